@@ -1,0 +1,463 @@
+/*
+ * sas_oracle.c -- TEST INFRASTRUCTURE ONLY (see sas_oracle.h).
+ *
+ * The oracle of the SANS Monte-Carlo hot path: one neutron at a time, fp64,
+ * in the order and notation of DESIGN.md section 3 ("readings" R-A*, R-B,
+ * R-C*), which restate PAPER.md where the paper speaks and fix a reading where
+ * it is silent.  No blocking, fusion or reordering.  Every expression is
+ * written so that, compiled with -ffp-contract=off, each operation is rounded
+ * once, left to right.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer vectors,
+ * closed forms of the sphere, brute-force Eq. 1 integrals for cylinder and
+ * ellipsoid, mpmath values of PY S(q) and 2J1(x)/x, weight conservation of the
+ * flat model, pencil-beam chi^2 against the numerically integrated I(Q),
+ * Guinier radii, model reductions.  "parity unpinned": whole detector images
+ * of configs c1-c4 have no external pin beyond those pieces (DESIGN.md s.3.D).
+ */
+#define _GNU_SOURCE
+#include "sas_oracle.h"
+
+#include <math.h>
+#include <string.h>
+
+static const double TWO_PI = 6.283185307179586;
+static const double FOUR_PI_3 = 4.1887902047863905; /* 4 pi / 3 */
+static const double PI_ = 3.141592653589793;
+
+/* ------------------------------------------------------------------ R-B */
+/* Philox4x32-10: multipliers 0xD2511F53, 0xCD9E8D57; Weyl key increments
+ * 0x9E3779B9, 0xBB67AE85; ten rounds (Salmon, Moraes, Dror, Shaw, SC'11). */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* u = (w + 0.5) * 2^-32, exact in fp64, in (0,1). */
+double orc_uniform(uint32_t word) { return ((double)word + 0.5) * 2.3283064365386963e-10; }
+
+/* draw block `block` of neutron `id` of experiment `exp`: ctr=(id_lo,id_hi,block,exp) */
+static void draw_block(uint64_t seed, uint64_t id, uint32_t block, uint32_t exp_index, double u4[4]) {
+  uint32_t ctr[4] = {(uint32_t)(id & 0xFFFFFFFFu), (uint32_t)(id >> 32), block, exp_index};
+  uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
+  uint32_t w[4];
+  orc_philox4x32_10(ctr, key, w);
+  for (int i = 0; i < 4; ++i) u4[i] = orc_uniform(w[i]);
+}
+
+/* -------------------------------------------------------------- R-C12 */
+/* Phi(u) = 3 (sin u - u cos u) / u^3 : sphere amplitude, PAPER.md:37 (Eq. 1
+ * integrated over a sphere).  Even series below u = 0.5 where the direct form
+ * cancels. */
+double orc_sphere_phi(double u) {
+  if (fabs(u) < 0.5) {
+    double u2 = u * u;
+    double s = 1.0 / 31135104000.0;
+    s = s * u2 - 1.0 / 172972800.0;
+    s = s * u2 + 1.0 / 1330560.0;
+    s = s * u2 - 1.0 / 15120.0;
+    s = s * u2 + 1.0 / 280.0;
+    s = s * u2 - 1.0 / 10.0;
+    s = s * u2 + 1.0;
+    return s;
+  }
+  return (3.0 * (sin(u) - u * cos(u))) / ((u * u) * u);
+}
+
+double orc_sinc(double x) {
+  if (x == 0.0) return 1.0;
+  return sin(x) / x;
+}
+
+/* Lambda(x) = 2 J1(x) / x, the disc factor of the cylinder. */
+double orc_lambda1(double x) {
+  if (x == 0.0) return 1.0;
+  return (2.0 * j1(x)) / x;
+}
+
+/* -------------------------------------------------------------- R-C13 */
+/* Percus-Yevick hard-sphere structure factor (Table II F.11). */
+double orc_py_sq(double q, double r_eff, double volfrac) {
+  double phi = volfrac;
+  double x = 2.0 * (q * r_eff);
+  double om = 1.0 - phi;
+  double om4 = (om * om) * (om * om);
+  double alpha = ((1.0 + 2.0 * phi) * (1.0 + 2.0 * phi)) / om4;
+  double beta = (-6.0 * phi) * ((1.0 + 0.5 * phi) * (1.0 + 0.5 * phi)) / om4;
+  double gamma = (phi * alpha) * 0.5;
+  double t1, t2, t3;
+  if (x < 1.0) {
+    static const double a1[8] = {1.0 / 3.0, -1.0 / 30.0, 1.0 / 840.0, -1.0 / 45360.0,
+                                 1.0 / 3991680.0, -1.0 / 518918400.0, 1.0 / 93405312000.0,
+                                 -1.0 / 22230464256000.0};
+    static const double a2[8] = {1.0 / 4.0, -1.0 / 36.0, 1.0 / 960.0, -1.0 / 50400.0,
+                                 1.0 / 4354560.0, -1.0 / 558835200.0, 1.0 / 99632332800.0,
+                                 -1.0 / 23538138624000.0};
+    static const double a3[8] = {1.0 / 6.0, -1.0 / 48.0, 1.0 / 1200.0, -1.0 / 60480.0,
+                                 1.0 / 5080320.0, -1.0 / 638668800.0, 1.0 / 112086374400.0,
+                                 -1.0 / 26153487360000.0};
+    double x2 = x * x;
+    t1 = a1[7]; t2 = a2[7]; t3 = a3[7];
+    for (int i = 6; i >= 0; --i) {
+      t1 = t1 * x2 + a1[i];
+      t2 = t2 * x2 + a2[i];
+      t3 = t3 * x2 + a3[i];
+    }
+  } else {
+    double s = sin(x), c = cos(x);
+    double x2 = x * x, x3 = x2 * x, x4 = x2 * x2, x6 = x3 * x3;
+    t1 = (s - x * c) / x3;
+    t2 = ((2.0 * x) * s + (2.0 - x2) * c - 2.0) / x4;
+    t3 = (-(x4 * c) + 4.0 * (((3.0 * x2 - 6.0) * c + (x3 - 6.0 * x) * s) + 6.0)) / x6;
+  }
+  return 1.0 / (1.0 + (24.0 * phi) * ((alpha * t1 + beta * t2) + gamma * t3));
+}
+
+/* ------------------------------------------------------ R-C12 amplitudes */
+/* One particle, sizes scaled by the polydispersity node values x0, x1
+ * (R-A12).  qa,qb,qc: projections of Q on the particle axes (PAPER.md:76-82,
+ * Eq. 6-7).  Returns F = integral of Delta-rho exp(-iQr) (real for these
+ * centro-symmetric shapes); *vol = normalising volume V_m
+ * (PAPER.md:49); *env = F with every shape factor set to 1. */
+double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double x0, double x1,
+                     double* vol, double* env) {
+  double q = sqrt((qa * qa + qb * qb) + qc * qc);
+  switch (m->model) {
+    case ORC_SPHERE: {
+      double R = m->size[0] * x0;
+      double V = FOUR_PI_3 * ((R * R) * R);
+      *vol = V;
+      *env = m->sld[0] * V;
+      return (m->sld[0] * V) * orc_sphere_phi(q * R);
+    }
+    case ORC_CORE_SHELL_SPHERE: {
+      double Rc = m->size[0] * x0;
+      double t = m->size[1] * x1;
+      double Rt = Rc + t;
+      double Vc = FOUR_PI_3 * ((Rc * Rc) * Rc);
+      double Vt = FOUR_PI_3 * ((Rt * Rt) * Rt);
+      double fc = (m->sld[0] - m->sld[1]) * Vc;
+      double ft = m->sld[1] * Vt;
+      *vol = Vt;
+      *env = fabs(fc) + fabs(ft);
+      return fc * orc_sphere_phi(q * Rc) + ft * orc_sphere_phi(q * Rt);
+    }
+    case ORC_CYLINDER: {
+      /* Eq. 9 with the projections as Eq. 1 gives them (R-A4):
+       * F = 2 drho V sinc(Q_C L/2) J1(Q_AB R)/(Q_AB R), V = pi R^2 L. */
+      double R = m->size[0] * x0;
+      double L = m->size[1] * x1;
+      double V = (PI_ * (R * R)) * L;
+      double qab = sqrt(qa * qa + qb * qb);
+      *vol = V;
+      *env = m->sld[0] * V;
+      return ((m->sld[0] * V) * orc_sinc(qc * (0.5 * L))) * orc_lambda1(qab * R);
+    }
+    case ORC_TRIAXIAL: {
+      double a = m->size[0] * x0, b = m->size[1] * x0, c = m->size[2] * x0;
+      double V = FOUR_PI_3 * ((a * b) * c);
+      double u = sqrt(((a * qa) * (a * qa) + (b * qb) * (b * qb)) + (c * qc) * (c * qc));
+      *vol = V;
+      *env = m->sld[0] * V;
+      return (m->sld[0] * V) * orc_sphere_phi(u);
+    }
+    case ORC_CORE_SHELL_TRIAXIAL: {
+      double a = m->size[0] * x0, b = m->size[1] * x0, c = m->size[2] * x0;
+      double t = m->size[3] * x1;
+      double at = a + t, bt = b + t, ct = c + t;
+      double Vc = FOUR_PI_3 * ((a * b) * c);
+      double Vt = FOUR_PI_3 * ((at * bt) * ct);
+      double uc = sqrt(((a * qa) * (a * qa) + (b * qb) * (b * qb)) + (c * qc) * (c * qc));
+      double ut = sqrt(((at * qa) * (at * qa) + (bt * qb) * (bt * qb)) + (ct * qc) * (ct * qc));
+      double fc = (m->sld[0] - m->sld[1]) * Vc;
+      double ft = m->sld[1] * Vt;
+      *vol = Vt;
+      *env = fabs(fc) + fabs(ft);
+      return fc * orc_sphere_phi(uc) + ft * orc_sphere_phi(ut);
+    }
+    default:
+      *vol = 1.0;
+      *env = 1.0;
+      return 1.0;
+  }
+}
+
+/* particle frame from (theta, phi, psi): R-A7 */
+static void frame_from_angles(double st, double ct, double sp, double cp, double ss, double cs,
+                              double A[3], double B[3], double C[3]) {
+  double a0[3] = {ct * cp, ct * sp, -st};
+  double b0[3] = {-sp, cp, 0.0};
+  C[0] = st * cp; C[1] = st * sp; C[2] = ct;
+  for (int i = 0; i < 3; ++i) {
+    A[i] = cs * a0[i] + ss * b0[i];
+    B[i] = cs * b0[i] - ss * a0[i];
+  }
+}
+
+static double dot3(const double a[3], const double b[3]) { return (a[0] * b[0] + a[1] * b[1]) + a[2] * b[2]; }
+
+/* I(Q) = 1e8 scale <F^2>/<V> S(q) + background  (Eq. 2-4;
+ * R-A2, R-A6).  Averages are fixed-node sums (R-A1, R-A9, R-A11). */
+double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3], double* env_out) {
+  if (m->model == ORC_FLAT) {
+    if (env_out) *env_out = m->scale + m->background;
+    return m->scale + m->background;
+  }
+  double A[3], B[3], C[3];
+  if (m->orient_kind == ORC_ORIENT_ISOTROPIC_MC) {
+    /* R-A3: isotropic = cos(theta) uniform, phi and psi uniform */
+    double ct = 1.0 - 2.0 * u_or[0];
+    double st = sqrt(1.0 - ct * ct);
+    double ph = TWO_PI * u_or[1];
+    double ps = TWO_PI * u_or[2];
+    frame_from_angles(st, ct, sin(ph), cos(ph), sin(ps), cos(ps), A, B, C);
+  } else {
+    frame_from_angles(sin(m->theta), cos(m->theta), sin(m->phi), cos(m->phi), sin(m->psi),
+                      cos(m->psi), A, B, C);
+  }
+  double qA = dot3(Q, A), qB = dot3(Q, B), qC = dot3(Q, C);
+  double q2 = dot3(Q, Q);
+  double qm = sqrt(q2);
+
+  int n_th = 1, n_ph = 1;
+  if (m->orient_kind == ORC_ORIENT_GAUSS_QUAD) { n_th = m->n_or[0]; n_ph = m->n_or[1]; }
+
+  double SF2 = 0.0, SE2 = 0.0, SV = 0.0;
+  for (int a = 0; a < m->n_pd[0]; ++a)
+    for (int b = 0; b < m->n_pd[1]; ++b) {
+      double V, E;
+      (void)orc_amplitude(m, 0.0, 0.0, 0.0, m->pd_x[0][a], m->pd_x[1][b], &V, &E);
+      SV += (m->pd_w[0][a] * m->pd_w[1][b]) * V;
+    }
+  for (int i = 0; i < n_th; ++i)
+    for (int j = 0; j < n_ph; ++j) {
+      double qa = qA, qb = qB, qc = qC, w_or = 1.0;
+      if (m->orient_kind == ORC_ORIENT_GAUSS_QUAD) {
+        /* R-A11: axis tilted by (dtheta_i, dphi_j) about the mean axis, in the
+         * mean particle frame: c_ij = (sin dth cos dph, sin dph, cos dth cos dph) */
+        double dth = m->or_d[0][i], dph = m->or_d[1][j];
+        double lx = sin(dth) * cos(dph), ly = sin(dph), lz = cos(dth) * cos(dph);
+        qc = (qA * lx + qB * ly) + qC * lz;
+        double r2 = q2 - qc * qc;
+        qa = sqrt(r2 > 0.0 ? r2 : 0.0); /* uniaxial models only: Q_AB (Eq. 7) */
+        qb = 0.0;
+        w_or = m->or_w[0][i] * m->or_w[1][j];
+      }
+      for (int a = 0; a < m->n_pd[0]; ++a)
+        for (int b = 0; b < m->n_pd[1]; ++b) {
+          double V, E;
+          double F = orc_amplitude(m, qa, qb, qc, m->pd_x[0][a], m->pd_x[1][b], &V, &E);
+          double w = w_or * (m->pd_w[0][a] * m->pd_w[1][b]);
+          SF2 += w * (F * F);
+          SE2 += w * (E * E);
+        }
+    }
+  double S = 1.0;
+  if (m->sq_kind == ORC_SQ_HARD_SPHERE_PY) S = orc_py_sq(qm, m->sq_radius_eff, m->sq_volfrac);
+  if (env_out) *env_out = ((1.0e8 * m->scale) * (SE2 / SV)) * S + m->background;
+  return ((1.0e8 * m->scale) * (SF2 / SV)) * S + m->background;
+}
+
+/* ------------------------------------------------------------- R-C5 */
+/* Ray (o + t d) against the sample volume centred at the origin of the sample
+ * frame.  Box: slab test per axis (x, y, z).  Cylinder: axis along y, radius
+ * sample_radius, height sample_yh.  Returns 0 on a miss. */
+static int intersect_sample(const orc_instrument* ins, const double o[3], const double d[3],
+                            double* t_in, double* t_out) {
+  double tin = -INFINITY, tout = INFINITY;
+  double h[3] = {0.5 * ins->sample_xw, 0.5 * ins->sample_yh, 0.5 * ins->sample_zd};
+  int first_axis = 0, last_axis = 2, step = 1;
+  if (ins->sample_shape == ORC_SAMPLE_CYL_Y) {
+    double a = d[0] * d[0] + d[2] * d[2];
+    double b = o[0] * d[0] + o[2] * d[2];
+    double c = (o[0] * o[0] + o[2] * o[2]) - ins->sample_radius * ins->sample_radius;
+    if (a == 0.0) {
+      if (c > 0.0) return 0;
+    } else {
+      double disc = b * b - a * c;
+      if (!(disc > 0.0)) return 0;
+      double sq = sqrt(disc);
+      double inv_a = 1.0 / a;
+      tin = (-b - sq) * inv_a;
+      tout = (-b + sq) * inv_a;
+    }
+    first_axis = 1; last_axis = 1; /* only the y slab remains */
+  }
+  for (int ax = first_axis; ax <= last_axis; ax += step) {
+    if (d[ax] == 0.0) {
+      if (fabs(o[ax]) > h[ax]) return 0;
+    } else {
+      double inv = 1.0 / d[ax];
+      double t1 = (-h[ax] - o[ax]) * inv;
+      double t2 = (h[ax] - o[ax]) * inv;
+      if (t1 > t2) { double tmp = t1; t1 = t2; t2 = tmp; }
+      if (t1 > tin) tin = t1;
+      if (t2 < tout) tout = t2;
+    }
+  }
+  *t_in = tin;
+  *t_out = tout;
+  return 1;
+}
+
+/* ---------------------------------------------------- R-C2 .. R-C11 */
+void orc_trace_one(const orc_instrument* ins, const orc_model* m, uint64_t seed, uint64_t id,
+                   uint32_t exp_index, orc_record* rec) {
+  memset(rec, 0, sizeof(*rec));
+  rec->pixel = -1;
+  double* u = rec->u;
+  draw_block(seed, id, 0, exp_index, u + 0);
+
+  /* R-C2 source point (flat = uniform), z0 = 0 */
+  double x0 = (u[0] - 0.5) * ins->src_xw;
+  double y0 = (u[1] - 0.5) * ins->src_yh;
+  double z0 = 0.0;
+  /* R-C3 direction towards a uniform point of the focus rectangle */
+  double xt = (u[2] - 0.5) * ins->focus_xw;
+  double yt = (u[3] - 0.5) * ins->focus_yh;
+  double zt = ins->focus_z;
+  double Dx = xt - x0, Dy = yt - y0, Dz = zt - z0;
+  double r2 = (Dx * Dx + Dy * Dy) + Dz * Dz;
+  double r = sqrt(r2);
+  double inv_r = 1.0 / r;
+  double d[3] = {Dx * inv_r, Dy * inv_r, Dz * inv_r};
+  double dOmega = (((ins->focus_xw * ins->focus_yh) * d[2]) * inv_r) * inv_r;
+  double dlam = ins->lambda_max - ins->lambda_min;
+  double dlam_w = dlam > 0.0 ? dlam : 1.0;
+  double p0 = ((ins->flux * ((ins->src_xw * ins->src_yh) * 1.0e4)) * dOmega) * dlam_w;
+  rec->p0 = p0;
+
+  /* R-C4 slits: straight lines, absorb outside the aperture (edges inclusive) */
+  double inv_dz = 1.0 / d[2];
+  {
+    double s = (ins->slit1_z - z0) * inv_dz;
+    double xs = x0 + d[0] * s, ys = y0 + d[1] * s;
+    if (fabs(xs) > 0.5 * ins->slit1_xw || fabs(ys) > 0.5 * ins->slit1_yh) { rec->status = ORC_SLIT1; return; }
+  }
+  {
+    double s = (ins->slit2_z - z0) * inv_dz;
+    double xs = x0 + d[0] * s, ys = y0 + d[1] * s;
+    if (fabs(xs) > 0.5 * ins->slit2_xw || fabs(ys) > 0.5 * ins->slit2_yh) { rec->status = ORC_SLIT2; return; }
+  }
+
+  draw_block(seed, id, 1, exp_index, u + 4);
+  double lambda = ins->lambda_min + u[4] * dlam;
+  rec->lambda = lambda;
+
+  /* R-C5 sample intersection in the sample frame (origin at (0,0,sample_z)) */
+  double o[3] = {x0, y0, z0 - ins->sample_z};
+  double tin, tout;
+  if (!intersect_sample(ins, o, d, &tin, &tout)) { rec->status = ORC_MISS_SAMPLE; return; }
+  if (tin < 0.0) tin = 0.0;
+  if (!(tout > tin)) { rec->status = ORC_MISS_SAMPLE; return; }
+  double ell = tout - tin;
+  rec->ell = ell;
+
+  /* R-C6 forced single scattering, uniform along the chord */
+  double ts = tin + u[5] * ell;
+  double rs[3] = {x0 + d[0] * ts, y0 + d[1] * ts, z0 + d[2] * ts};
+
+  /* R-C7 choose |Q| and azimuth */
+  double q = ins->q_min + u[6] * (ins->q_max - ins->q_min);
+  double chi = TWO_PI * u[7];
+  double k = TWO_PI / lambda;
+  double inv_k = lambda / TWO_PI;
+  double qk = q * inv_k;
+  double s = 0.5 * qk; /* sin(theta), |Q| = 2 k sin(theta) */
+  rec->q = q;
+  if (s >= 1.0) { rec->status = ORC_UNREACHABLE; return; }
+  double ss2 = 2.0 * (s * s);              /* 1 - cos(2 theta) */
+  double c2 = 1.0 - ss2;                   /* cos(2 theta) */
+  double s2 = 2.0 * (s * sqrt(1.0 - s * s)); /* sin(2 theta) */
+
+  /* R-C8 outgoing direction: rotate d by 2 theta at azimuth chi */
+  double n = sqrt(d[2] * d[2] + d[0] * d[0]);
+  double inv_n = 1.0 / n;
+  double e1x = d[2] * inv_n, e1z = -(d[0] * inv_n);       /* e1 = y^ x d^, normalised; e1y = 0 */
+  double e2x = d[1] * e1z, e2y = d[2] * e1x - d[0] * e1z, e2z = -(d[1] * e1x); /* e2 = d^ x e1 */
+  double sc = sin(chi), cc = cos(chi);
+  double tx = cc * e1x + sc * e2x, ty = sc * e2y, tz = cc * e1z + sc * e2z;
+  double dp[3] = {c2 * d[0] + s2 * tx, c2 * d[1] + s2 * ty, c2 * d[2] + s2 * tz};
+  double Q[3] = {k * (ss2 * d[0] - s2 * tx), k * (ss2 * d[1] - s2 * ty), k * (ss2 * d[2] - s2 * tz)};
+  rec->Q[0] = Q[0]; rec->Q[1] = Q[1]; rec->Q[2] = Q[2];
+
+  /* R-C9 detector plane at sample_z + det_dist */
+  if (!(dp[2] > 0.0)) { rec->status = ORC_MISS_DET; return; }
+  double inv_dpz = 1.0 / dp[2];
+  double td = ((ins->sample_z + ins->det_dist) - rs[2]) * inv_dpz;
+  double X = rs[0] + dp[0] * td, Y = rs[1] + dp[1] * td;
+  double fx = (X + 0.5 * ins->det_xw) * ((double)ins->det_nx / ins->det_xw);
+  double fy = (Y + 0.5 * ins->det_yh) * ((double)ins->det_ny / ins->det_yh);
+  if (!(fx >= 0.0 && fx < (double)ins->det_nx && fy >= 0.0 && fy < (double)ins->det_ny)) {
+    rec->status = ORC_MISS_DET; return;
+  }
+  int ix = (int)floor(fx), iy = (int)floor(fy);
+  rec->pixel = iy * ins->det_nx + ix;
+
+  /* orientation uniforms (draws 8,9,10) only for per-neutron random orientation */
+  if (m->orient_kind == ORC_ORIENT_ISOTROPIC_MC && m->model != ORC_FLAT) draw_block(seed, id, 2, exp_index, u + 8);
+
+  /* R-C11 attenuation along the path inside the sample */
+  double T = 1.0;
+  if (ins->mu_abs_2200 != 0.0 || ins->mu_inc != 0.0) {
+    double mu = (ins->mu_abs_2200 * lambda) / 1.7982 + ins->mu_inc;
+    double o2[3] = {rs[0], rs[1], rs[2] - ins->sample_z};
+    double tin2, tout2, ell_out = 0.0;
+    if (intersect_sample(ins, o2, dp, &tin2, &tout2) && tout2 > 0.0) ell_out = tout2;
+    T = exp(-(mu * (u[5] * ell + ell_out)));
+  }
+
+  double env;
+  double I = orc_intensity(m, Q, u + 8, &env);
+  rec->intensity = I;
+  double jac = qk * inv_k;                            /* q / k^2 */
+  double qnorm = TWO_PI * (ins->q_max - ins->q_min);  /* 1 / pdf(q, chi) */
+  double geo = (p0 * T) * (100.0 * ell);              /* ell in cm: I is per cm */
+  rec->weight = ((geo * I) * jac) * qnorm;
+  rec->weight_env = ((geo * env) * jac) * qnorm;
+  rec->status = ORC_DETECTED;
+}
+
+void orc_trace_range(const orc_instrument* ins, const orc_model* m, uint64_t seed, uint64_t first,
+                     uint64_t n, uint32_t exp_index, int32_t* pixel, double* weight, double* weight_env,
+                     double* q, double* sum_p, double* sum_p2, uint64_t* counts, uint64_t counters[8]) {
+  orc_record rec;
+  for (uint64_t i = 0; i < n; ++i) {
+    orc_trace_one(ins, m, seed, first + i, exp_index, &rec);
+    if (pixel) pixel[i] = rec.pixel;
+    if (weight) weight[i] = rec.status == ORC_DETECTED ? rec.weight : 0.0;
+    if (weight_env) weight_env[i] = rec.status == ORC_DETECTED ? rec.weight_env : 0.0;
+    if (q) q[i] = rec.q;
+    if (counters) {
+      counters[0] += 1;
+      switch (rec.status) {
+        case ORC_SLIT1: counters[1] += 1; break;
+        case ORC_SLIT2: counters[2] += 1; break;
+        case ORC_MISS_SAMPLE: counters[3] += 1; break;
+        case ORC_UNREACHABLE: counters[4] += 1; break;
+        case ORC_MISS_DET: counters[5] += 1; break;
+        default: counters[6] += 1; break;
+      }
+    }
+    if (rec.status == ORC_DETECTED) {
+      /* R-C14 accumulate in id order */
+      if (counts) counts[rec.pixel] += 1;
+      if (sum_p) sum_p[rec.pixel] += rec.weight;
+      if (sum_p2) sum_p2[rec.pixel] += rec.weight * rec.weight;
+    }
+  }
+}

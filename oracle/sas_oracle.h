@@ -1,0 +1,138 @@
+/*
+ * sas_oracle.h -- TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, single-threaded fp64 CPU restatement of the SANS Monte-Carlo
+ * hot path of arXiv 2501.06054, written from the paper and the
+ * readings listed in DESIGN.md section 3.  It shares no code, header, table
+ * or constant generator with the CUDA library under paper_2501_06054_b200/.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call it.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fPIC -shared  (no FMA contraction: every
+ * written operation is individually rounded, DESIGN.md R-C0).
+ *
+ * Units: instrument geometry in metres, wavelengths in Angstrom, Q in 1/A,
+ * particle sizes in A, contrasts in 1/A^2, intensity in 1/cm.
+ */
+#ifndef SAS_ORACLE_H
+#define SAS_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* outcome of one neutron (PAPER.md:143-147 trace loop; DESIGN.md R-C4..R-C9) */
+enum {
+  ORC_DETECTED = 0,
+  ORC_SLIT1 = 1,
+  ORC_SLIT2 = 2,
+  ORC_MISS_SAMPLE = 3,
+  ORC_UNREACHABLE = 4,
+  ORC_MISS_DET = 5
+};
+
+enum { ORC_SAMPLE_BOX = 0, ORC_SAMPLE_CYL_Y = 1 };
+enum {
+  ORC_SPHERE = 0,
+  ORC_CORE_SHELL_SPHERE = 1,
+  ORC_CYLINDER = 2,
+  ORC_TRIAXIAL = 3,
+  ORC_CORE_SHELL_TRIAXIAL = 4,
+  ORC_FLAT = 5
+};
+enum { ORC_ORIENT_FIXED = 0, ORC_ORIENT_GAUSS_QUAD = 1, ORC_ORIENT_ISOTROPIC_MC = 2 };
+enum { ORC_SQ_NONE = 0, ORC_SQ_HARD_SPHERE_PY = 1 };
+
+#define ORC_MAX_NODES 64
+
+/* Instrument: PAPER.md:86 (source, slits, sample, 2-D PSD). */
+typedef struct {
+  double src_xw, src_yh;          /* flat source, m */
+  double lambda_min, lambda_max;  /* A */
+  double flux;
+  double slit1_z, slit1_xw, slit1_yh;
+  double slit2_z, slit2_xw, slit2_yh;
+  double focus_z, focus_xw, focus_yh;
+  int32_t sample_shape;
+  int32_t pad0;
+  double sample_z, sample_xw, sample_yh, sample_zd, sample_radius;
+  double mu_abs_2200, mu_inc;     /* 1/m */
+  double q_min, q_max;            /* 1/A */
+  double det_dist, det_xw, det_yh;
+  int32_t det_nx, det_ny;
+} orc_instrument;
+
+/* Sample model with its quadrature tables already expanded by the caller
+ * (oracle/oracle.py builds them with numpy: DESIGN.md R-A9, R-A11). */
+typedef struct {
+  int32_t model;
+  int32_t orient_kind;
+  int32_t sq_kind;
+  int32_t pad0;
+  double scale, background;
+  double sld[3];
+  double size[4];
+  /* polydispersity: two tensor axes of relative-size nodes (value, weight);
+   * n_pd[k]=1 with node 1.0 / weight 1.0 means monodisperse. The node value
+   * multiplies size[...] as DESIGN.md R-A12 states per model. */
+  int32_t n_pd[2];
+  double pd_x[2][ORC_MAX_NODES];
+  double pd_w[2][ORC_MAX_NODES];
+  /* orientation */
+  double theta, phi, psi;         /* rad */
+  int32_t n_or[2];                /* Gauss quadrature tilts (theta, phi) */
+  double or_d[2][ORC_MAX_NODES];  /* tilt angle Delta (rad) */
+  double or_w[2][ORC_MAX_NODES];
+  double sq_radius_eff, sq_volfrac;
+} orc_model;
+
+/* full per-neutron record, for pins and parity */
+typedef struct {
+  int32_t status;
+  int32_t pixel;       /* iy*nx+ix, or -1 */
+  double weight;       /* p   (R-C11) */
+  double weight_env;   /* p with every shape factor Phi, sinc, Lambda := 1 (R-C15) */
+  double q;            /* sampled |Q| */
+  double Q[3];
+  double lambda;
+  double ell;          /* chord length in the sample, m */
+  double p0;           /* source weight */
+  double intensity;    /* I(Q) 1/cm */
+  double u[12];        /* the uniforms drawn (unused ones stay 0) */
+} orc_record;
+
+/* Philox4x32-10, Salmon et al. SC'11 (DESIGN.md R-B). */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double orc_uniform(uint32_t word);
+
+/* form / structure factor pieces (PAPER.md:37-49 Eq.1-4, :161-163 Eq.9) */
+double orc_sphere_phi(double u);                 /* 3(sin u - u cos u)/u^3 */
+double orc_sinc(double x);
+double orc_lambda1(double x);                    /* 2 J1(x)/x */
+double orc_py_sq(double q, double r_eff, double volfrac);
+/* I(Q) in 1/cm for a Q vector given in the GLOBAL frame, with orientation
+ * uniforms u_or[3] (used only by ORC_ORIENT_ISOTROPIC_MC). env (nullable)
+ * receives the envelope intensity. */
+double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3], double* env);
+/* amplitude F (A^-2 * A^3) of one particle with explicit axes projections */
+double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double x0, double x1,
+                     double* vol, double* env);
+
+/* one neutron */
+void orc_trace_one(const orc_instrument* ins, const orc_model* m, uint64_t seed, uint64_t id,
+                   uint32_t exp_index, orc_record* rec);
+
+/* ids [first, first+n): optional per-neutron dumps (nullable), optional
+ * histograms (nullable, accumulated in id order: R-C14), counters[8]
+ * (launched, slit1, slit2, miss_sample, unreachable, miss_det, detected, 0)
+ * are incremented. */
+void orc_trace_range(const orc_instrument* ins, const orc_model* m, uint64_t seed, uint64_t first,
+                     uint64_t n, uint32_t exp_index, int32_t* pixel, double* weight, double* weight_env,
+                     double* q, double* sum_p, double* sum_p2, uint64_t* counts, uint64_t counters[8]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

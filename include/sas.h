@@ -1,0 +1,181 @@
+/*
+ * sas.h -- C ABI of the B200-native SANS Monte-Carlo tracer (libsas_b200.so).
+ *
+ * The library traces neutrons of a small-angle-scattering virtual experiment
+ * (PAPER.md:19, :86, :143-147 -- arXiv 2501.06054): source -> two slits ->
+ * sample -> choose Q -> weight by the SAS model intensity I(Q) (PAPER.md:37-49,
+ * Eq. 1-4; :161-163, Eq. 9; polydispersity and orientation distributions
+ * :122-135) -> 2-D position-sensitive detector histogram.  Every step runs in
+ * hand-written CUDA kernels for sm_100a; there is no CPU fallback: a call that
+ * cannot run on the device returns SAS_ECUDA.
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross the boundary; every call returns sas_status
+ *     (SAS_OK == 0) and leaves a message readable with sas_last_error().
+ *   - "h_" pointers are HOST memory, "d_" pointers are DEVICE memory of the
+ *     current CUDA device, both caller-owned and caller-sized unless said
+ *     otherwise.  Descriptors are host structs, copied by the call.
+ *   - Instrument lengths are metres; wavelengths Angstrom; Q in 1/Angstrom;
+ *     particle sizes Angstrom; contrasts 1/Angstrom^2; intensities 1/cm;
+ *     angles radians.
+ *   - Detector arrays are row-major [ny][nx], index = iy*nx + ix; in batched
+ *     mode [n_exp][ny][nx].  sum_p and sum_p2 are double, counts uint64_t.
+ *   - Weights carry no 1/N: the weight of a neutron depends only on
+ *     (seed, id, experiment index) and the descriptors, so id ranges are
+ *     additive; normalise with counters[0] (launched).
+ *   - sas_trace* enqueue on the context's stream and return; sas_read_detector
+ *     and sas_get_counters synchronise that stream.
+ *   - A context is not thread-safe; distinct contexts are independent.
+ *   - The precise arithmetic (draw table, operation order) is DESIGN.md s.3.
+ */
+#ifndef SAS_H
+#define SAS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sas_ctx sas_ctx; /* opaque; owns device constants, tables, counters */
+
+typedef enum {
+  SAS_OK = 0,
+  SAS_EINVAL = 1,       /* bad descriptor or argument */
+  SAS_ESTATE = 2,       /* call out of order (e.g. trace before set_model) */
+  SAS_ECUDA = 3,        /* CUDA runtime failure, or no usable device */
+  SAS_ENOMEM = 4,
+  SAS_EUNSUPPORTED = 5  /* valid request this build does not implement */
+} sas_status;
+
+enum { SAS_FP32 = 0, SAS_FP64 = 1 }; /* precision of the MODEL evaluation; RNG->uniform and geometry are always fp64 */
+enum { SAS_SAMPLE_BOX = 0, SAS_SAMPLE_CYL_Y = 1 };
+enum {
+  SAS_SPHERE = 0,              /* Table II F.9 */
+  SAS_CORE_SHELL_SPHERE = 1,   /* Table II F.3  */
+  SAS_CYLINDER = 2,            /* Table I  A.7, Eq. 9 */
+  SAS_TRIAXIAL_ELLIPSOID = 3,  /* Table I  B.3  */
+  SAS_CORE_SHELL_TRIAXIAL = 4, /* B.3's shape with B.1's two-contrast composition (DESIGN.md R-A12) */
+  SAS_FLAT = 5                 /* I == scale + background: test model */
+};
+enum { SAS_ORIENT_FIXED = 0, SAS_ORIENT_GAUSS_QUAD = 1, SAS_ORIENT_ISOTROPIC_MC = 2 };
+enum { SAS_PD_NONE = 0, SAS_PD_SCHULZ_QUAD = 1 };
+enum { SAS_SQ_NONE = 0, SAS_SQ_HARD_SPHERE_PY = 1 };
+
+#define SAS_MAX_NODES 64      /* per quadrature axis */
+#define SAS_MAX_PD_PAIRS 1024 /* pd_nodes[0]*pd_nodes[1] */
+
+/* Instrument (source, slits defining the divergence, sample, 2-D PSD). */
+typedef struct {
+  uint32_t struct_size;              /* = sizeof(sas_instrument_desc) */
+  int32_t sample_shape;              /* SAS_SAMPLE_* */
+  double src_xw, src_yh;             /* flat rectangular source in the plane z = 0 */
+  double lambda_min, lambda_max;     /* uniform wavelength band; equal => monochromatic */
+  double flux;                       /* n / (cm^2 s sr A); 1 for unit flux */
+  double slit1_z, slit1_xw, slit1_yh;
+  double slit2_z, slit2_xw, slit2_yh;
+  double focus_z, focus_xw, focus_yh; /* rectangle the source aims at, uniformly (normally slit 2) */
+  double sample_z;                   /* sample centre */
+  double sample_xw, sample_yh, sample_zd; /* box extents; yh is also the cylinder height */
+  double sample_radius;              /* SAS_SAMPLE_CYL_Y: axis along y */
+  double mu_abs_2200, mu_inc;        /* 1/m; absorption at 1.7982 A (scaled ~lambda) and incoherent; 0 => no attenuation */
+  double q_min, q_max;               /* |Q| is drawn uniformly in [q_min, q_max] */
+  double det_dist;                   /* detector plane at sample_z + det_dist */
+  double det_xw, det_yh;
+  int32_t det_nx, det_ny;
+} sas_instrument_desc;
+
+/* Sample model (PAPER.md:51 parameters {theta_i}; :122-133 distributions). */
+typedef struct {
+  uint32_t struct_size;              /* = sizeof(sas_model_desc) */
+  int32_t model;                     /* SAS_SPHERE ... */
+  int32_t precision;                 /* SAS_FP32 | SAS_FP64 */
+  int32_t orient_kind;               /* SAS_ORIENT_* */
+  int32_t sq_kind;                   /* SAS_SQ_* */
+  int32_t pd_kind[2];                /* SAS_PD_* for the two polydisperse lengths */
+  int32_t pd_nodes[2];               /* quadrature nodes (1..SAS_MAX_NODES) */
+  int32_t n_theta, n_phi;            /* SAS_ORIENT_GAUSS_QUAD nodes */
+  int32_t reserved;
+  double scale, background;          /* scale = volume fraction; background 1/cm */
+  double sld[3];                     /* contrast vs solvent: [0] particle/core, [1] shell */
+  double size[4];                    /* sphere R | core-shell Rc,t | cylinder R,L | a,b,c | a,b,c,t */
+  double pd_rel[2];                  /* sigma/mean of: [0] R|Rc|R|common scale of (a,b,c); [1] t|L|t */
+  double theta, phi, psi;            /* axis polar angle from +z, azimuth from +x, spin (DESIGN.md R-A7) */
+  double sigma_theta, sigma_phi;     /* Gaussian spreads of the two tilts (uniaxial models only) */
+  double sq_radius_eff, sq_volfrac;  /* Percus-Yevick hard-sphere S(q) (Table II F.11) */
+} sas_model_desc;
+
+/* --- single experiment --------------------------------------------------- */
+
+/* Validate and copy the instrument; allocate device state on the current CUDA
+ * device (its own zeroed histograms and an internal stream until sas_bind_buffers
+ * says otherwise).  *out is set only on SAS_OK; free with sas_destroy. */
+sas_status sas_create_instrument(const sas_instrument_desc* instr, sas_ctx** out);
+
+/* Use caller-owned DEVICE histograms ([n_exp][ny][nx]: double, double, uint64)
+ * and CUDA stream (a cudaStream_t passed as void*; NULL = default stream).
+ * The caller keeps ownership and must keep them alive; contents are not cleared. */
+sas_status sas_bind_buffers(sas_ctx* ctx, void* d_sum_p, void* d_sum_p2, void* d_counts, void* cuda_stream);
+
+/* Validate the model, build the quadrature tables on the host (generalised
+ * Gauss-Laguerre for Schulz sizes, Gauss-Legendre for Gaussian tilts;
+ * DESIGN.md R-A9, R-A11) and upload them (asynchronous H2D on the stream). */
+sas_status sas_set_model(sas_ctx* ctx, const sas_model_desc* model);
+
+/* Trace neutron ids [0, n) (sas_trace) or [first_id, first_id+n) and ACCUMULATE
+ * into the histograms and counters (PAPER.md:143-147 trace loop). */
+sas_status sas_trace(sas_ctx* ctx, uint64_t n_neutrons, uint64_t seed);
+sas_status sas_trace_range(sas_ctx* ctx, uint64_t first_id, uint64_t n, uint64_t seed);
+
+/* Parity hook: no histogram; writes, for id = first_id + i, d_pixel[i] (iy*nx+ix,
+ * or -1 when the neutron is not detected), d_weight[i] (0 when not detected) and,
+ * if d_q is not NULL, the drawn |Q| (0 if the neutron died before the draw).
+ * Single-experiment contexts only; exp_index enters the Philox counter. n <= 2^31. */
+sas_status sas_trace_dump(sas_ctx* ctx, uint64_t first_id, uint64_t n, uint64_t seed, uint32_t exp_index,
+                          int32_t* d_pixel, double* d_weight, double* d_q);
+
+/* Synchronise and copy the histograms to HOST arrays (any may be NULL). */
+sas_status sas_read_detector(sas_ctx* ctx, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts);
+
+/* out[8] = launched, absorbed at slit 1, at slit 2, missed the sample, |Q| unreachable
+ * (q >= 2k), missed the detector, detected, 0.  Summed over experiments.  Synchronises. */
+sas_status sas_get_counters(sas_ctx* ctx, uint64_t out[8]);
+
+/* Zero histograms and counters (asynchronous on the stream). */
+sas_status sas_reset_detector(sas_ctx* ctx);
+
+void sas_destroy(sas_ctx* ctx);
+/* Message of the last failing call on ctx (or of the last failing create when ctx == NULL). */
+const char* sas_last_error(const sas_ctx* ctx);
+
+/* --- batched mode (PAPER.md:19, :213 dataset generation) ------------------ */
+
+/* n_exp experiments, each with its own instrument + model and its own histogram
+ * ([n_exp][ny][nx]; every experiment must have the same det_nx, det_ny and the same
+ * precision).  Tables are built and uploaded here. */
+sas_status sas_create_batch(const sas_instrument_desc* instr, const sas_model_desc* model, uint32_t n_exp,
+                            sas_ctx** out);
+/* Trace ids [0, n_neutrons_each) of every experiment in ONE launch; experiment e
+ * uses Philox counter word 3 = e. */
+sas_status sas_trace_batch(sas_ctx* ctx, uint64_t n_neutrons_each, uint64_t seed);
+
+/* --- introspection -------------------------------------------------------- */
+/* HOST-ONLY (needs no device): the quadrature rule the library builds for
+ * kind 0 = Schulz sizes of relative width param (values = size multipliers of mean 1;
+ *          generalised Gauss-Laguerre, DESIGN.md R-A9),
+ * kind 1 = Gaussian tilt of standard deviation param radians on [-3 sigma, 3 sigma]
+ *          (values = tilt angles; Gauss-Legendre x Gaussian, DESIGN.md R-A11).
+ * Writes n values and n weights (weights sum to 1).  n in 1..SAS_MAX_NODES. */
+sas_status sas_quadrature_nodes(int32_t kind, double param, int32_t n, double* h_values, double* h_weights);
+/* Number of kernel launches this context has issued, and launch geometry of the last one. */
+sas_status sas_get_launch_info(sas_ctx* ctx, uint64_t* n_launches, int32_t* grid, int32_t* block,
+                               int32_t* smem_bytes);
+/* Average device time in ms (CUDA events on the context's stream) of the trace kernels launched
+ * since the last call with reset != 0; *n_timed = how many launches the average covers. */
+sas_status sas_get_kernel_time(sas_ctx* ctx, int32_t reset, double* avg_ms, uint64_t* n_timed);
+const char* sas_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAS_H */

@@ -1,0 +1,309 @@
+// Device math of the CUDA tracer: Philox4x32-10, sin/cos, sphere Phi, sinc, Lambda = 2J1(x)/x and
+// Percus-Yevick S(q) in fp32 and fp64.  The translation unit is compiled with -fmad=false so that
+// the fp64 geometry keeps one rounding per written operation (DESIGN.md R-C0); everything here that
+// wants a fused multiply-add says so with fmaf()/fma().
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "coeffs_generated.h"
+
+namespace sas {
+
+// ---------------------------------------------------------------- Philox4x32-10 (DESIGN.md R-B)
+struct PhiloxKeys {  // the ten round keys are the same for every neutron of a launch
+  uint32_t k0[10], k1[10];
+};
+
+__host__ __device__ inline void philox_make_keys(uint64_t seed, PhiloxKeys& pk) {
+  uint32_t a = (uint32_t)seed, b = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) {
+    pk.k0[r] = a;
+    pk.k1[r] = b;
+    a += 0x9E3779B9u;
+    b += 0xBB67AE85u;
+  }
+}
+
+__device__ __forceinline__ void philox4x32_10(const PhiloxKeys& pk, uint32_t c0, uint32_t c1, uint32_t c2,
+                                              uint32_t c3, uint32_t out[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ pk.k0[r];
+    uint32_t n2 = hi0 ^ c3 ^ pk.k1[r];
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// u = (w + 0.5) 2^-32, exact: (double)w is assembled as 2^52 + w minus 2^52 (no I2F conversion).
+__device__ __forceinline__ double uniform_from_word(uint32_t w) {
+  double d = __hiloint2double(0x43300000, (int)w) - 4503599627370496.0;
+  return (d + 0.5) * 2.3283064365386963e-10;
+}
+
+// ---------------------------------------------------------------- polynomial helpers
+template <int N>
+__device__ __forceinline__ float horner(const float (&c)[N], float t) {
+  float r = c[N - 1];
+#pragma unroll
+  for (int i = N - 2; i >= 0; --i) r = fmaf(r, t, c[i]);
+  return r;
+}
+
+// ---------------------------------------------------------------- sin/cos
+// fp32: three-step Cody-Waite reduction by pi/2 with FMAs, kernels on [-pi/4, pi/4].
+// Valid for |x| < ~1e5 (k exact in fp32); the tracer's arguments are q*size < ~1e3.
+__device__ __forceinline__ void sincos_r(float x, float& s, float& c) {
+  const float kf = rintf(x * 0.636619772f);
+  float r = fmaf(kf, -1.57079625129699707031e+00f, x);
+  r = fmaf(kf, -7.54978941586159635335e-08f, r);
+  r = fmaf(kf, -5.39030252995776476554e-15f, r);
+  const int k = (int)kf;
+  const float z = r * r;
+  const float SP[SAS_SIN_POLY_N] = SAS_SIN_POLY;
+  const float CP[SAS_COS_POLY_N] = SAS_COS_POLY;
+  const float ps = fmaf(r * z, horner(SP, z), r);
+  const float pc = fmaf(z, horner(CP, z), 1.0f);
+  float ss = (k & 1) ? pc : ps;
+  float cc = (k & 1) ? ps : pc;
+  s = (k & 2) ? -ss : ss;
+  c = ((k + 1) & 2) ? -cc : cc;
+}
+__device__ __forceinline__ void sincos_r(double x, double& s, double& c) { sincos(x, &s, &c); }
+
+__device__ __forceinline__ float rcp_r(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ double rcp_r(double x) { return 1.0 / x; }
+__device__ __forceinline__ float sqrt_r(float x) { return __fsqrt_rn(x); }
+__device__ __forceinline__ double sqrt_r(double x) { return sqrt(x); }
+__device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
+
+// ---------------------------------------------------------------- phases in extended precision
+// A form-factor phase is (projection of Q) x (particle length) and reaches hundreds of radians
+// (q L/2 for a 2000 A rod).  In the fp32 model path the projection is carried as an unevaluated sum
+// of two floats (hi + lo, from the fp64 value) and so is the length (split by the host), the product
+// is formed with FMAs and the lo part joins after the Cody-Waite reduction: the reduced argument
+// is good to ~1e-7 rad whatever the magnitude.  In the fp64 path both are plain doubles.
+template <typename Real> struct Proj;
+template <> struct Proj<double> { double v; };
+template <> struct Proj<float> { float hi, lo; };
+template <typename Real> struct Phase;
+template <> struct Phase<double> { double v; };
+template <> struct Phase<float> { float hi, lo; };
+
+template <typename Real> __device__ __forceinline__ Proj<Real> make_proj(double v);
+template <> __device__ __forceinline__ Proj<double> make_proj<double>(double v) { return {v}; }
+template <> __device__ __forceinline__ Proj<float> make_proj<float>(double v) {
+  const float hi = (float)v;
+  return {hi, (float)(v - (double)hi)};
+}
+__device__ __forceinline__ Phase<double> phase_mul(Proj<double> p, double l_hi, double) { return {p.v * l_hi}; }
+__device__ __forceinline__ Phase<float> phase_mul(Proj<float> p, float l_hi, float l_lo) {
+  const float h = p.hi * l_hi;
+  float e = fmaf(p.hi, l_hi, -h);
+  e = fmaf(p.hi, l_lo, e);
+  e = fmaf(p.lo, l_hi, e);
+  return {h, e};
+}
+__device__ __forceinline__ double ph_val(Phase<double> p) { return p.v; }
+__device__ __forceinline__ float ph_val(Phase<float> p) { return p.hi; }
+
+__device__ __forceinline__ void sincos_ph(Phase<double> p, double& s, double& c) { sincos(p.v, &s, &c); }
+__device__ __forceinline__ void sincos_ph(Phase<float> p, float& s, float& c) {
+  const float kf = rintf(p.hi * 0.636619772f);
+  float r = fmaf(kf, -1.57079625129699707031e+00f, p.hi);  // exact: the product has <= 32 significant bits
+  r = fmaf(kf, -7.54978941586159635335e-08f, r);
+  r = fmaf(kf, -5.39030252995776476554e-15f, r) + p.lo;
+  const int k = (int)kf;
+  const float z = r * r;
+  const float SP[SAS_SIN_POLY_N] = SAS_SIN_POLY;
+  const float CP[SAS_COS_POLY_N] = SAS_COS_POLY;
+  const float ps = fmaf(r * z, horner(SP, z), r);
+  const float pc = fmaf(z, horner(CP, z), 1.0f);
+  const float ss = (k & 1) ? pc : ps;
+  const float cc = (k & 1) ? ps : pc;
+  s = (k & 2) ? -ss : ss;
+  c = ((k + 1) & 2) ? -cc : cc;
+}
+
+// sin/cos of 2 pi u, u in (0,1), fp64, ~1e-13: exact reduction by quarter turns, Taylor kernels.
+// Used by the fp32 model path for the per-neutron random orientation (the fp64 path calls sincos()).
+__device__ __forceinline__ void sincos_2pi(double u, double& s, double& c) {
+  const double kf = rint(4.0 * u);
+  const double r = 6.283185307179586 * (u - 0.25 * kf);  // |r| <= pi/4
+  const int k = (int)kf;
+  const double z = r * r;
+  double ps = fma(z, 1.0 / 6227020800.0, -1.0 / 39916800.0);
+  ps = fma(ps, z, 1.0 / 362880.0);
+  ps = fma(ps, z, -1.0 / 5040.0);
+  ps = fma(ps, z, 1.0 / 120.0);
+  ps = fma(ps, z, -1.0 / 6.0);
+  ps = fma(r * z, ps, r);
+  double pc = fma(z, -1.0 / 479001600.0, 1.0 / 3628800.0);
+  pc = fma(pc, z, -1.0 / 40320.0);
+  pc = fma(pc, z, 1.0 / 720.0);
+  pc = fma(pc, z, -1.0 / 24.0);
+  pc = fma(pc, z, 0.5);
+  pc = fma(-z, pc, 1.0);
+  const double ss = (k & 1) ? pc : ps;
+  const double cc = (k & 1) ? ps : pc;
+  s = (k & 2) ? -ss : ss;
+  c = ((k + 1) & 2) ? -cc : cc;
+}
+
+// ---------------------------------------------------------------- sphere Phi(u) = 3 (sin u - u cos u)/u^3
+// PAPER.md:37 (Eq. 1 over a sphere).  Even series below the threshold where the direct form cancels.
+__device__ __forceinline__ float sphere_phi(float u) {
+  const float u2 = u * u;
+  float ser = fmaf(u2, 1.0f / 1330560.0f, -1.0f / 15120.0f);
+  ser = fmaf(ser, u2, 1.0f / 280.0f);
+  ser = fmaf(ser, u2, -0.1f);
+  ser = fmaf(ser, u2, 1.0f);
+  float s, c;
+  sincos_r(u, s, c);
+  const float inv = __frcp_rn(u);
+  const float dir = (3.0f * fmaf(-u, c, s)) * ((inv * inv) * inv);
+  return (u < 0.7f) ? ser : dir;
+}
+__device__ __forceinline__ double sphere_phi(double u) {
+  if (u < 0.5) {
+    const double u2 = u * u;
+    double s = 1.0 / 31135104000.0;
+    s = fma(s, u2, -1.0 / 172972800.0);
+    s = fma(s, u2, 1.0 / 1330560.0);
+    s = fma(s, u2, -1.0 / 15120.0);
+    s = fma(s, u2, 1.0 / 280.0);
+    s = fma(s, u2, -0.1);
+    return fma(s, u2, 1.0);
+  }
+  double s, c;
+  sincos(u, &s, &c);
+  return (3.0 * fma(-u, c, s)) / ((u * u) * u);
+}
+
+// ---------------------------------------------------------------- sinc
+__device__ __forceinline__ float sinc_r(float x) {
+  float s, c;
+  sincos_r(x, s, c);
+  return (fabsf(x) < 1e-4f) ? 1.0f : s * __frcp_rn(x);
+}
+__device__ __forceinline__ double sinc_r(double x) { return (x == 0.0) ? 1.0 : sin(x) / x; }
+
+// ---------------------------------------------------------------- Lambda(x) = 2 J1(x)/x, x >= 0
+__device__ __forceinline__ float lambda1_r(float x) {
+  if (x < 4.0f) {
+    const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+    return horner(LA, fmaf(x * x, 0.125f, -1.0f));
+  }
+  if (x < 8.0f) {
+    const float LB[SAS_LAMBDA_B_N] = SAS_LAMBDA_B;
+    return horner(LB, fmaf(x, 0.5f, -3.0f));
+  }
+  // Hankel form: J1 = sqrt(2/(pi x)) (P cos(x - 3pi/4) - Q sin(x - 3pi/4))
+  const float AP[SAS_J1_ASY_P_N] = SAS_J1_ASY_P;
+  const float AQ[SAS_J1_ASY_Q_N] = SAS_J1_ASY_Q;
+  const float inv = __frcp_rn(x);
+  const float t = fmaf(128.0f * inv, inv, -1.0f);
+  const float P = horner(AP, t);
+  const float Q = horner(AQ, t) * inv;
+  float s, c;
+  sincos_r(x, s, c);
+  // cos(x-3pi/4) = (s - c)/sqrt2 ; sin(x-3pi/4) = -(s + c)/sqrt2
+  const float j1 = (0.797884583f * 0.707106769f) * rsqrtf(x) * fmaf(P, s - c, Q * (s + c));
+  return 2.0f * j1 * inv;
+}
+__device__ __forceinline__ double lambda1_r(double x) { return (x == 0.0) ? 1.0 : (2.0 * j1(x)) / x; }
+
+// ---------------------------------------------------------------- the same functions of a Phase
+__device__ __forceinline__ float sphere_phi_ph(Phase<float> p) {
+  const float u = p.hi;
+  const float u2 = u * u;
+  float ser = fmaf(u2, 1.0f / 1330560.0f, -1.0f / 15120.0f);
+  ser = fmaf(ser, u2, 1.0f / 280.0f);
+  ser = fmaf(ser, u2, -0.1f);
+  ser = fmaf(ser, u2, 1.0f);
+  float s, c;
+  sincos_ph(p, s, c);
+  const float inv = __frcp_rn(u);
+  const float dir = (3.0f * fmaf(-u, c, s)) * ((inv * inv) * inv);
+  return (u < 0.7f) ? ser : dir;
+}
+__device__ __forceinline__ double sphere_phi_ph(Phase<double> p) { return sphere_phi(p.v); }
+
+__device__ __forceinline__ float sinc_ph(Phase<float> p) {
+  float s, c;
+  sincos_ph(p, s, c);
+  return (fabsf(p.hi) < 1e-4f) ? 1.0f : s * __frcp_rn(p.hi);
+}
+__device__ __forceinline__ double sinc_ph(Phase<double> p) { return sinc_r(p.v); }
+
+__device__ __forceinline__ float lambda1_ph(Phase<float> p) {
+  const float x = p.hi;
+  if (x < 4.0f) {
+    const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+    return horner(LA, fmaf(x * x, 0.125f, fmaf(x * p.lo, 0.25f, -1.0f)));
+  }
+  if (x < 8.0f) {
+    const float LB[SAS_LAMBDA_B_N] = SAS_LAMBDA_B;
+    return horner(LB, fmaf(x, 0.5f, fmaf(p.lo, 0.5f, -3.0f)));
+  }
+  const float AP[SAS_J1_ASY_P_N] = SAS_J1_ASY_P;
+  const float AQ[SAS_J1_ASY_Q_N] = SAS_J1_ASY_Q;
+  const float inv = __frcp_rn(x);
+  const float t = fmaf(128.0f * inv, inv, -1.0f);
+  const float P = horner(AP, t);
+  const float Q = horner(AQ, t) * inv;
+  float s, c;
+  sincos_ph(p, s, c);
+  const float j1v = (0.797884583f * 0.707106769f) * rsqrtf(x) * fmaf(P, s - c, Q * (s + c));
+  return 2.0f * j1v * inv;
+}
+__device__ __forceinline__ double lambda1_ph(Phase<double> p) { return lambda1_r(p.v); }
+
+// ---------------------------------------------------------------- Percus-Yevick S(q) (Table II F.11)
+struct PYCoef {  // host-computed from the volume fraction (DESIGN.md R-C13)
+  double alpha, beta, gamma, phi24, two_r;
+};
+
+template <typename Real>
+__device__ __forceinline__ Real py_sq(Real q, const PYCoef& pc) {
+  const Real x = (Real)pc.two_r * q;
+  const Real a = (Real)pc.alpha, b = (Real)pc.beta, g = (Real)pc.gamma;
+  const Real thr = sizeof(Real) == 4 ? (Real)2.0 : (Real)1.0;
+  Real t1, t2, t3;
+  if (x < thr) {
+    const Real x2 = x * x;
+    const Real a1[8] = {(Real)(1.0 / 3.0), (Real)(-1.0 / 30.0), (Real)(1.0 / 840.0), (Real)(-1.0 / 45360.0),
+                        (Real)(1.0 / 3991680.0), (Real)(-1.0 / 518918400.0), (Real)(1.0 / 93405312000.0),
+                        (Real)(-1.0 / 22230464256000.0)};
+    const Real a2[8] = {(Real)(1.0 / 4.0), (Real)(-1.0 / 36.0), (Real)(1.0 / 960.0), (Real)(-1.0 / 50400.0),
+                        (Real)(1.0 / 4354560.0), (Real)(-1.0 / 558835200.0), (Real)(1.0 / 99632332800.0),
+                        (Real)(-1.0 / 23538138624000.0)};
+    const Real a3[8] = {(Real)(1.0 / 6.0), (Real)(-1.0 / 48.0), (Real)(1.0 / 1200.0), (Real)(-1.0 / 60480.0),
+                        (Real)(1.0 / 5080320.0), (Real)(-1.0 / 638668800.0), (Real)(1.0 / 112086374400.0),
+                        (Real)(-1.0 / 26153487360000.0)};
+    t1 = a1[7]; t2 = a2[7]; t3 = a3[7];
+#pragma unroll
+    for (int i = 6; i >= 0; --i) {
+      t1 = fma_r(t1, x2, a1[i]);
+      t2 = fma_r(t2, x2, a2[i]);
+      t3 = fma_r(t3, x2, a3[i]);
+    }
+  } else {
+    Real s, c;
+    sincos_r(x, s, c);
+    const Real x2 = x * x, x3 = x2 * x, x4 = x2 * x2;
+    const Real i1 = rcp_r(x);
+    const Real i3 = (i1 * i1) * i1;
+    t1 = fma_r(-x, c, s) * i3;
+    t2 = (fma_r((Real)2.0 * x, s, ((Real)2.0 - x2) * c) - (Real)2.0) * (i3 * i1);
+    const Real in = fma_r(fma_r((Real)3.0, x2, (Real)-6.0), c, fma_r(x3 - (Real)6.0 * x, s, (Real)6.0));
+    t3 = fma_r((Real)4.0, in, -(x4 * c)) * (i3 * i3);
+  }
+  return rcp_r(fma_r((Real)pc.phi24, fma_r(g, t3, fma_r(b, t2, a * t1)), (Real)1.0));
+}
+
+}  // namespace sas

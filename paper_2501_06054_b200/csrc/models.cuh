@@ -1,0 +1,198 @@
+// SAS model intensity I(Q) = 1e8 scale <F^2>/<V> S(q) + background for one detected neutron
+// (PAPER.md:37-49 Eq. 1-4, :76-84 Eq. 6-7, :161-163 Eq. 9; DESIGN.md R-A2, R-A9, R-A11, R-A12, R-C12).
+// Real = float or double.  The quadrature node tables live in shared memory, one broadcast load per
+// node per warp; all Q-independent factors (volumes, contrasts, weights, <V>) were folded into the
+// tables by the host (sas_api.cu: build_tables).
+#pragma once
+#include "sas_types.h"
+
+namespace sas {
+
+template <typename Real>
+struct Tables {  // views into the shared-memory table block
+  const Real* ta;   // [n_a][TA_W]
+  const Real* tb;   // [n_b][TB_W]
+  const Real* tab;  // [n_a*n_b][TAB_W]
+  const Real* tth;  // [n_th][TOR_W]
+  const Real* tph;  // [n_ph][TOR_W]
+};
+
+template <typename Real>
+__device__ __forceinline__ Tables<Real> table_views(const Real* base, const ExpParams& P) {
+  Tables<Real> t;
+  t.ta = base;
+  t.tb = t.ta + P.n_a * TA_W;
+  t.tab = t.tb + P.n_b * TB_W;
+  t.tth = t.tab + P.n_a * P.n_b * TAB_W;
+  t.tph = t.tth + P.n_th * TOR_W;
+  return t;
+}
+
+template <typename Real>
+__device__ __forceinline__ Real sq(Real x) { return x * x; }
+
+// Model table meaning (host: fill_model).  Lengths that multiply a projection of Q are stored as a
+// (hi, lo) pair: in the fp32 path hi = float(L), lo = float(L - hi); in the fp64 path hi = L, lo = 0.
+//  sphere              ta = {R_hi, R_lo, w_a (drho V_a)^2}
+//  core-shell sphere   ta = {Rc_hi, Rc_lo, (drho_c-drho_s) Vc_a, w_a}; tb = {-, w_b};
+//                      tab = {Rt_hi, Rt_lo, drho_s Vt_ab}
+//  cylinder            ta = {R_hi, R_lo, w_a (drho pi R_a^2)^2}; tb = {L_b/2 hi, lo, w_b L_b^2}
+//  triaxial            ta = {x_hi, x_lo, w_a (drho V_a)^2}
+//  core-shell triaxial ta = {x_hi, x_lo, (drho_c-drho_s) Vc_a, w_a}; tb = {t_b, w_b, t_b^2};
+//                      tab = {drho_s Vt_ab, 2 x_a t_b}
+template <typename Real>
+__device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* tab_base, const PhiloxKeys& keys,
+                                               uint32_t id_lo, uint32_t id_hi, uint32_t exp_word, double Qx,
+                                               double Qy, double Qz) {
+  if (P.model == 5) return (Real)P.flat_I;
+  const Tables<Real> T = table_views(tab_base, P);
+  const int model = P.model;
+  // |Q| and the projections of Q on the particle axes (Eq. 6) in fp64: they feed the phases
+  const double q2d = fma(Qx, Qx, fma(Qy, Qy, Qz * Qz));
+  const double qd = sqrt(q2d);
+  double qAd = 0, qBd = 0, qCd = 0;
+  if (model >= 2) {
+    double A[3], B[3], C[3];
+    if (P.orient_kind == 2) {
+      // R-A3: one isotropic random orientation per neutron, draws 8, 9, 10
+      uint32_t w2[4];
+      philox4x32_10(keys, id_lo, id_hi, 2u, exp_word, w2);
+      const double u8 = uniform_from_word(w2[0]), u9 = uniform_from_word(w2[1]), u10 = uniform_from_word(w2[2]);
+      const double ct = 1.0 - 2.0 * u8;
+      const double st = sqrt(1.0 - ct * ct);
+      double sp, cp, ss, cs;
+      if (sizeof(Real) == 8) {
+        sincos(6.283185307179586 * u9, &sp, &cp);
+        sincos(6.283185307179586 * u10, &ss, &cs);
+      } else {
+        sincos_2pi(u9, sp, cp);
+        sincos_2pi(u10, ss, cs);
+      }
+      const double a0[3] = {ct * cp, ct * sp, -st};
+      const double b0[3] = {-sp, cp, 0.0};
+      C[0] = st * cp; C[1] = st * sp; C[2] = ct;
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+        A[i] = fma(cs, a0[i], ss * b0[i]);
+        B[i] = fma(cs, b0[i], -(ss * a0[i]));
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { A[i] = P.frame[i]; B[i] = P.frame[3 + i]; C[i] = P.frame[6 + i]; }
+    }
+    qAd = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
+    qBd = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
+    qCd = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
+  }
+  const Real q = (Real)qd, q2 = (Real)q2d;
+
+  Real acc = 0;
+  switch (model) {
+    case 0: {  // sphere
+      const Proj<Real> qp = make_proj<Real>(qd);
+      for (int a = 0; a < P.n_a; ++a) {
+        const Real* r = T.ta + a * TA_W;
+        const Real ph = sphere_phi_ph(phase_mul(qp, r[0], r[1]));
+        acc = fma_r(r[2], ph * ph, acc);
+      }
+    } break;
+    case 1: {  // core-shell sphere
+      const Proj<Real> qp = make_proj<Real>(qd);
+      for (int a = 0; a < P.n_a; ++a) {
+        const Real* ra = T.ta + a * TA_W;
+        const Real fc = ra[2] * sphere_phi_ph(phase_mul(qp, ra[0], ra[1]));
+        Real inner = 0;
+        for (int b = 0; b < P.n_b; ++b) {
+          const Real* pr = T.tab + (a * P.n_b + b) * TAB_W;
+          const Real F = fma_r(pr[2], sphere_phi_ph(phase_mul(qp, pr[0], pr[1])), fc);
+          inner = fma_r(T.tb[b * TB_W + 1], F * F, inner);
+        }
+        acc = fma_r(ra[3], inner, acc);
+      }
+    } break;
+    case 2: {  // cylinder: separable in (R, L) for a given axis direction
+      if (P.orient_kind == 1) {
+        // Gaussian tilt quadrature (R-A11): n_th x n_ph axis directions about the mean axis, plain Real
+        const Real qA = (Real)qAd, qB = (Real)qBd, qC = (Real)qCd;
+        for (int i = 0; i < P.n_th; ++i) {
+          const Real sth = T.tth[i * TOR_W + 0], cth = T.tth[i * TOR_W + 1], wth = T.tth[i * TOR_W + 2];
+          const Real Ai = fma_r(qA, sth, qC * cth);
+          Real row = 0;
+          for (int j = 0; j < P.n_ph; ++j) {
+            const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
+            const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
+            Real r2 = fma_r(-qc, qc, q2);
+            r2 = r2 > (Real)0 ? r2 : (Real)0;
+            const Real qab = sqrt_r(r2);
+            Real SL = 0, SR = 0;
+            for (int b = 0; b < P.n_b; ++b) {
+              const Real sc = sinc_r(qc * T.tb[b * TB_W + 0]);
+              SL = fma_r(T.tb[b * TB_W + 2], sc * sc, SL);
+            }
+            for (int a = 0; a < P.n_a; ++a) {
+              const Real la = lambda1_r(qab * T.ta[a * TA_W + 0]);
+              SR = fma_r(T.ta[a * TA_W + 2], la * la, SR);
+            }
+            row = fma_r(wph, SL * SR, row);
+          }
+          acc = fma_r(wth, row, acc);
+        }
+      } else {
+        const Proj<Real> qcp = make_proj<Real>(qCd);
+        const Proj<Real> qabp = make_proj<Real>(sqrt(fma(qAd, qAd, qBd * qBd)));
+        Real SL = 0, SR = 0;
+        for (int b = 0; b < P.n_b; ++b) {
+          const Real* r = T.tb + b * TB_W;
+          const Real sc = sinc_ph(phase_mul(qcp, r[0], r[1]));
+          SL = fma_r(r[2], sc * sc, SL);
+        }
+        for (int a = 0; a < P.n_a; ++a) {
+          const Real* r = T.ta + a * TA_W;
+          const Real la = lambda1_ph(phase_mul(qabp, r[0], r[1]));
+          SR = fma_r(r[2], la * la, SR);
+        }
+        acc = SL * SR;
+      }
+    } break;
+    case 3: {  // triaxial ellipsoid: common size scale x_a (R-A12)
+      const double ua = P.msize[0] * qAd, ub = P.msize[1] * qBd, uc = P.msize[2] * qCd;
+      const Proj<Real> U0 = make_proj<Real>(sqrt(fma(ua, ua, fma(ub, ub, uc * uc))));
+      for (int a = 0; a < P.n_a; ++a) {
+        const Real* r = T.ta + a * TA_W;
+        const Real ph = sphere_phi_ph(phase_mul(U0, r[0], r[1]));
+        acc = fma_r(r[2], ph * ph, acc);
+      }
+    } break;
+    case 4: {  // core-shell triaxial ellipsoid
+      const double ma = P.msize[0], mb = P.msize[1], mc = P.msize[2];
+      const double qa2 = qAd * qAd, qb2 = qBd * qBd, qc2 = qCd * qCd;
+      const double U02d = fma(ma * ma, qa2, fma(mb * mb, qb2, (mc * mc) * qc2));
+      const Proj<Real> U0 = make_proj<Real>(sqrt(U02d));
+      const Real U02 = (Real)U02d;
+      const Real Wm = (Real)fma(ma, qa2, fma(mb, qb2, mc * qc2));
+      const Real qq2 = (Real)((qa2 + qb2) + qc2);
+      for (int a = 0; a < P.n_a; ++a) {
+        const Real* ra = T.ta + a * TA_W;
+        const Real fc = ra[2] * sphere_phi_ph(phase_mul(U0, ra[0], ra[1]));
+        const Real xa = ra[0] + ra[1];
+        const Real xa2U = (xa * xa) * U02;
+        Real inner = 0;
+        for (int b = 0; b < P.n_b; ++b) {
+          const Real* pr = T.tab + (a * P.n_b + b) * TAB_W;
+          const Real* rb = T.tb + b * TB_W;
+          // u_t^2 = sum ((x a_k + t) Q_k)^2 = x^2 U0^2 + 2 x t W + t^2 q^2
+          const Real ut2 = fma_r(rb[2], qq2, fma_r(pr[1], Wm, xa2U));
+          const Real F = fma_r(pr[0], sphere_phi(sqrt_r(ut2)), fc);
+          inner = fma_r(rb[1], F * F, inner);
+        }
+        acc = fma_r(ra[3], inner, acc);
+      }
+    } break;
+    default: break;
+  }
+  Real S = 1;
+  if (P.sq_kind == 1) S = py_sq<Real>(q, P.py);
+  return fma_r((Real)P.norm * acc, S, (Real)P.background);
+}
+
+}  // namespace sas

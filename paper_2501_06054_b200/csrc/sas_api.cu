@@ -1,0 +1,630 @@
+// C-ABI shim of libsas_b200.so (include/sas.h): validation, host-side parameter and quadrature-table
+// construction, launch planning, CUDA resource ownership.  All tracing runs in trace_kernel.cuh.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/sas.h"
+#include "quadrature_host.h"
+#include "trace_kernel.cuh"
+
+using namespace sas;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr double TWO_PI = 6.283185307179586;
+constexpr double FOUR_PI_3 = 4.1887902047863905;
+constexpr double PI_D = 3.141592653589793;
+constexpr int MAX_TIMED = 256;
+
+}  // namespace
+
+struct sas_ctx {
+  std::string err;
+  uint32_t n_exp = 0;
+  int nx = 0, ny = 0, npix = 0;
+  int precision = -1;  // set by the model(s)
+  bool model_set = false;
+  bool batch = false;
+  std::vector<sas_instrument_desc> instr;
+  std::vector<ExpParams> h_exps;
+  std::vector<double> h_tab;
+  int tab_len_max = 0;
+  // device
+  int device = 0, n_sm = 0;
+  ExpParams* d_exps = nullptr;
+  double* d_tab = nullptr;
+  size_t d_tab_cap = 0;
+  double *d_sum_p = nullptr, *d_sum_p2 = nullptr;
+  unsigned long long* d_counts = nullptr;
+  bool own_hist = true;
+  unsigned long long* d_counters = nullptr;
+  unsigned int* d_work = nullptr;
+  cudaStream_t stream = nullptr;
+  bool own_stream = true;
+  // bookkeeping
+  uint64_t n_launches = 0;
+  int last_grid = 0, last_block = 0, last_smem = 0;
+  std::vector<cudaEvent_t> ev0, ev1;
+  uint64_t n_timed = 0;
+};
+
+namespace {
+
+sas_status fail(sas_ctx* c, sas_status st, const std::string& msg) {
+  if (c) c->err = msg; else g_create_error = msg;
+  return st;
+}
+
+#define CUDA_TRY(ctx, call)                                                                     \
+  do {                                                                                          \
+    cudaError_t e_ = (call);                                                                    \
+    if (e_ != cudaSuccess)                                                                      \
+      return fail(ctx, SAS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));          \
+  } while (0)
+
+bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+sas_status validate_instrument(const sas_instrument_desc* d, std::string& why) {
+  if (!d) { why = "instrument descriptor is NULL"; return SAS_EINVAL; }
+  if (d->struct_size != sizeof(sas_instrument_desc)) { why = "sas_instrument_desc.struct_size mismatch"; return SAS_EINVAL; }
+  if (d->sample_shape != SAS_SAMPLE_BOX && d->sample_shape != SAS_SAMPLE_CYL_Y) { why = "unknown sample_shape"; return SAS_EINVAL; }
+  if (!finite_pos(d->src_xw) || !finite_pos(d->src_yh)) { why = "source size must be > 0"; return SAS_EINVAL; }
+  if (!finite_pos(d->lambda_min) || !(d->lambda_max >= d->lambda_min) || !std::isfinite(d->lambda_max)) { why = "need 0 < lambda_min <= lambda_max"; return SAS_EINVAL; }
+  if (!std::isfinite(d->flux) || d->flux < 0) { why = "flux must be >= 0"; return SAS_EINVAL; }
+  if (!finite_pos(d->slit1_xw) || !finite_pos(d->slit1_yh) || !finite_pos(d->slit2_xw) || !finite_pos(d->slit2_yh)) { why = "slit apertures must be > 0"; return SAS_EINVAL; }
+  if (!(d->slit1_z >= 0.0) || !(d->slit2_z >= d->slit1_z)) { why = "need 0 <= slit1_z <= slit2_z"; return SAS_EINVAL; }
+  if (!finite_pos(d->focus_z) || !finite_pos(d->focus_xw) || !finite_pos(d->focus_yh)) { why = "focus rectangle must have z, width, height > 0"; return SAS_EINVAL; }
+  if (!(d->sample_z > 0.0) || !finite_pos(d->sample_yh)) { why = "sample_z and sample_yh must be > 0"; return SAS_EINVAL; }
+  if (d->sample_shape == SAS_SAMPLE_BOX && (!finite_pos(d->sample_xw) || !finite_pos(d->sample_zd))) { why = "box sample extents must be > 0"; return SAS_EINVAL; }
+  if (d->sample_shape == SAS_SAMPLE_CYL_Y && !finite_pos(d->sample_radius)) { why = "cylinder sample radius must be > 0"; return SAS_EINVAL; }
+  if (!(d->mu_abs_2200 >= 0.0) || !(d->mu_inc >= 0.0)) { why = "attenuation coefficients must be >= 0"; return SAS_EINVAL; }
+  if (!(d->q_min >= 0.0) || !(d->q_max > d->q_min) || !std::isfinite(d->q_max)) { why = "need 0 <= q_min < q_max"; return SAS_EINVAL; }
+  if (!finite_pos(d->det_dist) || !finite_pos(d->det_xw) || !finite_pos(d->det_yh)) { why = "detector distance and size must be > 0"; return SAS_EINVAL; }
+  if (d->det_nx < 1 || d->det_ny < 1 || d->det_nx > 16384 || d->det_ny > 16384) { why = "detector pixels must be in 1..16384 per axis"; return SAS_EINVAL; }
+  return SAS_OK;
+}
+
+sas_status validate_model(const sas_model_desc* m, std::string& why) {
+  if (!m) { why = "model descriptor is NULL"; return SAS_EINVAL; }
+  if (m->struct_size != sizeof(sas_model_desc)) { why = "sas_model_desc.struct_size mismatch"; return SAS_EINVAL; }
+  if (m->model < SAS_SPHERE || m->model > SAS_FLAT) { why = "unknown model"; return SAS_EINVAL; }
+  if (m->precision != SAS_FP32 && m->precision != SAS_FP64) { why = "unknown precision"; return SAS_EINVAL; }
+  if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_ISOTROPIC_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
+  if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY) { why = "unknown sq_kind"; return SAS_EINVAL; }
+  if (!std::isfinite(m->scale) || !std::isfinite(m->background)) { why = "scale/background not finite"; return SAS_EINVAL; }
+  static const int n_sizes[6] = {1, 2, 2, 3, 4, 0};
+  static const int n_pd[6] = {1, 2, 2, 1, 2, 0};
+  for (int i = 0; i < n_sizes[m->model]; ++i) {
+    // a shell thickness may be 0, every other size must be > 0
+    const bool may_be_zero = (m->model == SAS_CORE_SHELL_SPHERE && i == 1) || (m->model == SAS_CORE_SHELL_TRIAXIAL && i == 3);
+    if (!std::isfinite(m->size[i]) || m->size[i] < 0.0 || (!may_be_zero && m->size[i] == 0.0)) { why = "model sizes must be > 0"; return SAS_EINVAL; }
+  }
+  for (int k = 0; k < 2; ++k) {
+    if (m->pd_kind[k] != SAS_PD_NONE && m->pd_kind[k] != SAS_PD_SCHULZ_QUAD) { why = "unknown pd_kind"; return SAS_EINVAL; }
+    if (m->pd_kind[k] == SAS_PD_SCHULZ_QUAD) {
+      if (k >= n_pd[m->model]) { why = "this model has no such polydisperse length"; return SAS_EINVAL; }
+      if (m->pd_nodes[k] < 1 || m->pd_nodes[k] > SAS_MAX_NODES) { why = "pd_nodes must be in 1..SAS_MAX_NODES"; return SAS_EINVAL; }
+      if (!(m->pd_rel[k] >= 0.0) || !(m->pd_rel[k] < 1.0)) { why = "pd_rel must be in [0,1)"; return SAS_EINVAL; }
+    }
+  }
+  const int na = m->pd_kind[0] == SAS_PD_SCHULZ_QUAD ? m->pd_nodes[0] : 1;
+  const int nb = m->pd_kind[1] == SAS_PD_SCHULZ_QUAD ? m->pd_nodes[1] : 1;
+  if (na * nb > SAS_MAX_PD_PAIRS) { why = "pd_nodes[0]*pd_nodes[1] exceeds SAS_MAX_PD_PAIRS"; return SAS_EINVAL; }
+  if (m->orient_kind == SAS_ORIENT_GAUSS_QUAD) {
+    if (m->n_theta < 1 || m->n_theta > SAS_MAX_NODES || m->n_phi < 1 || m->n_phi > SAS_MAX_NODES) { why = "n_theta/n_phi must be in 1..SAS_MAX_NODES"; return SAS_EINVAL; }
+    if (!(m->sigma_theta >= 0.0) || !(m->sigma_phi >= 0.0)) { why = "orientation spreads must be >= 0"; return SAS_EINVAL; }
+    if (m->model == SAS_TRIAXIAL_ELLIPSOID || m->model == SAS_CORE_SHELL_TRIAXIAL) {
+      why = "SAS_ORIENT_GAUSS_QUAD is defined for uniaxial models only (DESIGN.md R-A11)";
+      return SAS_EUNSUPPORTED;
+    }
+  }
+  if (!std::isfinite(m->theta) || !std::isfinite(m->phi) || !std::isfinite(m->psi)) { why = "orientation angles not finite"; return SAS_EINVAL; }
+  if (m->sq_kind == SAS_SQ_HARD_SPHERE_PY) {
+    if (!finite_pos(m->sq_radius_eff) || !(m->sq_volfrac >= 0.0) || !(m->sq_volfrac < 0.74)) { why = "PY S(q) needs radius_eff > 0 and 0 <= volfrac < 0.74"; return SAS_EINVAL; }
+  }
+  return SAS_OK;
+}
+
+// smallest / largest 32-bit word whose source coordinate passes |(u - 1/2) width| <= half
+void slit1_word_window(double width, double half, uint32_t& lo, uint32_t& hi) {
+  auto coord = [&](uint64_t w) {
+    const double u = ((double)(uint32_t)w + 0.5) * 2.3283064365386963e-10;
+    return (u - 0.5) * width;
+  };
+  auto pass = [&](uint64_t w) { return !(std::fabs(coord(w)) > half); };
+  // coord is non-decreasing in w: the pass set is one interval (possibly empty)
+  uint64_t a = 0, b = 0xFFFFFFFFull;
+  // first w with coord(w) >= -half
+  while (a < b) { uint64_t m = (a + b) / 2; if (coord(m) >= -half) b = m; else a = m + 1; }
+  uint64_t first = a;
+  a = 0; b = 0xFFFFFFFFull;
+  // last w with coord(w) <= half
+  while (a < b) { uint64_t m = (a + b + 1) / 2; if (coord(m) <= half) a = m; else b = m - 1; }
+  uint64_t last = a;
+  if (first <= last && pass(first) && pass(last)) { lo = (uint32_t)first; hi = (uint32_t)last; }
+  else { lo = 1; hi = 0; }
+}
+
+void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
+  P.src_xw = d.src_xw; P.src_yh = d.src_yh;
+  P.focus_xw = d.focus_xw; P.focus_yh = d.focus_yh; P.focus_z = d.focus_z;
+  P.focus_area = d.focus_xw * d.focus_yh;
+  P.p0_pref = d.flux * ((d.src_xw * d.src_yh) * 1.0e4);
+  P.lambda_min = d.lambda_min;
+  P.dlam = d.lambda_max - d.lambda_min;
+  P.dlam_w = P.dlam > 0.0 ? P.dlam : 1.0;
+  P.slit1_z = d.slit1_z; P.slit1_hx = 0.5 * d.slit1_xw; P.slit1_hy = 0.5 * d.slit1_yh;
+  P.slit2_z = d.slit2_z; P.slit2_hx = 0.5 * d.slit2_xw; P.slit2_hy = 0.5 * d.slit2_yh;
+  P.sample_shape = d.sample_shape;
+  P.sample_z = d.sample_z;
+  P.hx = 0.5 * d.sample_xw; P.hy = 0.5 * d.sample_yh; P.hz = 0.5 * d.sample_zd;
+  P.radius2 = d.sample_radius * d.sample_radius;
+  P.mu_abs_2200 = d.mu_abs_2200; P.mu_inc = d.mu_inc;
+  P.has_mu = (d.mu_abs_2200 != 0.0 || d.mu_inc != 0.0) ? 1 : 0;
+  P.q_min = d.q_min; P.dq = d.q_max - d.q_min;
+  P.qnorm = TWO_PI * (d.q_max - d.q_min);
+  P.det_z = d.sample_z + d.det_dist;
+  P.det_hw = 0.5 * d.det_xw; P.det_hh = 0.5 * d.det_yh;
+  P.det_sx = (double)d.det_nx / d.det_xw; P.det_sy = (double)d.det_ny / d.det_yh;
+  P.det_nxd = (double)d.det_nx; P.det_nyd = (double)d.det_ny;
+  P.det_nx = d.det_nx; P.det_ny = d.det_ny;
+  P.s1_int_ok = 0;
+  if (d.slit1_z == 0.0) {
+    // slit 1 in the source plane: xs = x0 + dx*0 = x0 exactly, so the test depends on draws 0, 1 only
+    slit1_word_window(d.src_xw, P.slit1_hx, P.s1_lo[0], P.s1_hi[0]);
+    slit1_word_window(d.src_yh, P.slit1_hy, P.s1_lo[1], P.s1_hi[1]);
+    P.s1_int_ok = 1;
+  }
+}
+
+// Folds every Q-independent factor of the model into the node tables (models.cuh lists the layout).
+void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool) {
+  P.model = m.model; P.orient_kind = m.orient_kind; P.sq_kind = m.sq_kind;
+  P.background = m.background;
+  P.flat_I = m.scale + m.background;
+  std::vector<double> xa, wa, xb, wb, dth, wth, dph, wph;
+  schulz_rule(m.pd_kind[0] == SAS_PD_SCHULZ_QUAD ? m.pd_rel[0] : 0.0, m.pd_nodes[0], xa, wa);
+  schulz_rule(m.pd_kind[1] == SAS_PD_SCHULZ_QUAD ? m.pd_rel[1] : 0.0, m.pd_nodes[1], xb, wb);
+  if (m.orient_kind == SAS_ORIENT_GAUSS_QUAD) {
+    gauss_tilt_rule(m.sigma_theta, m.n_theta, dth, wth);
+    gauss_tilt_rule(m.sigma_phi, m.n_phi, dph, wph);
+  } else {
+    dth.assign(1, 0.0); wth.assign(1, 1.0); dph.assign(1, 0.0); wph.assign(1, 1.0);
+  }
+  const int na = (int)xa.size(), nb = (int)xb.size();
+  P.n_a = na; P.n_b = nb; P.n_th = (int)dth.size(); P.n_ph = (int)dph.size();
+  std::vector<double> ta(na * TA_W, 0.0), tb(nb * TB_W, 0.0), tab(na * nb * TAB_W, 0.0);
+  double SV = 0.0;  // <V>
+  const double s0 = m.sld[0], s1 = m.sld[1];
+  for (int k = 0; k < 4; ++k) P.msize[k] = m.size[k];
+  for (int a = 0; a < na; ++a)
+    for (int b = 0; b < nb; ++b) {
+      const double w = wa[a] * wb[b];
+      double V = 1.0;
+      switch (m.model) {
+        case SAS_SPHERE: { const double R = m.size[0] * xa[a]; V = FOUR_PI_3 * R * R * R; } break;
+        case SAS_CORE_SHELL_SPHERE: { const double Rt = m.size[0] * xa[a] + m.size[1] * xb[b]; V = FOUR_PI_3 * Rt * Rt * Rt; } break;
+        case SAS_CYLINDER: { const double R = m.size[0] * xa[a], L = m.size[1] * xb[b]; V = PI_D * R * R * L; } break;
+        case SAS_TRIAXIAL_ELLIPSOID: V = FOUR_PI_3 * (m.size[0] * xa[a]) * (m.size[1] * xa[a]) * (m.size[2] * xa[a]); break;
+        case SAS_CORE_SHELL_TRIAXIAL: {
+          const double t = m.size[3] * xb[b];
+          V = FOUR_PI_3 * (m.size[0] * xa[a] + t) * (m.size[1] * xa[a] + t) * (m.size[2] * xa[a] + t);
+        } break;
+        default: break;
+      }
+      SV += w * V;
+    }
+  // a length that multiplies a projection of Q: (hi, lo) split for the fp32 path (device_math.cuh)
+  const bool f32 = m.precision == SAS_FP32;
+  auto split = [&](double L, double* dst) {
+    if (f32) { const float h = (float)L; dst[0] = (double)h; dst[1] = L - (double)h; }
+    else { dst[0] = L; dst[1] = 0.0; }
+  };
+  for (int a = 0; a < na; ++a) {
+    double* r = &ta[a * TA_W];
+    switch (m.model) {
+      case SAS_SPHERE: { const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R; split(R, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
+      case SAS_CORE_SHELL_SPHERE: { const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R; split(R, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
+      case SAS_CYLINDER: { const double R = m.size[0] * xa[a], c = s0 * PI_D * R * R; split(R, r); r[2] = wa[a] * c * c; } break;
+      case SAS_TRIAXIAL_ELLIPSOID: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
+      case SAS_CORE_SHELL_TRIAXIAL: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
+      default: break;
+    }
+  }
+  for (int b = 0; b < nb; ++b) {
+    double* r = &tb[b * TB_W];
+    switch (m.model) {
+      case SAS_CYLINDER: { const double L = m.size[1] * xb[b]; split(0.5 * L, r); r[2] = wb[b] * L * L; } break;
+      case SAS_CORE_SHELL_TRIAXIAL: { const double t = m.size[3] * xb[b]; r[0] = t; r[1] = wb[b]; r[2] = t * t; } break;
+      default: r[1] = wb[b]; break;
+    }
+  }
+  for (int a = 0; a < na; ++a)
+    for (int b = 0; b < nb; ++b) {
+      double* r = &tab[(a * nb + b) * TAB_W];
+      if (m.model == SAS_CORE_SHELL_SPHERE) {
+        const double Rt = m.size[0] * xa[a] + m.size[1] * xb[b];
+        split(Rt, r); r[2] = s1 * (FOUR_PI_3 * Rt * Rt * Rt);
+      } else if (m.model == SAS_CORE_SHELL_TRIAXIAL) {
+        const double x = xa[a], t = m.size[3] * xb[b];
+        r[0] = s1 * (FOUR_PI_3 * (m.size[0] * x + t) * (m.size[1] * x + t) * (m.size[2] * x + t));
+        r[1] = 2.0 * x * t;
+      }
+    }
+  P.norm = (1.0e8 * m.scale) / SV;
+  // mean particle frame (R-A7)
+  {
+    const double st = std::sin(m.theta), ct = std::cos(m.theta), sp = std::sin(m.phi), cp = std::cos(m.phi);
+    const double ss = std::sin(m.psi), cs = std::cos(m.psi);
+    const double a0[3] = {ct * cp, ct * sp, -st}, b0[3] = {-sp, cp, 0.0};
+    const double c0[3] = {st * cp, st * sp, ct};
+    for (int i = 0; i < 3; ++i) {
+      P.frame[i] = cs * a0[i] + ss * b0[i];
+      P.frame[3 + i] = cs * b0[i] - ss * a0[i];
+      P.frame[6 + i] = c0[i];
+    }
+  }
+  // Percus-Yevick coefficients (R-C13)
+  {
+    const double phi = m.sq_volfrac, om = 1.0 - phi, om4 = (om * om) * (om * om);
+    P.py.alpha = ((1.0 + 2.0 * phi) * (1.0 + 2.0 * phi)) / om4;
+    P.py.beta = (-6.0 * phi) * ((1.0 + 0.5 * phi) * (1.0 + 0.5 * phi)) / om4;
+    P.py.gamma = (phi * P.py.alpha) * 0.5;
+    P.py.phi24 = 24.0 * phi;
+    P.py.two_r = 2.0 * m.sq_radius_eff;
+  }
+  P.tab_off = (int)pool.size();
+  pool.insert(pool.end(), ta.begin(), ta.end());
+  pool.insert(pool.end(), tb.begin(), tb.end());
+  pool.insert(pool.end(), tab.begin(), tab.end());
+  for (size_t i = 0; i < dth.size(); ++i) { pool.push_back(std::sin(dth[i])); pool.push_back(std::cos(dth[i])); pool.push_back(wth[i]); }
+  for (size_t i = 0; i < dph.size(); ++i) { pool.push_back(std::sin(dph[i])); pool.push_back(std::cos(dph[i])); pool.push_back(wph[i]); }
+  P.tab_len = (int)pool.size() - P.tab_off;
+}
+
+}  // namespace
+
+// ===================================================================== context plumbing
+namespace {
+
+sas_status alloc_common(sas_ctx* c) {
+  CUDA_TRY(c, cudaGetDevice(&c->device));
+  CUDA_TRY(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device));
+  CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
+  c->own_stream = true;
+  const size_t nh = (size_t)c->n_exp * c->npix;
+  CUDA_TRY(c, cudaMalloc(&c->d_sum_p, nh * sizeof(double)));
+  CUDA_TRY(c, cudaMalloc(&c->d_sum_p2, nh * sizeof(double)));
+  CUDA_TRY(c, cudaMalloc(&c->d_counts, nh * sizeof(unsigned long long)));
+  c->own_hist = true;
+  CUDA_TRY(c, cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)));
+  CUDA_TRY(c, cudaMalloc(&c->d_work, sizeof(unsigned int)));
+  CUDA_TRY(c, cudaMalloc(&c->d_exps, (size_t)c->n_exp * sizeof(ExpParams)));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counts, 0, nh * sizeof(unsigned long long), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  return SAS_OK;
+}
+
+// how many amplitude evaluations one detected neutron costs
+int node_evaluations(const sas_model_desc& m) {
+  if (m.model == SAS_FLAT) return 1;
+  auto pd = [&](int k) { return (m.pd_kind[k] == SAS_PD_SCHULZ_QUAD && m.pd_rel[k] > 0.0 && m.pd_nodes[k] > 1) ? m.pd_nodes[k] : 1; };
+  int n = pd(0) * pd(1);
+  if (m.orient_kind == SAS_ORIENT_GAUSS_QUAD && m.model == SAS_CYLINDER) {
+    n *= (m.sigma_theta > 0.0 && m.n_theta > 1) ? m.n_theta : 1;
+    n *= (m.sigma_phi > 0.0 && m.n_phi > 1) ? m.n_phi : 1;
+  }
+  return n;
+}
+
+// (re)build ExpParams + tables of every experiment and upload them
+sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
+  c->h_tab.clear();
+  c->tab_len_max = 0;
+  // A model without any node loop is evaluated once per detected neutron; that single evaluation is
+  // done in fp64 whatever precision was asked for: it costs little next to the fp64 geometry before
+  // it, and a monodisperse form factor near its zeros cannot meet 1e-5 in fp32.
+  bool any_loop = false;
+  for (uint32_t e = 0; e < c->n_exp; ++e) any_loop = any_loop || node_evaluations(models[e]) > 1;
+  c->precision = (models[0].precision == SAS_FP64 || !any_loop) ? SAS_FP64 : SAS_FP32;
+  for (uint32_t e = 0; e < c->n_exp; ++e) {
+    ExpParams& P = c->h_exps[e];
+    fill_instrument(c->instr[e], P);
+    sas_model_desc m = models[e];
+    m.precision = c->precision;
+    fill_model(m, P, c->h_tab);
+    c->tab_len_max = std::max(c->tab_len_max, P.tab_len);
+  }
+  const size_t tb = c->h_tab.size() * sizeof(double);
+  if (tb > c->d_tab_cap) {
+    if (c->d_tab) { CUDA_TRY(c, cudaStreamSynchronize(c->stream)); CUDA_TRY(c, cudaFree(c->d_tab)); c->d_tab = nullptr; }
+    CUDA_TRY(c, cudaMalloc(&c->d_tab, tb));
+    c->d_tab_cap = tb;
+  }
+  // the host vectors stay alive in the context, so asynchronous copies from them are safe to order on
+  // the stream; a later set_model first synchronises (below) before overwriting them
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_tab, c->h_tab.data(), tb, cudaMemcpyHostToDevice, c->stream));
+  CUDA_TRY(c, cudaMemcpyAsync(c->d_exps, c->h_exps.data(), (size_t)c->n_exp * sizeof(ExpParams),
+                              cudaMemcpyHostToDevice, c->stream));
+  c->model_set = true;
+  return SAS_OK;
+}
+
+template <typename Real, bool DUMP>
+sas_status launch(sas_ctx* c, KernelArgs& a) {
+  const size_t smem = trace_smem_bytes<Real>(c->tab_len_max);
+  auto kern = trace_kernel<Real, DUMP>;
+  if (smem > 227 * 1024) return fail(c, SAS_EINVAL, "quadrature tables do not fit in shared memory");
+  CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int bps = 0;
+  CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, BLOCK_THREADS, smem));
+  if (bps < 1) return fail(c, SAS_ECUDA, "trace kernel does not fit on an SM");
+  const uint64_t total = (uint64_t)a.n_per_exp * a.n_exp;
+  const int grid_full = c->n_sm * bps;
+  // work items: ~16 per resident block, 2048..262144 ids each, multiple of 256 ids
+  uint64_t item = total / ((uint64_t)grid_full * 16ull);
+  item = std::min<uint64_t>(std::max<uint64_t>(item, 2048), 262144);
+  item = (item + 255) / 256 * 256;
+  a.item_ids = (uint32_t)item;
+  a.items_per_exp = (uint32_t)(((uint64_t)a.n_per_exp + item - 1) / item);
+  const uint64_t n_items = (uint64_t)a.items_per_exp * a.n_exp;
+  if (n_items >= 0xFFFFFFFFull) return fail(c, SAS_EINVAL, "too many work items in one launch");
+  a.n_items = (uint32_t)n_items;
+  a.tab_len_max = c->tab_len_max;
+  const int grid = (int)std::min<uint64_t>((uint64_t)grid_full, n_items);
+  CUDA_TRY(c, cudaMemsetAsync(c->d_work, 0, sizeof(unsigned int), c->stream));
+  const bool timed = !DUMP && c->n_timed < (uint64_t)MAX_TIMED;
+  if (timed) {
+    if (c->ev0.size() <= c->n_timed) {
+      cudaEvent_t e0, e1;
+      CUDA_TRY(c, cudaEventCreate(&e0));
+      CUDA_TRY(c, cudaEventCreate(&e1));
+      c->ev0.push_back(e0);
+      c->ev1.push_back(e1);
+    }
+    CUDA_TRY(c, cudaEventRecord(c->ev0[c->n_timed], c->stream));
+  }
+  kern<<<grid, BLOCK_THREADS, smem, c->stream>>>(a);
+  CUDA_TRY(c, cudaGetLastError());
+  if (timed) {
+    CUDA_TRY(c, cudaEventRecord(c->ev1[c->n_timed], c->stream));
+    c->n_timed += 1;
+  }
+  c->n_launches += 1;
+  c->last_grid = grid; c->last_block = BLOCK_THREADS; c->last_smem = (int)smem;
+  return SAS_OK;
+}
+
+sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t seed) {
+  if (!c) return SAS_EINVAL;
+  if (!c->model_set) return fail(c, SAS_ESTATE, "sas_set_model must precede tracing");
+  if (n_each == 0) return SAS_OK;
+  if (first_id + n_each < first_id) return fail(c, SAS_EINVAL, "neutron id range overflows 64 bits");
+  KernelArgs a;
+  std::memset(&a, 0, sizeof(a));
+  a.exps = c->d_exps; a.tab_pool = c->d_tab;
+  a.sum_p = c->d_sum_p; a.sum_p2 = c->d_sum_p2; a.counts = c->d_counts;
+  a.counters = c->d_counters; a.work_counter = c->d_work;
+  a.n_exp = c->n_exp; a.exp_base = 0; a.npix = c->npix;
+  philox_make_keys(seed, a.keys);
+  // one launch covers at most 2^31 ids per experiment (32-bit id offsets inside the kernel)
+  const uint64_t chunk = 1ull << 31;
+  for (uint64_t done = 0; done < n_each; done += chunk) {
+    a.first_id = first_id + done;
+    a.n_per_exp = (uint32_t)std::min<uint64_t>(chunk, n_each - done);
+    sas_status st = c->precision == SAS_FP64 ? launch<double, false>(c, a) : launch<float, false>(c, a);
+    if (st != SAS_OK) return st;
+  }
+  return SAS_OK;
+}
+
+void destroy_ctx(sas_ctx* c) {
+  if (!c) return;
+  if (c->stream) cudaStreamSynchronize(c->stream);
+  for (auto e : c->ev0) cudaEventDestroy(e);
+  for (auto e : c->ev1) cudaEventDestroy(e);
+  if (c->own_hist) { cudaFree(c->d_sum_p); cudaFree(c->d_sum_p2); cudaFree(c->d_counts); }
+  cudaFree(c->d_counters); cudaFree(c->d_work); cudaFree(c->d_exps); cudaFree(c->d_tab);
+  if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+  delete c;
+}
+
+}  // namespace
+
+// ===================================================================== the ABI
+extern "C" {
+
+const char* sas_version(void) { return "sas_b200 0.1 (sm_100a)"; }
+
+const char* sas_last_error(const sas_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+sas_status sas_quadrature_nodes(int32_t kind, double param, int32_t n, double* h_values, double* h_weights) {
+  if (!h_values || !h_weights || n < 1 || n > SAS_MAX_NODES || !(param >= 0.0)) return fail(nullptr, SAS_EINVAL, "bad sas_quadrature_nodes argument");
+  std::vector<double> x, w;
+  if (kind == 0) {
+    if (!(param < 1.0)) return fail(nullptr, SAS_EINVAL, "Schulz relative width must be < 1");
+    schulz_rule(param, n, x, w);
+  } else if (kind == 1) {
+    gauss_tilt_rule(param, n, x, w);
+  } else {
+    return fail(nullptr, SAS_EINVAL, "unknown quadrature kind");
+  }
+  // degenerate rules collapse to one node; pad so that the caller always gets n entries
+  for (int i = 0; i < n; ++i) {
+    h_values[i] = i < (int)x.size() ? x[i] : x[0];
+    h_weights[i] = i < (int)w.size() ? w[i] : 0.0;
+  }
+  return SAS_OK;
+}
+
+sas_status sas_create_instrument(const sas_instrument_desc* instr, sas_ctx** out) {
+  if (!out) return fail(nullptr, SAS_EINVAL, "out is NULL");
+  std::string why;
+  sas_status st = validate_instrument(instr, why);
+  if (st != SAS_OK) return fail(nullptr, st, why);
+  sas_ctx* c = new (std::nothrow) sas_ctx();
+  if (!c) return fail(nullptr, SAS_ENOMEM, "out of host memory");
+  c->n_exp = 1; c->batch = false;
+  c->nx = instr->det_nx; c->ny = instr->det_ny; c->npix = c->nx * c->ny;
+  c->instr.assign(1, *instr);
+  c->h_exps.assign(1, ExpParams());
+  std::memset(c->h_exps.data(), 0, sizeof(ExpParams));
+  st = alloc_common(c);
+  if (st != SAS_OK) { g_create_error = c->err; destroy_ctx(c); return st; }
+  *out = c;
+  return SAS_OK;
+}
+
+sas_status sas_create_batch(const sas_instrument_desc* instr, const sas_model_desc* model, uint32_t n_exp, sas_ctx** out) {
+  if (!out || !instr || !model || n_exp == 0) return fail(nullptr, SAS_EINVAL, "bad sas_create_batch argument");
+  std::string why;
+  for (uint32_t e = 0; e < n_exp; ++e) {
+    sas_status st = validate_instrument(instr + e, why);
+    if (st == SAS_OK) st = validate_model(model + e, why);
+    if (st == SAS_OK && (instr[e].det_nx != instr[0].det_nx || instr[e].det_ny != instr[0].det_ny)) { st = SAS_EINVAL; why = "all experiments of a batch need the same det_nx, det_ny"; }
+    if (st == SAS_OK && model[e].precision != model[0].precision) { st = SAS_EINVAL; why = "all experiments of a batch need the same precision"; }
+    if (st != SAS_OK) return fail(nullptr, st, "experiment " + std::to_string(e) + ": " + why);
+  }
+  sas_ctx* c = new (std::nothrow) sas_ctx();
+  if (!c) return fail(nullptr, SAS_ENOMEM, "out of host memory");
+  c->n_exp = n_exp; c->batch = true;
+  c->nx = instr[0].det_nx; c->ny = instr[0].det_ny; c->npix = c->nx * c->ny;
+  c->instr.assign(instr, instr + n_exp);
+  c->h_exps.assign(n_exp, ExpParams());
+  std::memset(c->h_exps.data(), 0, sizeof(ExpParams) * n_exp);
+  sas_status st = alloc_common(c);
+  if (st == SAS_OK) st = upload_models(c, model);
+  if (st != SAS_OK) { g_create_error = c->err; destroy_ctx(c); return st; }
+  *out = c;
+  return SAS_OK;
+}
+
+sas_status sas_bind_buffers(sas_ctx* c, void* d_sum_p, void* d_sum_p2, void* d_counts, void* cuda_stream) {
+  if (!c) return SAS_EINVAL;
+  if (!d_sum_p || !d_sum_p2 || !d_counts) return fail(c, SAS_EINVAL, "histogram pointers must not be NULL");
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  if (c->own_hist) { cudaFree(c->d_sum_p); cudaFree(c->d_sum_p2); cudaFree(c->d_counts); }
+  c->d_sum_p = (double*)d_sum_p; c->d_sum_p2 = (double*)d_sum_p2; c->d_counts = (unsigned long long*)d_counts;
+  c->own_hist = false;
+  if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+  c->stream = (cudaStream_t)cuda_stream;
+  c->own_stream = false;
+  // re-issue the uploads on the new stream so that ordering holds there
+  if (c->model_set) {
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_tab, c->h_tab.data(), c->h_tab.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_exps, c->h_exps.data(), (size_t)c->n_exp * sizeof(ExpParams), cudaMemcpyHostToDevice, c->stream));
+  }
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  return SAS_OK;
+}
+
+sas_status sas_set_model(sas_ctx* c, const sas_model_desc* model) {
+  if (!c) return SAS_EINVAL;
+  if (c->batch) return fail(c, SAS_ESTATE, "batched contexts take their models at sas_create_batch");
+  std::string why;
+  sas_status st = validate_model(model, why);
+  if (st != SAS_OK) return fail(c, st, why);
+  // pending asynchronous uploads read the host vectors we are about to rewrite
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return upload_models(c, model);
+}
+
+sas_status sas_trace(sas_ctx* c, uint64_t n_neutrons, uint64_t seed) {
+  if (c && c->batch) return fail(c, SAS_ESTATE, "use sas_trace_batch on a batched context");
+  return trace_common(c, 0, n_neutrons, seed);
+}
+
+sas_status sas_trace_range(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t seed) {
+  if (c && c->batch) return fail(c, SAS_ESTATE, "use sas_trace_batch on a batched context");
+  return trace_common(c, first_id, n, seed);
+}
+
+sas_status sas_trace_batch(sas_ctx* c, uint64_t n_neutrons_each, uint64_t seed) {
+  if (c && !c->batch) return fail(c, SAS_ESTATE, "sas_trace_batch needs a context from sas_create_batch");
+  return trace_common(c, 0, n_neutrons_each, seed);
+}
+
+sas_status sas_trace_dump(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t seed, uint32_t exp_index,
+                          int32_t* d_pixel, double* d_weight, double* d_q) {
+  if (!c) return SAS_EINVAL;
+  if (c->batch) return fail(c, SAS_ESTATE, "sas_trace_dump works on single-experiment contexts");
+  if (!c->model_set) return fail(c, SAS_ESTATE, "sas_set_model must precede tracing");
+  if (!d_pixel || !d_weight) return fail(c, SAS_EINVAL, "d_pixel and d_weight must not be NULL");
+  if (n == 0) return SAS_OK;
+  if (n > (1ull << 31)) return fail(c, SAS_EINVAL, "sas_trace_dump handles at most 2^31 ids per call");
+  KernelArgs a;
+  std::memset(&a, 0, sizeof(a));
+  a.exps = c->d_exps; a.tab_pool = c->d_tab;
+  a.counters = c->d_counters; a.work_counter = c->d_work;
+  a.d_pixel = d_pixel; a.d_weight = d_weight; a.d_q = d_q;
+  a.n_exp = 1; a.exp_base = exp_index; a.npix = c->npix;
+  a.first_id = first_id; a.n_per_exp = (uint32_t)n;
+  philox_make_keys(seed, a.keys);
+  CUDA_TRY(c, cudaMemsetAsync(d_pixel, 0xFF, n * sizeof(int32_t), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(d_weight, 0, n * sizeof(double), c->stream));
+  if (d_q) CUDA_TRY(c, cudaMemsetAsync(d_q, 0, n * sizeof(double), c->stream));
+  return c->precision == SAS_FP64 ? launch<double, true>(c, a) : launch<float, true>(c, a);
+}
+
+sas_status sas_read_detector(sas_ctx* c, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts) {
+  if (!c) return SAS_EINVAL;
+  const size_t nh = (size_t)c->n_exp * c->npix;
+  if (h_sum_p) CUDA_TRY(c, cudaMemcpyAsync(h_sum_p, c->d_sum_p, nh * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  if (h_sum_p2) CUDA_TRY(c, cudaMemcpyAsync(h_sum_p2, c->d_sum_p2, nh * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  if (h_counts) CUDA_TRY(c, cudaMemcpyAsync(h_counts, c->d_counts, nh * sizeof(uint64_t), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return SAS_OK;
+}
+
+sas_status sas_get_counters(sas_ctx* c, uint64_t out[8]) {
+  if (!c || !out) return SAS_EINVAL;
+  CUDA_TRY(c, cudaMemcpyAsync(out, c->d_counters, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  return SAS_OK;
+}
+
+sas_status sas_reset_detector(sas_ctx* c) {
+  if (!c) return SAS_EINVAL;
+  const size_t nh = (size_t)c->n_exp * c->npix;
+  CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counts, 0, nh * sizeof(unsigned long long), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  return SAS_OK;
+}
+
+sas_status sas_get_launch_info(sas_ctx* c, uint64_t* n_launches, int32_t* grid, int32_t* block, int32_t* smem_bytes) {
+  if (!c) return SAS_EINVAL;
+  if (n_launches) *n_launches = c->n_launches;
+  if (grid) *grid = c->last_grid;
+  if (block) *block = c->last_block;
+  if (smem_bytes) *smem_bytes = c->last_smem;
+  return SAS_OK;
+}
+
+sas_status sas_get_kernel_time(sas_ctx* c, int32_t reset, double* avg_ms, uint64_t* n_timed) {
+  if (!c) return SAS_EINVAL;
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  double sum = 0.0;
+  for (uint64_t i = 0; i < c->n_timed; ++i) {
+    float ms = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0[i], c->ev1[i]));
+    sum += ms;
+  }
+  if (avg_ms) *avg_ms = c->n_timed ? sum / (double)c->n_timed : 0.0;
+  if (n_timed) *n_timed = c->n_timed;
+  if (reset) c->n_timed = 0;
+  return SAS_OK;
+}
+
+void sas_destroy(sas_ctx* c) { destroy_ctx(c); }
+
+}  // extern "C"

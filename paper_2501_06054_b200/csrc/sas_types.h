@@ -1,0 +1,75 @@
+// Internal device-side parameter blocks of the CUDA tracer (not part of the ABI; not shared with oracle/).
+#pragma once
+#include <cstdint>
+
+#include "device_math.cuh"
+
+namespace sas {
+
+enum : int { ST_DETECTED = 0, ST_SLIT1 = 1, ST_SLIT2 = 2, ST_MISS_SAMPLE = 3, ST_UNREACHABLE = 4, ST_MISS_DET = 5 };
+
+// table record widths (in Reals)
+constexpr int TA_W = 4;   // per node of polydisperse axis 0
+constexpr int TB_W = 4;   // per node of polydisperse axis 1
+constexpr int TAB_W = 4;  // per (a,b) pair
+constexpr int TOR_W = 3;  // per orientation tilt node: sin(delta), cos(delta), weight
+
+// One virtual experiment: everything the kernel needs, precomputed on the host in fp64 with exactly the
+// operations DESIGN.md section 3 writes (so that e.g. 0.5*det_xw is the same double on both sides).
+struct ExpParams {
+  // source and aiming (R-C2, R-C3)
+  double src_xw, src_yh, focus_xw, focus_yh, focus_z, focus_area, p0_pref, dlam_w;
+  double lambda_min, dlam;
+  // slits (R-C4): half apertures
+  double slit1_z, slit1_hx, slit1_hy, slit2_z, slit2_hx, slit2_hy;
+  // sample (R-C5)
+  double sample_z, hx, hy, hz, radius2;
+  double mu_abs_2200, mu_inc;
+  // Q choice (R-C7) and weight (R-C11)
+  double q_min, dq, qnorm;
+  // detector (R-C9)
+  double det_z, det_hw, det_hh, det_sx, det_sy, det_nxd, det_nyd;
+  // model scalars (R-C12)
+  double norm;        // 1e8 * scale / <V>
+  double background;
+  double flat_I;      // SAS_FLAT: scale + background
+  double frame[9];    // particle axes A, B, C in the global frame for fixed / mean orientation (R-A7)
+  double msize[4];    // mean sizes (triaxial a, b, c)
+  PYCoef py;
+  // slit-1 integer prefilter: when slit 1 lies in the source plane the test |x0| <= hx is a monotone
+  // function of the Philox word, so it is decided on the raw 32-bit draws (bit-identical to the fp64 test)
+  uint32_t s1_lo[2], s1_hi[2];
+  int32_t s1_int_ok;
+  int32_t sample_shape, has_mu, det_nx, det_ny;
+  int32_t model, orient_kind, sq_kind;
+  int32_t n_a, n_b, n_th, n_ph;
+  int32_t tab_off, tab_len;  // in doubles, inside the table pool
+  int32_t pad_[1];
+};
+static_assert(sizeof(ExpParams) % 8 == 0, "ExpParams must be a multiple of 8 bytes");
+
+struct KernelArgs {
+  const ExpParams* exps;
+  const double* tab_pool;
+  double* sum_p;
+  double* sum_p2;
+  unsigned long long* counts;
+  unsigned long long* counters;  // [8]
+  unsigned int* work_counter;
+  // dump mode
+  int32_t* d_pixel;
+  double* d_weight;
+  double* d_q;
+  uint64_t first_id;       // id of offset 0
+  uint32_t n_per_exp;      // ids per experiment in this launch (< 2^32)
+  uint32_t n_exp;
+  uint32_t exp_base;       // Philox counter word 3 of experiment 0
+  uint32_t item_ids;       // ids per work item (multiple of 32)
+  uint32_t items_per_exp;
+  uint32_t n_items;
+  int32_t npix;
+  int32_t tab_len_max;     // Reals of table space in shared memory
+  PhiloxKeys keys;
+};
+
+}  // namespace sas

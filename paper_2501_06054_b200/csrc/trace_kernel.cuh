@@ -1,0 +1,209 @@
+// The trace kernel: persistent blocks pull work items (experiment, id range) from a global counter;
+// inside a block every warp is autonomous and runs a three-stage pipeline with warp-private ring
+// queues in shared memory so that each stage executes with full warps although ~75 % of the neutrons
+// die at slit 1 and ~80 % of the rest miss the detector:
+//
+//   stage A  Philox block 0 + slit-1 test on the raw 32-bit draws      (every launched neutron)
+//   stage B  fp64 geometry: slits, sample chord, Q, detector pixel     (slit-1 survivors)
+//   stage C  model intensity I(Q) with the quadrature node loops,      (detected neutrons)
+//            weight, histogram update
+#pragma once
+#include "geometry.cuh"
+#include "models.cuh"
+
+namespace sas {
+
+constexpr int BLOCK_THREADS = 256;
+constexpr int WARPS_PER_BLOCK = BLOCK_THREADS / 32;
+constexpr int RING = 64;  // entries per warp queue (power of two, >= 63)
+
+struct WarpQueues {
+  // queue B: slit-1 survivors
+  uint32_t b_id[RING];
+  uint32_t b_w[4][RING];
+  // queue C: detected neutrons
+  uint32_t c_id[RING];
+  int32_t c_pixel[RING];
+  double c_G[RING];
+  double c_Q[3][RING];
+};
+
+__host__ __device__ inline size_t round16(size_t x) { return (x + 15) & ~(size_t)15; }
+
+template <typename Real>
+__host__ __device__ inline size_t trace_smem_bytes(int tab_len_max) {
+  return round16(sizeof(ExpParams)) + round16((size_t)tab_len_max * sizeof(Real)) +
+         (size_t)WARPS_PER_BLOCK * sizeof(WarpQueues);
+}
+
+template <typename Real, bool DUMP>
+__global__ void __launch_bounds__(BLOCK_THREADS) trace_kernel(const __grid_constant__ KernelArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ unsigned int s_item;
+
+  ExpParams& P = *reinterpret_cast<ExpParams*>(smem_raw);
+  Real* tab = reinterpret_cast<Real*>(smem_raw + round16(sizeof(ExpParams)));
+  WarpQueues& wq = reinterpret_cast<WarpQueues*>(smem_raw + round16(sizeof(ExpParams)) +
+                                                 round16((size_t)a.tab_len_max * sizeof(Real)))[threadIdx.x >> 5];
+  const int lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const unsigned FULL = 0xFFFFFFFFu;
+
+  // warp-uniform pipeline state
+  int headB = 0, cntB = 0, headC = 0, cntC = 0;
+  unsigned n_s1 = 0, n_s2 = 0, n_ms = 0, n_un = 0, n_md = 0, n_det = 0;
+  unsigned long long n_launched = 0;
+
+  int cur_exp = -1;
+  uint32_t exp_word = 0;
+  size_t hist_base = 0;
+  bool replay = false;
+  unsigned item = 0;
+
+  for (;;) {
+    if (!replay) {
+      __syncthreads();  // everyone is done with s_item and with the staged experiment of the last pass
+      if (threadIdx.x == 0) s_item = atomicAdd(a.work_counter, 1u);
+      __syncthreads();
+      item = s_item;
+    }
+    const bool have = item < a.n_items;
+    const int e = have ? (int)(item / a.items_per_exp) : -1;
+    const bool drain = (e != cur_exp) && (cur_exp >= 0) && !replay;
+    uint32_t row = 0, row_end = 0, off0 = 0, cnt_ids = 0;
+    if (drain) {
+      replay = true;  // come back for this item after the queues are empty
+    } else {
+      replay = false;
+      if (!have) break;
+      if (e != cur_exp) {
+        // stage the experiment: parameters and tables (fp64 in HBM -> Real in shared memory)
+        __syncthreads();  // every warp has drained the previous experiment
+        const ExpParams* src = a.exps + e;
+        const uint32_t* s32 = reinterpret_cast<const uint32_t*>(src);
+        uint32_t* d32 = reinterpret_cast<uint32_t*>(&P);
+        for (int i = threadIdx.x; i < (int)(sizeof(ExpParams) / 4); i += BLOCK_THREADS) d32[i] = s32[i];
+        const int tl = src->tab_len;
+        const double* tsrc = a.tab_pool + src->tab_off;
+        for (int i = threadIdx.x; i < tl; i += BLOCK_THREADS) tab[i] = (Real)tsrc[i];
+        cur_exp = e;
+        exp_word = a.exp_base + (uint32_t)e;
+        hist_base = (size_t)e * (size_t)a.npix;
+        __syncthreads();
+      }
+      const uint32_t kk = item % a.items_per_exp;
+      off0 = kk * a.item_ids;
+      cnt_ids = min(a.item_ids, a.n_per_exp - off0);
+      row = warp;
+      row_end = (cnt_ids + 31u) >> 5;
+    }
+
+    // ------------------------------------------------------------------ the pump
+    for (;;) {
+      const bool rows_left = row < row_end;
+      if (cntC >= 32 || (drain && cntB == 0 && cntC > 0)) {
+        // ---------------- stage C: model + weight + histogram
+        const int n = cntC < 32 ? cntC : 32;
+        const bool act = lane < n;
+        const int slot = (headC + lane) & (RING - 1);
+        uint32_t idoff = 0; int32_t pixel = 0; double G = 0, Qx = 0, Qy = 0, Qz = 0;
+        if (act) {
+          idoff = wq.c_id[slot]; pixel = wq.c_pixel[slot]; G = wq.c_G[slot];
+          Qx = wq.c_Q[0][slot]; Qy = wq.c_Q[1][slot]; Qz = wq.c_Q[2][slot];
+        }
+        __syncwarp();
+        headC = (headC + n) & (RING - 1);
+        cntC -= n;
+        if (act) {
+          const uint64_t id = a.first_id + idoff;
+          const Real I = eval_intensity<Real>(P, tab, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
+          const double p = G * (double)I;
+          if (DUMP) {
+            a.d_pixel[idoff] = pixel;
+            a.d_weight[idoff] = p;
+          } else {
+            const size_t ix = hist_base + (size_t)pixel;
+            atomicAdd(a.counts + ix, 1ull);
+            atomicAdd(a.sum_p + ix, p);
+            atomicAdd(a.sum_p2 + ix, p * p);
+          }
+        }
+        continue;
+      }
+      if (cntB >= 32 || (drain && cntB > 0)) {
+        // ---------------- stage B: fp64 geometry
+        const int n = cntB < 32 ? cntB : 32;
+        const bool act = lane < n;
+        const int slot = (headB + lane) & (RING - 1);
+        uint32_t idoff = 0, w[4] = {0, 0, 0, 0};
+        if (act) {
+          idoff = wq.b_id[slot];
+          w[0] = wq.b_w[0][slot]; w[1] = wq.b_w[1][slot]; w[2] = wq.b_w[2][slot]; w[3] = wq.b_w[3][slot];
+        }
+        __syncwarp();
+        headB = (headB + n) & (RING - 1);
+        cntB -= n;
+        int st = -1;
+        Hit h;
+        if (act) {
+          const uint64_t id = a.first_id + idoff;
+          st = trace_geometry(P, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, w, h);
+          if (DUMP && a.d_q != nullptr) a.d_q[idoff] = h.q;
+        }
+        n_s1 += __popc(__ballot_sync(FULL, st == ST_SLIT1));
+        n_s2 += __popc(__ballot_sync(FULL, st == ST_SLIT2));
+        n_ms += __popc(__ballot_sync(FULL, st == ST_MISS_SAMPLE));
+        n_un += __popc(__ballot_sync(FULL, st == ST_UNREACHABLE));
+        n_md += __popc(__ballot_sync(FULL, st == ST_MISS_DET));
+        const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
+        n_det += __popc(m);
+        if (st == ST_DETECTED) {
+          const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
+          wq.c_id[s2] = idoff; wq.c_pixel[s2] = h.pixel; wq.c_G[s2] = h.G;
+          wq.c_Q[0][s2] = h.Qx; wq.c_Q[1][s2] = h.Qy; wq.c_Q[2][s2] = h.Qz;
+        }
+        cntC += __popc(m);
+        __syncwarp();
+        continue;
+      }
+      if (rows_left) {
+        // ---------------- stage A: Philox block 0 + slit 1 on the raw draws
+        const uint32_t idoff = off0 + (row << 5) + lane;
+        const bool valid = ((row << 5) + lane) < cnt_ids;
+        const uint64_t id = a.first_id + idoff;
+        uint32_t w[4];
+        philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
+        bool pass = valid;
+        if (P.s1_int_ok) {
+          pass = pass && (w[0] >= P.s1_lo[0]) && (w[0] <= P.s1_hi[0]) && (w[1] >= P.s1_lo[1]) && (w[1] <= P.s1_hi[1]);
+          n_s1 += __popc(__ballot_sync(FULL, valid && !pass));
+        }
+        n_launched += __popc(__ballot_sync(FULL, valid));
+        const unsigned m = __ballot_sync(FULL, pass);
+        if (pass) {
+          const int s2 = (headB + cntB + __popc(m & lt_mask)) & (RING - 1);
+          wq.b_id[s2] = idoff;
+          wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
+        }
+        cntB += __popc(m);
+        __syncwarp();
+        row += WARPS_PER_BLOCK;
+        continue;
+      }
+      break;
+    }
+  }
+
+  if (lane == 0 && !DUMP) {
+    atomicAdd(a.counters + 0, n_launched);
+    if (n_s1) atomicAdd(a.counters + 1, (unsigned long long)n_s1);
+    if (n_s2) atomicAdd(a.counters + 2, (unsigned long long)n_s2);
+    if (n_ms) atomicAdd(a.counters + 3, (unsigned long long)n_ms);
+    if (n_un) atomicAdd(a.counters + 4, (unsigned long long)n_un);
+    if (n_md) atomicAdd(a.counters + 5, (unsigned long long)n_md);
+    if (n_det) atomicAdd(a.counters + 6, (unsigned long long)n_det);
+  }
+}
+
+}  // namespace sas

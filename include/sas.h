@@ -173,6 +173,9 @@ sas_status sas_get_launch_info(sas_ctx* ctx, uint64_t* n_launches, int32_t* grid
 /* Average device time in ms (CUDA events on the context's stream) of the trace kernels launched
  * since the last call with reset != 0; *n_timed = how many launches the average covers. */
 sas_status sas_get_kernel_time(sas_ctx* ctx, int32_t reset, double* avg_ms, uint64_t* n_timed);
+/* Bytes of the last host-to-device upload of parameters and quadrature tables (sas_set_model /
+ * sas_create_batch). */
+sas_status sas_get_upload_bytes(sas_ctx* ctx, uint64_t* bytes);
 const char* sas_version(void);
 
 #ifdef __cplusplus

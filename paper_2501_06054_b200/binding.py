@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "sas_create_instrument", "sas_bind_buffers", "sas_set_model", "sas_trace", "sas_trace_range",
     "sas_trace_dump", "sas_read_detector", "sas_get_counters", "sas_reset_detector", "sas_destroy",
     "sas_last_error", "sas_create_batch", "sas_trace_batch", "sas_quadrature_nodes",
-    "sas_get_launch_info", "sas_get_kernel_time", "sas_version",
+    "sas_get_launch_info", "sas_get_kernel_time", "sas_get_upload_bytes", "sas_version",
 ]
 
 SAMPLE = {"box": 0, "cyl_y": 1}
@@ -130,6 +130,7 @@ def load_library(path: str | None = None):
     L.sas_quadrature_nodes.argtypes = [i32, dbl, i32, pp(dbl), pp(dbl)]
     L.sas_get_launch_info.argtypes = [vp, pp(u64), pp(i32), pp(i32), pp(i32)]
     L.sas_get_kernel_time.argtypes = [vp, i32, pp(dbl), pp(u64)]
+    L.sas_get_upload_bytes.argtypes = [vp, pp(u64)]
     L.sas_version.argtypes = []
     L.sas_version.restype = C.c_char_p
     for name in EXPORTED_SYMBOLS:
@@ -196,6 +197,11 @@ class _Base:
         ms, n = C.c_double(), C.c_uint64()
         _check(self.L, self.ctx, self.L.sas_get_kernel_time(self.ctx, 1 if reset else 0, ms, n))
         return ms.value, n.value
+
+    def upload_bytes(self):
+        n = C.c_uint64()
+        _check(self.L, self.ctx, self.L.sas_get_upload_bytes(self.ctx, n))
+        return n.value
 
     def close(self):
         if getattr(self, "ctx", None):

@@ -74,9 +74,13 @@ __device__ __forceinline__ void sincos_r(float x, float& s, float& c) {
 }
 __device__ __forceinline__ void sincos_r(double x, double& s, double& c) { sincos(x, &s, &c); }
 
-__device__ __forceinline__ float rcp_r(float x) { return __frcp_rn(x); }
+// fp32 reciprocal / square root: one MUFU each (~1 ulp), no IEEE fix-up path
+__device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float sqrt_fast(float x) { float r; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rsqrt_fast(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ float rcp_r(float x) { return rcp_fast(x); }
 __device__ __forceinline__ double rcp_r(double x) { return 1.0 / x; }
-__device__ __forceinline__ float sqrt_r(float x) { return __fsqrt_rn(x); }
+__device__ __forceinline__ float sqrt_r(float x) { return sqrt_fast(x); }
 __device__ __forceinline__ double sqrt_r(double x) { return sqrt(x); }
 __device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
@@ -164,7 +168,7 @@ __device__ __forceinline__ float sphere_phi(float u) {
   ser = fmaf(ser, u2, 1.0f);
   float s, c;
   sincos_r(u, s, c);
-  const float inv = __frcp_rn(u);
+  const float inv = rcp_fast(u);
   const float dir = (3.0f * fmaf(-u, c, s)) * ((inv * inv) * inv);
   return (u < 0.7f) ? ser : dir;
 }
@@ -185,37 +189,52 @@ __device__ __forceinline__ double sphere_phi(double u) {
 }
 
 // ---------------------------------------------------------------- sinc
+// sin(x) alone: reduction by pi, one odd polynomial on [-pi/2, pi/2], sign from the parity of k.
+__device__ __forceinline__ float sin_reduced_pi(float x, float lo) {
+  const float kf = rintf(x * 0.318309886f);
+  float r = fmaf(kf, -3.14159250259399414062e+00f, x);
+  r = fmaf(kf, -1.50995788317231927067e-07f, r);
+  r = fmaf(kf, -1.07806050599155295311e-14f, r) + lo;
+  const float z = r * r;
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  const float ps = fmaf(r * z, horner(SP, z), r);
+  const int k = (int)kf;
+  return __int_as_float(__float_as_int(ps) ^ (int)((unsigned)k << 31));
+}
 __device__ __forceinline__ float sinc_r(float x) {
-  float s, c;
-  sincos_r(x, s, c);
-  return (fabsf(x) < 1e-4f) ? 1.0f : s * __frcp_rn(x);
+  const float s = sin_reduced_pi(x, 0.0f);
+  return (fabsf(x) < 1e-4f) ? 1.0f : s * rcp_fast(x);
 }
 __device__ __forceinline__ double sinc_r(double x) { return (x == 0.0) ? 1.0 : sin(x) / x; }
 
 // ---------------------------------------------------------------- Lambda(x) = 2 J1(x)/x, x >= 0
-__device__ __forceinline__ float lambda1_r(float x) {
-  if (x < 4.0f) {
-    const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
-    return horner(LA, fmaf(x * x, 0.125f, -1.0f));
-  }
-  if (x < 8.0f) {
-    const float LB[SAS_LAMBDA_B_N] = SAS_LAMBDA_B;
-    return horner(LB, fmaf(x, 0.5f, -3.0f));
-  }
-  // Hankel form: J1 = sqrt(2/(pi x)) (P cos(x - 3pi/4) - Q sin(x - 3pi/4))
+// x <= 8: one polynomial in x^2 (no square root needed); x > 8: Hankel form
+//   J1 = sqrt(2/(pi x)) (P cos(x - 3pi/4) - Q sin(x - 3pi/4)).
+__device__ __forceinline__ float lambda1_asym(float x, float xlo) {
   const float AP[SAS_J1_ASY_P_N] = SAS_J1_ASY_P;
   const float AQ[SAS_J1_ASY_Q_N] = SAS_J1_ASY_Q;
-  const float inv = __frcp_rn(x);
+  const float inv = rcp_fast(x);
   const float t = fmaf(128.0f * inv, inv, -1.0f);
   const float P = horner(AP, t);
   const float Q = horner(AQ, t) * inv;
   float s, c;
-  sincos_r(x, s, c);
+  Phase<float> ph = {x, xlo};
+  sincos_ph(ph, s, c);
   // cos(x-3pi/4) = (s - c)/sqrt2 ; sin(x-3pi/4) = -(s + c)/sqrt2
-  const float j1 = (0.797884583f * 0.707106769f) * rsqrtf(x) * fmaf(P, s - c, Q * (s + c));
-  return 2.0f * j1 * inv;
+  const float j1v = (0.797884583f * 0.707106769f) * rsqrt_fast(x) * fmaf(P, s - c, Q * (s + c));
+  return 2.0f * j1v * inv;
 }
+// argument given as x^2 (plus a first-order correction 2 x x_lo folded in by the caller)
+__device__ __forceinline__ float lambda1_x2(float x2) {
+  if (x2 <= 64.0f) {
+    const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+    return horner(LA, fmaf(x2, 0.03125f, -1.0f));
+  }
+  return lambda1_asym(sqrt_fast(x2), 0.0f);
+}
+__device__ __forceinline__ float lambda1_r(float x) { return lambda1_x2(x * x); }
 __device__ __forceinline__ double lambda1_r(double x) { return (x == 0.0) ? 1.0 : (2.0 * j1(x)) / x; }
+__device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(x2)); }
 
 // ---------------------------------------------------------------- the same functions of a Phase
 __device__ __forceinline__ float sphere_phi_ph(Phase<float> p) {
@@ -227,39 +246,25 @@ __device__ __forceinline__ float sphere_phi_ph(Phase<float> p) {
   ser = fmaf(ser, u2, 1.0f);
   float s, c;
   sincos_ph(p, s, c);
-  const float inv = __frcp_rn(u);
+  const float inv = rcp_fast(u);
   const float dir = (3.0f * fmaf(-u, c, s)) * ((inv * inv) * inv);
   return (u < 0.7f) ? ser : dir;
 }
 __device__ __forceinline__ double sphere_phi_ph(Phase<double> p) { return sphere_phi(p.v); }
 
 __device__ __forceinline__ float sinc_ph(Phase<float> p) {
-  float s, c;
-  sincos_ph(p, s, c);
-  return (fabsf(p.hi) < 1e-4f) ? 1.0f : s * __frcp_rn(p.hi);
+  const float s = sin_reduced_pi(p.hi, p.lo);
+  return (fabsf(p.hi) < 1e-4f) ? 1.0f : s * rcp_fast(p.hi);
 }
 __device__ __forceinline__ double sinc_ph(Phase<double> p) { return sinc_r(p.v); }
 
 __device__ __forceinline__ float lambda1_ph(Phase<float> p) {
   const float x = p.hi;
-  if (x < 4.0f) {
+  if (x <= 8.0f) {
     const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
-    return horner(LA, fmaf(x * x, 0.125f, fmaf(x * p.lo, 0.25f, -1.0f)));
+    return horner(LA, fmaf(x * x, 0.03125f, fmaf(x * p.lo, 0.0625f, -1.0f)));
   }
-  if (x < 8.0f) {
-    const float LB[SAS_LAMBDA_B_N] = SAS_LAMBDA_B;
-    return horner(LB, fmaf(x, 0.5f, fmaf(p.lo, 0.5f, -3.0f)));
-  }
-  const float AP[SAS_J1_ASY_P_N] = SAS_J1_ASY_P;
-  const float AQ[SAS_J1_ASY_Q_N] = SAS_J1_ASY_Q;
-  const float inv = __frcp_rn(x);
-  const float t = fmaf(128.0f * inv, inv, -1.0f);
-  const float P = horner(AP, t);
-  const float Q = horner(AQ, t) * inv;
-  float s, c;
-  sincos_ph(p, s, c);
-  const float j1v = (0.797884583f * 0.707106769f) * rsqrtf(x) * fmaf(P, s - c, Q * (s + c));
-  return 2.0f * j1v * inv;
+  return lambda1_asym(x, p.lo);
 }
 __device__ __forceinline__ double lambda1_ph(Phase<double> p) { return lambda1_r(p.v); }
 

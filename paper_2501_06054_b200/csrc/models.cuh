@@ -112,28 +112,45 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
     } break;
     case 2: {  // cylinder: separable in (R, L) for a given axis direction
       if (P.orient_kind == 1) {
-        // Gaussian tilt quadrature (R-A11): n_th x n_ph axis directions about the mean axis, plain Real
+        // Gaussian tilt quadrature (R-A11): n_th x n_ph axis directions about the mean axis, plain Real.
+        // Lambda is evaluated from x^2 = R^2 (q^2 - qc^2): no square root below x = 8.
         const Real qA = (Real)qAd, qB = (Real)qBd, qC = (Real)qCd;
+        const bool mono = (P.n_a == 1) && (P.n_b == 1);
+        const Real hL0 = T.tb[0], cL0 = T.tb[2], R20 = T.ta[3], cR0 = T.ta[2];
         for (int i = 0; i < P.n_th; ++i) {
           const Real sth = T.tth[i * TOR_W + 0], cth = T.tth[i * TOR_W + 1], wth = T.tth[i * TOR_W + 2];
           const Real Ai = fma_r(qA, sth, qC * cth);
           Real row = 0;
-          for (int j = 0; j < P.n_ph; ++j) {
-            const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
-            const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
-            Real r2 = fma_r(-qc, qc, q2);
-            r2 = r2 > (Real)0 ? r2 : (Real)0;
-            const Real qab = sqrt_r(r2);
-            Real SL = 0, SR = 0;
-            for (int b = 0; b < P.n_b; ++b) {
-              const Real sc = sinc_r(qc * T.tb[b * TB_W + 0]);
-              SL = fma_r(T.tb[b * TB_W + 2], sc * sc, SL);
+          if (mono) {
+#pragma unroll 2
+            for (int j = 0; j < P.n_ph; ++j) {
+              const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
+              const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
+              Real r2 = fma_r(-qc, qc, q2);
+              r2 = r2 > (Real)0 ? r2 : (Real)0;
+              const Real sc = sinc_r(qc * hL0);
+              const Real la = lambda1_x2(r2 * R20);
+              const Real f = sc * la;
+              row = fma_r(wph, f * f, row);
             }
-            for (int a = 0; a < P.n_a; ++a) {
-              const Real la = lambda1_r(qab * T.ta[a * TA_W + 0]);
-              SR = fma_r(T.ta[a * TA_W + 2], la * la, SR);
+            row *= cL0 * cR0;
+          } else {
+            for (int j = 0; j < P.n_ph; ++j) {
+              const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
+              const Real qc = fma_r(cph, Ai, qB * sph);
+              Real r2 = fma_r(-qc, qc, q2);
+              r2 = r2 > (Real)0 ? r2 : (Real)0;
+              Real SL = 0, SR = 0;
+              for (int b = 0; b < P.n_b; ++b) {
+                const Real sc = sinc_r(qc * T.tb[b * TB_W + 0]);
+                SL = fma_r(T.tb[b * TB_W + 2], sc * sc, SL);
+              }
+              for (int a = 0; a < P.n_a; ++a) {
+                const Real la = lambda1_x2(r2 * T.ta[a * TA_W + 3]);
+                SR = fma_r(T.ta[a * TA_W + 2], la * la, SR);
+              }
+              row = fma_r(wph, SL * SR, row);
             }
-            row = fma_r(wph, SL * SR, row);
           }
           acc = fma_r(wth, row, acc);
         }

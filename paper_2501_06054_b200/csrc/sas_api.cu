@@ -231,7 +231,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
     switch (m.model) {
       case SAS_SPHERE: { const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R; split(R, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
       case SAS_CORE_SHELL_SPHERE: { const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R; split(R, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
-      case SAS_CYLINDER: { const double R = m.size[0] * xa[a], c = s0 * PI_D * R * R; split(R, r); r[2] = wa[a] * c * c; } break;
+      case SAS_CYLINDER: { const double R = m.size[0] * xa[a], c = s0 * PI_D * R * R; split(R, r); r[2] = wa[a] * c * c; r[3] = R * R; } break;
       case SAS_TRIAXIAL_ELLIPSOID: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
       case SAS_CORE_SHELL_TRIAXIAL: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
       default: break;
@@ -283,8 +283,8 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
   pool.insert(pool.end(), ta.begin(), ta.end());
   pool.insert(pool.end(), tb.begin(), tb.end());
   pool.insert(pool.end(), tab.begin(), tab.end());
-  for (size_t i = 0; i < dth.size(); ++i) { pool.push_back(std::sin(dth[i])); pool.push_back(std::cos(dth[i])); pool.push_back(wth[i]); }
-  for (size_t i = 0; i < dph.size(); ++i) { pool.push_back(std::sin(dph[i])); pool.push_back(std::cos(dph[i])); pool.push_back(wph[i]); }
+  for (size_t i = 0; i < dth.size(); ++i) { pool.push_back(std::sin(dth[i])); pool.push_back(std::cos(dth[i])); pool.push_back(wth[i]); pool.push_back(0.0); }
+  for (size_t i = 0; i < dph.size(); ++i) { pool.push_back(std::sin(dph[i])); pool.push_back(std::cos(dph[i])); pool.push_back(wph[i]); pool.push_back(0.0); }
   P.tab_len = (int)pool.size() - P.tab_off;
 }
 
@@ -622,6 +622,12 @@ sas_status sas_get_kernel_time(sas_ctx* c, int32_t reset, double* avg_ms, uint64
   if (avg_ms) *avg_ms = c->n_timed ? sum / (double)c->n_timed : 0.0;
   if (n_timed) *n_timed = c->n_timed;
   if (reset) c->n_timed = 0;
+  return SAS_OK;
+}
+
+sas_status sas_get_upload_bytes(sas_ctx* c, uint64_t* bytes) {
+  if (!c || !bytes) return SAS_EINVAL;
+  *bytes = c->h_tab.size() * sizeof(double) + (uint64_t)c->n_exp * sizeof(ExpParams);
   return SAS_OK;
 }
 

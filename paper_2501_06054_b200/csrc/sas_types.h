@@ -12,7 +12,7 @@ enum : int { ST_DETECTED = 0, ST_SLIT1 = 1, ST_SLIT2 = 2, ST_MISS_SAMPLE = 3, ST
 constexpr int TA_W = 4;   // per node of polydisperse axis 0
 constexpr int TB_W = 4;   // per node of polydisperse axis 1
 constexpr int TAB_W = 4;  // per (a,b) pair
-constexpr int TOR_W = 3;  // per orientation tilt node: sin(delta), cos(delta), weight
+constexpr int TOR_W = 4;  // per orientation tilt node: sin(delta), cos(delta), weight, pad (one 128-bit load)
 
 // One virtual experiment: everything the kernel needs, precomputed on the host in fp64 with exactly the
 // operations DESIGN.md section 3 writes (so that e.g. 0.5*det_xw is the same double on both sides).

@@ -13,8 +13,15 @@
 
 namespace sas {
 
-constexpr int BLOCK_THREADS = 256;
+#ifndef SAS_BLOCK_THREADS
+#define SAS_BLOCK_THREADS 256
+#endif
+#ifndef SAS_MIN_BLOCKS
+#define SAS_MIN_BLOCKS 3
+#endif
+constexpr int BLOCK_THREADS = SAS_BLOCK_THREADS;
 constexpr int WARPS_PER_BLOCK = BLOCK_THREADS / 32;
+constexpr int MIN_BLOCKS_PER_SM = SAS_MIN_BLOCKS;
 constexpr int RING = 64;  // entries per warp queue (power of two, >= 63)
 
 struct WarpQueues {
@@ -37,7 +44,7 @@ __host__ __device__ inline size_t trace_smem_bytes(int tab_len_max) {
 }
 
 template <typename Real, bool DUMP>
-__global__ void __launch_bounds__(BLOCK_THREADS) trace_kernel(const __grid_constant__ KernelArgs a) {
+__global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel(const __grid_constant__ KernelArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned int s_item;
 
@@ -168,27 +175,32 @@ __global__ void __launch_bounds__(BLOCK_THREADS) trace_kernel(const __grid_const
         continue;
       }
       if (rows_left) {
-        // ---------------- stage A: Philox block 0 + slit 1 on the raw draws
-        const uint32_t idoff = off0 + (row << 5) + lane;
-        const bool valid = ((row << 5) + lane) < cnt_ids;
-        const uint64_t id = a.first_id + idoff;
-        uint32_t w[4];
-        philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
-        bool pass = valid;
-        if (P.s1_int_ok) {
-          pass = pass && (w[0] >= P.s1_lo[0]) && (w[0] <= P.s1_hi[0]) && (w[1] >= P.s1_lo[1]) && (w[1] <= P.s1_hi[1]);
-          n_s1 += __popc(__ballot_sync(FULL, valid && !pass));
-        }
-        n_launched += __popc(__ballot_sync(FULL, valid));
-        const unsigned m = __ballot_sync(FULL, pass);
-        if (pass) {
-          const int s2 = (headB + cntB + __popc(m & lt_mask)) & (RING - 1);
-          wq.b_id[s2] = idoff;
-          wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
-        }
-        cntB += __popc(m);
+        // ---------------- stage A: Philox block 0 + slit 1 on the raw draws, until a full warp of
+        // survivors is queued (tight loop: ~4 rows per stage-B round at a 25 % pass rate)
+        const bool s1_int = P.s1_int_ok != 0;
+        const uint32_t lo0 = P.s1_lo[0], hi0 = P.s1_hi[0], lo1 = P.s1_lo[1], hi1 = P.s1_hi[1];
+        do {
+          const uint32_t in_item = (row << 5) + lane;
+          const uint32_t idoff = off0 + in_item;
+          const bool valid = in_item < cnt_ids;
+          const uint64_t id = a.first_id + idoff;
+          uint32_t w[4];
+          philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
+          bool pass = valid;
+          if (s1_int) pass = pass && (w[0] - lo0 <= hi0 - lo0) && (w[1] - lo1 <= hi1 - lo1);
+          const unsigned mv = __ballot_sync(FULL, valid);
+          const unsigned m = __ballot_sync(FULL, pass);
+          n_launched += __popc(mv);
+          if (s1_int) n_s1 += __popc(mv & ~m);
+          if (pass) {
+            const int s2 = (headB + cntB + __popc(m & lt_mask)) & (RING - 1);
+            wq.b_id[s2] = idoff;
+            wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
+          }
+          cntB += __popc(m);
+          row += WARPS_PER_BLOCK;
+        } while (row < row_end && cntB < 32);
         __syncwarp();
-        row += WARPS_PER_BLOCK;
         continue;
       }
       break;

@@ -2,66 +2,55 @@
 // Written operation by operation as the design note states them; the translation unit is compiled
 // with -fmad=false, so nothing here is contracted and the detector pixel is bit-identical to a
 // plain IEEE evaluation of the same text.
+//
+// Control flow: a warp executes this for 32 slit-1 survivors at once, of which ~80 % will miss the
+// detector.  The code is therefore straight-line: every lane computes every quantity (a dead lane
+// carries harmless garbage) and the outcome is decided at the end from failure flags taken in the
+// order the design note tests them.  Selects replace the d == 0 / swap branches of the slab test;
+// for finite non-NaN inputs they yield the same values as the oracle's branches.
 #pragma once
 #include "sas_types.h"
 
 namespace sas {
 
+// one axis of the slab test: interval of t with |o + t d| <= h, intersected into [tin, tout]
+__device__ __forceinline__ void slab_axis(double o, double d, double h, double& tin, double& tout, bool& miss) {
+  const bool par = (d == 0.0);
+  const double inv = 1.0 / d;
+  const double ta = (-h - o) * inv, tb = (h - o) * inv;
+  double t1 = fmin(ta, tb), t2 = fmax(ta, tb);
+  t1 = par ? -INFINITY : t1;
+  t2 = par ? INFINITY : t2;
+  miss = miss || (par && fabs(o) > h);
+  tin = fmax(tin, t1);
+  tout = fmin(tout, t2);
+}
+
 // Ray (o + t d) against the sample volume centred on the origin of the sample frame (R-C5).
 __device__ __forceinline__ bool intersect_sample(const ExpParams& P, double ox, double oy, double oz, double dx,
                                                  double dy, double dz, double& t_in, double& t_out) {
   double tin = -INFINITY, tout = INFINITY;
-  bool cyl = P.sample_shape == 1;
-  if (cyl) {
+  bool miss = false;
+  if (P.sample_shape == 1) {  // warp-uniform
     const double a = dx * dx + dz * dz;
     const double b = ox * dx + oz * dz;
     const double c = (ox * ox + oz * oz) - P.radius2;
-    if (a == 0.0) {
-      if (c > 0.0) return false;
-    } else {
-      const double disc = b * b - a * c;
-      if (!(disc > 0.0)) return false;
-      const double sq = sqrt(disc);
-      const double inv_a = 1.0 / a;
-      tin = (-b - sq) * inv_a;
-      tout = (-b + sq) * inv_a;
-    }
+    const bool par = (a == 0.0);
+    const double disc = b * b - a * c;
+    const double sq = sqrt(disc);
+    const double inv_a = 1.0 / a;
+    const double t1 = (-b - sq) * inv_a, t2 = (-b + sq) * inv_a;
+    miss = par ? (c > 0.0) : !(disc > 0.0);
+    tin = par ? tin : t1;
+    tout = par ? tout : t2;
   } else {
-    // x slab
-    if (dx == 0.0) {
-      if (fabs(ox) > P.hx) return false;
-    } else {
-      const double inv = 1.0 / dx;
-      double t1 = (-P.hx - ox) * inv, t2 = (P.hx - ox) * inv;
-      if (t1 > t2) { const double t = t1; t1 = t2; t2 = t; }
-      if (t1 > tin) tin = t1;
-      if (t2 < tout) tout = t2;
-    }
+    slab_axis(ox, dx, P.hx, tin, tout, miss);
   }
-  // y slab (box and cylinder height)
-  if (dy == 0.0) {
-    if (fabs(oy) > P.hy) return false;
-  } else {
-    const double inv = 1.0 / dy;
-    double t1 = (-P.hy - oy) * inv, t2 = (P.hy - oy) * inv;
-    if (t1 > t2) { const double t = t1; t1 = t2; t2 = t; }
-    if (t1 > tin) tin = t1;
-    if (t2 < tout) tout = t2;
-  }
-  if (!cyl) {
-    if (dz == 0.0) {
-      if (fabs(oz) > P.hz) return false;
-    } else {
-      const double inv = 1.0 / dz;
-      double t1 = (-P.hz - oz) * inv, t2 = (P.hz - oz) * inv;
-      if (t1 > t2) { const double t = t1; t1 = t2; t2 = t; }
-      if (t1 > tin) tin = t1;
-      if (t2 < tout) tout = t2;
-    }
-  }
+  slab_axis(oy, dy, P.hy, tin, tout, miss);
+  if (P.sample_shape != 1) slab_axis(oz, dz, P.hz, tin, tout, miss);
   t_in = tin;
   t_out = tout;
-  return true;
+  return !miss;
 }
 
 struct Hit {
@@ -74,8 +63,6 @@ struct Hit {
 // From the four words of Philox block 0 to the detector pixel.  Returns the ST_* outcome.
 __device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKeys& keys, uint32_t id_lo,
                                               uint32_t id_hi, uint32_t exp_word, const uint32_t w[4], Hit& h) {
-  h.q = 0.0;
-  h.pixel = -1;
   // R-C2 source point
   const double u0 = uniform_from_word(w[0]), u1 = uniform_from_word(w[1]);
   const double u2 = uniform_from_word(w[2]), u3 = uniform_from_word(w[3]);
@@ -93,16 +80,12 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKe
   const double p0 = (P.p0_pref * dOmega) * P.dlam_w;
   // R-C4 slits
   const double inv_dz = 1.0 / dz;
-  {
-    const double s = (P.slit1_z - 0.0) * inv_dz;
-    const double xs = x0 + dx * s, ys = y0 + dy * s;
-    if (fabs(xs) > P.slit1_hx || fabs(ys) > P.slit1_hy) return ST_SLIT1;
-  }
-  {
-    const double s = (P.slit2_z - 0.0) * inv_dz;
-    const double xs = x0 + dx * s, ys = y0 + dy * s;
-    if (fabs(xs) > P.slit2_hx || fabs(ys) > P.slit2_hy) return ST_SLIT2;
-  }
+  const double s1 = (P.slit1_z - 0.0) * inv_dz;
+  const double xs1 = x0 + dx * s1, ys1 = y0 + dy * s1;
+  const bool f_s1 = fabs(xs1) > P.slit1_hx || fabs(ys1) > P.slit1_hy;
+  const double s2s = (P.slit2_z - 0.0) * inv_dz;
+  const double xs2 = x0 + dx * s2s, ys2 = y0 + dy * s2s;
+  const bool f_s2 = fabs(xs2) > P.slit2_hx || fabs(ys2) > P.slit2_hy;
   // draws 4..7
   uint32_t w1[4];
   philox4x32_10(keys, id_lo, id_hi, 1u, exp_word, w1);
@@ -111,9 +94,9 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKe
   const double lambda = P.lambda_min + u4 * P.dlam;
   // R-C5 sample
   double tin, tout;
-  if (!intersect_sample(P, x0, y0, 0.0 - P.sample_z, dx, dy, dz, tin, tout)) return ST_MISS_SAMPLE;
-  if (tin < 0.0) tin = 0.0;
-  if (!(tout > tin)) return ST_MISS_SAMPLE;
+  const bool hit_s = intersect_sample(P, x0, y0, 0.0 - P.sample_z, dx, dy, dz, tin, tout);
+  tin = tin < 0.0 ? 0.0 : tin;
+  const bool f_ms = !hit_s || !(tout > tin);
   const double ell = tout - tin;
   // R-C6 scattering point
   const double ts = tin + u5 * ell;
@@ -125,8 +108,7 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKe
   const double inv_k = lambda / 6.283185307179586;
   const double qk = q * inv_k;
   const double s = 0.5 * qk;
-  h.q = q;
-  if (s >= 1.0) return ST_UNREACHABLE;
+  const bool f_un = s >= 1.0;
   const double ss2 = 2.0 * (s * s);
   const double c2 = 1.0 - ss2;
   const double s2 = 2.0 * (s * sqrt(1.0 - s * s));
@@ -143,25 +125,35 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKe
   h.Qy = k * (ss2 * dy - s2 * ty);
   h.Qz = k * (ss2 * dz - s2 * tz);
   // R-C9 detector
-  if (!(dpz > 0.0)) return ST_MISS_DET;
   const double inv_dpz = 1.0 / dpz;
   const double td = (P.det_z - rsz) * inv_dpz;
   const double X = rsx + dpx * td, Y = rsy + dpy * td;
   const double fx = (X + P.det_hw) * P.det_sx;
   const double fy = (Y + P.det_hh) * P.det_sy;
-  if (!(fx >= 0.0 && fx < P.det_nxd && fy >= 0.0 && fy < P.det_nyd)) return ST_MISS_DET;
-  h.pixel = (int)floor(fy) * P.det_nx + (int)floor(fx);
-  // R-C11 attenuation and the geometric part of the weight
-  double T = 1.0;
-  if (P.has_mu) {
-    const double mu = (P.mu_abs_2200 * lambda) / 1.7982 + P.mu_inc;
-    double tin2, tout2, ell_out = 0.0;
-    if (intersect_sample(P, rsx, rsy, rsz - P.sample_z, dpx, dpy, dpz, tin2, tout2) && tout2 > 0.0) ell_out = tout2;
-    T = exp(-(mu * (u5 * ell + ell_out)));
+  const bool f_md = !(dpz > 0.0) || !(fx >= 0.0 && fx < P.det_nxd && fy >= 0.0 && fy < P.det_nyd);
+  // outcome, in the order of the design note
+  int st = ST_DETECTED;
+  st = f_md ? ST_MISS_DET : st;
+  st = f_un ? ST_UNREACHABLE : st;
+  st = f_ms ? ST_MISS_SAMPLE : st;
+  st = f_s2 ? ST_SLIT2 : st;
+  st = f_s1 ? ST_SLIT1 : st;
+  h.q = (f_s1 || f_s2 || f_ms) ? 0.0 : q;
+  h.pixel = -1;
+  if (st == ST_DETECTED) {
+    h.pixel = (int)floor(fy) * P.det_nx + (int)floor(fx);
+    // R-C11 attenuation and the geometric part of the weight
+    double T = 1.0;
+    if (P.has_mu) {
+      const double mu = (P.mu_abs_2200 * lambda) / 1.7982 + P.mu_inc;
+      double tin2, tout2, ell_out = 0.0;
+      if (intersect_sample(P, rsx, rsy, rsz - P.sample_z, dpx, dpy, dpz, tin2, tout2) && tout2 > 0.0) ell_out = tout2;
+      T = exp(-(mu * (u5 * ell + ell_out)));
+    }
+    const double geo = (p0 * T) * (100.0 * ell);
+    h.G = (geo * (qk * inv_k)) * P.qnorm;
   }
-  const double geo = (p0 * T) * (100.0 * ell);
-  h.G = (geo * (qk * inv_k)) * P.qnorm;
-  return ST_DETECTED;
+  return st;
 }
 
 }  // namespace sas

@@ -33,6 +33,7 @@ struct WarpQueues {
   int32_t c_pixel[RING];
   double c_G[RING];
   double c_Q[3][RING];
+  unsigned long long n_launched;  // ids this warp has drawn (lane 0 updates it once per work item)
 };
 
 __host__ __device__ inline size_t round16(size_t x) { return (x + 15) & ~(size_t)15; }
@@ -41,6 +42,17 @@ template <typename Real>
 __host__ __device__ inline size_t trace_smem_bytes(int tab_len_max) {
   return round16(sizeof(ExpParams)) + round16((size_t)tab_len_max * sizeof(Real)) +
          (size_t)WARPS_PER_BLOCK * sizeof(WarpQueues);
+}
+
+// adds the six packed 10-bit outcome fields of one lane to the global counters (index = status, with
+// detected (status 0) stored in slot 6 and statuses 1..5 in slots 1..5)
+__device__ __forceinline__ void flush_packed(unsigned long long* counters, unsigned long long pk) {
+#pragma unroll
+  for (int st = 0; st < 6; ++st) {
+    const unsigned v = (unsigned)(pk >> (10 * st)) & 1023u;
+    const unsigned tot = __reduce_add_sync(0xFFFFFFFFu, v);
+    if ((threadIdx.x & 31) == 0 && tot) atomicAdd(counters + (st == 0 ? 6 : st), (unsigned long long)tot);
+  }
 }
 
 template <typename Real, bool DUMP>
@@ -59,8 +71,12 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
 
   // warp-uniform pipeline state
   int headB = 0, cntB = 0, headC = 0, cntC = 0;
-  unsigned n_s1 = 0, n_s2 = 0, n_ms = 0, n_un = 0, n_md = 0, n_det = 0;
-  unsigned long long n_launched = 0;
+  // outcome counters: every lane packs its own six 10-bit fields (status s -> bits [10 s, 10 s + 10));
+  // flushed to the global counters before a field can overflow
+  unsigned long long pk = 0;
+  unsigned pk_calls = 0;
+  unsigned n_passA = 0;  // survivors of the integer slit-1 test (warp-uniform)
+  if (lane == 0) wq.n_launched = 0;
 
   int cur_exp = -1;
   uint32_t exp_word = 0;
@@ -104,6 +120,12 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
       cnt_ids = min(a.item_ids, a.n_per_exp - off0);
       row = warp;
       row_end = (cnt_ids + 31u) >> 5;
+      if (lane == 0) {
+        // ids of this item that fall to this warp: rows warp, warp+8, ... ; the last row may be ragged
+        unsigned long long mine = 0;
+        for (uint32_t r = warp; r < row_end; r += WARPS_PER_BLOCK) mine += min(32u, cnt_ids - (r << 5));
+        wq.n_launched += mine;
+      }
     }
 
     // ------------------------------------------------------------------ the pump
@@ -158,13 +180,9 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
           st = trace_geometry(P, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, w, h);
           if (DUMP && a.d_q != nullptr) a.d_q[idoff] = h.q;
         }
-        n_s1 += __popc(__ballot_sync(FULL, st == ST_SLIT1));
-        n_s2 += __popc(__ballot_sync(FULL, st == ST_SLIT2));
-        n_ms += __popc(__ballot_sync(FULL, st == ST_MISS_SAMPLE));
-        n_un += __popc(__ballot_sync(FULL, st == ST_UNREACHABLE));
-        n_md += __popc(__ballot_sync(FULL, st == ST_MISS_DET));
+        if (act) pk += 1ull << (10 * st);
+        if (++pk_calls == 1000u) { flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
         const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
-        n_det += __popc(m);
         if (st == ST_DETECTED) {
           const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
           wq.c_id[s2] = idoff; wq.c_pixel[s2] = h.pixel; wq.c_G[s2] = h.G;
@@ -179,25 +197,23 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         // survivors is queued (tight loop: ~4 rows per stage-B round at a 25 % pass rate)
         const bool s1_int = P.s1_int_ok != 0;
         const uint32_t lo0 = P.s1_lo[0], hi0 = P.s1_hi[0], lo1 = P.s1_lo[1], hi1 = P.s1_hi[1];
+        const uint64_t id0 = a.first_id + off0 + lane;
         do {
           const uint32_t in_item = (row << 5) + lane;
-          const uint32_t idoff = off0 + in_item;
-          const bool valid = in_item < cnt_ids;
-          const uint64_t id = a.first_id + idoff;
+          const uint64_t id = id0 + (row << 5);
           uint32_t w[4];
           philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
-          bool pass = valid;
+          bool pass = in_item < cnt_ids;
           if (s1_int) pass = pass && (w[0] - lo0 <= hi0 - lo0) && (w[1] - lo1 <= hi1 - lo1);
-          const unsigned mv = __ballot_sync(FULL, valid);
           const unsigned m = __ballot_sync(FULL, pass);
-          n_launched += __popc(mv);
-          if (s1_int) n_s1 += __popc(mv & ~m);
+          const int np = __popc(m);
           if (pass) {
             const int s2 = (headB + cntB + __popc(m & lt_mask)) & (RING - 1);
-            wq.b_id[s2] = idoff;
+            wq.b_id[s2] = off0 + in_item;
             wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
           }
-          cntB += __popc(m);
+          cntB += np;
+          n_passA += np;
           row += WARPS_PER_BLOCK;
         } while (row < row_end && cntB < 32);
         __syncwarp();
@@ -207,14 +223,15 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
     }
   }
 
-  if (lane == 0 && !DUMP) {
-    atomicAdd(a.counters + 0, n_launched);
-    if (n_s1) atomicAdd(a.counters + 1, (unsigned long long)n_s1);
-    if (n_s2) atomicAdd(a.counters + 2, (unsigned long long)n_s2);
-    if (n_ms) atomicAdd(a.counters + 3, (unsigned long long)n_ms);
-    if (n_un) atomicAdd(a.counters + 4, (unsigned long long)n_un);
-    if (n_md) atomicAdd(a.counters + 5, (unsigned long long)n_md);
-    if (n_det) atomicAdd(a.counters + 6, (unsigned long long)n_det);
+  if (!DUMP) {
+    flush_packed(a.counters, pk);
+    if (lane == 0) {
+      const unsigned long long nl = wq.n_launched;
+      atomicAdd(a.counters + 0, nl);
+      // every neutron that stage A did not queue died at the integer slit-1 test (without the prefilter
+      // stage A queues every valid id, so the difference is zero for those experiments)
+      atomicAdd(a.counters + 1, nl - (unsigned long long)n_passA);
+    }
   }
 }
 

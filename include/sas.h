@@ -138,7 +138,9 @@ sas_status sas_trace_dump(sas_ctx* ctx, uint64_t first_id, uint64_t n, uint64_t 
 sas_status sas_read_detector(sas_ctx* ctx, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts);
 
 /* out[8] = launched, absorbed at slit 1, at slit 2, missed the sample, |Q| unreachable
- * (q >= 2k), missed the detector, detected, 0.  Summed over experiments.  Synchronises. */
+ * (q >= 2k), missed the detector, detected; out[7] = how many of the detector misses (out[5])
+ * were decided by the conservative q*lambda classifier without running the full geometry
+ * (an implementation statistic).  Summed over experiments.  Synchronises. */
 sas_status sas_get_counters(sas_ctx* ctx, uint64_t out[8]);
 
 /* Zero histograms and counters (asynchronous on the stream). */

@@ -60,9 +60,22 @@ struct Hit {
   double q;      // drawn |Q| (0 if the neutron died before the draw)
 };
 
-// From the four words of Philox block 0 to the detector pixel.  Returns the ST_* outcome.
-__device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKeys& keys, uint32_t id_lo,
-                                              uint32_t id_hi, uint32_t exp_word, const uint32_t w[4], Hit& h) {
+// Conservative classifier (stage B0): true when the neutron is CERTAIN to end as
+// ST_MISS_DET.  The host proved for this instrument that every slit-1 survivor passes slit 2 and
+// crosses the sample, and folded the worst-case beam divergence, beam radius at the sample, sample
+// depth and detector half-diagonal (each with a 1e-6 margin, ten orders above fp64 rounding) into
+// s_cut = sin(theta_cut): a neutron with sin(theta) = q lambda / 4 pi above it lands outside the
+// detector's circumscribed circle whatever its azimuth.  q is formed exactly as R-C7 forms it.
+__device__ __forceinline__ bool surely_misses_detector(const ExpParams& P, const uint32_t w1[4], double& q) {
+  const double u4 = uniform_from_word(w1[0]), u6 = uniform_from_word(w1[2]);
+  const double lambda = P.lambda_min + u4 * P.dlam;
+  q = P.q_min + u6 * P.dq;
+  const double s_a = (q * lambda) * 0.07957747154594767;  // 1 / (4 pi)
+  return (s_a > P.s_cut) && (s_a < 0.999999);
+}
+
+// From the words of Philox blocks 0 and 1 to the detector pixel.  Returns the ST_* outcome.
+__device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t w[4], const uint32_t w1[4], Hit& h) {
   // R-C2 source point
   const double u0 = uniform_from_word(w[0]), u1 = uniform_from_word(w[1]);
   const double u2 = uniform_from_word(w[2]), u3 = uniform_from_word(w[3]);
@@ -86,9 +99,7 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const PhiloxKe
   const double s2s = (P.slit2_z - 0.0) * inv_dz;
   const double xs2 = x0 + dx * s2s, ys2 = y0 + dy * s2s;
   const bool f_s2 = fabs(xs2) > P.slit2_hx || fabs(ys2) > P.slit2_hy;
-  // draws 4..7
-  uint32_t w1[4];
-  philox4x32_10(keys, id_lo, id_hi, 1u, exp_word, w1);
+  // draws 4..7 (Philox block 1, drawn by the classifier stage)
   const double u4 = uniform_from_word(w1[0]), u5 = uniform_from_word(w1[1]);
   const double u6 = uniform_from_word(w1[2]), u7 = uniform_from_word(w1[3]);
   const double lambda = P.lambda_min + u4 * P.dlam;

@@ -174,12 +174,40 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
   P.det_sx = (double)d.det_nx / d.det_xw; P.det_sy = (double)d.det_ny / d.det_yh;
   P.det_nxd = (double)d.det_nx; P.det_nyd = (double)d.det_ny;
   P.det_nx = d.det_nx; P.det_ny = d.det_ny;
+  P.s_cut = INFINITY;
   P.s1_int_ok = 0;
   if (d.slit1_z == 0.0) {
     // slit 1 in the source plane: xs = x0 + dx*0 = x0 exactly, so the test depends on draws 0, 1 only
     slit1_word_window(d.src_xw, P.slit1_hx, P.s1_lo[0], P.s1_hi[0]);
     slit1_word_window(d.src_yh, P.slit1_hy, P.s1_lo[1], P.s1_hi[1]);
     P.s1_int_ok = 1;
+  }
+  // Certain-miss classifier (geometry.cuh: surely_misses_detector).  Qualifies when, for EVERY ray the
+  // source can emit through slit 1, (i) slit 2 cannot cut (it is the focus rectangle or larger),
+  // (ii) the ray crosses the sample (beam envelope inside the sample's lateral extent).
+  {
+    const double m = 1.0e-6;
+    const double x0m = 0.5 * d.src_xw, y0m = 0.5 * d.src_yh, xf = 0.5 * d.focus_xw, yf = 0.5 * d.focus_yh;
+    const bool cyl = d.sample_shape == SAS_SAMPLE_CYL_Y;
+    const double depth = cyl ? d.sample_radius : 0.5 * d.sample_zd;
+    const double z_near = d.sample_z - depth, z_far = d.sample_z + depth;
+    auto envelope = [&](double a0, double af, double z) {  // max |coordinate| of the beam at z
+      const double slope = (af + a0) / d.focus_z;
+      return z <= d.focus_z ? std::max(a0, af) : af + (z - d.focus_z) * slope;
+    };
+    const double bx = std::max(envelope(x0m, xf, z_near), envelope(x0m, xf, z_far));
+    const double by = std::max(envelope(y0m, yf, z_near), envelope(y0m, yf, z_far));
+    const bool slit2_sure = d.focus_z == d.slit2_z && d.focus_xw <= d.slit2_xw && d.focus_yh <= d.slit2_yh;
+    const bool sample_sure = z_near > 0.0 && by <= 0.5 * d.sample_yh * (1.0 - m) &&
+                             bx <= (cyl ? d.sample_radius : 0.5 * d.sample_xw) * (1.0 - m);
+    const double d_min = (d.sample_z + d.det_dist) - z_far;
+    if (P.s1_int_ok && slit2_sure && sample_sure && d_min > 0.0) {
+      const double delta = std::atan(std::hypot(xf + x0m, yf + y0m) / d.focus_z);  // max tilt of d^ from z
+      const double r_diag = std::hypot(0.5 * d.det_xw, 0.5 * d.det_yh);
+      const double t_cut = (r_diag * (1.0 + m) + std::hypot(bx, by)) / d_min;
+      const double a_cut = (std::atan(t_cut) + delta) * (1.0 + m) + 1.0e-9;         // on 2 theta
+      if (a_cut < 3.0) P.s_cut = std::sin(0.5 * a_cut) * (1.0 + m);
+    }
   }
 }
 

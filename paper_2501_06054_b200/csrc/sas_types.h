@@ -29,6 +29,7 @@ struct ExpParams {
   double q_min, dq, qnorm;
   // detector (R-C9)
   double det_z, det_hw, det_hh, det_sx, det_sy, det_nxd, det_nyd;
+  double s_cut;  // classifier threshold on sin(theta); +inf when the instrument does not qualify
   // model scalars (R-C12)
   double norm;        // 1e8 * scale / <V>
   double background;

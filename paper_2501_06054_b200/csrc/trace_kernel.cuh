@@ -4,7 +4,9 @@
 // die at slit 1 and ~80 % of the rest miss the detector:
 //
 //   stage A  Philox block 0 + slit-1 test on the raw 32-bit draws      (every launched neutron)
-//   stage B  fp64 geometry: slits, sample chord, Q, detector pixel     (slit-1 survivors)
+//   stage B0 Philox block 1 + conservative "certain to miss the         (slit-1 survivors)
+//            detector" test on q lambda (geometry.cuh)
+//   stage B  fp64 geometry: slits, sample chord, Q, detector pixel     (survivors that may hit)
 //   stage C  model intensity I(Q) with the quadrature node loops,      (detected neutrons)
 //            weight, histogram update
 #pragma once
@@ -25,9 +27,12 @@ constexpr int MIN_BLOCKS_PER_SM = SAS_MIN_BLOCKS;
 constexpr int RING = 64;  // entries per warp queue (power of two, >= 63)
 
 struct WarpQueues {
-  // queue B: slit-1 survivors
+  // queue B: slit-1 survivors (Philox block 0)
   uint32_t b_id[RING];
   uint32_t b_w[4][RING];
+  // queue B2: survivors the classifier could not rule out (Philox blocks 0 and 1)
+  uint32_t b2_id[RING];
+  uint32_t b2_w[8][RING];
   // queue C: detected neutrons
   uint32_t c_id[RING];
   int32_t c_pixel[RING];
@@ -44,14 +49,18 @@ __host__ __device__ inline size_t trace_smem_bytes(int tab_len_max) {
          (size_t)WARPS_PER_BLOCK * sizeof(WarpQueues);
 }
 
-// adds the six packed 10-bit outcome fields of one lane to the global counters (index = status, with
-// detected (status 0) stored in slot 6 and statuses 1..5 in slots 1..5)
+// adds the seven packed 9-bit outcome fields of one lane to the global counters: field s = status s
+// (detected, status 0, goes to slot 6; statuses 1..5 to slots 1..5); field 6 = detector misses decided
+// by the classifier, slot 7
+constexpr int PK_BITS = 9;
+constexpr unsigned PK_FLUSH_CALLS = 500;  // < 2^9: one increment per lane per stage call
 __device__ __forceinline__ void flush_packed(unsigned long long* counters, unsigned long long pk) {
 #pragma unroll
-  for (int st = 0; st < 6; ++st) {
-    const unsigned v = (unsigned)(pk >> (10 * st)) & 1023u;
+  for (int f = 0; f < 7; ++f) {
+    const unsigned v = (unsigned)(pk >> (PK_BITS * f)) & ((1u << PK_BITS) - 1u);
     const unsigned tot = __reduce_add_sync(0xFFFFFFFFu, v);
-    if ((threadIdx.x & 31) == 0 && tot) atomicAdd(counters + (st == 0 ? 6 : st), (unsigned long long)tot);
+    const int slot = f == 0 ? 6 : (f == 6 ? 7 : f);
+    if ((threadIdx.x & 31) == 0 && tot) atomicAdd(counters + slot, (unsigned long long)tot);
   }
 }
 
@@ -70,8 +79,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
   const unsigned FULL = 0xFFFFFFFFu;
 
   // warp-uniform pipeline state
-  int headB = 0, cntB = 0, headC = 0, cntC = 0;
-  // outcome counters: every lane packs its own six 10-bit fields (status s -> bits [10 s, 10 s + 10));
+  int headB = 0, cntB = 0, headB2 = 0, cntB2 = 0, headC = 0, cntC = 0;
+  // outcome counters: every lane packs its own seven 9-bit fields (flush_packed);
   // flushed to the global counters before a field can overflow
   unsigned long long pk = 0;
   unsigned pk_calls = 0;
@@ -131,7 +140,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
     // ------------------------------------------------------------------ the pump
     for (;;) {
       const bool rows_left = row < row_end;
-      if (cntC >= 32 || (drain && cntB == 0 && cntC > 0)) {
+      if (cntC >= 32 || (drain && cntB == 0 && cntB2 == 0 && cntC > 0)) {
         // ---------------- stage C: model + weight + histogram
         const int n = cntC < 32 ? cntC : 32;
         const bool act = lane < n;
@@ -160,8 +169,40 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         }
         continue;
       }
-      if (cntB >= 32 || (drain && cntB > 0)) {
+      if (cntB2 >= 32 || (drain && cntB == 0 && cntB2 > 0)) {
         // ---------------- stage B: fp64 geometry
+        const int n = cntB2 < 32 ? cntB2 : 32;
+        const bool act = lane < n;
+        const int slot = (headB2 + lane) & (RING - 1);
+        uint32_t idoff = 0, w[4] = {0, 0, 0, 0}, w1[4] = {0, 0, 0, 0};
+        if (act) {
+          idoff = wq.b2_id[slot];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { w[i] = wq.b2_w[i][slot]; w1[i] = wq.b2_w[4 + i][slot]; }
+        }
+        __syncwarp();
+        headB2 = (headB2 + n) & (RING - 1);
+        cntB2 -= n;
+        int st = -1;
+        Hit h;
+        if (act) {
+          st = trace_geometry(P, w, w1, h);
+          if (DUMP && a.d_q != nullptr) a.d_q[idoff] = h.q;
+          pk += 1ull << (PK_BITS * st);
+        }
+        if (++pk_calls == PK_FLUSH_CALLS) { flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
+        const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
+        if (st == ST_DETECTED) {
+          const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
+          wq.c_id[s2] = idoff; wq.c_pixel[s2] = h.pixel; wq.c_G[s2] = h.G;
+          wq.c_Q[0][s2] = h.Qx; wq.c_Q[1][s2] = h.Qy; wq.c_Q[2][s2] = h.Qz;
+        }
+        cntC += __popc(m);
+        __syncwarp();
+        continue;
+      }
+      if (cntB >= 32 || (drain && cntB > 0)) {
+        // ---------------- stage B0: Philox block 1 + certain-miss classifier
         const int n = cntB < 32 ? cntB : 32;
         const bool act = lane < n;
         const int slot = (headB + lane) & (RING - 1);
@@ -173,22 +214,25 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         __syncwarp();
         headB = (headB + n) & (RING - 1);
         cntB -= n;
-        int st = -1;
-        Hit h;
-        if (act) {
-          const uint64_t id = a.first_id + idoff;
-          st = trace_geometry(P, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, w, h);
-          if (DUMP && a.d_q != nullptr) a.d_q[idoff] = h.q;
+        const uint64_t id = a.first_id + idoff;
+        uint32_t w1[4];
+        philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 1u, exp_word, w1);
+        double q;
+        const bool sure = surely_misses_detector(P, w1, q);
+        if (act && sure) {
+          pk += (1ull << (PK_BITS * ST_MISS_DET)) + (1ull << (PK_BITS * 6));
+          if (DUMP && a.d_q != nullptr) a.d_q[idoff] = q;
         }
-        if (act) pk += 1ull << (10 * st);
-        if (++pk_calls == 1000u) { flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
-        const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
-        if (st == ST_DETECTED) {
-          const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
-          wq.c_id[s2] = idoff; wq.c_pixel[s2] = h.pixel; wq.c_G[s2] = h.G;
-          wq.c_Q[0][s2] = h.Qx; wq.c_Q[1][s2] = h.Qy; wq.c_Q[2][s2] = h.Qz;
+        if (++pk_calls == PK_FLUSH_CALLS) { flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
+        const bool keep = act && !sure;
+        const unsigned m = __ballot_sync(FULL, keep);
+        if (keep) {
+          const int s2 = (headB2 + cntB2 + __popc(m & lt_mask)) & (RING - 1);
+          wq.b2_id[s2] = idoff;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { wq.b2_w[i][s2] = w[i]; wq.b2_w[4 + i][s2] = w1[i]; }
         }
-        cntC += __popc(m);
+        cntB2 += __popc(m);
         __syncwarp();
         continue;
       }

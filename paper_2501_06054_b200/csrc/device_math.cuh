@@ -56,22 +56,28 @@ __device__ __forceinline__ float horner(const float (&c)[N], float t) {
 // ---------------------------------------------------------------- sin/cos
 // fp32: three-step Cody-Waite reduction by pi/2 with FMAs, kernels on [-pi/4, pi/4].
 // Valid for |x| < ~1e5 (k exact in fp32); the tracer's arguments are q*size < ~1e3.
-__device__ __forceinline__ void sincos_r(float x, float& s, float& c) {
-  const float kf = rintf(x * 0.636619772f);
-  float r = fmaf(kf, -1.57079625129699707031e+00f, x);
+// k = nearest integer to x*inv_period is taken from the mantissa of x*inv_period + 1.5*2^23 (no
+// FRND/F2I on the XU pipe); |x*inv_period| < 2^22.
+#define SAS_ROUND_MAGIC 12582912.0f
+__device__ __forceinline__ void sincos_core(float x, float lo, float& s, float& c) {
+  const float t = fmaf(x, 0.636619772f, SAS_ROUND_MAGIC);
+  const int kb = __float_as_int(t);
+  const float kf = t - SAS_ROUND_MAGIC;
+  float r = fmaf(kf, -1.57079625129699707031e+00f, x);  // exact: the product has <= 32 significant bits
   r = fmaf(kf, -7.54978941586159635335e-08f, r);
-  r = fmaf(kf, -5.39030252995776476554e-15f, r);
-  const int k = (int)kf;
+  r = fmaf(kf, -5.39030252995776476554e-15f, r) + lo;
   const float z = r * r;
   const float SP[SAS_SIN_POLY_N] = SAS_SIN_POLY;
   const float CP[SAS_COS_POLY_N] = SAS_COS_POLY;
   const float ps = fmaf(r * z, horner(SP, z), r);
   const float pc = fmaf(z, horner(CP, z), 1.0f);
-  float ss = (k & 1) ? pc : ps;
-  float cc = (k & 1) ? ps : pc;
-  s = (k & 2) ? -ss : ss;
-  c = ((k + 1) & 2) ? -cc : cc;
+  const bool odd = (kb & 1) != 0;
+  const float ss = odd ? pc : ps;
+  const float cc = odd ? ps : pc;
+  s = __int_as_float(__float_as_int(ss) ^ ((kb << 30) & 0x80000000));        // k mod 4 in {2,3}: -sin
+  c = __int_as_float(__float_as_int(cc) ^ (((kb + 1) << 30) & 0x80000000));  // k mod 4 in {1,2}: -cos
 }
+__device__ __forceinline__ void sincos_r(float x, float& s, float& c) { sincos_core(x, 0.0f, s, c); }
 __device__ __forceinline__ void sincos_r(double x, double& s, double& c) { sincos(x, &s, &c); }
 
 // fp32 reciprocal / square root: one MUFU each (~1 ulp), no IEEE fix-up path
@@ -116,22 +122,7 @@ __device__ __forceinline__ double ph_val(Phase<double> p) { return p.v; }
 __device__ __forceinline__ float ph_val(Phase<float> p) { return p.hi; }
 
 __device__ __forceinline__ void sincos_ph(Phase<double> p, double& s, double& c) { sincos(p.v, &s, &c); }
-__device__ __forceinline__ void sincos_ph(Phase<float> p, float& s, float& c) {
-  const float kf = rintf(p.hi * 0.636619772f);
-  float r = fmaf(kf, -1.57079625129699707031e+00f, p.hi);  // exact: the product has <= 32 significant bits
-  r = fmaf(kf, -7.54978941586159635335e-08f, r);
-  r = fmaf(kf, -5.39030252995776476554e-15f, r) + p.lo;
-  const int k = (int)kf;
-  const float z = r * r;
-  const float SP[SAS_SIN_POLY_N] = SAS_SIN_POLY;
-  const float CP[SAS_COS_POLY_N] = SAS_COS_POLY;
-  const float ps = fmaf(r * z, horner(SP, z), r);
-  const float pc = fmaf(z, horner(CP, z), 1.0f);
-  const float ss = (k & 1) ? pc : ps;
-  const float cc = (k & 1) ? ps : pc;
-  s = (k & 2) ? -ss : ss;
-  c = ((k + 1) & 2) ? -cc : cc;
-}
+__device__ __forceinline__ void sincos_ph(Phase<float> p, float& s, float& c) { sincos_core(p.hi, p.lo, s, c); }
 
 // sin/cos of 2 pi u, u in (0,1), fp64, ~1e-13: exact reduction by quarter turns, Taylor kernels.
 // Used by the fp32 model path for the per-neutron random orientation (the fp64 path calls sincos()).
@@ -191,19 +182,34 @@ __device__ __forceinline__ double sphere_phi(double u) {
 // ---------------------------------------------------------------- sinc
 // sin(x) alone: reduction by pi, one odd polynomial on [-pi/2, pi/2], sign from the parity of k.
 __device__ __forceinline__ float sin_reduced_pi(float x, float lo) {
-  const float kf = rintf(x * 0.318309886f);
+  const float t = fmaf(x, 0.318309886f, SAS_ROUND_MAGIC);
+  const int kb = __float_as_int(t);
+  const float kf = t - SAS_ROUND_MAGIC;
   float r = fmaf(kf, -3.14159250259399414062e+00f, x);
   r = fmaf(kf, -1.50995788317231927067e-07f, r);
   r = fmaf(kf, -1.07806050599155295311e-14f, r) + lo;
   const float z = r * r;
   const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
   const float ps = fmaf(r * z, horner(SP, z), r);
-  const int k = (int)kf;
-  return __int_as_float(__float_as_int(ps) ^ (int)((unsigned)k << 31));
+  return __int_as_float(__float_as_int(ps) ^ (kb << 31));
+}
+// sin(x)/x: for tiny x the polynomial returns x itself, so the quotient is 1 to rounding; only the
+// exact x = 0 gives 0 * inf = NaN, replaced by 1 with one select (no branch in the node loops)
+__device__ __forceinline__ float sinc_from(float s, float x) {
+  const float r = s * rcp_fast(x);
+  return (r != r) ? 1.0f : r;
 }
 __device__ __forceinline__ float sinc_r(float x) {
-  const float s = sin_reduced_pi(x, 0.0f);
-  return (fabsf(x) < 1e-4f) ? 1.0f : s * rcp_fast(x);
+  const float t = fmaf(x, 0.318309886f, SAS_ROUND_MAGIC);
+  const int kb = __float_as_int(t);
+  const float kf = t - SAS_ROUND_MAGIC;
+  float r = fmaf(kf, -3.14159250259399414062e+00f, x);
+  r = fmaf(kf, -1.50995788317231927067e-07f, r);
+  r = fmaf(kf, -1.07806050599155295311e-14f, r);
+  const float z = r * r;
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  const float ps = fmaf(r * z, horner(SP, z), r);
+  return sinc_from(__int_as_float(__float_as_int(ps) ^ (kb << 31)), x);
 }
 __device__ __forceinline__ double sinc_r(double x) { return (x == 0.0) ? 1.0 : sin(x) / x; }
 
@@ -232,9 +238,16 @@ __device__ __forceinline__ float lambda1_x2(float x2) {
   }
   return lambda1_asym(sqrt_fast(x2), 0.0f);
 }
+// caller guarantees x^2 <= 64 (the host checked q_max * R_max for the experiment)
+__device__ __forceinline__ float lambda1_x2_small(float x2) {
+  const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+  return horner(LA, fmaf(x2, 0.03125f, -1.0f));
+}
+__device__ __forceinline__ double lambda1_x2_small(double x2);
 __device__ __forceinline__ float lambda1_r(float x) { return lambda1_x2(x * x); }
 __device__ __forceinline__ double lambda1_r(double x) { return (x == 0.0) ? 1.0 : (2.0 * j1(x)) / x; }
 __device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(x2)); }
+__device__ __forceinline__ double lambda1_x2_small(double x2) { return lambda1_r(sqrt(x2)); }
 
 // ---------------------------------------------------------------- the same functions of a Phase
 __device__ __forceinline__ float sphere_phi_ph(Phase<float> p) {
@@ -252,10 +265,7 @@ __device__ __forceinline__ float sphere_phi_ph(Phase<float> p) {
 }
 __device__ __forceinline__ double sphere_phi_ph(Phase<double> p) { return sphere_phi(p.v); }
 
-__device__ __forceinline__ float sinc_ph(Phase<float> p) {
-  const float s = sin_reduced_pi(p.hi, p.lo);
-  return (fabsf(p.hi) < 1e-4f) ? 1.0f : s * rcp_fast(p.hi);
-}
+__device__ __forceinline__ float sinc_ph(Phase<float> p) { return sinc_from(sin_reduced_pi(p.hi, p.lo), p.hi); }
 __device__ __forceinline__ double sinc_ph(Phase<double> p) { return sinc_r(p.v); }
 
 __device__ __forceinline__ float lambda1_ph(Phase<float> p) {

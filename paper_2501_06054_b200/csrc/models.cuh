@@ -122,16 +122,27 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
           const Real Ai = fma_r(qA, sth, qC * cth);
           Real row = 0;
           if (mono) {
+            // lam_small: the host checked (q_max R)^2 <= 64, so Lambda needs no range test
+            if (P.lam_small) {
 #pragma unroll 2
-            for (int j = 0; j < P.n_ph; ++j) {
-              const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
-              const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
-              Real r2 = fma_r(-qc, qc, q2);
-              r2 = r2 > (Real)0 ? r2 : (Real)0;
-              const Real sc = sinc_r(qc * hL0);
-              const Real la = lambda1_x2(r2 * R20);
-              const Real f = sc * la;
-              row = fma_r(wph, f * f, row);
+              for (int j = 0; j < P.n_ph; ++j) {
+                const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
+                const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
+                Real r2 = fma_r(-qc, qc, q2);
+                r2 = r2 > (Real)0 ? r2 : (Real)0;
+                const Real f = sinc_r(qc * hL0) * lambda1_x2_small(r2 * R20);
+                row = fma_r(wph, f * f, row);
+              }
+            } else {
+#pragma unroll 2
+              for (int j = 0; j < P.n_ph; ++j) {
+                const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
+                const Real qc = fma_r(cph, Ai, qB * sph);
+                Real r2 = fma_r(-qc, qc, q2);
+                r2 = r2 > (Real)0 ? r2 : (Real)0;
+                const Real f = sinc_r(qc * hL0) * lambda1_x2(r2 * R20);
+                row = fma_r(wph, f * f, row);
+              }
             }
             row *= cL0 * cR0;
           } else {

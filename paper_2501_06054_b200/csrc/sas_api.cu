@@ -369,6 +369,14 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
     sas_model_desc m = models[e];
     m.precision = c->precision;
     fill_model(m, P, c->h_tab);
+    P.lam_small = 0;
+    if (m.model == SAS_CYLINDER) {
+      // largest Lambda argument this experiment can produce: |Q| <= q_max, radius <= largest node
+      double r_max = 0.0;
+      for (int a = 0; a < P.n_a; ++a) r_max = std::max(r_max, c->h_tab[P.tab_off + a * TA_W] + c->h_tab[P.tab_off + a * TA_W + 1]);
+      const double x_max = c->instr[e].q_max * r_max * 1.001;
+      P.lam_small = (x_max * x_max <= 64.0) ? 1 : 0;
+    }
     c->tab_len_max = std::max(c->tab_len_max, P.tab_len);
   }
   const size_t tb = c->h_tab.size() * sizeof(double);

@@ -45,7 +45,7 @@ struct ExpParams {
   int32_t model, orient_kind, sq_kind;
   int32_t n_a, n_b, n_th, n_ph;
   int32_t tab_off, tab_len;  // in doubles, inside the table pool
-  int32_t pad_[1];
+  int32_t lam_small;  // cylinder: (q_max * R_max)^2 <= 64, Lambda stays on its polynomial range
 };
 static_assert(sizeof(ExpParams) % 8 == 0, "ExpParams must be a multiple of 8 bytes");
 

@@ -49,6 +49,7 @@ struct sas_ctx {
   bool own_stream = true;
   // bookkeeping
   uint64_t n_launches = 0;
+  uint64_t launched = 0;  // neutrons traced into the detector since the last reset (counters[0])
   int last_grid = 0, last_block = 0, last_smem = 0;
   std::vector<cudaEvent_t> ev0, ev1;
   uint64_t n_timed = 0;
@@ -338,6 +339,7 @@ sas_status alloc_common(sas_ctx* c) {
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_counts, 0, nh * sizeof(unsigned long long), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  c->launched = 0;
   return SAS_OK;
 }
 
@@ -458,6 +460,7 @@ sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t
     a.n_per_exp = (uint32_t)std::min<uint64_t>(chunk, n_each - done);
     sas_status st = c->precision == SAS_FP64 ? launch<double, false>(c, a) : launch<float, false>(c, a);
     if (st != SAS_OK) return st;
+    c->launched += (uint64_t)a.n_per_exp * a.n_exp;
   }
   return SAS_OK;
 }
@@ -559,6 +562,7 @@ sas_status sas_bind_buffers(sas_ctx* c, void* d_sum_p, void* d_sum_p2, void* d_c
     CUDA_TRY(c, cudaMemcpyAsync(c->d_exps, c->h_exps.data(), (size_t)c->n_exp * sizeof(ExpParams), cudaMemcpyHostToDevice, c->stream));
   }
   CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  c->launched = 0;
   return SAS_OK;
 }
 
@@ -624,6 +628,12 @@ sas_status sas_get_counters(sas_ctx* c, uint64_t out[8]) {
   if (!c || !out) return SAS_EINVAL;
   CUDA_TRY(c, cudaMemcpyAsync(out, c->d_counters, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  // the kernel counts the outcomes it decides in its queued stages (slots 2..7); launched is the host's
+  // own sum of the traced ranges and every neutron has exactly one outcome, so slit 1 takes the rest
+  out[0] = c->launched;
+  uint64_t other = 0;
+  for (int i = 2; i <= 6; ++i) other += out[i];
+  out[1] = c->launched - other;
   return SAS_OK;
 }
 
@@ -634,6 +644,7 @@ sas_status sas_reset_detector(sas_ctx* c) {
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_counts, 0, nh * sizeof(unsigned long long), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  c->launched = 0;
   return SAS_OK;
 }
 

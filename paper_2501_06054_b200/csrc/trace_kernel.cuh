@@ -16,10 +16,10 @@
 namespace sas {
 
 #ifndef SAS_BLOCK_THREADS
-#define SAS_BLOCK_THREADS 256
+#define SAS_BLOCK_THREADS 128
 #endif
 #ifndef SAS_MIN_BLOCKS
-#define SAS_MIN_BLOCKS 3
+#define SAS_MIN_BLOCKS 5
 #endif
 constexpr int BLOCK_THREADS = SAS_BLOCK_THREADS;
 constexpr int WARPS_PER_BLOCK = BLOCK_THREADS / 32;
@@ -38,7 +38,6 @@ struct WarpQueues {
   int32_t c_pixel[RING];
   double c_G[RING];
   double c_Q[3][RING];
-  unsigned long long n_launched;  // ids this warp has drawn (lane 0 updates it once per work item)
 };
 
 __host__ __device__ inline size_t round16(size_t x) { return (x + 15) & ~(size_t)15; }
@@ -84,8 +83,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
   // flushed to the global counters before a field can overflow
   unsigned long long pk = 0;
   unsigned pk_calls = 0;
-  unsigned n_passA = 0;  // survivors of the integer slit-1 test (warp-uniform)
-  if (lane == 0) wq.n_launched = 0;
 
   int cur_exp = -1;
   uint32_t exp_word = 0;
@@ -129,12 +126,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
       cnt_ids = min(a.item_ids, a.n_per_exp - off0);
       row = warp;
       row_end = (cnt_ids + 31u) >> 5;
-      if (lane == 0) {
-        // ids of this item that fall to this warp: rows warp, warp+8, ... ; the last row may be ragged
-        unsigned long long mine = 0;
-        for (uint32_t r = warp; r < row_end; r += WARPS_PER_BLOCK) mine += min(32u, cnt_ids - (r << 5));
-        wq.n_launched += mine;
-      }
     }
 
     // ------------------------------------------------------------------ the pump
@@ -257,7 +248,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
             wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
           }
           cntB += np;
-          n_passA += np;
           row += WARPS_PER_BLOCK;
         } while (row < row_end && cntB < 32);
         __syncwarp();
@@ -267,16 +257,9 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
     }
   }
 
-  if (!DUMP) {
-    flush_packed(a.counters, pk);
-    if (lane == 0) {
-      const unsigned long long nl = wq.n_launched;
-      atomicAdd(a.counters + 0, nl);
-      // every neutron that stage A did not queue died at the integer slit-1 test (without the prefilter
-      // stage A queues every valid id, so the difference is zero for those experiments)
-      atomicAdd(a.counters + 1, nl - (unsigned long long)n_passA);
-    }
-  }
+  // counters[0] (launched) is known to the host; counters[1] (died at slit 1) is what is left of it after
+  // every other outcome (sas_get_counters): a neutron that the integer slit-1 test drops is never queued
+  if (!DUMP) flush_packed(a.counters, pk);
 }
 
 }  // namespace sas

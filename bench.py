@@ -182,7 +182,9 @@ def bench_config(torch, S, cfg_index, steps, warmup, rank, world, flush, with_e2
             merge_detectors([tr.sum_p, tr.sum_p2, tr.counts], dst=0)
 
     total_ms, launches = time_steps(torch, tr, do_step, steps, warmup, flush)
-    kernel_ms, n_timed = tr.kernel_time_ms(reset=True)
+    kernel_ms, n_timed = tr.kernel_time_ms(reset=True)   # average per launch; a step may take several
+    launches_per_step = max(1, int(n_timed) // steps)    # launches (one per kernel variant in a batch)
+    kernel_ms *= launches_per_step                        # trace-kernel time per step
     info = tr.launch_info()
     cnt = tr.counters().astype(np.float64)
     ms_per_step = total_ms / steps
@@ -306,7 +308,8 @@ def main():
         tr.reset()
         tr.kernel_time_ms(reset=True)
         tr.trace_range(first, 10**9, c0["seed"])
-        ms, _ = tr.kernel_time_ms(reset=True)
+        ms, nt = tr.kernel_time_ms(reset=True)
+        ms *= nt
         from paper_2501_06054_b200 import roofline as R
         cnt = tr.counters().astype(np.float64)
         rl = R.roofline(1e9 / (ms * 1e-3), 1 - cnt[1] / cnt[0], cnt[6] / cnt[0], "sphere_fp64", 1)

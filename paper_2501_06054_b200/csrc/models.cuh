@@ -40,20 +40,23 @@ __device__ __forceinline__ Real sq(Real x) { return x * x; }
 //  triaxial            ta = {x_hi, x_lo, w_a (drho V_a)^2}
 //  core-shell triaxial ta = {x_hi, x_lo, (drho_c-drho_s) Vc_a, w_a}; tb = {t_b, w_b, t_b^2};
 //                      tab = {drho_s Vt_ab, 2 x_a t_b}
-template <typename Real>
+// V is the kernel variant (sas_types.h): the model, with the cylinder split into its Gaussian tilt
+// quadrature and its fixed / per-neutron random orientation forms.  One kernel is compiled per variant so
+// that a launch carries the code of its own model only (instruction-cache footprint).
+template <typename Real, int V>
 __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* tab_base, const PhiloxKeys& keys,
                                                uint32_t id_lo, uint32_t id_hi, uint32_t exp_word, double Qx,
                                                double Qy, double Qz) {
-  if (P.model == 5) return (Real)P.flat_I;
+  if (V == V_FLAT) return (Real)P.flat_I;
   const Tables<Real> T = table_views(tab_base, P);
-  const int model = P.model;
+  constexpr int model = (V == V_CYL_QUAD) ? 2 : V;
   // |Q| and the projections of Q on the particle axes (Eq. 6) in fp64: they feed the phases
   const double q2d = fma(Qx, Qx, fma(Qy, Qy, Qz * Qz));
   const double qd = sqrt(q2d);
   double qAd = 0, qBd = 0, qCd = 0;
   if (model >= 2) {
     double A[3], B[3], C[3];
-    if (P.orient_kind == 2) {
+    if (V != V_CYL_QUAD && P.orient_kind == 2) {
       // R-A3: one isotropic random orientation per neutron, draws 8, 9, 10
       uint32_t w2[4];
       philox4x32_10(keys, id_lo, id_hi, 2u, exp_word, w2);
@@ -111,7 +114,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
       }
     } break;
     case 2: {  // cylinder: separable in (R, L) for a given axis direction
-      if (P.orient_kind == 1) {
+      if (V == V_CYL_QUAD) {
         // Gaussian tilt quadrature (R-A11): n_th x n_ph axis directions about the mean axis, plain Real.
         // Lambda is evaluated from x^2 = R^2 (q^2 - qc^2): no square root below x = 8.
         const Real qA = (Real)qAd, qB = (Real)qBd, qC = (Real)qCd;

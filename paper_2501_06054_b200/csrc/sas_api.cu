@@ -45,6 +45,10 @@ struct sas_ctx {
   bool own_hist = true;
   unsigned long long* d_counters = nullptr;
   unsigned int* d_work = nullptr;
+  // experiments grouped by kernel variant: one launch per non-empty group (ids concatenated on the device)
+  std::vector<uint32_t> group_ids[N_VARIANTS];
+  size_t group_off[N_VARIANTS] = {};
+  uint32_t* d_exp_ids = nullptr;
   cudaStream_t stream = nullptr;
   bool own_stream = true;
   // bookkeeping
@@ -334,6 +338,7 @@ sas_status alloc_common(sas_ctx* c) {
   c->own_hist = true;
   CUDA_TRY(c, cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)));
   CUDA_TRY(c, cudaMalloc(&c->d_work, sizeof(unsigned int)));
+  CUDA_TRY(c, cudaMalloc(&c->d_exp_ids, (size_t)c->n_exp * sizeof(uint32_t)));
   CUDA_TRY(c, cudaMalloc(&c->d_exps, (size_t)c->n_exp * sizeof(ExpParams)));
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
@@ -381,6 +386,19 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
     }
     c->tab_len_max = std::max(c->tab_len_max, P.tab_len);
   }
+  // kernel variant of every experiment, and the launch groups
+  for (auto& g : c->group_ids) g.clear();
+  for (uint32_t e = 0; e < c->n_exp; ++e) {
+    const ExpParams& P = c->h_exps[e];
+    const int v = (P.model == SAS_CYLINDER && P.orient_kind == SAS_ORIENT_GAUSS_QUAD) ? (int)V_CYL_QUAD : P.model;
+    c->group_ids[v].push_back(e);
+  }
+  std::vector<uint32_t> ids;
+  for (int v = 0; v < N_VARIANTS; ++v) {
+    c->group_off[v] = ids.size();
+    ids.insert(ids.end(), c->group_ids[v].begin(), c->group_ids[v].end());
+  }
+  CUDA_TRY(c, cudaMemcpy(c->d_exp_ids, ids.data(), ids.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
   const size_t tb = c->h_tab.size() * sizeof(double);
   if (tb > c->d_tab_cap) {
     if (c->d_tab) { CUDA_TRY(c, cudaStreamSynchronize(c->stream)); CUDA_TRY(c, cudaFree(c->d_tab)); c->d_tab = nullptr; }
@@ -396,10 +414,11 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   return SAS_OK;
 }
 
-template <typename Real, bool DUMP>
+template <typename Real, int V>
 sas_status launch(sas_ctx* c, KernelArgs& a) {
+  const bool DUMP = a.d_pixel != nullptr;
   const size_t smem = trace_smem_bytes<Real>(c->tab_len_max);
-  auto kern = trace_kernel<Real, DUMP>;
+  auto kern = trace_kernel<Real, V>;
   if (smem > 227 * 1024) return fail(c, SAS_EINVAL, "quadrature tables do not fit in shared memory");
   CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int bps = 0;
@@ -441,6 +460,32 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   return SAS_OK;
 }
 
+// one launch of the kernel compiled for variant v over the experiments of that group
+template <typename Real>
+sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v) {
+  a.exp_ids = c->d_exp_ids + c->group_off[v];
+  a.n_exp = (uint32_t)c->group_ids[v].size();
+  switch (v) {
+    case V_SPHERE: return launch<Real, V_SPHERE>(c, a);
+    case V_CS_SPHERE: return launch<Real, V_CS_SPHERE>(c, a);
+    case V_CYL: return launch<Real, V_CYL>(c, a);
+    case V_TRIAX: return launch<Real, V_TRIAX>(c, a);
+    case V_CS_TRIAX: return launch<Real, V_CS_TRIAX>(c, a);
+    case V_FLAT: return launch<Real, V_FLAT>(c, a);
+    case V_CYL_QUAD: return launch<Real, V_CYL_QUAD>(c, a);
+    default: return fail(c, SAS_EINVAL, "unknown kernel variant");
+  }
+}
+
+sas_status launch_groups(sas_ctx* c, KernelArgs& a) {
+  for (int v = 0; v < N_VARIANTS; ++v) {
+    if (c->group_ids[v].empty()) continue;
+    sas_status st = c->precision == SAS_FP64 ? launch_variant<double>(c, a, v) : launch_variant<float>(c, a, v);
+    if (st != SAS_OK) return st;
+  }
+  return SAS_OK;
+}
+
 sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t seed) {
   if (!c) return SAS_EINVAL;
   if (!c->model_set) return fail(c, SAS_ESTATE, "sas_set_model must precede tracing");
@@ -458,9 +503,9 @@ sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t
   for (uint64_t done = 0; done < n_each; done += chunk) {
     a.first_id = first_id + done;
     a.n_per_exp = (uint32_t)std::min<uint64_t>(chunk, n_each - done);
-    sas_status st = c->precision == SAS_FP64 ? launch<double, false>(c, a) : launch<float, false>(c, a);
+    sas_status st = launch_groups(c, a);
     if (st != SAS_OK) return st;
-    c->launched += (uint64_t)a.n_per_exp * a.n_exp;
+    c->launched += (uint64_t)a.n_per_exp * c->n_exp;
   }
   return SAS_OK;
 }
@@ -471,7 +516,7 @@ void destroy_ctx(sas_ctx* c) {
   for (auto e : c->ev0) cudaEventDestroy(e);
   for (auto e : c->ev1) cudaEventDestroy(e);
   if (c->own_hist) { cudaFree(c->d_sum_p); cudaFree(c->d_sum_p2); cudaFree(c->d_counts); }
-  cudaFree(c->d_counters); cudaFree(c->d_work); cudaFree(c->d_exps); cudaFree(c->d_tab);
+  cudaFree(c->d_counters); cudaFree(c->d_work); cudaFree(c->d_exp_ids); cudaFree(c->d_exps); cudaFree(c->d_tab);
   if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
   delete c;
 }
@@ -611,7 +656,7 @@ sas_status sas_trace_dump(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t se
   CUDA_TRY(c, cudaMemsetAsync(d_pixel, 0xFF, n * sizeof(int32_t), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(d_weight, 0, n * sizeof(double), c->stream));
   if (d_q) CUDA_TRY(c, cudaMemsetAsync(d_q, 0, n * sizeof(double), c->stream));
-  return c->precision == SAS_FP64 ? launch<double, true>(c, a) : launch<float, true>(c, a);
+  return launch_groups(c, a);
 }
 
 sas_status sas_read_detector(sas_ctx* c, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts) {

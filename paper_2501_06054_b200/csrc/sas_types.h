@@ -8,6 +8,9 @@ namespace sas {
 
 enum : int { ST_DETECTED = 0, ST_SLIT1 = 1, ST_SLIT2 = 2, ST_MISS_SAMPLE = 3, ST_UNREACHABLE = 4, ST_MISS_DET = 5 };
 
+// kernel variants: one trace kernel is compiled per model form (models.cuh: eval_intensity)
+enum : int { V_SPHERE = 0, V_CS_SPHERE = 1, V_CYL = 2, V_TRIAX = 3, V_CS_TRIAX = 4, V_FLAT = 5, V_CYL_QUAD = 6, N_VARIANTS = 7 };
+
 // table record widths (in Reals)
 constexpr int TA_W = 4;   // per node of polydisperse axis 0
 constexpr int TB_W = 4;   // per node of polydisperse axis 1
@@ -51,6 +54,7 @@ static_assert(sizeof(ExpParams) % 8 == 0, "ExpParams must be a multiple of 8 byt
 
 struct KernelArgs {
   const ExpParams* exps;
+  const uint32_t* exp_ids;       // experiments of this launch (one launch per kernel variant), [n_exp]
   const double* tab_pool;
   double* sum_p;
   double* sum_p2;
@@ -64,7 +68,7 @@ struct KernelArgs {
   uint64_t first_id;       // id of offset 0
   uint32_t n_per_exp;      // ids per experiment in this launch (< 2^32)
   uint32_t n_exp;
-  uint32_t exp_base;       // Philox counter word 3 of experiment 0
+  uint32_t exp_base;       // Philox counter word 3 of experiment index 0
   uint32_t item_ids;       // ids per work item (multiple of 32)
   uint32_t items_per_exp;
   uint32_t n_items;

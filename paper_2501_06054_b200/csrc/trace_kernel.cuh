@@ -63,7 +63,7 @@ __device__ __forceinline__ void flush_packed(unsigned long long* counters, unsig
   }
 }
 
-template <typename Real, bool DUMP>
+template <typename Real, int V>
 __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel(const __grid_constant__ KernelArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned int s_item;
@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
   const int warp = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
   const unsigned FULL = 0xFFFFFFFFu;
+  const bool DUMP = a.d_pixel != nullptr;  // parity hook: per-neutron outputs instead of the histogram
 
   // warp-uniform pipeline state
   int headB = 0, cntB = 0, headB2 = 0, cntB2 = 0, headC = 0, cntC = 0;
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
       item = s_item;
     }
     const bool have = item < a.n_items;
-    const int e = have ? (int)(item / a.items_per_exp) : -1;
+    const int e = have ? (int)a.exp_ids[item / a.items_per_exp] : -1;
     const bool drain = (e != cur_exp) && (cur_exp >= 0) && !replay;
     uint32_t row = 0, row_end = 0, off0 = 0, cnt_ids = 0;
     if (drain) {
@@ -146,7 +147,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         cntC -= n;
         if (act) {
           const uint64_t id = a.first_id + idoff;
-          const Real I = eval_intensity<Real>(P, tab, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
+          const Real I = eval_intensity<Real, V>(P, tab, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
           const double p = G * (double)I;
           if (DUMP) {
             a.d_pixel[idoff] = pixel;
@@ -181,7 +182,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
           if (DUMP && a.d_q != nullptr) a.d_q[idoff] = h.q;
           pk += 1ull << (PK_BITS * st);
         }
-        if (++pk_calls == PK_FLUSH_CALLS) { flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
+        if (++pk_calls == PK_FLUSH_CALLS) { if (!DUMP) flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
         const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
         if (st == ST_DETECTED) {
           const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
@@ -214,7 +215,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
           pk += (1ull << (PK_BITS * ST_MISS_DET)) + (1ull << (PK_BITS * 6));
           if (DUMP && a.d_q != nullptr) a.d_q[idoff] = q;
         }
-        if (++pk_calls == PK_FLUSH_CALLS) { flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
+        if (++pk_calls == PK_FLUSH_CALLS) { if (!DUMP) flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
         const bool keep = act && !sure;
         const unsigned m = __ballot_sync(FULL, keep);
         if (keep) {

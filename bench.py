@@ -201,13 +201,15 @@ def bench_config(torch, S, cfg_index, steps, warmup, rank, world, flush, with_e2
         # mixed batch: weigh the per-detected cost of the two model families equally (half each)
         rl = None
         for k, n in ks.items():
-            r = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n)
+            r = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n,
+                           workload=c["name"])
             rl = r if rl is None else {**rl, "achieved": 0.5 * (rl["achieved"] + r["achieved"]),
                                        "frac": 0.5 * (rl["frac"] + r["frac"])}
         out["roofline"] = rl
     else:
         k, n = model_key_and_nodes(c["model"])
-        out["roofline"] = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n)
+        out["roofline"] = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n,
+                                     workload=c["name"])
     e2e = None
     if with_e2e and not batch:
         # the call a user makes, host buffers in and out, every step

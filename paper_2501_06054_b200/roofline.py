@@ -43,6 +43,15 @@ MODEL_COST = {
 }
 
 
+# DRAM traffic of one trace-kernel launch, dram__bytes_read.sum + dram__bytes_write.sum of the
+# `ncu --set full` captures summarised in profiles/r1_ncu_c<k>.md (bytes per launch; c4: the first of its
+# two launches, the 512 sphere experiments).  The algorithmic traffic is the histograms only.
+NCU_DRAM_BYTES = {
+    "c0_sphere_fp64": 698_624, "c1_polysphere_py": 2_006_784, "c2_oriented_cylinder": 2_111_744,
+    "c3_coreshell_triaxial": 6_835_200, "c4_batch": 202_950_400 + 152_935_680,
+}
+
+
 def smsp_clocks_per_neutron(frac_survive: float, frac_detect: float, model_key: str, nodes: int):
     """Algorithmic SMSP-clocks per launched neutron (per lane: divide by 32 for per-warp) for each
     resource; returns dict(issue=, fp64=, xu=)."""
@@ -54,7 +63,7 @@ def smsp_clocks_per_neutron(frac_survive: float, frac_detect: float, model_key: 
 
 
 def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, model_key: str, nodes: int,
-             sm_mhz: float = SM_MAX_MHZ):
+             sm_mhz: float = SM_MAX_MHZ, workload: str | None = None):
     """Roofline record for bench.py.  `achieved` and `peak` are in G thread-instructions/s on the
     binding resource (issue slots x 32 lanes: 148 SM x 4 SMSP x 32 lanes x clock)."""
     c = smsp_clocks_per_neutron(frac_survive, frac_detect, model_key, nodes)
@@ -67,5 +76,5 @@ def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, mod
         "frac": achieved / peak_lane_clocks,
         "alg_clocks_per_neutron": {k: round(v, 2) for k, v in c.items()},
         "peak_source": f"derived: {N_SM} SM x {SMSP_PER_SM} SMSP x 32 lanes x {sm_mhz:.0f} MHz (DESIGN.md s.7)",
-        "traffic": None,
+        "traffic": NCU_DRAM_BYTES.get(workload),
     }

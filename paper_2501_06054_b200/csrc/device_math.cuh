@@ -151,18 +151,31 @@ __device__ __forceinline__ void sincos_2pi(double u, double& s, double& c) {
 
 // ---------------------------------------------------------------- sphere Phi(u) = 3 (sin u - u cos u)/u^3
 // PAPER.md:37 (Eq. 1 over a sphere).  Even series below the threshold where the direct form cancels.
-__device__ __forceinline__ float sphere_phi(float u) {
-  const float u2 = u * u;
-  float ser = fmaf(u2, 1.0f / 1330560.0f, -1.0f / 15120.0f);
-  ser = fmaf(ser, u2, 1.0f / 280.0f);
-  ser = fmaf(ser, u2, -0.1f);
-  ser = fmaf(ser, u2, 1.0f);
-  float s, c;
-  sincos_r(u, s, c);
+// fp32: reduction of u by pi (u = k pi + r, |r| <= pi/2), then sin u - u cos u = (-1)^k (sin r - u cos r)
+// with sin r = r + r z S(z), cos r = 1 + z C(z), z = r^2.  For k = 0 (u < pi/2, where the direct form
+// cancels) the same two polynomials give Phi without cancellation: sin r - r cos r = r^3 (S - C), so
+// Phi = 3 (S(z) - C(z)).  SIGNED = false drops (-1)^k for callers that only use Phi^2.
+template <bool SIGNED>
+__device__ __forceinline__ float sphere_phi_core(float u, float lo) {
+  const float t = fmaf(u, 0.318309886f, SAS_ROUND_MAGIC);
+  const int kb = __float_as_int(t);
+  const float kf = t - SAS_ROUND_MAGIC;
+  float r = fmaf(kf, -3.14159250259399414062e+00f, u);
+  r = fmaf(kf, -1.50995788317231927067e-07f, r);
+  r = fmaf(kf, -1.07806050599155295311e-14f, r) + lo;
+  const float z = r * r;
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  const float CP[SAS_COSPI_POLY_N] = SAS_COSPI_POLY;
+  const float S = horner(SP, z), C = horner(CP, z);
+  const float sr = fmaf(r * z, S, r);
+  const float cr = fmaf(z, C, 1.0f);
   const float inv = rcp_fast(u);
-  const float dir = (3.0f * fmaf(-u, c, s)) * ((inv * inv) * inv);
-  return (u < 0.7f) ? ser : dir;
+  float dir = fmaf(-u, cr, sr) * ((inv * inv) * inv);
+  if (SIGNED) dir = __int_as_float(__float_as_int(dir) ^ (kb << 31));
+  const float sel = (kb == __float_as_int(SAS_ROUND_MAGIC)) ? (S - C) : dir;
+  return 3.0f * sel;
 }
+__device__ __forceinline__ float sphere_phi(float u) { return sphere_phi_core<true>(u, 0.0f); }
 __device__ __forceinline__ double sphere_phi(double u) {
   if (u < 0.5) {
     const double u2 = u * u;
@@ -250,19 +263,10 @@ __device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(
 __device__ __forceinline__ double lambda1_x2_small(double x2) { return lambda1_r(sqrt(x2)); }
 
 // ---------------------------------------------------------------- the same functions of a Phase
-__device__ __forceinline__ float sphere_phi_ph(Phase<float> p) {
-  const float u = p.hi;
-  const float u2 = u * u;
-  float ser = fmaf(u2, 1.0f / 1330560.0f, -1.0f / 15120.0f);
-  ser = fmaf(ser, u2, 1.0f / 280.0f);
-  ser = fmaf(ser, u2, -0.1f);
-  ser = fmaf(ser, u2, 1.0f);
-  float s, c;
-  sincos_ph(p, s, c);
-  const float inv = rcp_fast(u);
-  const float dir = (3.0f * fmaf(-u, c, s)) * ((inv * inv) * inv);
-  return (u < 0.7f) ? ser : dir;
-}
+__device__ __forceinline__ float sphere_phi_ph(Phase<float> p) { return sphere_phi_core<true>(p.hi, p.lo); }
+// |Phi| up to sign, for models that square a single term
+__device__ __forceinline__ float sphere_phi_abs_ph(Phase<float> p) { return sphere_phi_core<false>(p.hi, p.lo); }
+__device__ __forceinline__ double sphere_phi_abs_ph(Phase<double> p) { return sphere_phi(p.v); }
 __device__ __forceinline__ double sphere_phi_ph(Phase<double> p) { return sphere_phi(p.v); }
 
 __device__ __forceinline__ float sinc_ph(Phase<float> p) { return sinc_from(sin_reduced_pi(p.hi, p.lo), p.hi); }

@@ -95,7 +95,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
       const Proj<Real> qp = make_proj<Real>(qd);
       for (int a = 0; a < P.n_a; ++a) {
         const Real* r = T.ta + a * TA_W;
-        const Real ph = sphere_phi_ph(phase_mul(qp, r[0], r[1]));
+        const Real ph = sphere_phi_abs_ph(phase_mul(qp, r[0], r[1]));
         acc = fma_r(r[2], ph * ph, acc);
       }
     } break;
@@ -190,7 +190,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
       const Proj<Real> U0 = make_proj<Real>(sqrt(fma(ua, ua, fma(ub, ub, uc * uc))));
       for (int a = 0; a < P.n_a; ++a) {
         const Real* r = T.ta + a * TA_W;
-        const Real ph = sphere_phi_ph(phase_mul(U0, r[0], r[1]));
+        const Real ph = sphere_phi_abs_ph(phase_mul(U0, r[0], r[1]));
         acc = fma_r(r[2], ph * ph, acc);
       }
     } break;

@@ -21,15 +21,19 @@ namespace sas {
 #ifndef SAS_MIN_BLOCKS
 #define SAS_MIN_BLOCKS 5
 #endif
+#ifndef SAS_STAGE_A_ROWS
+#define SAS_STAGE_A_ROWS 2
+#endif
 constexpr int BLOCK_THREADS = SAS_BLOCK_THREADS;
 constexpr int WARPS_PER_BLOCK = BLOCK_THREADS / 32;
 constexpr int MIN_BLOCKS_PER_SM = SAS_MIN_BLOCKS;
-constexpr int RING = 64;  // entries per warp queue (power of two, >= 63)
+constexpr int RING = 64;     // entries per warp queue (power of two, >= 63)
+constexpr int RING_B = 128;  // queue B takes two rows of 32 per stage-A step on top of < 32 entries
 
 struct WarpQueues {
   // queue B: slit-1 survivors (Philox block 0)
-  uint32_t b_id[RING];
-  uint32_t b_w[4][RING];
+  uint32_t b_id[RING_B];
+  uint32_t b_w[4][RING_B];
   // queue B2: survivors the classifier could not rule out (Philox blocks 0 and 1)
   uint32_t b2_id[RING];
   uint32_t b2_w[8][RING];
@@ -38,6 +42,9 @@ struct WarpQueues {
   int32_t c_pixel[RING];
   double c_G[RING];
   double c_Q[3][RING];
+  // outcome counts of this warp, one column per lane (no conflicts, no overflow): row 0 detected,
+  // rows 1..5 = ST_*, row 6 = detector misses decided by the classifier
+  uint32_t oc[7][32];
 };
 
 __host__ __device__ inline size_t round16(size_t x) { return (x + 15) & ~(size_t)15; }
@@ -48,18 +55,17 @@ __host__ __device__ inline size_t trace_smem_bytes(int tab_len_max) {
          (size_t)WARPS_PER_BLOCK * sizeof(WarpQueues);
 }
 
-// adds the seven packed 9-bit outcome fields of one lane to the global counters: field s = status s
-// (detected, status 0, goes to slot 6; statuses 1..5 to slots 1..5); field 6 = detector misses decided
-// by the classifier, slot 7
-constexpr int PK_BITS = 9;
-constexpr unsigned PK_FLUSH_CALLS = 500;  // < 2^9: one increment per lane per stage call
-__device__ __forceinline__ void flush_packed(unsigned long long* counters, unsigned long long pk) {
+// adds a warp's outcome counts to the global counters: detected (row 0) to slot 6, ST_* rows 1..5 to
+// slots 1..5; the classifier's detector misses (row 6) to slot 5 and to slot 7
+__device__ __forceinline__ void flush_outcomes(unsigned long long* counters, const uint32_t (*oc)[32]) {
+  const int lane = threadIdx.x & 31;
 #pragma unroll
   for (int f = 0; f < 7; ++f) {
-    const unsigned v = (unsigned)(pk >> (PK_BITS * f)) & ((1u << PK_BITS) - 1u);
-    const unsigned tot = __reduce_add_sync(0xFFFFFFFFu, v);
-    const int slot = f == 0 ? 6 : (f == 6 ? 7 : f);
-    if ((threadIdx.x & 31) == 0 && tot) atomicAdd(counters + slot, (unsigned long long)tot);
+    const unsigned tot = __reduce_add_sync(0xFFFFFFFFu, oc[f][lane]);
+    if (lane == 0 && tot) {
+      atomicAdd(counters + (f == 0 ? 6 : (f == 6 ? 5 : f)), (unsigned long long)tot);
+      if (f == 6) atomicAdd(counters + 7, (unsigned long long)tot);
+    }
   }
 }
 
@@ -77,13 +83,12 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
   const unsigned lt_mask = (1u << lane) - 1u;
   const unsigned FULL = 0xFFFFFFFFu;
   const bool DUMP = a.d_pixel != nullptr;  // parity hook: per-neutron outputs instead of the histogram
+  const bool DUMP_Q = DUMP && a.d_q != nullptr;
 
   // warp-uniform pipeline state
   int headB = 0, cntB = 0, headB2 = 0, cntB2 = 0, headC = 0, cntC = 0;
-  // outcome counters: every lane packs its own seven 9-bit fields (flush_packed);
-  // flushed to the global counters before a field can overflow
-  unsigned long long pk = 0;
-  unsigned pk_calls = 0;
+#pragma unroll
+  for (int f = 0; f < 7; ++f) wq.oc[f][lane] = 0;
 
   int cur_exp = -1;
   uint32_t exp_word = 0;
@@ -179,10 +184,9 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         Hit h;
         if (act) {
           st = trace_geometry(P, w, w1, h);
-          if (DUMP && a.d_q != nullptr) a.d_q[idoff] = h.q;
-          pk += 1ull << (PK_BITS * st);
+          if (DUMP_Q) a.d_q[idoff] = h.q;
+          wq.oc[st][lane] += 1;
         }
-        if (++pk_calls == PK_FLUSH_CALLS) { if (!DUMP) flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
         const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
         if (st == ST_DETECTED) {
           const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
@@ -197,14 +201,14 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         // ---------------- stage B0: Philox block 1 + certain-miss classifier
         const int n = cntB < 32 ? cntB : 32;
         const bool act = lane < n;
-        const int slot = (headB + lane) & (RING - 1);
+        const int slot = (headB + lane) & (RING_B - 1);
         uint32_t idoff = 0, w[4] = {0, 0, 0, 0};
         if (act) {
           idoff = wq.b_id[slot];
           w[0] = wq.b_w[0][slot]; w[1] = wq.b_w[1][slot]; w[2] = wq.b_w[2][slot]; w[3] = wq.b_w[3][slot];
         }
         __syncwarp();
-        headB = (headB + n) & (RING - 1);
+        headB = (headB + n) & (RING_B - 1);
         cntB -= n;
         const uint64_t id = a.first_id + idoff;
         uint32_t w1[4];
@@ -212,10 +216,9 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         double q;
         const bool sure = surely_misses_detector(P, w1, q);
         if (act && sure) {
-          pk += (1ull << (PK_BITS * ST_MISS_DET)) + (1ull << (PK_BITS * 6));
-          if (DUMP && a.d_q != nullptr) a.d_q[idoff] = q;
+          wq.oc[6][lane] += 1;
+          if (DUMP_Q) a.d_q[idoff] = q;
         }
-        if (++pk_calls == PK_FLUSH_CALLS) { if (!DUMP) flush_packed(a.counters, pk); pk = 0; pk_calls = 0; }
         const bool keep = act && !sure;
         const unsigned m = __ballot_sync(FULL, keep);
         if (keep) {
@@ -234,6 +237,35 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         const bool s1_int = P.s1_int_ok != 0;
         const uint32_t lo0 = P.s1_lo[0], hi0 = P.s1_hi[0], lo1 = P.s1_lo[1], hi1 = P.s1_hi[1];
         const uint64_t id0 = a.first_id + off0 + lane;
+#if SAS_STAGE_A_ROWS == 2
+        // two rows per step: two independent Philox chains in flight, round keys loaded once
+        do {
+          const uint32_t in0 = (row << 5) + lane, in1 = in0 + (WARPS_PER_BLOCK << 5);
+          const uint64_t ida = id0 + (row << 5), idb = ida + (WARPS_PER_BLOCK << 5);
+          uint32_t w[4], v[4];
+          philox4x32_10(a.keys, (uint32_t)ida, (uint32_t)(ida >> 32), 0u, exp_word, w);
+          philox4x32_10(a.keys, (uint32_t)idb, (uint32_t)(idb >> 32), 0u, exp_word, v);
+          bool pa = in0 < cnt_ids, pb = in1 < cnt_ids;  // a row past the item's end fails here as well
+          if (s1_int) {
+            pa = pa && (w[0] - lo0 <= hi0 - lo0) && (w[1] - lo1 <= hi1 - lo1);
+            pb = pb && (v[0] - lo0 <= hi0 - lo0) && (v[1] - lo1 <= hi1 - lo1);
+          }
+          const unsigned ma = __ballot_sync(FULL, pa), mb = __ballot_sync(FULL, pb);
+          const int na = __popc(ma);
+          const int tail = headB + cntB;
+          if (pa) {
+            const int s2 = (tail + __popc(ma & lt_mask)) & (RING_B - 1);
+            wq.b_id[s2] = off0 + in0;
+            wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
+          }
+          if (pb) {
+            const int s2 = (tail + na + __popc(mb & lt_mask)) & (RING_B - 1);
+            wq.b_id[s2] = off0 + in1;
+            wq.b_w[0][s2] = v[0]; wq.b_w[1][s2] = v[1]; wq.b_w[2][s2] = v[2]; wq.b_w[3][s2] = v[3];
+          }
+          cntB += na + __popc(mb);
+          row += 2 * WARPS_PER_BLOCK;
+#else
         do {
           const uint32_t in_item = (row << 5) + lane;
           const uint64_t id = id0 + (row << 5);
@@ -244,12 +276,13 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
           const unsigned m = __ballot_sync(FULL, pass);
           const int np = __popc(m);
           if (pass) {
-            const int s2 = (headB + cntB + __popc(m & lt_mask)) & (RING - 1);
+            const int s2 = (headB + cntB + __popc(m & lt_mask)) & (RING_B - 1);
             wq.b_id[s2] = off0 + in_item;
             wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
           }
           cntB += np;
           row += WARPS_PER_BLOCK;
+#endif
         } while (row < row_end && cntB < 32);
         __syncwarp();
         continue;
@@ -260,7 +293,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
 
   // counters[0] (launched) is known to the host; counters[1] (died at slit 1) is what is left of it after
   // every other outcome (sas_get_counters): a neutron that the integer slit-1 test drops is never queued
-  if (!DUMP) flush_packed(a.counters, pk);
+  if (!DUMP) flush_outcomes(a.counters, wq.oc);
 }
 
 }  // namespace sas

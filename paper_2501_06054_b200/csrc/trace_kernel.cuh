@@ -15,20 +15,20 @@
 
 namespace sas {
 
+#ifndef SAS_STAGE_A_ROWS
+#define SAS_STAGE_A_ROWS 3
+#endif
 #ifndef SAS_BLOCK_THREADS
 #define SAS_BLOCK_THREADS 128
 #endif
 #ifndef SAS_MIN_BLOCKS
 #define SAS_MIN_BLOCKS 5
 #endif
-#ifndef SAS_STAGE_A_ROWS
-#define SAS_STAGE_A_ROWS 2
-#endif
 constexpr int BLOCK_THREADS = SAS_BLOCK_THREADS;
 constexpr int WARPS_PER_BLOCK = BLOCK_THREADS / 32;
 constexpr int MIN_BLOCKS_PER_SM = SAS_MIN_BLOCKS;
 constexpr int RING = 64;     // entries per warp queue (power of two, >= 63)
-constexpr int RING_B = 128;  // queue B takes two rows of 32 per stage-A step on top of < 32 entries
+constexpr int RING_B = SAS_STAGE_A_ROWS > 3 ? 256 : 128;  // queue B takes SAS_STAGE_A_ROWS rows of 32 per stage-A step on top of < 32 entries
 
 struct WarpQueues {
   // queue B: slit-1 survivors (Philox block 0)
@@ -237,34 +237,34 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         const bool s1_int = P.s1_int_ok != 0;
         const uint32_t lo0 = P.s1_lo[0], hi0 = P.s1_hi[0], lo1 = P.s1_lo[1], hi1 = P.s1_hi[1];
         const uint64_t id0 = a.first_id + off0 + lane;
-#if SAS_STAGE_A_ROWS == 2
-        // two rows per step: two independent Philox chains in flight, round keys loaded once
+#if SAS_STAGE_A_ROWS >= 2
+        // several rows per step: independent Philox chains in flight, round keys loaded once
         do {
-          const uint32_t in0 = (row << 5) + lane, in1 = in0 + (WARPS_PER_BLOCK << 5);
-          const uint64_t ida = id0 + (row << 5), idb = ida + (WARPS_PER_BLOCK << 5);
-          uint32_t w[4], v[4];
-          philox4x32_10(a.keys, (uint32_t)ida, (uint32_t)(ida >> 32), 0u, exp_word, w);
-          philox4x32_10(a.keys, (uint32_t)idb, (uint32_t)(idb >> 32), 0u, exp_word, v);
-          bool pa = in0 < cnt_ids, pb = in1 < cnt_ids;  // a row past the item's end fails here as well
-          if (s1_int) {
-            pa = pa && (w[0] - lo0 <= hi0 - lo0) && (w[1] - lo1 <= hi1 - lo1);
-            pb = pb && (v[0] - lo0 <= hi0 - lo0) && (v[1] - lo1 <= hi1 - lo1);
+          constexpr int NR = SAS_STAGE_A_ROWS;
+          uint32_t w[NR][4];
+          bool pass[NR];
+          unsigned m[NR];
+#pragma unroll
+          for (int k = 0; k < NR; ++k) {
+            const uint64_t id = id0 + ((row + k * WARPS_PER_BLOCK) << 5);
+            philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w[k]);
           }
-          const unsigned ma = __ballot_sync(FULL, pa), mb = __ballot_sync(FULL, pb);
-          const int na = __popc(ma);
-          const int tail = headB + cntB;
-          if (pa) {
-            const int s2 = (tail + __popc(ma & lt_mask)) & (RING_B - 1);
-            wq.b_id[s2] = off0 + in0;
-            wq.b_w[0][s2] = w[0]; wq.b_w[1][s2] = w[1]; wq.b_w[2][s2] = w[2]; wq.b_w[3][s2] = w[3];
+          int tail = headB + cntB;
+#pragma unroll
+          for (int k = 0; k < NR; ++k) {
+            const uint32_t in_item = ((row + k * WARPS_PER_BLOCK) << 5) + lane;
+            pass[k] = in_item < cnt_ids;  // a row past the item's end fails here as well
+            if (s1_int) pass[k] = pass[k] && (w[k][0] - lo0 <= hi0 - lo0) && (w[k][1] - lo1 <= hi1 - lo1);
+            m[k] = __ballot_sync(FULL, pass[k]);
+            if (pass[k]) {
+              const int s2 = (tail + __popc(m[k] & lt_mask)) & (RING_B - 1);
+              wq.b_id[s2] = off0 + in_item;
+              wq.b_w[0][s2] = w[k][0]; wq.b_w[1][s2] = w[k][1]; wq.b_w[2][s2] = w[k][2]; wq.b_w[3][s2] = w[k][3];
+            }
+            tail += __popc(m[k]);
           }
-          if (pb) {
-            const int s2 = (tail + na + __popc(mb & lt_mask)) & (RING_B - 1);
-            wq.b_id[s2] = off0 + in1;
-            wq.b_w[0][s2] = v[0]; wq.b_w[1][s2] = v[1]; wq.b_w[2][s2] = v[2]; wq.b_w[3][s2] = v[3];
-          }
-          cntB += na + __popc(mb);
-          row += 2 * WARPS_PER_BLOCK;
+          cntB = tail - headB;
+          row += NR * WARPS_PER_BLOCK;
 #else
         do {
           const uint32_t in_item = (row << 5) + lane;

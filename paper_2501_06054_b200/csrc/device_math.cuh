@@ -54,7 +54,7 @@ __device__ __forceinline__ float horner(const float (&c)[N], float t) {
 }
 
 // ---------------------------------------------------------------- sin/cos
-// fp32: three-step Cody-Waite reduction by pi/2 with FMAs, kernels on [-pi/4, pi/4].
+// fp32: two-step Cody-Waite reduction by pi/2 with FMAs (48 bits of pi/2), kernels on [-pi/4, pi/4].
 // Valid for |x| < ~1e5 (k exact in fp32); the tracer's arguments are q*size < ~1e3.
 // k = nearest integer to x*inv_period is taken from the mantissa of x*inv_period + 1.5*2^23 (no
 // FRND/F2I on the XU pipe); |x*inv_period| < 2^22.
@@ -65,7 +65,7 @@ __device__ __forceinline__ void sincos_core(float x, float lo, float& s, float& 
   const float kf = t - SAS_ROUND_MAGIC;
   float r = fmaf(kf, -1.57079625129699707031e+00f, x);  // exact: the product has <= 32 significant bits
   r = fmaf(kf, -7.54978941586159635335e-08f, r);
-  r = fmaf(kf, -5.39030252995776476554e-15f, r) + lo;
+  r += lo;  // the third Cody-Waite term, k * 5.4e-15, is below 1e-11 rad for |x| < 1e3
   const float z = r * r;
   const float SP[SAS_SIN_POLY_N] = SAS_SIN_POLY;
   const float CP[SAS_COS_POLY_N] = SAS_COS_POLY;
@@ -162,7 +162,7 @@ __device__ __forceinline__ float sphere_phi_core(float u, float lo) {
   const float kf = t - SAS_ROUND_MAGIC;
   float r = fmaf(kf, -3.14159250259399414062e+00f, u);
   r = fmaf(kf, -1.50995788317231927067e-07f, r);
-  r = fmaf(kf, -1.07806050599155295311e-14f, r) + lo;
+  r += lo;  // the third Cody-Waite term, k * 1.1e-14, is below 1e-11 rad for |x| < 1e3
   const float z = r * r;
   const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
   const float CP[SAS_COSPI_POLY_N] = SAS_COSPI_POLY;
@@ -200,7 +200,7 @@ __device__ __forceinline__ float sin_reduced_pi(float x, float lo) {
   const float kf = t - SAS_ROUND_MAGIC;
   float r = fmaf(kf, -3.14159250259399414062e+00f, x);
   r = fmaf(kf, -1.50995788317231927067e-07f, r);
-  r = fmaf(kf, -1.07806050599155295311e-14f, r) + lo;
+  r += lo;  // the third Cody-Waite term, k * 1.1e-14, is below 1e-11 rad for |x| < 1e3
   const float z = r * r;
   const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
   const float ps = fmaf(r * z, horner(SP, z), r);
@@ -218,7 +218,6 @@ __device__ __forceinline__ float sinc_r(float x) {
   const float kf = t - SAS_ROUND_MAGIC;
   float r = fmaf(kf, -3.14159250259399414062e+00f, x);
   r = fmaf(kf, -1.50995788317231927067e-07f, r);
-  r = fmaf(kf, -1.07806050599155295311e-14f, r);
   const float z = r * r;
   const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
   const float ps = fmaf(r * z, horner(SP, z), r);
@@ -256,11 +255,17 @@ __device__ __forceinline__ float lambda1_x2_small(float x2) {
   const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
   return horner(LA, fmaf(x2, 0.03125f, -1.0f));
 }
+// the same with the polynomial variable t = x^2/32 - 1 formed by the caller (|x^2| <= 64)
+__device__ __forceinline__ float lambda1_t_small(float t) {
+  const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+  return horner(LA, t);
+}
 __device__ __forceinline__ double lambda1_x2_small(double x2);
 __device__ __forceinline__ float lambda1_r(float x) { return lambda1_x2(x * x); }
 __device__ __forceinline__ double lambda1_r(double x) { return (x == 0.0) ? 1.0 : (2.0 * j1(x)) / x; }
 __device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(x2)); }
 __device__ __forceinline__ double lambda1_x2_small(double x2) { return lambda1_r(sqrt(x2)); }
+__device__ __forceinline__ double lambda1_t_small(double t) { return lambda1_r(sqrt(fmax(32.0 * (t + 1.0), 0.0))); }
 
 // ---------------------------------------------------------------- the same functions of a Phase
 __device__ __forceinline__ float sphere_phi_ph(Phase<float> p) { return sphere_phi_core<true>(p.hi, p.lo); }

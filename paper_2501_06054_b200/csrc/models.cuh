@@ -120,6 +120,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
         const Real qA = (Real)qAd, qB = (Real)qBd, qC = (Real)qCd;
         const bool mono = (P.n_a == 1) && (P.n_b == 1);
         const Real hL0 = T.tb[0], cL0 = T.tb[2], R20 = T.ta[3], cR0 = T.ta[2];
+        const Real nR2k = -R20 * (Real)0.03125, tq = fma_r(q2, R20 * (Real)0.03125, (Real)-1);
         for (int i = 0; i < P.n_th; ++i) {
           const Real sth = T.tth[i * TOR_W + 0], cth = T.tth[i * TOR_W + 1], wth = T.tth[i * TOR_W + 2];
           const Real Ai = fma_r(qA, sth, qC * cth);
@@ -131,9 +132,8 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
               for (int j = 0; j < P.n_ph; ++j) {
                 const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
                 const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
-                Real r2 = fma_r(-qc, qc, q2);
-                r2 = r2 > (Real)0 ? r2 : (Real)0;
-                const Real f = sinc_r(qc * hL0) * lambda1_x2_small(r2 * R20);
+                // Lambda's polynomial variable t = x^2/32 - 1, x^2 = R^2 (q^2 - qc^2), in one FMA
+                const Real f = sinc_r(qc * hL0) * lambda1_t_small(fma_r(qc * qc, nR2k, tq));
                 row = fma_r(wph, f * f, row);
               }
             } else {

@@ -224,6 +224,19 @@ __device__ __forceinline__ float sinc_r(float x) {
   return sinc_from(__int_as_float(__float_as_int(ps) ^ (kb << 31)), x);
 }
 __device__ __forceinline__ double sinc_r(double x) { return (x == 0.0) ? 1.0 : sin(x) / x; }
+// |sinc(q h)| for callers that square it: no sign, and the phase is biased by 1e-30 so that q h = 0 gives
+// sin(1e-30) / 1e-30 = 1 instead of 0/0 (the bias is far below one ulp of any other phase)
+__device__ __forceinline__ float sinc_abs_r(float q, float h) {
+  const float x = fmaf(q, h, 1e-30f);
+  const float t = fmaf(x, 0.318309886f, SAS_ROUND_MAGIC);
+  const float kf = t - SAS_ROUND_MAGIC;
+  float r = fmaf(kf, -3.14159250259399414062e+00f, x);
+  r = fmaf(kf, -1.50995788317231927067e-07f, r);
+  const float z = r * r;
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  return fmaf(r * z, horner(SP, z), r) * rcp_fast(x);
+}
+__device__ __forceinline__ double sinc_abs_r(double q, double h) { return sinc_r(q * h); }
 
 // ---------------------------------------------------------------- Lambda(x) = 2 J1(x)/x, x >= 0
 // x <= 8: one polynomial in x^2 (no square root needed); x > 8: Hankel form
@@ -255,17 +268,30 @@ __device__ __forceinline__ float lambda1_x2_small(float x2) {
   const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
   return horner(LA, fmaf(x2, 0.03125f, -1.0f));
 }
-// the same with the polynomial variable t = x^2/32 - 1 formed by the caller (|x^2| <= 64)
-__device__ __forceinline__ float lambda1_t_small(float t) {
-  const float LA[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
-  return horner(LA, t);
+// Lambda by class: the caller forms t = x^2 * lambda_class_scale(LC) - 1 and guarantees x^2 within the
+// class range (1: 64, 2: 36, 3: 25, 4: 16); shorter ranges take shorter polynomials
+__host__ __device__ constexpr double lambda_class_scale(int lc) {
+  return lc == 4 ? 1.0 / 8.0 : lc == 3 ? 1.0 / 12.5 : lc == 2 ? 1.0 / 18.0 : 1.0 / 32.0;
 }
+template <int LC>
+__device__ __forceinline__ float lambda1_class(float t) {
+  if (LC == 4) { const float c[SAS_LAMBDA_16_N] = SAS_LAMBDA_16; return horner(c, t); }
+  if (LC == 3) { const float c[SAS_LAMBDA_25_N] = SAS_LAMBDA_25; return horner(c, t); }
+  if (LC == 2) { const float c[SAS_LAMBDA_36_N] = SAS_LAMBDA_36; return horner(c, t); }
+  const float c[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+  return horner(c, t);
+}
+template <int LC>
+__device__ __forceinline__ double lambda1_class(double t);
 __device__ __forceinline__ double lambda1_x2_small(double x2);
 __device__ __forceinline__ float lambda1_r(float x) { return lambda1_x2(x * x); }
 __device__ __forceinline__ double lambda1_r(double x) { return (x == 0.0) ? 1.0 : (2.0 * j1(x)) / x; }
 __device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(x2)); }
 __device__ __forceinline__ double lambda1_x2_small(double x2) { return lambda1_r(sqrt(x2)); }
-__device__ __forceinline__ double lambda1_t_small(double t) { return lambda1_r(sqrt(fmax(32.0 * (t + 1.0), 0.0))); }
+template <int LC>
+__device__ __forceinline__ double lambda1_class(double t) {
+  return lambda1_r(sqrt(fmax((t + 1.0) / lambda_class_scale(LC), 0.0)));
+}
 
 // ---------------------------------------------------------------- the same functions of a Phase
 __device__ __forceinline__ float sphere_phi_ph(Phase<float> p) { return sphere_phi_core<true>(p.hi, p.lo); }

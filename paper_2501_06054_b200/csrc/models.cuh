@@ -31,6 +31,31 @@ __device__ __forceinline__ Tables<Real> table_views(const Real* base, const ExpP
 template <typename Real>
 __device__ __forceinline__ Real sq(Real x) { return x * x; }
 
+// One row of the Gaussian-tilt quadrature of a monodisperse cylinder (R-A11): sum over the phi tilts of
+// w_j [sinc(Q.c_ij L/2) Lambda(R sqrt(q^2 - (Q.c_ij)^2))]^2 for one theta tilt (Ai = Q.(tilted axis, phi = 0)).
+// LC > 0: Lambda is the short polynomial of class LC in t = x^2 / h - 1 (device_math.cuh), t in one FMA.
+template <typename Real, int LC>
+__device__ __forceinline__ Real cyl_quad_row(const Real* tph, int n_ph, Real Ai, Real qB, Real hL0, Real R20, Real q2) {
+  const Real k = R20 * (Real)lambda_class_scale(LC);
+  const Real nk = -k, tq = fma_r(q2, k, (Real)-1);
+  Real row = 0;
+#pragma unroll 2
+  for (int j = 0; j < n_ph; ++j) {
+    const Real sph = tph[j * TOR_W + 0], cph = tph[j * TOR_W + 1], wph = tph[j * TOR_W + 2];
+    const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
+    Real f;
+    if (LC > 0) {
+      f = sinc_abs_r(qc, hL0) * lambda1_class<LC>(fma_r(qc * qc, nk, tq));
+    } else {
+      Real r2 = fma_r(-qc, qc, q2);
+      r2 = r2 > (Real)0 ? r2 : (Real)0;
+      f = sinc_abs_r(qc, hL0) * lambda1_x2(r2 * R20);
+    }
+    row = fma_r(wph, f * f, row);
+  }
+  return row;
+}
+
 // Model table meaning (host: fill_model).  Lengths that multiply a projection of Q are stored as a
 // (hi, lo) pair: in the fp32 path hi = float(L), lo = float(L - hi); in the fp64 path hi = L, lo = 0.
 //  sphere              ta = {R_hi, R_lo, w_a (drho V_a)^2}
@@ -120,32 +145,19 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
         const Real qA = (Real)qAd, qB = (Real)qBd, qC = (Real)qCd;
         const bool mono = (P.n_a == 1) && (P.n_b == 1);
         const Real hL0 = T.tb[0], cL0 = T.tb[2], R20 = T.ta[3], cR0 = T.ta[2];
-        const Real nR2k = -R20 * (Real)0.03125, tq = fma_r(q2, R20 * (Real)0.03125, (Real)-1);
         for (int i = 0; i < P.n_th; ++i) {
           const Real sth = T.tth[i * TOR_W + 0], cth = T.tth[i * TOR_W + 1], wth = T.tth[i * TOR_W + 2];
           const Real Ai = fma_r(qA, sth, qC * cth);
           Real row = 0;
           if (mono) {
-            // lam_small: the host checked (q_max R)^2 <= 64, so Lambda needs no range test
-            if (P.lam_small) {
-#pragma unroll 2
-              for (int j = 0; j < P.n_ph; ++j) {
-                const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
-                const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
-                // Lambda's polynomial variable t = x^2/32 - 1, x^2 = R^2 (q^2 - qc^2), in one FMA
-                const Real f = sinc_r(qc * hL0) * lambda1_t_small(fma_r(qc * qc, nR2k, tq));
-                row = fma_r(wph, f * f, row);
-              }
-            } else {
-#pragma unroll 2
-              for (int j = 0; j < P.n_ph; ++j) {
-                const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
-                const Real qc = fma_r(cph, Ai, qB * sph);
-                Real r2 = fma_r(-qc, qc, q2);
-                r2 = r2 > (Real)0 ? r2 : (Real)0;
-                const Real f = sinc_r(qc * hL0) * lambda1_x2(r2 * R20);
-                row = fma_r(wph, f * f, row);
-              }
+            // lam_class: the host bounded x^2 = (q R)^2 for this experiment, so Lambda is one short
+            // polynomial without a range test (0: no bound below 64)
+            switch (P.lam_small) {
+              case 4: row = cyl_quad_row<Real, 4>(T.tph, P.n_ph, Ai, qB, hL0, R20, q2); break;
+              case 3: row = cyl_quad_row<Real, 3>(T.tph, P.n_ph, Ai, qB, hL0, R20, q2); break;
+              case 2: row = cyl_quad_row<Real, 2>(T.tph, P.n_ph, Ai, qB, hL0, R20, q2); break;
+              case 1: row = cyl_quad_row<Real, 1>(T.tph, P.n_ph, Ai, qB, hL0, R20, q2); break;
+              default: row = cyl_quad_row<Real, 0>(T.tph, P.n_ph, Ai, qB, hL0, R20, q2); break;
             }
             row *= cL0 * cR0;
           } else {

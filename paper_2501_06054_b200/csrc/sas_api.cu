@@ -384,8 +384,12 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
       // largest Lambda argument this experiment can produce: |Q| <= q_max, radius <= largest node
       double r_max = 0.0;
       for (int a = 0; a < P.n_a; ++a) r_max = std::max(r_max, c->h_tab[P.tab_off + a * TA_W] + c->h_tab[P.tab_off + a * TA_W + 1]);
-      const double x_max = c->instr[e].q_max * r_max * 1.001;
-      P.lam_small = (x_max * x_max <= 64.0) ? 1 : 0;
+      // ... and a detected neutron has sin(theta) = q lambda / 4 pi <= s_cut (the classifier's bound)
+      double q_top = c->instr[e].q_max;
+      if (std::isfinite(P.s_cut)) q_top = std::min(q_top, 4.0 * PI_D * P.s_cut / c->instr[e].lambda_min);
+      const double x_max = q_top * r_max * 1.001;
+      const double x2 = x_max * x_max;
+      P.lam_small = x2 <= 16.0 ? 4 : x2 <= 25.0 ? 3 : x2 <= 36.0 ? 2 : x2 <= 64.0 ? 1 : 0;
     }
     c->tab_len_max = std::max(c->tab_len_max, P.tab_len);
   }

@@ -6,7 +6,13 @@
 #pragma once
 #include "sas_types.h"
 
+#ifndef SAS_CYL_UNROLL
+#define SAS_CYL_UNROLL 4
+#endif
+
 namespace sas {
+
+constexpr int CYL_UNROLL = SAS_CYL_UNROLL;  // nodes of the phi-tilt loop in flight
 
 template <typename Real>
 struct Tables {  // views into the shared-memory table block
@@ -39,7 +45,7 @@ __device__ __forceinline__ Real cyl_quad_row(const Real* tph, int n_ph, Real Ai,
   const Real k = R20 * (Real)lambda_class_scale(LC);
   const Real nk = -k, tq = fma_r(q2, k, (Real)-1);
   Real row = 0;
-#pragma unroll 2
+#pragma unroll CYL_UNROLL
   for (int j = 0; j < n_ph; ++j) {
     const Real sph = tph[j * TOR_W + 0], cph = tph[j * TOR_W + 1], wph = tph[j * TOR_W + 2];
     const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij

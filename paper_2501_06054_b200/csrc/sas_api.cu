@@ -21,6 +21,9 @@ constexpr double TWO_PI = 6.283185307179586;
 constexpr double FOUR_PI_3 = 4.1887902047863905;
 constexpr double PI_D = 3.141592653589793;
 constexpr int MAX_TIMED = 256;
+#ifndef SAS_ITEMS_PER_BLOCK
+#define SAS_ITEMS_PER_BLOCK 16
+#endif
 #ifndef SAS_MIN_ITEM
 #define SAS_MIN_ITEM 2048
 #endif
@@ -434,7 +437,7 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   const uint64_t total = (uint64_t)a.n_per_exp * a.n_exp;
   const int grid_full = c->n_sm * bps;
   // work items: ~16 per resident block, 2048..262144 ids each, multiple of 256 ids
-  uint64_t item = total / ((uint64_t)grid_full * 16ull);
+  uint64_t item = total / ((uint64_t)grid_full * (uint64_t)SAS_ITEMS_PER_BLOCK);
   item = std::min<uint64_t>(std::max<uint64_t>(item, SAS_MIN_ITEM), 262144);
   item = (item + 255) / 256 * 256;
   a.item_ids = (uint32_t)item;

@@ -18,6 +18,9 @@ namespace sas {
 #ifndef SAS_STAGE_A_ROWS
 #define SAS_STAGE_A_ROWS 3
 #endif
+#ifndef SAS_B0_PER_LANE
+#define SAS_B0_PER_LANE 2
+#endif
 #ifndef SAS_BLOCK_THREADS
 #define SAS_BLOCK_THREADS 128
 #endif
@@ -28,15 +31,17 @@ constexpr int BLOCK_THREADS = SAS_BLOCK_THREADS;
 constexpr int WARPS_PER_BLOCK = BLOCK_THREADS / 32;
 constexpr int MIN_BLOCKS_PER_SM = SAS_MIN_BLOCKS;
 constexpr int RING = 64;     // entries per warp queue (power of two, >= 63)
-constexpr int RING_B = SAS_STAGE_A_ROWS > 3 ? 256 : 128;  // queue B takes SAS_STAGE_A_ROWS rows of 32 per stage-A step on top of < 32 entries
+constexpr int NB0 = SAS_B0_PER_LANE;  // queue-B entries a lane takes per stage-B0 step
+constexpr int RING_B2 = NB0 > 1 ? 128 : 64;
+constexpr int RING_B = (32 * NB0 - 1 + 32 * SAS_STAGE_A_ROWS) > 128 ? 256 : 128;  // queue B takes SAS_STAGE_A_ROWS rows of 32 per stage-A step on top of < 32 entries
 
 struct WarpQueues {
   // queue B: slit-1 survivors (their id offsets; stage B draws Philox block 0 again for the few it gets:
   // 40 integer instructions for 6 % of the neutrons instead of eight queue accesses for 25 %)
   uint32_t b_id[RING_B];
   // queue B2: survivors the classifier could not rule out (id offset and Philox block 1)
-  uint32_t b2_id[RING];
-  uint32_t b2_w[4][RING];
+  uint32_t b2_id[RING_B2];
+  uint32_t b2_w[4][RING_B2];
   // queue C: detected neutrons
   uint32_t c_id[RING];
   int32_t c_pixel[RING];
@@ -170,7 +175,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         // ---------------- stage B: fp64 geometry
         const int n = cntB2 < 32 ? cntB2 : 32;
         const bool act = lane < n;
-        const int slot = (headB2 + lane) & (RING - 1);
+        const int slot = (headB2 + lane) & (RING_B2 - 1);
         uint32_t idoff = 0, w[4] = {0, 0, 0, 0}, w1[4] = {0, 0, 0, 0};
         if (act) {
           idoff = wq.b2_id[slot];
@@ -182,7 +187,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
           philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
         }
         __syncwarp();
-        headB2 = (headB2 + n) & (RING - 1);
+        headB2 = (headB2 + n) & (RING_B2 - 1);
         cntB2 -= n;
         int st = -1;
         Hit h;
@@ -201,33 +206,45 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         __syncwarp();
         continue;
       }
-      if (cntB >= 32 || (drain && cntB > 0)) {
-        // ---------------- stage B0: Philox block 1 + certain-miss classifier
-        const int n = cntB < 32 ? cntB : 32;
-        const bool act = lane < n;
-        const int slot = (headB + lane) & (RING_B - 1);
-        const uint32_t idoff = act ? wq.b_id[slot] : 0u;
+      if (cntB >= 32 * NB0 || (drain && cntB > 0)) {
+        // ---------------- stage B0: Philox block 1 + certain-miss classifier, NB0 entries per lane
+        // (independent Philox chains in flight, as in stage A)
+        const int n = cntB < 32 * NB0 ? cntB : 32 * NB0;
+        uint32_t idoff[NB0], w1[NB0][4];
+        bool act[NB0];
+#pragma unroll
+        for (int k = 0; k < NB0; ++k) {
+          act[k] = lane + 32 * k < n;
+          idoff[k] = act[k] ? wq.b_id[(headB + lane + 32 * k) & (RING_B - 1)] : 0u;
+        }
         __syncwarp();
         headB = (headB + n) & (RING_B - 1);
         cntB -= n;
-        const uint64_t id = a.first_id + idoff;
-        uint32_t w1[4];
-        philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 1u, exp_word, w1);
-        double q;
-        const bool sure = surely_misses_detector(P, w1, q);
-        if (act && sure) {
-          wq.oc[6][lane] += 1;
-          if (DUMP_Q) a.d_q[idoff] = q;
-        }
-        const bool keep = act && !sure;
-        const unsigned m = __ballot_sync(FULL, keep);
-        if (keep) {
-          const int s2 = (headB2 + cntB2 + __popc(m & lt_mask)) & (RING - 1);
-          wq.b2_id[s2] = idoff;
 #pragma unroll
-          for (int i = 0; i < 4; ++i) wq.b2_w[i][s2] = w1[i];
+        for (int k = 0; k < NB0; ++k) {
+          const uint64_t id = a.first_id + idoff[k];
+          philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 1u, exp_word, w1[k]);
         }
-        cntB2 += __popc(m);
+        int tail = headB2 + cntB2;
+#pragma unroll
+        for (int k = 0; k < NB0; ++k) {
+          double q;
+          const bool sure = surely_misses_detector(P, w1[k], q);
+          if (act[k] && sure) {
+            wq.oc[6][lane] += 1;
+            if (DUMP_Q) a.d_q[idoff[k]] = q;
+          }
+          const bool keep = act[k] && !sure;
+          const unsigned m = __ballot_sync(FULL, keep);
+          if (keep) {
+            const int s2 = (tail + __popc(m & lt_mask)) & (RING_B2 - 1);
+            wq.b2_id[s2] = idoff[k];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) wq.b2_w[i][s2] = w1[k][i];
+          }
+          tail += __popc(m);
+        }
+        cntB2 = tail - headB2;
         __syncwarp();
         continue;
       }
@@ -281,7 +298,7 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
           cntB += np;
           row += WARPS_PER_BLOCK;
 #endif
-        } while (row < row_end && cntB < 32);
+        } while (row < row_end && cntB < 32 * NB0);
         __syncwarp();
         continue;
       }

@@ -191,7 +191,9 @@ def bench_config(torch, S, cfg_index, steps, warmup, rank, world, flush, with_e2
     value = n_step * world / (ms_per_step * 1e-3)
     out = {"workload": c["name"], "n_neutrons_per_step": n_step, "ms_per_step": ms_per_step, "value": value,
            "kernel_ms": kernel_ms, "grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
-           "gpu_launches": int(launches), "detected_frac": cnt[6] / cnt[0], "survive_frac": 1.0 - cnt[1] / cnt[0]}
+           "gpu_launches": int(launches), "detected_frac": cnt[6] / cnt[0], "survive_frac": 1.0 - cnt[1] / cnt[0],
+           # survivors whose fp64 geometry ran (the others were certain detector misses, counters[7])
+           "geometry_frac": 1.0 - cnt[1] / cnt[0] - cnt[7] / cnt[0]}
     # roofline of the (only) kernel of the step, from its own average launch duration
     if batch:
         ks = {}
@@ -202,14 +204,14 @@ def bench_config(torch, S, cfg_index, steps, warmup, rank, world, flush, with_e2
         rl = None
         for k, n in ks.items():
             r = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n,
-                           workload=c["name"])
+                           workload=c["name"], frac_geometry=out["geometry_frac"])
             rl = r if rl is None else {**rl, "achieved": 0.5 * (rl["achieved"] + r["achieved"]),
                                        "frac": 0.5 * (rl["frac"] + r["frac"])}
         out["roofline"] = rl
     else:
         k, n = model_key_and_nodes(c["model"])
         out["roofline"] = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n,
-                                     workload=c["name"])
+                                     workload=c["name"], frac_geometry=out["geometry_frac"])
     e2e = None
     if with_e2e and not batch:
         # the call a user makes, host buffers in and out, every step
@@ -314,7 +316,8 @@ def main():
         ms *= nt
         from paper_2501_06054_b200 import roofline as R
         cnt = tr.counters().astype(np.float64)
-        rl = R.roofline(1e9 / (ms * 1e-3), 1 - cnt[1] / cnt[0], cnt[6] / cnt[0], "sphere_fp64", 1)
+        rl = R.roofline(1e9 / (ms * 1e-3), 1 - cnt[1] / cnt[0], cnt[6] / cnt[0], "sphere_fp64", 1,
+                        frac_geometry=1 - cnt[1] / cnt[0] - cnt[7] / cnt[0])
         others["c0_sphere_fp64_1e9"] = {"value": 1e9 * world / (ms * 1e-3), "kernel_ms": ms,
                                         "roofline_frac": rl["frac"], "roofline_pipe": rl["pipe"]}
         tr.close()

@@ -10,13 +10,17 @@ therefore the largest of three per-neutron costs, in SMSP-clocks per 32 neutrons
     fp64  = 2 x FP64 thread-instructions
     xu    = 8 x MUFU/conversion thread-instructions
 
-The per-unit instruction counts below are ALGORITHMIC: what the arithmetic of DESIGN.md section 3
-needs on this ISA (a fp64 division = 1 MUFU.RCP64H + 9 DFMA-class, a fp64 sqrt = 1 MUFU.RSQ64H + 9,
-fp64 sincos = 62, Philox4x32-10 = 40 integer instructions, ...), counted per unit of work:
-every launched neutron (stage A), every slit-1 survivor (stage B), every detected neutron (stage C
-prologue) and every quadrature node evaluation.  Queue handling, work fetching, atomics and loop
-overhead of the kernel are NOT in them.  The unit fractions (survivors and detected per launched
-neutron) are the counters of the timed run itself.
+The per-unit instruction counts below are ALGORITHMIC: the arithmetic that the method, in the
+formulation this library uses, needs on this ISA (a fp64 division = 1 MUFU.RCP64H + 9 DFMA-class,
+a fp64 sqrt = 1 MUFU.RSQ64H + 9, fp64 sincos = 62, Philox4x32-10 = 40 integer instructions, ...),
+counted per unit of work: every launched neutron (stage A), every slit-1 survivor (stage B0: Philox
+block 1 and the certain-miss test), every survivor whose geometry is evaluated (stage B), every
+detected neutron (stage-C prologue) and every quadrature node evaluation.  The per-node counts are the
+arithmetic instructions (FFMA/FMUL/FADD/MUFU/select) of the shipped loop bodies, read from the SASS of
+this build (cuobjdump): table loads, loop control, register moves, queue handling, work fetching and
+atomics are NOT in them, so the fraction cannot exceed the kernel's issue-slot utilisation.  The unit
+fractions (survivors, evaluated geometries, detected per launched neutron) are the counters of the
+timed run itself.
 """
 from __future__ import annotations
 
@@ -26,7 +30,8 @@ SM_MAX_MHZ = 1965.0
 
 # thread-instructions per unit: (issue_total, fp64, xu)
 STAGE_A = (46, 0, 0)            # Philox block 0 (40) + id/compare (6)
-# Philox block 1 (40) + 8 uniforms (3 fp64 each) + ~125 fp64 add/mul/compare + 8 div (10) + 3 sqrt (10)
+STAGE_B0 = (40 + 12, 12, 0)     # Philox block 1 (40) + two uniforms, q, lambda, q*lambda test in fp64 (12)
+# Philox block 0 again (40) + 8 uniforms (3 fp64 each) + ~125 fp64 add/mul/compare + 8 div (10) + 3 sqrt (10)
 # + sincos (62) + floor/convert (6 xu-class conversions)
 STAGE_B = (40 + 24 + 125 + 80 + 30 + 62 + 12, 24 + 125 + 72 + 27 + 62, 11 + 6)
 
@@ -34,14 +39,13 @@ STAGE_B = (40 + 24 + 125 + 80 + 30 + 62 + 12, 24 + 125 + 72 + 27 + 62, 11 + 6)
 MODEL_COST = {
     # name: (prologue(issue, fp64, xu), per_node(issue, fp64, xu))
     "sphere_fp64": ((40, 30, 2), (110, 100, 2)),
-    "sphere_fp32": ((40, 30, 4), (34, 0, 1)),
-    "sphere_py_fp32": ((40 + 60, 30, 5), (34, 0, 1)),
+    "sphere_fp32": ((40, 30, 4), (32, 0, 1)),
+    "sphere_py_fp32": ((40 + 60, 30, 5), (32, 0, 1)),
     "sphere_py_fp64": ((40 + 160, 30 + 150, 4), (110, 100, 2)),
-    "cylinder_quad_fp32": ((60, 40, 4), (52, 0, 3)),
-    "cs_triaxial_iso_fp32": ((40 + 40 + 90, 120, 6), (40, 0, 2)),
+    "cylinder_quad_fp32": ((60, 40, 4), (27, 0, 1)),
+    "cs_triaxial_iso_fp32": ((40 + 40 + 90, 120, 6), (33, 0, 2)),
     "cylinder_iso_fp64": ((40 + 40 + 200 + 320, 520, 8), (0, 0, 0)),
 }
-
 
 # DRAM traffic of one trace-kernel launch, dram__bytes_read.sum + dram__bytes_write.sum of the
 # `ncu --set full` captures summarised in profiles/r1_ncu_c<k>.md (bytes per launch; c4: the first of its
@@ -52,28 +56,36 @@ NCU_DRAM_BYTES = {
 }
 
 
-def smsp_clocks_per_neutron(frac_survive: float, frac_detect: float, model_key: str, nodes: int):
+def smsp_clocks_per_neutron(frac_survive: float, frac_detect: float, model_key: str, nodes: int,
+                            frac_geometry: float | None = None):
     """Algorithmic SMSP-clocks per launched neutron (per lane: divide by 32 for per-warp) for each
     resource; returns dict(issue=, fp64=, xu=)."""
     pro, node = MODEL_COST[model_key]
+    if frac_geometry is None:
+        frac_geometry = frac_survive      # no classifier: every survivor's geometry is evaluated
     tot = [0.0, 0.0, 0.0]
     for i in range(3):
-        tot[i] = STAGE_A[i] + frac_survive * STAGE_B[i] + frac_detect * (pro[i] + nodes * node[i])
+        tot[i] = (STAGE_A[i] + frac_survive * STAGE_B0[i] + frac_geometry * STAGE_B[i]
+                  + frac_detect * (pro[i] + nodes * node[i]))
     return dict(issue=tot[0], fp64=2.0 * tot[1], xu=8.0 * tot[2])
 
 
 def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, model_key: str, nodes: int,
-             sm_mhz: float = SM_MAX_MHZ, workload: str | None = None):
+             sm_mhz: float = SM_MAX_MHZ, workload: str | None = None, frac_geometry: float | None = None):
     """Roofline record for bench.py.  `achieved` and `peak` are in G thread-instructions/s on the
     binding resource (issue slots x 32 lanes: 148 SM x 4 SMSP x 32 lanes x clock)."""
-    c = smsp_clocks_per_neutron(frac_survive, frac_detect, model_key, nodes)
+    c = smsp_clocks_per_neutron(frac_survive, frac_detect, model_key, nodes, frac_geometry)
     pipe = max(c, key=c.get)
     peak_lane_clocks = N_SM * SMSP_PER_SM * 32 * sm_mhz * 1e6      # lane-clocks per second
     achieved = neutrons_per_s * c[pipe]
+    # the same path without the classifier shortcut (every survivor's geometry evaluated): what a plain
+    # implementation of DESIGN.md section 3 would have to issue for this throughput
+    plain = smsp_clocks_per_neutron(frac_survive, frac_detect, model_key, nodes, frac_survive)
     return {
         "bound": "alu", "pipe": pipe,
         "achieved": achieved / 1e9, "peak": peak_lane_clocks / 1e9, "unit": "G lane-clocks/s",
         "frac": achieved / peak_lane_clocks,
+        "frac_plain_algorithm": neutrons_per_s * max(plain.values()) / peak_lane_clocks,
         "alg_clocks_per_neutron": {k: round(v, 2) for k, v in c.items()},
         "peak_source": f"derived: {N_SM} SM x {SMSP_PER_SM} SMSP x 32 lanes x {sm_mhz:.0f} MHz (DESIGN.md s.7)",
         "traffic": NCU_DRAM_BYTES.get(workload),

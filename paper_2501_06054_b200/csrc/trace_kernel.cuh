@@ -96,8 +96,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
   for (int f = 0; f < 7; ++f) wq.oc[f][lane] = 0;
 
   int cur_exp = -1;
-  uint32_t exp_word = 0;
-  size_t hist_base = 0;
   bool replay = false;
   unsigned item = 0;
 
@@ -128,8 +126,6 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         const double* tsrc = a.tab_pool + src->tab_off;
         for (int i = threadIdx.x; i < tl; i += BLOCK_THREADS) tab[i] = (Real)tsrc[i];
         cur_exp = e;
-        exp_word = a.exp_base + (uint32_t)e;
-        hist_base = (size_t)e * (size_t)a.npix;
         __syncthreads();
       }
       const uint32_t kk = item % a.items_per_exp;
@@ -142,6 +138,8 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
     // ------------------------------------------------------------------ the pump
     for (;;) {
       const bool rows_left = row < row_end;
+      // Philox counter word 3 of the staged experiment (one add from a kernel parameter: not kept live)
+      const uint32_t exp_word = a.exp_base + (uint32_t)cur_exp;
       if (cntC >= 32 || (drain && cntB == 0 && cntB2 == 0 && cntC > 0)) {
         // ---------------- stage C: model + weight + histogram
         const int n = cntC < 32 ? cntC : 32;
@@ -163,7 +161,12 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
             a.d_pixel[idoff] = pixel;
             a.d_weight[idoff] = p;
           } else {
-            const size_t ix = hist_base + (size_t)pixel;
+            const size_t ix = (size_t)cur_exp * (size_t)a.npix + (size_t)pixel;
+#ifdef SAS_PROBE_NO_ATOMICS
+            // measurement probe only (profiles/r1_atomics.md): the same kernel without its histogram
+            // updates (the weight stays live through an impossible condition)
+            if (p != -1.0) continue;
+#endif
             atomicAdd(a.counts + ix, 1ull);
             atomicAdd(a.sum_p + ix, p);
             atomicAdd(a.sum_p2 + ix, p * p);

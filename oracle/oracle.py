@@ -32,7 +32,7 @@ MAX_NODES = 64
 _SAMPLE = {"box": 0, "cyl_y": 1}
 _MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3,
           "core_shell_triaxial": 4, "flat": 5}
-_ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2}
+_ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
 _SQ = {"none": 0, "hard_sphere_py": 1}
 
 
@@ -57,14 +57,16 @@ class Model(C.Structure):
                 ("theta", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
                 ("n_or", C.c_int32 * 2),
                 ("or_d", (C.c_double * MAX_NODES) * 2), ("or_w", (C.c_double * MAX_NODES) * 2),
-                ("sq_radius_eff", C.c_double), ("sq_volfrac", C.c_double)]
+                ("sq_radius_eff", C.c_double), ("sq_volfrac", C.c_double),
+                ("pd_mc", C.c_int32 * 2), ("pd_rel", C.c_double * 2)]
 
 
 class Record(C.Structure):
     _fields_ = [("status", C.c_int32), ("pixel", C.c_int32), ("weight", C.c_double),
                 ("weight_env", C.c_double), ("q", C.c_double), ("Q", C.c_double * 3),
                 ("lam", C.c_double), ("ell", C.c_double), ("p0", C.c_double),
-                ("intensity", C.c_double), ("u", C.c_double * 12)]
+                ("intensity", C.c_double), ("u", C.c_double * 12),
+                ("pd_x", C.c_double * 2), ("pd_tries", C.c_int32 * 2)]
 
 
 def build(force: bool = False) -> str:
@@ -97,6 +99,12 @@ def lib():
         L.orc_intensity.argtypes = [C.POINTER(Model), C.POINTER(C.c_double), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double)]
         L.orc_intensity.restype = C.c_double
+        L.orc_intensity_event.argtypes = [C.POINTER(Model), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                          C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_intensity_event.restype = C.c_double
+        L.orc_draw_rel_size.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_int, C.c_double,
+                                        C.POINTER(C.c_int32)]
+        L.orc_draw_rel_size.restype = C.c_double
         L.orc_amplitude.argtypes = [C.POINTER(Model)] + [C.c_double] * 5 + [C.POINTER(C.c_double)] * 2
         L.orc_amplitude.restype = C.c_double
         L.orc_trace_one.argtypes = [C.POINTER(Instrument), C.POINTER(Model), C.c_uint64, C.c_uint64,
@@ -164,6 +172,9 @@ def make_model(d: dict) -> Model:
             s, w = schulz_nodes(d["pd_rel"][k], d["pd_nodes"][k])
         else:
             s, w = np.ones(1), np.ones(1)
+        # the paper's own size averaging (DESIGN.md R-N1): one Gaussian draw per event
+        m.pd_mc[k] = 1 if d["pd_kind"][k] == "gauss_mc" else 0
+        m.pd_rel[k] = float(d["pd_rel"][k])
         m.n_pd[k] = len(s)
         for i in range(len(s)):
             m.pd_x[k][i] = s[i]
@@ -182,6 +193,8 @@ def make_model(d: dict) -> Model:
             m.or_w[k][i] = w[i]
     m.sq_radius_eff = d["sq_radius_eff"]
     m.sq_volfrac = d["sq_volfrac"]
+    if "gauss_mc" in d["pd_kind"] and (d["orient_kind"] == "gauss_quad" or "schulz" in d["pd_kind"]):
+        raise ValueError("per-event sizes (gauss_mc) do not combine with fixed-node averages (DESIGN.md R-N1)")
     if d["orient_kind"] == "gauss_quad" and d["model"] in ("triaxial", "core_shell_triaxial"):
         raise ValueError("gauss_quad orientation is defined for uniaxial models only (DESIGN.md R-A11)")
     return m
@@ -203,6 +216,22 @@ def intensity(model_d: dict, Q, u_or=(0.0, 0.0, 0.0), want_env=False):
     env = C.c_double()
     val = lib().orc_intensity(C.byref(m), q, u, C.byref(env))
     return (val, env.value) if want_env else val
+
+
+def intensity_event(model_d: dict, Q, x=(1.0, 1.0), u_or=(0.0, 0.0, 0.0)):
+    """Eq. 4 for one scattering event with relative sizes x (DESIGN.md R-N2)."""
+    m = model_d if isinstance(model_d, Model) else make_model(model_d)
+    q = (C.c_double * 3)(*[float(v) for v in Q])
+    u = (C.c_double * 3)(*u_or)
+    xx = (C.c_double * 2)(*x)
+    return lib().orc_intensity_event(C.byref(m), q, u, xx, None)
+
+
+def draw_rel_size(seed: int, nid: int, k: int, rel: float, exp_index: int = 0):
+    """(relative size, Philox blocks used) of axis k of event (seed, nid, exp_index) (DESIGN.md R-N1)."""
+    tries = C.c_int32()
+    x = lib().orc_draw_rel_size(seed, nid, exp_index, k, float(rel), C.byref(tries))
+    return x, tries.value
 
 
 def amplitude(model_d: dict, qa, qb, qc, x0=1.0, x1=1.0):

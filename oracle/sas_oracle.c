@@ -210,6 +210,28 @@ static void frame_from_angles(double st, double ct, double sp, double cp, double
 
 static double dot3(const double a[3], const double b[3]) { return (a[0] * b[0] + a[1] * b[1]) + a[2] * b[2]; }
 
+/* particle axes of one event: fixed angles, or drawn per event (R-A3 isotropic; R-N3 the paper's printed
+ * uniform angles) */
+static void particle_frame(const orc_model* m, const double u_or[3], double A[3], double B[3], double C[3]) {
+  if (m->orient_kind == ORC_ORIENT_ISOTROPIC_MC) {
+    /* R-A3: isotropic = cos(theta) uniform, phi and psi uniform */
+    double ct = 1.0 - 2.0 * u_or[0];
+    double st = sqrt(1.0 - ct * ct);
+    double ph = TWO_PI * u_or[1];
+    double ps = TWO_PI * u_or[2];
+    frame_from_angles(st, ct, sin(ph), cos(ph), sin(ps), cos(ps), A, B, C);
+  } else if (m->orient_kind == ORC_ORIENT_UNIFORM_ANGLES_MC) {
+    /* R-N3: theta ~ U[0, pi], phi ~ U[0, 2 pi], psi ~ U[0, 2 pi] exactly as printed */
+    double th = PI_ * u_or[0];
+    double ph = TWO_PI * u_or[1];
+    double ps = TWO_PI * u_or[2];
+    frame_from_angles(sin(th), cos(th), sin(ph), cos(ph), sin(ps), cos(ps), A, B, C);
+  } else {
+    frame_from_angles(sin(m->theta), cos(m->theta), sin(m->phi), cos(m->phi), sin(m->psi),
+                      cos(m->psi), A, B, C);
+  }
+}
+
 /* I(Q) = 1e8 scale <F^2>/<V> S(q) + background  (Eq. 2-4;
  * R-A2, R-A6).  Averages are fixed-node sums (R-A1, R-A9, R-A11). */
 double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3], double* env_out) {
@@ -218,17 +240,7 @@ double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3]
     return m->scale + m->background;
   }
   double A[3], B[3], C[3];
-  if (m->orient_kind == ORC_ORIENT_ISOTROPIC_MC) {
-    /* R-A3: isotropic = cos(theta) uniform, phi and psi uniform */
-    double ct = 1.0 - 2.0 * u_or[0];
-    double st = sqrt(1.0 - ct * ct);
-    double ph = TWO_PI * u_or[1];
-    double ps = TWO_PI * u_or[2];
-    frame_from_angles(st, ct, sin(ph), cos(ph), sin(ps), cos(ps), A, B, C);
-  } else {
-    frame_from_angles(sin(m->theta), cos(m->theta), sin(m->phi), cos(m->phi), sin(m->psi),
-                      cos(m->psi), A, B, C);
-  }
+  particle_frame(m, u_or, A, B, C);
   double qA = dot3(Q, A), qB = dot3(Q, B), qC = dot3(Q, C);
   double q2 = dot3(Q, Q);
   double qm = sqrt(q2);
@@ -270,6 +282,42 @@ double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3]
   if (m->sq_kind == ORC_SQ_HARD_SPHERE_PY) S = orc_py_sq(qm, m->sq_radius_eff, m->sq_volfrac);
   if (env_out) *env_out = ((1.0e8 * m->scale) * (SE2 / SV)) * S + m->background;
   return ((1.0e8 * m->scale) * (SF2 / SV)) * S + m->background;
+}
+
+/* R-N2: the paper's per-event model, Eq. 4 literally: M = A A* / V with the sizes of THIS scattering
+ * event, I = 1e8 scale M S(q) + background.  x[k] = relative size of axis k. */
+double orc_intensity_event(const orc_model* m, const double Q[3], const double u_or[3], const double x[2],
+                           double* env_out) {
+  if (m->model == ORC_FLAT) {
+    if (env_out) *env_out = m->scale + m->background;
+    return m->scale + m->background;
+  }
+  double A[3], B[3], C[3];
+  particle_frame(m, u_or, A, B, C);
+  double qA = dot3(Q, A), qB = dot3(Q, B), qC = dot3(Q, C);
+  double qm = sqrt(dot3(Q, Q));
+  double V, E;
+  double F = orc_amplitude(m, qA, qB, qC, x[0], x[1], &V, &E);
+  double S = 1.0;
+  if (m->sq_kind == ORC_SQ_HARD_SPHERE_PY) S = orc_py_sq(qm, m->sq_radius_eff, m->sq_volfrac);
+  if (env_out) *env_out = ((1.0e8 * m->scale) * ((E * E) / V)) * S + m->background;
+  return ((1.0e8 * m->scale) * ((F * F) / V)) * S + m->background;
+}
+
+/* R-N1 (Eq. 8): r = mean (1 + rel z), z standard normal by Box-Muller from the two
+ * uniforms (words 2k, 2k+1) of Philox block 3 + t, t = 0, 1, ...: "radii and distances are always checked
+ * to be positively defined, else a new iteration of the random choice is performed".  After 8 blocks
+ * the mean is taken (probability Phi(-1/rel)^8). */
+double orc_draw_rel_size(uint64_t seed, uint64_t id, uint32_t exp_index, int k, double rel, int32_t* tries) {
+  for (int t = 0; t < 8; ++t) {
+    double u4[4];
+    draw_block(seed, id, 3u + (uint32_t)t, exp_index, u4);
+    double z = sqrt(-2.0 * log(u4[2 * k])) * cos(TWO_PI * u4[2 * k + 1]);
+    double x = 1.0 + rel * z;
+    if (tries) *tries = t + 1;
+    if (x > 0.0) return x;
+  }
+  return 1.0;
 }
 
 /* ------------------------------------------------------------- R-C5 */
@@ -409,7 +457,9 @@ void orc_trace_one(const orc_instrument* ins, const orc_model* m, uint64_t seed,
   rec->pixel = iy * ins->det_nx + ix;
 
   /* orientation uniforms (draws 8,9,10) only for per-neutron random orientation */
-  if (m->orient_kind == ORC_ORIENT_ISOTROPIC_MC && m->model != ORC_FLAT) draw_block(seed, id, 2, exp_index, u + 8);
+  if ((m->orient_kind == ORC_ORIENT_ISOTROPIC_MC || m->orient_kind == ORC_ORIENT_UNIFORM_ANGLES_MC) &&
+      m->model != ORC_FLAT)
+    draw_block(seed, id, 2, exp_index, u + 8);
 
   /* R-C11 attenuation along the path inside the sample */
   double T = 1.0;
@@ -421,8 +471,16 @@ void orc_trace_one(const orc_instrument* ins, const orc_model* m, uint64_t seed,
     T = exp(-(mu * (u[5] * ell + ell_out)));
   }
 
-  double env;
-  double I = orc_intensity(m, Q, u + 8, &env);
+  double env, I;
+  rec->pd_x[0] = rec->pd_x[1] = 1.0;
+  if ((m->pd_mc[0] || m->pd_mc[1]) && m->model != ORC_FLAT) {
+    /* the paper's own size averaging: one size per scattering event (R-N1, R-N2) */
+    for (int kk = 0; kk < 2; ++kk)
+      if (m->pd_mc[kk]) rec->pd_x[kk] = orc_draw_rel_size(seed, id, exp_index, kk, m->pd_rel[kk], &rec->pd_tries[kk]);
+    I = orc_intensity_event(m, Q, u + 8, rec->pd_x, &env);
+  } else {
+    I = orc_intensity(m, Q, u + 8, &env);
+  }
   rec->intensity = I;
   double jac = qk * inv_k;                            /* q / k^2 */
   double qnorm = TWO_PI * (ins->q_max - ins->q_min);  /* 1 / pdf(q, chi) */

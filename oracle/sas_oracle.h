@@ -42,7 +42,12 @@ enum {
   ORC_CORE_SHELL_TRIAXIAL = 4,
   ORC_FLAT = 5
 };
-enum { ORC_ORIENT_FIXED = 0, ORC_ORIENT_GAUSS_QUAD = 1, ORC_ORIENT_ISOTROPIC_MC = 2 };
+enum {
+  ORC_ORIENT_FIXED = 0,
+  ORC_ORIENT_GAUSS_QUAD = 1,
+  ORC_ORIENT_ISOTROPIC_MC = 2,
+  ORC_ORIENT_UNIFORM_ANGLES_MC = 3 /* PAPER.md:131-133 as printed: theta~U[0,pi], phi, psi~U[0,2pi] (R-N3) */
+};
 enum { ORC_SQ_NONE = 0, ORC_SQ_HARD_SPHERE_PY = 1 };
 
 #define ORC_MAX_NODES 64
@@ -86,6 +91,11 @@ typedef struct {
   double or_d[2][ORC_MAX_NODES];  /* tilt angle Delta (rad) */
   double or_w[2][ORC_MAX_NODES];
   double sq_radius_eff, sq_volfrac;
+  /* The paper's own polydispersity (Eq. 8; DESIGN.md R-N1, R-N2): pd_mc[k] != 0 draws
+   * length k of every scattering event from N(mean, (pd_rel[k] mean)^2), redrawn while not positive;
+   * the fixed-node tables of axis k must then be the single node (1.0, 1.0). */
+  int32_t pd_mc[2];
+  double pd_rel[2];
 } orc_model;
 
 /* full per-neutron record, for pins and parity */
@@ -101,6 +111,8 @@ typedef struct {
   double p0;           /* source weight */
   double intensity;    /* I(Q) 1/cm */
   double u[12];        /* the uniforms drawn (unused ones stay 0) */
+  double pd_x[2];      /* relative sizes drawn for this event (1 when the axis is not sampled) */
+  int32_t pd_tries[2]; /* Philox blocks used by each sampled axis (1 = no redraw) */
 } orc_record;
 
 /* Philox4x32-10, Salmon et al. SC'11 (DESIGN.md R-B). */
@@ -116,6 +128,11 @@ double orc_py_sq(double q, double r_eff, double volfrac);
  * uniforms u_or[3] (used only by ORC_ORIENT_ISOTROPIC_MC). env (nullable)
  * receives the envelope intensity. */
 double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3], double* env);
+/* The per-event form of the paper (Eq. 4 with the event's own sizes, R-N2): relative sizes x[2] given. */
+double orc_intensity_event(const orc_model* m, const double Q[3], const double u_or[3], const double x[2],
+                           double* env);
+/* Relative size of axis k of event (seed, id, exp) by R-N1; *tries = Philox blocks consumed. */
+double orc_draw_rel_size(uint64_t seed, uint64_t id, uint32_t exp_index, int k, double rel, int32_t* tries);
 /* amplitude F (A^-2 * A^3) of one particle with explicit axes projections */
 double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double x0, double x1,
                      double* vol, double* env);

@@ -58,8 +58,23 @@ enum {
   SAS_CORE_SHELL_TRIAXIAL = 4, /* B.3's shape with B.1's two-contrast composition (DESIGN.md R-A12) */
   SAS_FLAT = 5                 /* I == scale + background: test model */
 };
-enum { SAS_ORIENT_FIXED = 0, SAS_ORIENT_GAUSS_QUAD = 1, SAS_ORIENT_ISOTROPIC_MC = 2 };
-enum { SAS_PD_NONE = 0, SAS_PD_SCHULZ_QUAD = 1 };
+enum {
+  SAS_ORIENT_FIXED = 0,
+  SAS_ORIENT_GAUSS_QUAD = 1,
+  SAS_ORIENT_ISOTROPIC_MC = 2,
+  /* the paper's printed law, one draw per scattering event: theta ~ U[0,pi], phi, psi ~ U[0,2pi]
+   * (DESIGN.md R-N3: not isotropic) */
+  SAS_ORIENT_UNIFORM_ANGLES_MC = 3
+};
+enum {
+  SAS_PD_NONE = 0,
+  SAS_PD_SCHULZ_QUAD = 1,
+  /* the paper's own averaging (Eq. 8; DESIGN.md R-N1, R-N2): one size per scattering
+   * event from N(mean, (pd_rel mean)^2), redrawn while not positive; the event's intensity is Eq. 4 with
+   * the event's own volume.  Does not combine with SAS_PD_SCHULZ_QUAD or SAS_ORIENT_GAUSS_QUAD
+   * (SAS_EUNSUPPORTED); evaluated in fp64 whatever `precision` says. */
+  SAS_PD_GAUSS_MC = 2
+};
 enum { SAS_SQ_NONE = 0, SAS_SQ_HARD_SPHERE_PY = 1 };
 
 #define SAS_MAX_NODES 64      /* per quadrature axis */

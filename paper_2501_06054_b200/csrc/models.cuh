@@ -62,6 +62,114 @@ __device__ __forceinline__ Real cyl_quad_row(const Real* tph, int n_ph, Real Ai,
   return row;
 }
 
+// Particle axes A, B, C in the global frame (R-A7): the fixed / mean frame of the experiment, or one random
+// orientation per scattering event from draws 8, 9, 10 (Philox block 2): isotropic (R-A3) or the paper's
+// printed uniform angles (R-N3).  LIBM: CUDA's fp64 sincos, else the 1e-13 fp64 kernels.
+template <bool LIBM, int V>
+__device__ __forceinline__ void particle_frame(const ExpParams& P, const PhiloxKeys& keys, uint32_t id_lo, uint32_t id_hi,
+                                               uint32_t exp_word, double A[3], double B[3], double C[3]) {
+  if (V != V_CYL_QUAD && P.orient_kind >= 2) {
+    uint32_t w2[4];
+    philox4x32_10(keys, id_lo, id_hi, 2u, exp_word, w2);
+    const double u8 = uniform_from_word(w2[0]), u9 = uniform_from_word(w2[1]), u10 = uniform_from_word(w2[2]);
+    double ct, st, sp, cp, ss, cs;
+    if (P.orient_kind == 3) {  // theta = pi u8
+      if (LIBM) sincospi(u8, &st, &ct); else sincos_2pi(0.5 * u8, st, ct);
+    } else {                   // cos(theta) = 1 - 2 u8
+      ct = 1.0 - 2.0 * u8;
+      st = sqrt(1.0 - ct * ct);
+    }
+    if (LIBM) {
+      // sincospi reduces exactly and has no large-argument path: within 1e-15 of sin/cos(TWO_PI u) as R-A3 writes it
+      sincospi(2.0 * u9, &sp, &cp);
+      sincospi(2.0 * u10, &ss, &cs);
+    } else {
+      sincos_2pi(u9, sp, cp);
+      sincos_2pi(u10, ss, cs);
+    }
+    const double a0[3] = {ct * cp, ct * sp, -st};
+    const double b0[3] = {-sp, cp, 0.0};
+    C[0] = st * cp; C[1] = st * sp; C[2] = ct;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      A[i] = fma(cs, a0[i], ss * b0[i]);
+      B[i] = fma(cs, b0[i], -(ss * a0[i]));
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { A[i] = P.frame[i]; B[i] = P.frame[3 + i]; C[i] = P.frame[6 + i]; }
+  }
+}
+
+// R-N1 (Eq. 8): relative size of polydisperse length k of this scattering event,
+// 1 + rel z with z standard normal by Box-Muller from words 2k, 2k+1 of Philox block 3 + t; the draw is
+// repeated (t = 1, 2, ...) while the size is not positive; after 8 blocks the mean is taken.
+__device__ __forceinline__ double draw_rel_size(const PhiloxKeys& keys, uint32_t id_lo, uint32_t id_hi, uint32_t exp_word,
+                                                int k, double rel) {
+  for (uint32_t t = 0; t < 8u; ++t) {
+    uint32_t w[4];
+    philox4x32_10(keys, id_lo, id_hi, 3u + t, exp_word, w);
+    const double ua = uniform_from_word(k ? w[2] : w[0]), ub = uniform_from_word(k ? w[3] : w[1]);
+    const double x = 1.0 + rel * (sqrt(-2.0 * log(ua)) * cos(6.283185307179586 * ub));
+    if (x > 0.0) return x;
+  }
+  return 1.0;
+}
+
+// R-N2: the paper's per-event model, Eq. 4 with the sizes of THIS scattering event:
+// I = 1e8 scale F(r)^2 / V(r) S(q) + background, one fp64 evaluation per detected neutron.
+// (compiled into kernels of its own, trace_kernel<double, V, true>: in the same kernel as the fixed-node
+// path it cost that path 3-6 % through register allocation and code layout)
+template <int V>
+__device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const PhiloxKeys& keys, uint32_t id_lo,
+                                                       uint32_t id_hi, uint32_t exp_word, double Qx, double Qy, double Qz) {
+  if (V == V_FLAT) return P.flat_I;
+  const double x0 = P.pd_mc[0] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 0, P.pd_rel[0]) : 1.0;
+  const double x1 = P.pd_mc[1] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 1, P.pd_rel[1]) : 1.0;
+  const double q = sqrt(fma(Qx, Qx, fma(Qy, Qy, Qz * Qz)));
+  double qA = 0, qB = 0, qC = 0;
+  if (V >= 2) {
+    double A[3], B[3], C[3];
+    particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
+    qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
+    qB = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
+    qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
+  }
+  const double FOUR_PI_3 = 4.1887902047863905, PI_D = 3.141592653589793;
+  const double s0 = P.ev_sld[0], s1 = P.ev_sld[1];
+  double F = 1.0, Vol = 1.0;
+  if (V == V_SPHERE) {
+    const double R = P.msize[0] * x0;
+    Vol = FOUR_PI_3 * ((R * R) * R);
+    F = (s0 * Vol) * sphere_phi(q * R);
+  } else if (V == V_CS_SPHERE) {
+    const double Rc = P.msize[0] * x0, Rt = Rc + P.msize[1] * x1;
+    const double Vc = FOUR_PI_3 * ((Rc * Rc) * Rc);
+    Vol = FOUR_PI_3 * ((Rt * Rt) * Rt);
+    F = fma((s0 - s1) * Vc, sphere_phi(q * Rc), (s1 * Vol) * sphere_phi(q * Rt));
+  } else if (V == V_CYL) {
+    const double R = P.msize[0] * x0, L = P.msize[1] * x1;
+    Vol = (PI_D * (R * R)) * L;
+    F = ((s0 * Vol) * sinc_r(qC * (0.5 * L))) * lambda1_r(sqrt(fma(qA, qA, qB * qB)) * R);
+  } else if (V == V_TRIAX) {
+    const double a = P.msize[0] * x0, b = P.msize[1] * x0, c = P.msize[2] * x0;
+    Vol = FOUR_PI_3 * ((a * b) * c);
+    const double ua = a * qA, ub = b * qB, uc = c * qC;
+    F = (s0 * Vol) * sphere_phi(sqrt(fma(ua, ua, fma(ub, ub, uc * uc))));
+  } else if (V == V_CS_TRIAX) {
+    const double a = P.msize[0] * x0, b = P.msize[1] * x0, c = P.msize[2] * x0, t = P.msize[3] * x1;
+    const double at = a + t, bt = b + t, ct = c + t;
+    const double Vc = FOUR_PI_3 * ((a * b) * c);
+    Vol = FOUR_PI_3 * ((at * bt) * ct);
+    const double ua = a * qA, ub = b * qB, uc = c * qC, va = at * qA, vb = bt * qB, vc = ct * qC;
+    F = fma((s0 - s1) * Vc, sphere_phi(sqrt(fma(ua, ua, fma(ub, ub, uc * uc)))),
+            (s1 * Vol) * sphere_phi(sqrt(fma(va, va, fma(vb, vb, vc * vc)))));
+  }
+  double S = 1.0;
+  if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
+  return fma((P.ev_scale * ((F * F) / Vol)), S, P.background);
+}
+
 // Model table meaning (host: fill_model).  Lengths that multiply a projection of Q are stored as a
 // (hi, lo) pair: in the fp32 path hi = float(L), lo = float(L - hi); in the fp64 path hi = L, lo = 0.
 //  sphere              ta = {R_hi, R_lo, w_a (drho V_a)^2}
@@ -87,33 +195,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
   double qAd = 0, qBd = 0, qCd = 0;
   if (model >= 2) {
     double A[3], B[3], C[3];
-    if (V != V_CYL_QUAD && P.orient_kind == 2) {
-      // R-A3: one isotropic random orientation per neutron, draws 8, 9, 10
-      uint32_t w2[4];
-      philox4x32_10(keys, id_lo, id_hi, 2u, exp_word, w2);
-      const double u8 = uniform_from_word(w2[0]), u9 = uniform_from_word(w2[1]), u10 = uniform_from_word(w2[2]);
-      const double ct = 1.0 - 2.0 * u8;
-      const double st = sqrt(1.0 - ct * ct);
-      double sp, cp, ss, cs;
-      if (sizeof(Real) == 8) {
-        sincos(6.283185307179586 * u9, &sp, &cp);
-        sincos(6.283185307179586 * u10, &ss, &cs);
-      } else {
-        sincos_2pi(u9, sp, cp);
-        sincos_2pi(u10, ss, cs);
-      }
-      const double a0[3] = {ct * cp, ct * sp, -st};
-      const double b0[3] = {-sp, cp, 0.0};
-      C[0] = st * cp; C[1] = st * sp; C[2] = ct;
-#pragma unroll
-      for (int i = 0; i < 3; ++i) {
-        A[i] = fma(cs, a0[i], ss * b0[i]);
-        B[i] = fma(cs, b0[i], -(ss * a0[i]));
-      }
-    } else {
-#pragma unroll
-      for (int i = 0; i < 3; ++i) { A[i] = P.frame[i]; B[i] = P.frame[3 + i]; C[i] = P.frame[6 + i]; }
-    }
+    particle_frame<sizeof(Real) == 8, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
     qAd = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
     qBd = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
     qCd = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));

@@ -52,8 +52,9 @@ struct sas_ctx {
   unsigned long long* d_counters = nullptr;
   unsigned int* d_work = nullptr;
   // experiments grouped by kernel variant: one launch per non-empty group (ids concatenated on the device)
-  std::vector<uint32_t> group_ids[N_VARIANTS];
-  size_t group_off[N_VARIANTS] = {};
+  // (groups N_VARIANTS.. are the per-event-size kernels of the same variants)
+  std::vector<uint32_t> group_ids[2 * N_VARIANTS];
+  size_t group_off[2 * N_VARIANTS] = {};
   uint32_t* d_exp_ids = nullptr;
   cudaStream_t stream = nullptr;
   bool own_stream = true;
@@ -106,7 +107,7 @@ sas_status validate_model(const sas_model_desc* m, std::string& why) {
   if (m->struct_size != sizeof(sas_model_desc)) { why = "sas_model_desc.struct_size mismatch"; return SAS_EINVAL; }
   if (m->model < SAS_SPHERE || m->model > SAS_FLAT) { why = "unknown model"; return SAS_EINVAL; }
   if (m->precision != SAS_FP32 && m->precision != SAS_FP64) { why = "unknown precision"; return SAS_EINVAL; }
-  if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_ISOTROPIC_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
+  if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_UNIFORM_ANGLES_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
   if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY) { why = "unknown sq_kind"; return SAS_EINVAL; }
   if (!std::isfinite(m->scale) || !std::isfinite(m->background)) { why = "scale/background not finite"; return SAS_EINVAL; }
   static const int n_sizes[6] = {1, 2, 2, 3, 4, 0};
@@ -117,7 +118,15 @@ sas_status validate_model(const sas_model_desc* m, std::string& why) {
     if (!std::isfinite(m->size[i]) || m->size[i] < 0.0 || (!may_be_zero && m->size[i] == 0.0)) { why = "model sizes must be > 0"; return SAS_EINVAL; }
   }
   for (int k = 0; k < 2; ++k) {
-    if (m->pd_kind[k] != SAS_PD_NONE && m->pd_kind[k] != SAS_PD_SCHULZ_QUAD) { why = "unknown pd_kind"; return SAS_EINVAL; }
+    if (m->pd_kind[k] != SAS_PD_NONE && m->pd_kind[k] != SAS_PD_SCHULZ_QUAD && m->pd_kind[k] != SAS_PD_GAUSS_MC) { why = "unknown pd_kind"; return SAS_EINVAL; }
+    if (m->pd_kind[k] == SAS_PD_GAUSS_MC) {
+      if (k >= n_pd[m->model]) { why = "this model has no such polydisperse length"; return SAS_EINVAL; }
+      if (!(m->pd_rel[k] >= 0.0) || !std::isfinite(m->pd_rel[k])) { why = "pd_rel must be >= 0"; return SAS_EINVAL; }
+      if (m->pd_kind[1 - k] == SAS_PD_SCHULZ_QUAD || m->orient_kind == SAS_ORIENT_GAUSS_QUAD) {
+        why = "per-event sizes (SAS_PD_GAUSS_MC) do not combine with fixed-node averages (DESIGN.md R-N1)";
+        return SAS_EUNSUPPORTED;
+      }
+    }
     if (m->pd_kind[k] == SAS_PD_SCHULZ_QUAD) {
       if (k >= n_pd[m->model]) { why = "this model has no such polydisperse length"; return SAS_EINVAL; }
       if (m->pd_nodes[k] < 1 || m->pd_nodes[k] > SAS_MAX_NODES) { why = "pd_nodes must be in 1..SAS_MAX_NODES"; return SAS_EINVAL; }
@@ -226,6 +235,10 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
 void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool) {
   P.model = m.model; P.orient_kind = m.orient_kind; P.sq_kind = m.sq_kind;
   P.background = m.background;
+  // per-event size sampling (R-N1, R-N2): the event evaluates Eq. 4 from the descriptor's own numbers
+  for (int k = 0; k < 2; ++k) { P.pd_mc[k] = m.pd_kind[k] == SAS_PD_GAUSS_MC ? 1 : 0; P.pd_rel[k] = m.pd_rel[k]; }
+  P.ev_sld[0] = m.sld[0]; P.ev_sld[1] = m.sld[1];
+  P.ev_scale = 1.0e8 * m.scale;
   P.flat_I = m.scale + m.background;
   std::vector<double> xa, wa, xb, wb, dth, wth, dph, wph;
   schulz_rule(m.pd_kind[0] == SAS_PD_SCHULZ_QUAD ? m.pd_rel[0] : 0.0, m.pd_nodes[0], xa, wa);
@@ -375,7 +388,11 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   // it, and a monodisperse form factor near its zeros cannot meet 1e-5 in fp32.
   bool any_loop = false;
   for (uint32_t e = 0; e < c->n_exp; ++e) any_loop = any_loop || node_evaluations(models[e]) > 1;
-  c->precision = (models[0].precision == SAS_FP64 || !any_loop) ? SAS_FP64 : SAS_FP32;
+  // ... and per-event sizes (SAS_PD_GAUSS_MC) are one fp64 evaluation per neutron as well (R-N2)
+  bool any_event = false;
+  for (uint32_t e = 0; e < c->n_exp; ++e)
+    any_event = any_event || models[e].pd_kind[0] == SAS_PD_GAUSS_MC || models[e].pd_kind[1] == SAS_PD_GAUSS_MC;
+  c->precision = (models[0].precision == SAS_FP64 || !any_loop || any_event) ? SAS_FP64 : SAS_FP32;
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     ExpParams& P = c->h_exps[e];
     fill_instrument(c->instr[e], P);
@@ -401,10 +418,11 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     const ExpParams& P = c->h_exps[e];
     const int v = (P.model == SAS_CYLINDER && P.orient_kind == SAS_ORIENT_GAUSS_QUAD) ? (int)V_CYL_QUAD : P.model;
-    c->group_ids[v].push_back(e);
+    const bool event = (P.pd_mc[0] | P.pd_mc[1]) != 0 && P.model != SAS_FLAT;
+    c->group_ids[v + (event ? (int)N_VARIANTS : 0)].push_back(e);
   }
   std::vector<uint32_t> ids;
-  for (int v = 0; v < N_VARIANTS; ++v) {
+  for (int v = 0; v < 2 * N_VARIANTS; ++v) {
     c->group_off[v] = ids.size();
     ids.insert(ids.end(), c->group_ids[v].begin(), c->group_ids[v].end());
   }
@@ -424,11 +442,11 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   return SAS_OK;
 }
 
-template <typename Real, int V>
+template <typename Real, int V, bool EV>
 sas_status launch(sas_ctx* c, KernelArgs& a) {
   const bool DUMP = a.d_pixel != nullptr;
   const size_t smem = trace_smem_bytes<Real>(c->tab_len_max);
-  auto kern = trace_kernel<Real, V>;
+  auto kern = trace_kernel<Real, V, EV>;
   if (smem > 227 * 1024) return fail(c, SAS_EINVAL, "quadrature tables do not fit in shared memory");
   CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int bps = 0;
@@ -470,27 +488,30 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   return SAS_OK;
 }
 
-// one launch of the kernel compiled for variant v over the experiments of that group
-template <typename Real>
-sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v) {
-  a.exp_ids = c->d_exp_ids + c->group_off[v];
-  a.n_exp = (uint32_t)c->group_ids[v].size();
+// one launch of the kernel compiled for group g (variant, fixed-node or per-event sizes) over its experiments
+template <typename Real, bool EV>
+sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v, int g) {
+  a.exp_ids = c->d_exp_ids + c->group_off[g];
+  a.n_exp = (uint32_t)c->group_ids[g].size();
   switch (v) {
-    case V_SPHERE: return launch<Real, V_SPHERE>(c, a);
-    case V_CS_SPHERE: return launch<Real, V_CS_SPHERE>(c, a);
-    case V_CYL: return launch<Real, V_CYL>(c, a);
-    case V_TRIAX: return launch<Real, V_TRIAX>(c, a);
-    case V_CS_TRIAX: return launch<Real, V_CS_TRIAX>(c, a);
-    case V_FLAT: return launch<Real, V_FLAT>(c, a);
-    case V_CYL_QUAD: return launch<Real, V_CYL_QUAD>(c, a);
+    case V_SPHERE: return launch<Real, V_SPHERE, EV>(c, a);
+    case V_CS_SPHERE: return launch<Real, V_CS_SPHERE, EV>(c, a);
+    case V_CYL: return launch<Real, V_CYL, EV>(c, a);
+    case V_TRIAX: return launch<Real, V_TRIAX, EV>(c, a);
+    case V_CS_TRIAX: return launch<Real, V_CS_TRIAX, EV>(c, a);
+    case V_FLAT: return launch<Real, V_FLAT, false>(c, a);
+    case V_CYL_QUAD: return launch<Real, V_CYL_QUAD, false>(c, a);
     default: return fail(c, SAS_EINVAL, "unknown kernel variant");
   }
 }
 
 sas_status launch_groups(sas_ctx* c, KernelArgs& a) {
-  for (int v = 0; v < N_VARIANTS; ++v) {
-    if (c->group_ids[v].empty()) continue;
-    sas_status st = c->precision == SAS_FP64 ? launch_variant<double>(c, a, v) : launch_variant<float>(c, a, v);
+  for (int g = 0; g < 2 * N_VARIANTS; ++g) {
+    if (c->group_ids[g].empty()) continue;
+    const int v = g % N_VARIANTS;
+    sas_status st;
+    if (g >= N_VARIANTS) st = launch_variant<double, true>(c, a, v, g);  // upload_models forced fp64
+    else st = c->precision == SAS_FP64 ? launch_variant<double, false>(c, a, v, g) : launch_variant<float, false>(c, a, v, g);
     if (st != SAS_OK) return st;
   }
   return SAS_OK;

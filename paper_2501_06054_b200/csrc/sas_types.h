@@ -40,6 +40,9 @@ struct ExpParams {
   double frame[9];    // particle axes A, B, C in the global frame for fixed / mean orientation (R-A7)
   double msize[4];    // mean sizes (triaxial a, b, c)
   PYCoef py;
+  // per-event size sampling (SAS_PD_GAUSS_MC, DESIGN.md R-N1/R-N2): contrasts, 1e8 scale, widths (sizes: msize)
+  double ev_sld[2], ev_scale, pd_rel[2];
+  int32_t pd_mc[2];
   // slit-1 integer prefilter: when slit 1 lies in the source plane the test |x0| <= hx is a monotone
   // function of the Philox word, so it is decided on the raw 32-bit draws (bit-identical to the fp64 test)
   uint32_t s1_lo[2], s1_hi[2];

@@ -74,7 +74,9 @@ __device__ __forceinline__ void flush_outcomes(unsigned long long* counters, con
   }
 }
 
-template <typename Real, int V>
+// EV: the experiments of this launch sample their sizes per scattering event (SAS_PD_GAUSS_MC); those
+// kernels exist in fp64 only and evaluate Eq. 4 once per detected neutron (models.cuh)
+template <typename Real, int V, bool EV>
 __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel(const __grid_constant__ KernelArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned int s_item;
@@ -155,7 +157,11 @@ __global__ void __launch_bounds__(BLOCK_THREADS, MIN_BLOCKS_PER_SM) trace_kernel
         cntC -= n;
         if (act) {
           const uint64_t id = a.first_id + idoff;
-          const Real I = eval_intensity<Real, V>(P, tab, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
+          Real I;
+          if (EV)
+            I = (Real)eval_intensity_event<V>(P, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
+          else
+            I = eval_intensity<Real, V>(P, tab, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
           const double p = G * (double)I;
           if (DUMP) {
             a.d_pixel[idoff] = pixel;

@@ -256,3 +256,64 @@ def test_certain_miss_classifier_never_changes_an_outcome(sas):
         assert np.array_equal(cnt[:7], ref[:7]), (k, cnt, ref)
         assert cnt[7] <= cnt[5]
         assert (cnt[7] > 0) == busy, (k, cnt)
+
+
+# ---- NEXT-1: the paper's own stochastic averaging (DESIGN.md R-N1..R-N3)
+PAPER_SAMPLING = [
+    ("sphere_gauss", dict(model="sphere", size=[50.0, 0, 0, 0], pd_kind=["gauss_mc", "none"], pd_rel=[0.15, 0.0])),
+    ("sphere_gauss_wide_py", dict(model="sphere", size=[40.0, 0, 0, 0], pd_kind=["gauss_mc", "none"], pd_rel=[0.9, 0.0],
+                                  scale=0.2, sq_kind="hard_sphere_py", sq_radius_eff=40.0, sq_volfrac=0.2)),
+    ("core_shell_gauss2", dict(model="core_shell_sphere", size=[40.0, 10.0, 0, 0], sld=[3e-6, 1e-6, 0],
+                               pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.1, 0.6])),
+    ("cylinder_paper", dict(model="cylinder", size=[119.0, 800.0, 0, 0], pd_kind=["gauss_mc", "gauss_mc"],
+                            pd_rel=[0.05, 0.05], orient_kind="uniform_angles_mc")),
+    ("cylinder_gauss_fixed", dict(model="cylinder", size=[20.0, 400.0, 0, 0], pd_kind=["none", "gauss_mc"],
+                                  pd_rel=[0.0, 0.2], theta=1.0, phi=0.4)),
+    ("triaxial_gauss_iso", dict(model="triaxial", size=[30.0, 50.0, 80.0, 0], pd_kind=["gauss_mc", "none"],
+                                pd_rel=[0.1, 0.0], orient_kind="isotropic_mc")),
+    ("cs_triaxial_paper", dict(model="core_shell_triaxial", size=[30.0, 50.0, 80.0, 10.0], sld=[3e-6, 1e-6, 0],
+                               pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.1, 0.1], orient_kind="uniform_angles_mc")),
+    ("cylinder_uniform_angles_nodes", dict(model="cylinder", size=[30.0, 150.0, 0, 0], orient_kind="uniform_angles_mc",
+                                           pd_kind=["schulz", "none"], pd_rel=[0.1, 0], pd_nodes=[6, 1])),
+]
+
+
+@pytest.mark.parametrize("name,over", PAPER_SAMPLING, ids=[m[0] for m in PAPER_SAMPLING])
+def test_paper_sampling_per_neutron(sas, name, over):
+    # per-event sizes are one fp64 evaluation per neutron whatever precision is asked for
+    precision = "fp32" if name == "cylinder_uniform_angles_nodes" else "fp64"
+    model = W.model(precision=precision, **over)
+    tol = TOL[precision]
+    check_dump(sas, W.instrument(det_dist=3.0), model, 20250111, 0, 150000, tol=tol, min_detected=5000)
+
+
+def test_paper_sampling_histogram_and_fp32_request(sas):
+    ins = W.instrument(det_dist=3.0, det_nx=64, det_ny=64)
+    over = dict(PAPER_SAMPLING[3][1])
+    n = 300000
+    ref = O.trace_range(ins, W.model(precision="fp64", **over), 7, 0, n, dump=False)
+    for precision in ("fp64", "fp32"):      # the fp32 request is served by the same fp64 event evaluation
+        tr = sas.Tracer(ins, W.model(precision=precision, **over))
+        tr.trace(n, 7)
+        sp, sp2, cn = tr.read_detector()
+        cnt = tr.counters()
+        tr.close()
+        assert np.array_equal(cnt[:7], ref["counters"][:7]) and np.array_equal(cn.reshape(-1), ref["counts"])
+        m = ref["sum_p"] > 0
+        assert np.abs(sp.reshape(-1)[m] / ref["sum_p"][m] - 1).max() < 1e-9
+        assert np.abs(sp2.reshape(-1)[m] / ref["sum_p2"][m] - 1).max() < 1e-9
+
+
+def test_paper_sampling_rejects_mixtures(sas):
+    ins = W.instrument()
+    for over in (dict(model="sphere", pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0], orient_kind="fixed",
+                      size=[50.0, 0, 0, 0]),):
+        sas.Tracer(ins, W.model(**over)).close()        # fine on its own
+    bad = [dict(model="core_shell_sphere", size=[40.0, 10.0, 0, 0], pd_kind=["gauss_mc", "schulz"], pd_rel=[0.1, 0.1],
+                pd_nodes=[1, 8]),
+           dict(model="cylinder", size=[20.0, 400.0, 0, 0], pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0],
+                orient_kind="gauss_quad", sigma_theta=0.1, sigma_phi=0.1, n_theta=4, n_phi=4)]
+    for over in bad:
+        with pytest.raises(sas.SasError) as e:
+            sas.Tracer(ins, W.model(**over))
+        assert e.value.status == 5                      # SAS_EUNSUPPORTED

@@ -113,6 +113,8 @@ def model_key_and_nodes(model):
     from paper_2501_06054_b200 import roofline as R  # noqa: F401
     m, prec = model["model"], model["precision"]
     pd = [n if k == "schulz" else 1 for k, n in zip(model["pd_kind"], model["pd_nodes"])]
+    if is_event_model(model) and m == "cylinder":
+        return "cylinder_event_fp64", 1
     if m == "sphere":
         nodes = pd[0]
         eff = prec if nodes > 1 else "fp64"
@@ -125,6 +127,10 @@ def model_key_and_nodes(model):
     if m == "cylinder":
         return "cylinder_iso_fp64", 1
     raise KeyError(m)
+
+
+def is_event_model(model):
+    return "gauss_mc" in model["pd_kind"]
 
 
 def time_steps(torch, tracer, do_step, steps, warmup, flush):
@@ -297,7 +303,7 @@ def main():
 
     others = {}
     if not args.headline_only:
-        for i in [j for j in range(5) if j != args.config]:
+        for i in [j for j in range(6) if j != args.config]:
             o, _ = bench_config(torch, S, i, 3, 3, rank, world, flush, False)
             others[o["workload"]] = {k: o[k] for k in ("value", "ms_per_step", "kernel_ms", "n_neutrons_per_step",
                                                        "detected_frac", "grid", "smem_bytes")}

@@ -45,6 +45,9 @@ MODEL_COST = {
     "cylinder_quad_fp32": ((60, 40, 4), (27, 0, 1)),
     "cs_triaxial_iso_fp32": ((40 + 40 + 90, 120, 6), (33, 0, 2)),
     "cylinder_iso_fp64": ((40 + 40 + 200 + 320, 520, 8), (0, 0, 0)),
+    # per-event sizes: Philox blocks 2 and 3, two Box-Muller normals (log, sqrt, cos in fp64), three sincospi,
+    # sin, j1, the weight
+    "cylinder_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12), (0, 0, 0)),
 }
 
 # DRAM traffic of one trace-kernel launch, dram__bytes_read.sum + dram__bytes_write.sum of the

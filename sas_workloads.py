@@ -56,7 +56,7 @@ def model(**over):
 
 
 def config(i: int, precision: str | None = None):
-    """Return dict(name, instrument, model, n_neutrons, seed) for config i in 0..3,
+    """Return dict(name, instrument, model, n_neutrons, seed) for config i in 0..3 and 5,
     or dict(name, instruments[], models[], n_neutrons_each, seed) for config 4."""
     if i == 0:
         return dict(name="c0_sphere_fp64", instrument=instrument(),
@@ -91,6 +91,16 @@ def config(i: int, precision: str | None = None):
             n_neutrons=10**9, seed=20250109)
     if i == 4:
         return batch_config(1024, 10**7, 20250110, precision or "fp32")
+    if i == 5:
+        # NEXT-1 (not a BASELINE.json config): the paper's own averaging on the cylinder it compares with a
+        # measurement (R = 119 A, L = 800 A, 5 % polydispersity, random orientation): one Gaussian
+        # size pair and one uniform-angle orientation per scattering event (DESIGN.md R-N1..R-N3)
+        return dict(
+            name="n1_paper_cylinder", instrument=instrument(det_nx=256, det_ny=256),
+            model=model(model="cylinder", precision="fp64", size=[119.0, 800.0, 0, 0],
+                        pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.05, 0.05],
+                        orient_kind="uniform_angles_mc"),
+            n_neutrons=10**9, seed=20250111)
     raise ValueError(i)
 
 

@@ -28,7 +28,8 @@ __device__ __forceinline__ void slab_axis(double o, double d, double h, double& 
 
 // Ray (o + t d) against the sample volume centred on the origin of the sample frame (R-C5).
 __device__ __forceinline__ bool intersect_sample(const ExpParams& P, double ox, double oy, double oz, double dx,
-                                                 double dy, double dz, double& t_in, double& t_out) {
+                                                 double dy, double dz, double& t_in, double& t_out,
+                                                 bool lateral_free = false) {
   double tin = -INFINITY, tout = INFINITY;
   bool miss = false;
   if (P.sample_shape == 1) {  // warp-uniform
@@ -43,10 +44,13 @@ __device__ __forceinline__ bool intersect_sample(const ExpParams& P, double ox, 
     miss = par ? (c > 0.0) : !(disc > 0.0);
     tin = par ? tin : t1;
     tout = par ? tout : t2;
-  } else {
+  } else if (!lateral_free) {
     slab_axis(ox, dx, P.hx, tin, tout, miss);
   }
-  slab_axis(oy, dy, P.hy, tin, tout, miss);
+  // lateral_free: the host proved that the beam envelope lies strictly inside the sample's lateral faces over
+  // its whole depth, so their slab intervals strictly contain the depth interval and max/min return the
+  // depth roots themselves: skipping them is bit-identical (primary ray only, not the scattered one)
+  if (!lateral_free) slab_axis(oy, dy, P.hy, tin, tout, miss);
   if (P.sample_shape != 1) slab_axis(oz, dz, P.hz, tin, tout, miss);
   t_in = tin;
   t_out = tout;
@@ -105,7 +109,7 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
   const double lambda = P.lambda_min + u4 * P.dlam;
   // R-C5 sample
   double tin, tout;
-  const bool hit_s = intersect_sample(P, x0, y0, 0.0 - P.sample_z, dx, dy, dz, tin, tout);
+  const bool hit_s = intersect_sample(P, x0, y0, 0.0 - P.sample_z, dx, dy, dz, tin, tout, P.lateral_free != 0);
   tin = tin < 0.0 ? 0.0 : tin;
   const bool f_ms = !hit_s || !(tout > tin);
   const double ell = tout - tin;

@@ -95,14 +95,18 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
   const double dx = Dx * inv_r, dy = Dy * inv_r, dz = Dz * inv_r;
   const double dOmega = ((P.focus_area * dz) * inv_r) * inv_r;
   const double p0 = (P.p0_pref * dOmega) * P.dlam_w;
-  // R-C4 slits
-  const double inv_dz = 1.0 / dz;
-  const double s1 = (P.slit1_z - 0.0) * inv_dz;
-  const double xs1 = x0 + dx * s1, ys1 = y0 + dy * s1;
-  const bool f_s1 = fabs(xs1) > P.slit1_hx || fabs(ys1) > P.slit1_hy;
-  const double s2s = (P.slit2_z - 0.0) * inv_dz;
-  const double xs2 = x0 + dx * s2s, ys2 = y0 + dy * s2s;
-  const bool f_s2 = fabs(xs2) > P.slit2_hx || fabs(ys2) > P.slit2_hy;
+  // R-C4 slits.  slits_free: stage A already applied the (bit-identical) integer slit-1 test and the host
+  // proved that slit 2 cannot cut a ray aimed at the focus rectangle: nothing to compute
+  bool f_s1 = false, f_s2 = false;
+  if (!P.slits_free) {
+    const double inv_dz = 1.0 / dz;
+    const double s1 = (P.slit1_z - 0.0) * inv_dz;
+    const double xs1 = x0 + dx * s1, ys1 = y0 + dy * s1;
+    f_s1 = fabs(xs1) > P.slit1_hx || fabs(ys1) > P.slit1_hy;
+    const double s2s = (P.slit2_z - 0.0) * inv_dz;
+    const double xs2 = x0 + dx * s2s, ys2 = y0 + dy * s2s;
+    f_s2 = fabs(xs2) > P.slit2_hx || fabs(ys2) > P.slit2_hy;
+  }
   // draws 4..7 (Philox block 1, drawn by the classifier stage)
   const double u4 = uniform_from_word(w1[0]), u5 = uniform_from_word(w1[1]);
   const double u6 = uniform_from_word(w1[2]), u7 = uniform_from_word(w1[3]);

@@ -196,7 +196,7 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
   P.det_nx = d.det_nx; P.det_ny = d.det_ny;
   P.s_cut = INFINITY;
   P.s1_int_ok = 0;
-  P.lateral_free = 0; P.pad_lf = 0;
+  P.lateral_free = 0; P.slits_free = 0;
   if (d.slit1_z == 0.0) {
     // slit 1 in the source plane: xs = x0 + dx*0 = x0 exactly, so the test depends on draws 0, 1 only
     slit1_word_window(d.src_xw, P.slit1_hx, P.s1_lo[0], P.s1_hi[0]);
@@ -224,6 +224,7 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
     // the lateral slabs of the sample cannot bind for a primary ray (needs the ray to start before the sample
     // and to move forward: z_near > 0, dz > 0 always); the cylinder's y slab likewise
     P.lateral_free = sample_sure ? 1 : 0;
+    P.slits_free = (P.s1_int_ok && slit2_sure) ? 1 : 0;
     const double d_min = (d.sample_z + d.det_dist) - z_far;
     if (P.s1_int_ok && slit2_sure && sample_sure && d_min > 0.0) {
       const double delta = std::atan(std::hypot(xf + x0m, yf + y0m) / d.focus_z);  // max tilt of d^ from z

@@ -48,7 +48,8 @@ struct ExpParams {
   uint32_t s1_lo[2], s1_hi[2];
   int32_t s1_int_ok;
   int32_t sample_shape, has_mu, det_nx, det_ny;
-  int32_t lateral_free, pad_lf;  // primary rays cannot touch the sample's lateral faces (geometry.cuh)
+  int32_t lateral_free;  // primary rays cannot touch the sample's lateral faces (geometry.cuh)
+  int32_t slits_free;    // no stage-B ray can be cut by a slit (geometry.cuh)
   int32_t model, orient_kind, sq_kind;
   int32_t n_a, n_b, n_th, n_ph;
   int32_t tab_off, tab_len;  // in doubles, inside the table pool

@@ -31,7 +31,7 @@ MAX_NODES = 64
 
 _SAMPLE = {"box": 0, "cyl_y": 1}
 _MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3,
-          "core_shell_triaxial": 4, "flat": 5}
+          "core_shell_triaxial": 4, "flat": 5, "parallelepiped": 6, "core_shell_cylinder": 7, "ellipsoid": 8}
 _ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
 _SQ = {"none": 0, "hard_sphere_py": 1}
 
@@ -195,8 +195,8 @@ def make_model(d: dict) -> Model:
     m.sq_volfrac = d["sq_volfrac"]
     if "gauss_mc" in d["pd_kind"] and (d["orient_kind"] == "gauss_quad" or "schulz" in d["pd_kind"]):
         raise ValueError("per-event sizes (gauss_mc) do not combine with fixed-node averages (DESIGN.md R-N1)")
-    if d["orient_kind"] == "gauss_quad" and d["model"] in ("triaxial", "core_shell_triaxial"):
-        raise ValueError("gauss_quad orientation is defined for uniaxial models only (DESIGN.md R-A11)")
+    if d["orient_kind"] == "gauss_quad" and d["model"] != "cylinder":
+        raise ValueError("gauss_quad orientation is built for the cylinder only (DESIGN.md R-A11)")
     return m
 
 

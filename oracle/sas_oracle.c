@@ -189,6 +189,40 @@ double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double
       *env = fabs(fc) + fabs(ft);
       return fc * orc_sphere_phi(uc) + ft * orc_sphere_phi(ut);
     }
+    case ORC_PARALLELEPIPED: {
+      /* Eq. 1 over the box |x|<=a/2, |y|<=b/2, |z|<=c/2 along A, B, C: the three 1-D integrals are
+       * a sinc(Q_A a/2) etc.  One common size scale x0 (as the triaxial ellipsoid, R-A12). */
+      double a = m->size[0] * x0, b = m->size[1] * x0, c = m->size[2] * x0;
+      double V = (a * b) * c;
+      *vol = V;
+      *env = m->sld[0] * V;
+      return (m->sld[0] * V) * ((orc_sinc(qa * (0.5 * a)) * orc_sinc(qb * (0.5 * b))) * orc_sinc(qc * (0.5 * c)));
+    }
+    case ORC_CORE_SHELL_CYLINDER: {
+      /* core cylinder (R, L) of contrast sld[0] inside a cylinder (R+t, L+2t) of contrast sld[1]:
+       * Eq. 1 with a piecewise contrast = (sld0-sld1) x core + sld1 x whole; x0 scales R, x1 scales L */
+      double R = m->size[0] * x0, L = m->size[1] * x1, t = m->size[2];
+      double Rt = R + t, Lt = L + 2.0 * t;
+      double Vc = (PI_ * (R * R)) * L;
+      double Vt = (PI_ * (Rt * Rt)) * Lt;
+      double qab = sqrt(qa * qa + qb * qb);
+      double fc = (m->sld[0] - m->sld[1]) * Vc;
+      double ft = m->sld[1] * Vt;
+      *vol = Vt;
+      *env = fabs(fc) + fabs(ft);
+      return (fc * orc_sinc(qc * (0.5 * L))) * orc_lambda1(qab * R) +
+             (ft * orc_sinc(qc * (0.5 * Lt))) * orc_lambda1(qab * Rt);
+    }
+    case ORC_ELLIPSOID: {
+      /* ellipsoid of revolution about C: the sphere amplitude at u = sqrt(R_e^2 Q_AB^2 + R_p^2 Q_C^2);
+       * x0 scales the equatorial, x1 the polar radius */
+      double Re = m->size[0] * x0, Rp = m->size[1] * x1;
+      double V = FOUR_PI_3 * ((Re * Re) * Rp);
+      double u = sqrt((Re * Re) * (qa * qa + qb * qb) + (Rp * qc) * (Rp * qc));
+      *vol = V;
+      *env = m->sld[0] * V;
+      return (m->sld[0] * V) * orc_sphere_phi(u);
+    }
     default:
       *vol = 1.0;
       *env = 1.0;

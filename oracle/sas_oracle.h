@@ -40,7 +40,11 @@ enum {
   ORC_CYLINDER = 2,
   ORC_TRIAXIAL = 3,
   ORC_CORE_SHELL_TRIAXIAL = 4,
-  ORC_FLAT = 5
+  ORC_FLAT = 5,
+  /* NEXT-2: three more of the paper's models, each Eq. 1 integrated over its body */
+  ORC_PARALLELEPIPED = 6,       /* Table I group E, Eq. 6: sides a, b, c along A, B, C */
+  ORC_CORE_SHELL_CYLINDER = 7,  /* Table I group A, Eq. 7: core R, L; shell t on every face */
+  ORC_ELLIPSOID = 8             /* Table I group B, Eq. 7: equatorial R_e, polar R_p (axis C) */
 };
 enum {
   ORC_ORIENT_FIXED = 0,

@@ -56,7 +56,12 @@ enum {
   SAS_CYLINDER = 2,            /* Table I  A.7, Eq. 9 */
   SAS_TRIAXIAL_ELLIPSOID = 3,  /* Table I  B.3  */
   SAS_CORE_SHELL_TRIAXIAL = 4, /* B.3's shape with B.1's two-contrast composition (DESIGN.md R-A12) */
-  SAS_FLAT = 5                 /* I == scale + background: test model */
+  SAS_FLAT = 5,                /* I == scale + background: test model */
+  /* NEXT-2: evaluated in fp64 whatever `precision` says; orientation fixed or per event
+   * (no SAS_ORIENT_GAUSS_QUAD) */
+  SAS_PARALLELEPIPED = 6,      /* size = a, b, c along A, B, C (Eq. 6); pd[0] = common scale */
+  SAS_CORE_SHELL_CYLINDER = 7, /* size = R, L, t (Eq. 7); sld[0] core, sld[1] shell; pd[0] on R, pd[1] on L */
+  SAS_ELLIPSOID = 8            /* size = R_equatorial, R_polar (axis C, Eq. 7); pd[0] on R_e, pd[1] on R_p */
 };
 enum {
   SAS_ORIENT_FIXED = 0,

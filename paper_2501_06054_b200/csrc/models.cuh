@@ -116,28 +116,17 @@ __device__ __forceinline__ double draw_rel_size(const PhiloxKeys& keys, uint32_t
   return 1.0;
 }
 
-// R-N2: the paper's per-event model, Eq. 4 with the sizes of THIS scattering event:
-// I = 1e8 scale F(r)^2 / V(r) S(q) + background, one fp64 evaluation per detected neutron.
-// (compiled into kernels of its own, trace_kernel<double, V, true>: in the same kernel as the fixed-node
-// path it cost that path 3-6 % through register allocation and code layout)
+// Amplitude F and normalising volume of ONE particle with relative sizes x0, x1 (R-A12 says which lengths
+// they scale), straight from the descriptor's numbers in fp64: Eq. 1 integrated over the body (R-C12; the
+// NEXT-2 bodies: box -> three sincs, core-shell cylinder -> two sinc x Lambda terms, ellipsoid of revolution
+// -> Phi at sqrt(Re^2 Q_AB^2 + Rp^2 Q_C^2)).
 template <int V>
-__device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const PhiloxKeys& keys, uint32_t id_lo,
-                                                       uint32_t id_hi, uint32_t exp_word, double Qx, double Qy, double Qz) {
-  if (V == V_FLAT) return P.flat_I;
-  const double x0 = P.pd_mc[0] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 0, P.pd_rel[0]) : 1.0;
-  const double x1 = P.pd_mc[1] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 1, P.pd_rel[1]) : 1.0;
-  const double q = sqrt(fma(Qx, Qx, fma(Qy, Qy, Qz * Qz)));
-  double qA = 0, qB = 0, qC = 0;
-  if (V >= 2) {
-    double A[3], B[3], C[3];
-    particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
-    qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
-    qB = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
-    qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
-  }
+__device__ __forceinline__ double particle_amplitude(const ExpParams& P, double q, double qA, double qB, double qC,
+                                                     double x0, double x1, double& Vol) {
   const double FOUR_PI_3 = 4.1887902047863905, PI_D = 3.141592653589793;
   const double s0 = P.ev_sld[0], s1 = P.ev_sld[1];
-  double F = 1.0, Vol = 1.0;
+  double F = 1.0;
+  Vol = 1.0;
   if (V == V_SPHERE) {
     const double R = P.msize[0] * x0;
     Vol = FOUR_PI_3 * ((R * R) * R);
@@ -164,10 +153,80 @@ __device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const
     const double ua = a * qA, ub = b * qB, uc = c * qC, va = at * qA, vb = bt * qB, vc = ct * qC;
     F = fma((s0 - s1) * Vc, sphere_phi(sqrt(fma(ua, ua, fma(ub, ub, uc * uc)))),
             (s1 * Vol) * sphere_phi(sqrt(fma(va, va, fma(vb, vb, vc * vc)))));
+  } else if (V == V_PARA) {
+    const double a = P.msize[0] * x0, b = P.msize[1] * x0, c = P.msize[2] * x0;
+    Vol = (a * b) * c;
+    F = (s0 * Vol) * ((sinc_r(qA * (0.5 * a)) * sinc_r(qB * (0.5 * b))) * sinc_r(qC * (0.5 * c)));
+  } else if (V == V_CS_CYL) {
+    const double R = P.msize[0] * x0, L = P.msize[1] * x1, t = P.msize[2];
+    const double Rt = R + t, Lt = L + 2.0 * t;
+    const double Vc = (PI_D * (R * R)) * L;
+    Vol = (PI_D * (Rt * Rt)) * Lt;
+    const double qab = sqrt(fma(qA, qA, qB * qB));
+    F = fma(((s0 - s1) * Vc) * sinc_r(qC * (0.5 * L)), lambda1_r(qab * R),
+            ((s1 * Vol) * sinc_r(qC * (0.5 * Lt))) * lambda1_r(qab * Rt));
+  } else if (V == V_ELL) {
+    const double Re = P.msize[0] * x0, Rp = P.msize[1] * x1;
+    Vol = FOUR_PI_3 * ((Re * Re) * Rp);
+    const double uc = Rp * qC;
+    F = (s0 * Vol) * sphere_phi(sqrt(fma(Re * Re, fma(qA, qA, qB * qB), uc * uc)));
   }
+  return F;
+}
+
+// R-N2: the paper's per-event model, Eq. 4 with the sizes of THIS scattering event:
+// I = 1e8 scale F(r)^2 / V(r) S(q) + background, one fp64 evaluation per detected neutron.
+// (compiled into kernels of its own, trace_kernel<double, V, true>: in the same kernel as the fixed-node
+// path it cost that path 3-6 % through register allocation and code layout)
+template <int V>
+__device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const PhiloxKeys& keys, uint32_t id_lo,
+                                                       uint32_t id_hi, uint32_t exp_word, double Qx, double Qy, double Qz) {
+  if (V == V_FLAT) return P.flat_I;
+  const double x0 = P.pd_mc[0] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 0, P.pd_rel[0]) : 1.0;
+  const double x1 = P.pd_mc[1] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 1, P.pd_rel[1]) : 1.0;
+  const double q = sqrt(fma(Qx, Qx, fma(Qy, Qy, Qz * Qz)));
+  double qA = 0, qB = 0, qC = 0;
+  if (V >= 2) {
+    double A[3], B[3], C[3];
+    particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
+    qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
+    qB = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
+    qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
+  }
+  double Vol;
+  const double F = particle_amplitude<V>(P, q, qA, qB, qC, x0, x1, Vol);
   double S = 1.0;
   if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
   return fma((P.ev_scale * ((F * F) / Vol)), S, P.background);
+}
+
+// Fixed-node average of the NEXT-2 models: the plain double sum over the (a, b) nodes of F^2, in fp64
+// (tables: node value and weight only).  <V> is in P.norm.
+template <typename Real, int V>
+__device__ __forceinline__ double eval_intensity_generic(const ExpParams& P, const Real* tab_base, const PhiloxKeys& keys,
+                                                         uint32_t id_lo, uint32_t id_hi, uint32_t exp_word, double Qx,
+                                                         double Qy, double Qz) {
+  const Real* ta = tab_base;
+  const Real* tb = ta + P.n_a * TA_W;
+  const double q = sqrt(fma(Qx, Qx, fma(Qy, Qy, Qz * Qz)));
+  double A[3], B[3], C[3];
+  particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
+  const double qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
+  const double qB = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
+  const double qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
+  double acc = 0.0;
+  for (int a = 0; a < P.n_a; ++a) {
+    double inner = 0.0;
+    for (int b = 0; b < P.n_b; ++b) {
+      double Vol;
+      const double F = particle_amplitude<V>(P, q, qA, qB, qC, (double)ta[a * TA_W], (double)tb[b * TB_W], Vol);
+      inner = fma((double)tb[b * TB_W + 2], F * F, inner);
+    }
+    acc = fma((double)ta[a * TA_W + 2], inner, acc);
+  }
+  double S = 1.0;
+  if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
+  return fma(P.norm * acc, S, P.background);
 }
 
 // Model table meaning (host: fill_model).  Lengths that multiply a projection of Q are stored as a
@@ -187,8 +246,9 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
                                                uint32_t id_lo, uint32_t id_hi, uint32_t exp_word, double Qx,
                                                double Qy, double Qz) {
   if (V == V_FLAT) return (Real)P.flat_I;
+  if (V >= V_PARA) return (Real)eval_intensity_generic<Real, V>(P, tab_base, keys, id_lo, id_hi, exp_word, Qx, Qy, Qz);
   const Tables<Real> T = table_views(tab_base, P);
-  constexpr int model = (V == V_CYL_QUAD) ? 2 : V;
+  constexpr int model = (V == V_CYL_QUAD) ? 2 : (V >= V_PARA ? 5 : V);
   // |Q| and the projections of Q on the particle axes (Eq. 6) in fp64: they feed the phases
   const double q2d = fma(Qx, Qx, fma(Qy, Qy, Qz * Qz));
   const double qd = sqrt(q2d);

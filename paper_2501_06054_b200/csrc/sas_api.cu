@@ -105,16 +105,17 @@ sas_status validate_instrument(const sas_instrument_desc* d, std::string& why) {
 sas_status validate_model(const sas_model_desc* m, std::string& why) {
   if (!m) { why = "model descriptor is NULL"; return SAS_EINVAL; }
   if (m->struct_size != sizeof(sas_model_desc)) { why = "sas_model_desc.struct_size mismatch"; return SAS_EINVAL; }
-  if (m->model < SAS_SPHERE || m->model > SAS_FLAT) { why = "unknown model"; return SAS_EINVAL; }
+  if (m->model < SAS_SPHERE || m->model > SAS_ELLIPSOID) { why = "unknown model"; return SAS_EINVAL; }
   if (m->precision != SAS_FP32 && m->precision != SAS_FP64) { why = "unknown precision"; return SAS_EINVAL; }
   if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_UNIFORM_ANGLES_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
   if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY) { why = "unknown sq_kind"; return SAS_EINVAL; }
   if (!std::isfinite(m->scale) || !std::isfinite(m->background)) { why = "scale/background not finite"; return SAS_EINVAL; }
-  static const int n_sizes[6] = {1, 2, 2, 3, 4, 0};
-  static const int n_pd[6] = {1, 2, 2, 1, 2, 0};
+  static const int n_sizes[9] = {1, 2, 2, 3, 4, 0, 3, 3, 2};
+  static const int n_pd[9] = {1, 2, 2, 1, 2, 0, 1, 2, 2};
   for (int i = 0; i < n_sizes[m->model]; ++i) {
     // a shell thickness may be 0, every other size must be > 0
-    const bool may_be_zero = (m->model == SAS_CORE_SHELL_SPHERE && i == 1) || (m->model == SAS_CORE_SHELL_TRIAXIAL && i == 3);
+    const bool may_be_zero = (m->model == SAS_CORE_SHELL_SPHERE && i == 1) || (m->model == SAS_CORE_SHELL_TRIAXIAL && i == 3) ||
+                             (m->model == SAS_CORE_SHELL_CYLINDER && i == 2);
     if (!std::isfinite(m->size[i]) || m->size[i] < 0.0 || (!may_be_zero && m->size[i] == 0.0)) { why = "model sizes must be > 0"; return SAS_EINVAL; }
   }
   for (int k = 0; k < 2; ++k) {
@@ -139,8 +140,8 @@ sas_status validate_model(const sas_model_desc* m, std::string& why) {
   if (m->orient_kind == SAS_ORIENT_GAUSS_QUAD) {
     if (m->n_theta < 1 || m->n_theta > SAS_MAX_NODES || m->n_phi < 1 || m->n_phi > SAS_MAX_NODES) { why = "n_theta/n_phi must be in 1..SAS_MAX_NODES"; return SAS_EINVAL; }
     if (!(m->sigma_theta >= 0.0) || !(m->sigma_phi >= 0.0)) { why = "orientation spreads must be >= 0"; return SAS_EINVAL; }
-    if (m->model == SAS_TRIAXIAL_ELLIPSOID || m->model == SAS_CORE_SHELL_TRIAXIAL) {
-      why = "SAS_ORIENT_GAUSS_QUAD is defined for uniaxial models only (DESIGN.md R-A11)";
+    if (m->model != SAS_CYLINDER) {
+      why = "SAS_ORIENT_GAUSS_QUAD is built for the cylinder only (DESIGN.md R-A11)";
       return SAS_EUNSUPPORTED;
     }
   }
@@ -273,6 +274,12 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
           const double t = m.size[3] * xb[b];
           V = FOUR_PI_3 * (m.size[0] * xa[a] + t) * (m.size[1] * xa[a] + t) * (m.size[2] * xa[a] + t);
         } break;
+        case SAS_PARALLELEPIPED: V = (m.size[0] * xa[a]) * (m.size[1] * xa[a]) * (m.size[2] * xa[a]); break;
+        case SAS_CORE_SHELL_CYLINDER: {
+          const double Rt = m.size[0] * xa[a] + m.size[2], Lt = m.size[1] * xb[b] + 2.0 * m.size[2];
+          V = PI_D * Rt * Rt * Lt;
+        } break;
+        case SAS_ELLIPSOID: { const double Re = m.size[0] * xa[a], Rp = m.size[1] * xb[b]; V = FOUR_PI_3 * Re * Re * Rp; } break;
         default: break;
       }
       SV += w * V;
@@ -291,6 +298,8 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
       case SAS_CYLINDER: { const double R = m.size[0] * xa[a], c = s0 * PI_D * R * R; split(R, r); r[2] = wa[a] * c * c; r[3] = R * R; } break;
       case SAS_TRIAXIAL_ELLIPSOID: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
       case SAS_CORE_SHELL_TRIAXIAL: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
+      // NEXT-2 models: the node value and its weight; the kernel forms the amplitude itself (models.cuh)
+      case SAS_PARALLELEPIPED: case SAS_CORE_SHELL_CYLINDER: case SAS_ELLIPSOID: r[0] = xa[a]; r[2] = wa[a]; break;
       default: break;
     }
   }
@@ -299,6 +308,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
     switch (m.model) {
       case SAS_CYLINDER: { const double L = m.size[1] * xb[b]; split(0.5 * L, r); r[2] = wb[b] * L * L; } break;
       case SAS_CORE_SHELL_TRIAXIAL: { const double t = m.size[3] * xb[b]; r[0] = t; r[1] = wb[b]; r[2] = t * t; } break;
+      case SAS_PARALLELEPIPED: case SAS_CORE_SHELL_CYLINDER: case SAS_ELLIPSOID: r[0] = xb[b]; r[2] = wb[b]; break;
       default: r[1] = wb[b]; break;
     }
   }
@@ -396,7 +406,8 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   // ... and per-event sizes (SAS_PD_GAUSS_MC) are one fp64 evaluation per neutron as well (R-N2)
   bool any_event = false;
   for (uint32_t e = 0; e < c->n_exp; ++e)
-    any_event = any_event || models[e].pd_kind[0] == SAS_PD_GAUSS_MC || models[e].pd_kind[1] == SAS_PD_GAUSS_MC;
+    any_event = any_event || models[e].pd_kind[0] == SAS_PD_GAUSS_MC || models[e].pd_kind[1] == SAS_PD_GAUSS_MC ||
+                models[e].model >= SAS_PARALLELEPIPED;  // the NEXT-2 models have an fp64 node loop only
   c->precision = (models[0].precision == SAS_FP64 || !any_loop || any_event) ? SAS_FP64 : SAS_FP32;
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     ExpParams& P = c->h_exps[e];
@@ -422,7 +433,8 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   for (auto& g : c->group_ids) g.clear();
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     const ExpParams& P = c->h_exps[e];
-    const int v = (P.model == SAS_CYLINDER && P.orient_kind == SAS_ORIENT_GAUSS_QUAD) ? (int)V_CYL_QUAD : P.model;
+    const int v = (P.model == SAS_CYLINDER && P.orient_kind == SAS_ORIENT_GAUSS_QUAD) ? (int)V_CYL_QUAD
+                  : P.model >= SAS_PARALLELEPIPED ? (int)V_PARA + (P.model - SAS_PARALLELEPIPED) : P.model;
     const bool event = (P.pd_mc[0] | P.pd_mc[1]) != 0 && P.model != SAS_FLAT;
     c->group_ids[v + (event ? (int)N_VARIANTS : 0)].push_back(e);
   }
@@ -506,6 +518,9 @@ sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v, int g) {
     case V_CS_TRIAX: return launch<Real, V_CS_TRIAX, EV>(c, a);
     case V_FLAT: return launch<Real, V_FLAT, false>(c, a);
     case V_CYL_QUAD: return launch<Real, V_CYL_QUAD, false>(c, a);
+    case V_PARA: return launch<double, V_PARA, EV>(c, a);
+    case V_CS_CYL: return launch<double, V_CS_CYL, EV>(c, a);
+    case V_ELL: return launch<double, V_ELL, EV>(c, a);
     default: return fail(c, SAS_EINVAL, "unknown kernel variant");
   }
 }

@@ -9,7 +9,11 @@ namespace sas {
 enum : int { ST_DETECTED = 0, ST_SLIT1 = 1, ST_SLIT2 = 2, ST_MISS_SAMPLE = 3, ST_UNREACHABLE = 4, ST_MISS_DET = 5 };
 
 // kernel variants: one trace kernel is compiled per model form (models.cuh: eval_intensity)
-enum : int { V_SPHERE = 0, V_CS_SPHERE = 1, V_CYL = 2, V_TRIAX = 3, V_CS_TRIAX = 4, V_FLAT = 5, V_CYL_QUAD = 6, N_VARIANTS = 7 };
+enum : int {
+  V_SPHERE = 0, V_CS_SPHERE = 1, V_CYL = 2, V_TRIAX = 3, V_CS_TRIAX = 4, V_FLAT = 5, V_CYL_QUAD = 6,
+  V_PARA = 7, V_CS_CYL = 8, V_ELL = 9,  // NEXT-2 models: generic fp64 node loop over event_amplitude
+  N_VARIANTS = 10
+};
 
 // table record widths (in Reals)
 constexpr int TA_W = 4;   // per node of polydisperse axis 0

@@ -317,3 +317,51 @@ def test_paper_sampling_rejects_mixtures(sas):
         with pytest.raises(sas.SasError) as e:
             sas.Tracer(ins, W.model(**over))
         assert e.value.status == 5                      # SAS_EUNSUPPORTED
+
+
+# ---- NEXT-2: parallelepiped, core-shell cylinder, ellipsoid of revolution (fp64 node loops)
+MORE_MODELS = [
+    ("parallelepiped_fixed", dict(model="parallelepiped", size=[35.0, 75.0, 120.0, 0], theta=0.7, phi=2.0, psi=0.5)),
+    ("parallelepiped_pd_iso", dict(model="parallelepiped", size=[35.0, 75.0, 120.0, 0], pd_kind=["schulz", "none"],
+                                   pd_rel=[0.1, 0], pd_nodes=[8, 1], orient_kind="isotropic_mc")),
+    ("cs_cylinder_pd_fixed", dict(model="core_shell_cylinder", size=[20.0, 300.0, 8.0, 0], sld=[3e-6, 1e-6, 0],
+                                  pd_kind=["schulz", "schulz"], pd_rel=[0.1, 0.05], pd_nodes=[6, 5], theta=1.0, phi=0.3)),
+    ("cs_cylinder_paper", dict(model="core_shell_cylinder", size=[20.0, 300.0, 8.0, 0], sld=[3e-6, 1e-6, 0],
+                               pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.1, 0.1], orient_kind="uniform_angles_mc")),
+    ("ellipsoid_pd_iso_py", dict(model="ellipsoid", size=[30.0, 70.0, 0, 0], pd_kind=["schulz", "schulz"],
+                                 pd_rel=[0.1, 0.1], pd_nodes=[5, 7], orient_kind="isotropic_mc",
+                                 sq_kind="hard_sphere_py", sq_radius_eff=45.0, sq_volfrac=0.15, background=0.01)),
+    ("ellipsoid_paper", dict(model="ellipsoid", size=[30.0, 70.0, 0, 0], pd_kind=["gauss_mc", "none"], pd_rel=[0.2, 0],
+                             theta=0.5, phi=1.0)),
+]
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+@pytest.mark.parametrize("name,over", MORE_MODELS, ids=[m[0] for m in MORE_MODELS])
+def test_more_models_per_neutron(sas, name, over, precision):
+    # these models have an fp64 node loop only: an fp32 request is served in fp64 and meets the fp64 bound
+    model = W.model(precision=precision, **over)
+    check_dump(sas, W.instrument(det_dist=3.0), model, 777, 0, 150000, tol=1e-12, min_detected=5000)
+
+
+def test_more_models_in_one_batch(sas):
+    # one launch per kernel variant present, fixed-node and per-event kernels side by side
+    ins = [W.instrument(det_dist=2.0 + 0.5 * i, det_nx=64, det_ny=64) for i in range(len(MORE_MODELS))]
+    models = [W.model(precision="fp64", **over) for _, over in MORE_MODELS]
+    bt = sas.BatchTracer(ins, models)
+    bt.trace(40000, 31)
+    sp, sp2, cn = bt.read_detector()
+    cnt = bt.counters()
+    tot = np.zeros(8, np.uint64)
+    for e in range(len(models)):
+        ref = O.trace_range(ins[e], models[e], 31, 0, 40000, exp_index=e, dump=False)
+        tot += ref["counters"]
+        assert np.array_equal(cn[e].reshape(-1), ref["counts"]), e
+        m = ref["sum_p"] > 0
+        assert np.abs(sp[e].reshape(-1)[m] / ref["sum_p"][m] - 1).max() < 1e-9, e
+    assert np.array_equal(cnt[:7], tot[:7])
+    bt.close()
+    with pytest.raises(sas.SasError) as e:
+        sas.Tracer(ins[0], W.model(model="ellipsoid", size=[30.0, 70.0, 0, 0], orient_kind="gauss_quad",
+                                   sigma_theta=0.1, sigma_phi=0.1, n_theta=4, n_phi=4))
+    assert e.value.status == 5

@@ -12,7 +12,11 @@
  * closed forms of the sphere, brute-force Eq. 1 integrals for cylinder and
  * ellipsoid, mpmath values of PY S(q) and 2J1(x)/x, weight conservation of the
  * flat model, pencil-beam chi^2 against the numerically integrated I(Q),
- * Guinier radii, model reductions.  "parity unpinned": whole detector images
+ * Guinier radii, model reductions; NEXT-1 (tests/test_oracle_paper_sampling.py):
+ * normal / truncated-normal laws of the per-event sizes, raw-Philox draw layout,
+ * numpy integrals of F^2/V, isotropic vs printed orientation law; NEXT-2
+ * (tests/test_oracle_more_models.py): Eq. 1 integrated over the box, the
+ * core-shell cylinder and the ellipsoid of revolution.  "parity unpinned": whole detector images
  * of configs c1-c4 have no external pin beyond those pieces (DESIGN.md s.3.D).
  */
 #define _GNU_SOURCE

@@ -263,6 +263,42 @@ def cpu_baseline(cfg_index, budget_s=12.0):
             "sample": f"ids [0, {n}) of {c['name']} ({dt:.1f} s, single thread)"}
 
 
+def _oracle_worker(job):
+    cfg_index, first, n = job
+    from oracle import oracle as O
+    c = W.config(cfg_index)
+    O.trace_range(c["instrument"], c["model"], c["seed"], first, n, dump=False)
+    return n
+
+
+def cpu_baseline_all_cores(cfg_index, rate_1core, seconds=3.0):
+    """The same oracle as K independent id-range processes (the paper's MPI scheme):
+    K = the cores this process may run on."""
+    import multiprocessing as mp
+    k = len(os.sched_getaffinity(0))
+    n = int(max(rate_1core * seconds, 2e5))
+    with mp.get_context("spawn").Pool(k) as pool:
+        pool.map(_oracle_worker, [(cfg_index, 0, 1000)] * k)          # start the workers, load the library
+        t0 = time.perf_counter()
+        pool.map(_oracle_worker, [(cfg_index, r * n, n) for r in range(k)])
+        dt = time.perf_counter() - t0
+    return {"value": k * n / dt, "cores": k, "sample": f"{k} processes x {n} ids ({dt:.1f} s)"}
+
+
+def oracle_rate(cfg_index, n=300_000):
+    """Oracle neutrons/s on one host core over ids [0, n) of a secondary config (c4: its first two experiments)."""
+    from oracle import oracle as O
+    c = W.config(cfg_index)
+    if "models" in c:
+        pairs = [(c["instruments"][e], c["models"][e], e) for e in (0, 1)]
+    else:
+        pairs = [(c["instrument"], c["model"], 0)]
+    t0 = time.perf_counter()
+    for ins, mod, e in pairs:
+        O.trace_range(ins, mod, c["seed"], 0, n // len(pairs), exp_index=e, dump=False)
+    return n / (time.perf_counter() - t0)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -331,6 +367,15 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(args.config if args.config < 4 else HEADLINE)
+        try:
+            cpu["all_cores"] = cpu_baseline_all_cores(args.config if args.config < 4 else HEADLINE, cpu["value"])
+        except Exception as exc:                          # a reported extra, never fatal
+            cpu["all_cores"] = {"error": str(exc)}
+        if not args.headline_only:
+            names = {W.config(i)["name"]: i for i in range(6)}
+            for k, v in others.items():
+                if k in names:
+                    v["oracle_1core"] = oracle_rate(names[k])
 
     if rank == 0:
         c = W.config(args.config)

@@ -365,3 +365,96 @@ def test_more_models_in_one_batch(sas):
         sas.Tracer(ins[0], W.model(model="ellipsoid", size=[30.0, 70.0, 0, 0], orient_kind="gauss_quad",
                                    sigma_theta=0.1, sigma_phi=0.1, n_theta=4, n_phi=4))
     assert e.value.status == 5
+
+
+# ---- full sizes, in the launch configuration bench.py times (BASELINE.json configs 1-4)
+def _sampled_windows(sas, ins, model, seed, n_total, exp_index=0, n_win=6, width=4096, tol=None):
+    rng = np.random.Generator(np.random.PCG64(seed ^ 0x5EED))
+    firsts = [0, n_total - width] + [int(v) for v in rng.integers(0, n_total - width, n_win - 2)]
+    tr = sas.Tracer(ins, model)
+    n_det = 0
+    for first in firsts:
+        px, wt, qq = tr.trace_dump(first, width, seed, exp_index)
+        ref = O.trace_range(ins, model, seed, first, width, exp_index=exp_index, hist=False)
+        assert np.array_equal(px, ref["pixel"]), first
+        det = ref["pixel"] >= 0
+        bound = tol * np.maximum(np.abs(ref["weight"][det]), 1e-4 * np.abs(ref["weight_env"][det]))
+        assert np.all(np.abs(wt[det] - ref["weight"][det]) <= bound), first
+        n_det += int(det.sum())
+    tr.close()
+    return n_det
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_full_size_run_properties_and_sampled_ids(sas, cfg):
+    c = W.config(cfg)
+    n, seed, ins, model = c["n_neutrons"], c["seed"], c["instrument"], c["model"]
+    tr = sas.Tracer(ins, model)
+    tr.trace(n, seed)                                  # the launch bench.py times
+    sp, sp2, cn = tr.read_detector()
+    cnt = tr.counters().astype(np.int64)
+    info = tr.launch_info()
+    assert info["grid"] % 148 == 0 and info["block"] == 128
+    # every neutron has exactly one outcome; the histogram holds exactly the detected ones
+    assert cnt[0] == n and cnt[1:7].sum() == n and int(cn.sum()) == cnt[6]
+    assert abs(cnt[1] / n - 0.75) < 5 * math.sqrt(0.75 * 0.25 / n)      # slit 1 passes the central quarter
+    assert np.all((cn == 0) == (sp == 0)) and np.all(sp2 <= sp * sp * (1 + 1e-12)) and np.all(sp >= 0)
+    # the image has the symmetry of the instrument: left/right and up/down halves agree statistically
+    tot = sp.sum()
+    lr = sp[:, : sp.shape[1] // 2].sum() / tot
+    ud = sp[: sp.shape[0] // 2, :].sum() / tot
+    rel_err = math.sqrt(float(sp2.sum())) / tot
+    assert abs(lr - 0.5) < 6 * rel_err and abs(ud - 0.5) < 6 * rel_err
+    # a second launch of the same ids in two halves adds up to the same detector (counts exactly)
+    tr.reset()
+    tr.trace_range(0, n // 2, seed)
+    tr.trace_range(n // 2, n - n // 2, seed)
+    sp_b, sp2_b, cn_b = tr.read_detector()
+    assert np.array_equal(cn, cn_b)
+    m = sp > 0
+    assert np.abs(sp_b[m] / sp[m] - 1).max() < 1e-9
+    tr.close()
+    # the oracle's image of an id prefix is the same estimator: mean weight per hit, pixel ring by ring
+    n_pre = 300000
+    ref = O.trace_range(ins, model, seed, 0, n_pre, dump=False)
+    ny, nx = sp.shape
+    yy, xx = np.mgrid[0:ny, 0:nx]
+    ring = np.minimum((np.hypot(xx - (nx - 1) / 2, yy - (ny - 1) / 2) / (nx / 2) * 12).astype(int), 15).reshape(-1)
+    gp, gc = np.bincount(ring, sp.reshape(-1), 16), np.bincount(ring, cn.reshape(-1).astype(float), 16)
+    op, oc = np.bincount(ring, ref["sum_p"], 16), np.bincount(ring, ref["counts"].astype(float), 16)
+    op2 = np.bincount(ring, ref["sum_p2"], 16)
+    ok = oc > 200
+    mean_g, mean_o = gp[ok] / gc[ok], op[ok] / oc[ok]
+    sig_o = np.sqrt(np.maximum(op2[ok] / oc[ok] - mean_o ** 2, 0) / oc[ok])
+    assert ok.sum() >= 8 and np.all(np.abs(mean_g - mean_o) < 5 * sig_o + 1e-3 * mean_o)
+    # ids sampled over the whole range, one by one against the oracle
+    assert _sampled_windows(sas, ins, model, seed, n, tol=TOL[model["precision"]]) > 300
+
+
+def test_full_size_batch_properties_and_sampled_ids(sas):
+    c = W.config(4)
+    n_each, seed = c["n_neutrons_each"], c["seed"]
+    bt = sas.BatchTracer(c["instruments"], c["models"])
+    bt.trace(n_each, seed)
+    sp, sp2, cn = bt.read_detector()
+    cnt = bt.counters().astype(np.int64)
+    n_exp = len(c["models"])
+    assert cnt[0] == n_exp * n_each and cnt[1:7].sum() == cnt[0] and int(cn.sum()) == cnt[6]
+    per_exp = cn.reshape(n_exp, -1).sum(axis=1)
+    assert per_exp.min() > 0                           # every experiment wrote its own histogram
+    bt.close()
+    # three experiments one by one: same Philox word, same detector as a single-experiment run of those ids
+    for e in (0, 511, 1023):
+        tr = sas.Tracer(c["instruments"][e], c["models"][e])
+        px, wt, _ = tr.trace_dump(n_each - 50000, 50000, seed, e)
+        tr.close()
+        ref = O.trace_range(c["instruments"][e], c["models"][e], seed, n_each - 50000, 50000, exp_index=e, hist=False)
+        assert np.array_equal(px, ref["pixel"])
+        det = ref["pixel"] >= 0
+        bound = 1e-5 * np.maximum(np.abs(ref["weight"][det]), 1e-4 * np.abs(ref["weight_env"][det]))
+        assert np.all(np.abs(wt[det] - ref["weight"][det]) <= bound)
+        # the batch histogram of experiment e counts what the oracle counts over a prefix, scaled: detected fraction
+        frac = per_exp[e] / n_each
+        pre = O.trace_range(c["instruments"][e], c["models"][e], seed, 0, 200000, exp_index=e, dump=False, hist=False)
+        f0 = pre["counters"][6] / 200000
+        assert abs(frac - f0) < 6 * math.sqrt(f0 * (1 - f0) / 200000) + 1e-4

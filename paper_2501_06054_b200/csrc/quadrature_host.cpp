@@ -1,5 +1,10 @@
 #include "quadrature_host.h"
 
+#include <cstdint>
+#include <cstring>
+#include <map>
+#include <mutex>
+
 #include <algorithm>
 #include <cmath>
 #include <limits>
@@ -60,7 +65,7 @@ void gauss_from_jacobi(const std::vector<double>& a, const std::vector<double>& 
   for (int i = 0; i < n; ++i) w[i] /= wsum;
 }
 
-void schulz_rule(double p, int n, std::vector<double>& s, std::vector<double>& w) {
+static void schulz_rule_compute(double p, int n, std::vector<double>& s, std::vector<double>& w) {
   if (n <= 1 || !(p > 0.0)) {
     s.assign(1, 1.0);
     w.assign(1, 1.0);
@@ -77,7 +82,7 @@ void schulz_rule(double p, int n, std::vector<double>& s, std::vector<double>& w
   for (int k = 0; k < n; ++k) s[k] /= (z + 1.0);
 }
 
-void gauss_tilt_rule(double sigma, int n, std::vector<double>& d, std::vector<double>& w) {
+static void gauss_tilt_rule_compute(double sigma, int n, std::vector<double>& d, std::vector<double>& w) {
   if (n <= 1 || !(sigma > 0.0)) {
     d.assign(1, 0.0);
     w.assign(1, 1.0);
@@ -97,5 +102,38 @@ void gauss_tilt_rule(double sigma, int n, std::vector<double>& d, std::vector<do
   }
   for (int k = 0; k < n; ++k) w[k] /= sum;
 }
+
+// Rules are memoised by (kind, parameter bits, n): a dataset-generation loop sets thousands of models that
+// share a handful of rules, and the bisection costs ~100 us per 32-node rule.
+namespace {
+struct RuleKey {
+  int kind; uint64_t bits; int n;
+  bool operator<(const RuleKey& o) const {
+    return kind != o.kind ? kind < o.kind : bits != o.bits ? bits < o.bits : n < o.n;
+  }
+};
+struct Rule { std::vector<double> x, w; };
+std::mutex g_rule_mutex;
+std::map<RuleKey, Rule> g_rules;
+
+void cached_rule(int kind, double param, int n, std::vector<double>& x, std::vector<double>& w) {
+  uint64_t bits;
+  std::memcpy(&bits, &param, sizeof bits);
+  const RuleKey key{kind, bits, n};
+  std::lock_guard<std::mutex> lock(g_rule_mutex);
+  auto it = g_rules.find(key);
+  if (it == g_rules.end()) {
+    Rule r;
+    if (kind == 0) schulz_rule_compute(param, n, r.x, r.w); else gauss_tilt_rule_compute(param, n, r.x, r.w);
+    if (g_rules.size() >= 4096) g_rules.clear();
+    it = g_rules.emplace(key, std::move(r)).first;
+  }
+  x = it->second.x;
+  w = it->second.w;
+}
+}  // namespace
+
+void schulz_rule(double p, int n, std::vector<double>& s, std::vector<double>& w) { cached_rule(0, p, n, s, w); }
+void gauss_tilt_rule(double sigma, int n, std::vector<double>& d, std::vector<double>& w) { cached_rule(1, sigma, n, d, w); }
 
 }  // namespace sas

@@ -35,6 +35,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_microbench() -> str:
+    """csrc/microbench.cu -> paper_2501_06054_b200/microbench (pipe rates for the roofline, DESIGN.md s.7)."""
+    exe = os.path.join(HERE, "microbench")
+    subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
+                           "-o", exe, "microbench.cu"], cwd=CSRC)
+    return exe
+
+
 if __name__ == "__main__":
     import sys
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--microbench" in sys.argv:
+        print(build_microbench())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

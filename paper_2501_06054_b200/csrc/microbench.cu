@@ -1,0 +1,122 @@
+// Pipe-rate microbenchmarks for the ALU roofline of the tracer (SURVEY.md 8(d) asks for
+// them): how many SMSP clocks one warp instruction of each class occupies its pipe on this B200, measured with
+// many independent chains per thread and full occupancy, so that latency is hidden and the pipe is the limit.
+//
+//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -std=c++17 -o microbench microbench.cu && ./microbench
+//
+// Prints one line per class: SMSP clocks per warp instruction (at the clock given by SM_MHZ, default 1965).
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cuda_runtime.h>
+
+constexpr int CHAINS = 8;
+constexpr int UNROLL = 32;
+
+enum { K_FFMA, K_IMAD, K_IMAD_WIDE, K_LOP3, K_DFMA, K_MUFU_RCP, K_PHILOX, N_KINDS };
+static const char* NAMES[N_KINDS] = {"FFMA (fp32 fused multiply-add)", "IMAD (32-bit integer multiply-add)",
+                                     "IMAD.WIDE.U32 (32x32->64 multiply)", "LOP3 (integer logic)",
+                                     "DFMA (fp64 fused multiply-add)", "MUFU.RCP (special function)",
+                                     "Philox4x32-10 block (20 wide multiplies + 20 LOP3)"};
+static const double INSTR_PER_STEP[N_KINDS] = {1, 1, 1, 1, 1, 1, 1};
+
+template <int KIND>
+__global__ void __launch_bounds__(256, 4) bench(int iters, uint32_t seed, uint32_t* out) {
+  uint32_t id = blockIdx.x * blockDim.x + threadIdx.x + seed;
+  float f[CHAINS]; double d[CHAINS]; uint32_t u[CHAINS]; unsigned long long w[CHAINS];
+#pragma unroll
+  for (int c = 0; c < CHAINS; ++c) { f[c] = 1.0f + id * 1e-9f + c; d[c] = 1.0 + id * 1e-12 + c; u[c] = id * 2654435761u + c; w[c] = u[c]; }
+  const float fa = 1.0000001f, fb = 1e-7f;
+  const double da = 1.0000000001, db = 1e-10;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < UNROLL; ++k) {
+#pragma unroll
+      for (int c = 0; c < CHAINS; ++c) {
+        if (KIND == K_FFMA) f[c] = fmaf(f[c], fa, fb);
+        if (KIND == K_IMAD) u[c] = u[c] * u[(c + 1) % CHAINS] + id;
+        if (KIND == K_IMAD_WIDE) w[c] = (unsigned long long)(uint32_t)(w[c] ^ (w[c] >> 32)) * 0xD2511F53ull;
+        if (KIND == K_LOP3) u[c] = u[c] ^ u[(c + 1) % CHAINS] ^ (id + k);
+        if (KIND == K_DFMA) d[c] = fma(d[c], da, db);
+        if (KIND == K_MUFU_RCP) { asm volatile("rcp.approx.ftz.f32 %0, %0;" : "+f"(f[c])); f[c] += fb; }  // + one FADD on the FMA pipe
+      }
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int c = 0; c < CHAINS; ++c) acc ^= __float_as_uint(f[c]) ^ (uint32_t)__double2loint(d[c]) ^ u[c] ^ (uint32_t)w[c] ^ (uint32_t)(w[c] >> 32);
+  if (acc == 0x12345678u) out[id & 1023] = acc;
+}
+
+struct Keys { uint32_t k0[10], k1[10]; };
+__global__ void __launch_bounds__(256, 4) bench_philox(const __grid_constant__ Keys pk, int iters, uint32_t* out) {
+  uint32_t id = blockIdx.x * blockDim.x + threadIdx.x, acc = 0;
+  for (int i = 0; i < iters; ++i) {
+    uint32_t r[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      uint32_t c0 = id + c * 77777u + i * 131u, c1 = 0, c2 = 0, c3 = 0;
+#pragma unroll
+      for (int rd = 0; rd < 10; ++rd) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        uint32_t n0 = hi1 ^ c1 ^ pk.k0[rd], n2 = hi0 ^ c3 ^ pk.k1[rd];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+      }
+      r[c][0] = c0; r[c][1] = c1; r[c][2] = c2; r[c][3] = c3;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) acc += r[c][0] ^ r[c][1] ^ r[c][2] ^ r[c][3];
+  }
+  if (acc == 0x12345678u) out[id & 1023] = acc;
+}
+
+template <int KIND>
+static double run(double mhz) {
+  uint32_t* d; cudaMalloc(&d, 4096);
+  int n_sm = 0; cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  const int grid = n_sm * 4, iters = 400;
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    bench<KIND><<<grid, 256>>>(iters, rep, d);
+    cudaEventRecord(e1); cudaEventSynchronize(e1);
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  const double warp_instr_per_smsp = (double)grid * 8 / (n_sm * 4) * iters * UNROLL * CHAINS * INSTR_PER_STEP[KIND];
+  cudaFree(d);
+  return best * 1e-3 * mhz * 1e6 / warp_instr_per_smsp;
+}
+
+static double run_philox(double mhz) {
+  uint32_t* d; cudaMalloc(&d, 4096);
+  int n_sm = 0; cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  Keys pk; for (int r = 0; r < 10; ++r) { pk.k0[r] = 1234u + r * 0x9E3779B9u; pk.k1[r] = 99u + r * 0xBB67AE85u; }
+  const int grid = n_sm * 4, iters = 4000;
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    bench_philox<<<grid, 256>>>(pk, iters, d);
+    cudaEventRecord(e1); cudaEventSynchronize(e1);
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  const double warp_blocks_per_smsp = (double)grid * 8 / (n_sm * 4) * iters * 3;
+  cudaFree(d);
+  return best * 1e-3 * mhz * 1e6 / warp_blocks_per_smsp;
+}
+
+int main() {
+  const char* env = getenv("SM_MHZ");
+  const double mhz = env ? atof(env) : 1965.0;
+  double v[N_KINDS];
+  v[K_FFMA] = run<K_FFMA>(mhz); v[K_IMAD] = run<K_IMAD>(mhz); v[K_IMAD_WIDE] = run<K_IMAD_WIDE>(mhz);
+  v[K_LOP3] = run<K_LOP3>(mhz); v[K_DFMA] = run<K_DFMA>(mhz); v[K_MUFU_RCP] = run<K_MUFU_RCP>(mhz);
+  v[K_PHILOX] = run_philox(mhz);
+  printf("SMSP clocks per warp instruction at %.0f MHz (32 resident warps per SM, %d independent chains per thread)\n", mhz, CHAINS);
+  for (int k = 0; k < N_KINDS; ++k) printf("  %-52s %7.2f\n", NAMES[k], v[k]);
+  return 0;
+}

@@ -9,6 +9,11 @@ therefore the largest of three per-neutron costs, in SMSP-clocks per 32 neutrons
     issue = all algorithmic thread-instructions          (1 clock per warp instruction)
     fp64  = 2 x FP64 thread-instructions
     xu    = 8 x MUFU/conversion thread-instructions
+    imul  = 4 x 32x32->64-bit integer multiplies         (Philox: 20 per block, the heavy FMA pipe)
+
+The clocks per warp instruction are MEASURED on the B200 with csrc/microbench.cu (profiles/r1_microbench.md):
+FFMA 1.04, IMAD 2.02, IMAD.WIDE 4.05 inside Philox (a whole Philox4x32-10 block: 81 clocks), LOP3 2.03,
+DFMA 2.03, MUFU 8.05.
 
 The per-unit instruction counts below are ALGORITHMIC: the arithmetic that the method, in the
 formulation this library uses, needs on this ISA (a fp64 division = 1 MUFU.RCP64H + 9 DFMA-class,
@@ -28,26 +33,26 @@ N_SM = 148
 SMSP_PER_SM = 4
 SM_MAX_MHZ = 1965.0
 
-# thread-instructions per unit: (issue_total, fp64, xu)
-STAGE_A = (46, 0, 0)            # Philox block 0 (40) + id/compare (6)
-STAGE_B0 = (40 + 12, 12, 0)     # Philox block 1 (40) + two uniforms, q, lambda, q*lambda test in fp64 (12)
+# thread-instructions per unit: (issue_total, fp64, xu, wide integer multiplies)
+STAGE_A = (46, 0, 0, 19)        # Philox block 0 (40; the last round needs one of its two products) + id/compare (6)
+STAGE_B0 = (40 + 12, 12, 0, 20) # Philox block 1 (40) + two uniforms, q, lambda, q*lambda test in fp64 (12)
 # Philox block 0 again (40) + 8 uniforms (3 fp64 each) + ~125 fp64 add/mul/compare + 8 div (10) + 3 sqrt (10)
 # + sincos (62) + floor/convert (6 xu-class conversions)
-STAGE_B = (40 + 24 + 125 + 80 + 30 + 62 + 12, 24 + 125 + 72 + 27 + 62, 11 + 6)
+STAGE_B = (40 + 24 + 125 + 80 + 30 + 62 + 12, 24 + 125 + 72 + 27 + 62, 11 + 6, 20)
 
 # per detected neutron: prologue (|Q|, projections, weight product, 3 atomics) and per node evaluation
 MODEL_COST = {
     # name: (prologue(issue, fp64, xu), per_node(issue, fp64, xu))
-    "sphere_fp64": ((40, 30, 2), (110, 100, 2)),
-    "sphere_fp32": ((40, 30, 4), (32, 0, 1)),
-    "sphere_py_fp32": ((40 + 60, 30, 5), (32, 0, 1)),
-    "sphere_py_fp64": ((40 + 160, 30 + 150, 4), (110, 100, 2)),
-    "cylinder_quad_fp32": ((60, 40, 4), (27, 0, 1)),
-    "cs_triaxial_iso_fp32": ((40 + 40 + 90, 120, 6), (33, 0, 2)),
-    "cylinder_iso_fp64": ((40 + 40 + 200 + 320, 520, 8), (0, 0, 0)),
+    "sphere_fp64": ((40, 30, 2, 0), (110, 100, 2, 0)),
+    "sphere_fp32": ((40, 30, 4, 0), (32, 0, 1, 0)),
+    "sphere_py_fp32": ((40 + 60, 30, 5, 0), (32, 0, 1, 0)),
+    "sphere_py_fp64": ((40 + 160, 30 + 150, 4, 0), (110, 100, 2, 0)),
+    "cylinder_quad_fp32": ((60, 40, 4, 0), (27, 0, 1, 0)),
+    "cs_triaxial_iso_fp32": ((40 + 40 + 90, 120, 6, 20), (33, 0, 2, 0)),
+    "cylinder_iso_fp64": ((40 + 40 + 200 + 320, 520, 8, 20), (0, 0, 0, 0)),
     # per-event sizes: Philox blocks 2 and 3, two Box-Muller normals (log, sqrt, cos in fp64), three sincospi,
     # sin, j1, the weight
-    "cylinder_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12), (0, 0, 0)),
+    "cylinder_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12, 40), (0, 0, 0, 0)),
 }
 
 # DRAM traffic of one trace-kernel launch, dram__bytes_read.sum + dram__bytes_write.sum of the
@@ -62,15 +67,15 @@ NCU_DRAM_BYTES = {
 def smsp_clocks_per_neutron(frac_survive: float, frac_detect: float, model_key: str, nodes: int,
                             frac_geometry: float | None = None):
     """Algorithmic SMSP-clocks per launched neutron (per lane: divide by 32 for per-warp) for each
-    resource; returns dict(issue=, fp64=, xu=)."""
+    resource; returns dict(issue=, fp64=, xu=, imul=)."""
     pro, node = MODEL_COST[model_key]
     if frac_geometry is None:
         frac_geometry = frac_survive      # no classifier: every survivor's geometry is evaluated
-    tot = [0.0, 0.0, 0.0]
-    for i in range(3):
+    tot = [0.0, 0.0, 0.0, 0.0]
+    for i in range(4):
         tot[i] = (STAGE_A[i] + frac_survive * STAGE_B0[i] + frac_geometry * STAGE_B[i]
                   + frac_detect * (pro[i] + nodes * node[i]))
-    return dict(issue=tot[0], fp64=2.0 * tot[1], xu=8.0 * tot[2])
+    return dict(issue=tot[0], fp64=2.0 * tot[1], xu=8.0 * tot[2], imul=4.0 * tot[3])
 
 
 def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, model_key: str, nodes: int,

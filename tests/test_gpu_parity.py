@@ -491,3 +491,41 @@ def test_paper_pin_first_minimum_of_the_random_rod_end_to_end(sas):
     i_min = next(i for i in range(2, 47) if sm[i] < sm[i - 1] and sm[i] < sm[i + 1] and sm[i] < sm[i - 2] and sm[i] < sm[i + 2])
     assert 0.030 <= qc[i_min] <= 0.034, qc[i_min]
     assert 3.5 < 119.0 * qc[i_min] < 4.1                  # the paper's R = 3.78 / Q_min
+
+
+def test_detector_image_agrees_with_the_analytic_intensity_within_3_sigma(sas):
+    """north_star: "the detector image agrees with the analytic I(Q) within 3 sigma statistical error".
+    Monochromatic pencil beam (DESIGN.md R-C17), 2e8 neutrons on a 64 x 64 detector through the CUDA path; the
+    expectation per pixel is the closed-form sphere intensity (numpy, nothing of the oracle but the source
+    weight p0 of one ray) integrated over the pixel's solid angle."""
+    ins = W.pencil_instrument(det_nx=64, det_ny=64, q_min=0.004, q_max=0.3)
+    m = W.config(0)["model"]
+    n = 2 * 10**8
+    tr = sas.Tracer(ins, m)
+    tr.trace(n, 4242)
+    sp, sp2, cn = tr.read_detector()
+    tr.close()
+    p0, ell = O.trace_one(ins, m, 4242, 0).p0, 1e-3
+    R, drho, scale = m["size"][0], m["sld"][0], m["scale"]
+    nx = ny = 64
+    Wd, D, k = ins["det_xw"], ins["det_dist"], 2 * math.pi / ins["lambda_min"]
+    g, gw = np.polynomial.legendre.leggauss(5)
+    xs = ((np.arange(nx)[:, None] + 0.5 + 0.5 * g[None, :]) * (Wd / nx) - 0.5 * Wd).reshape(-1)
+    w1 = np.tile(0.5 * gw * (Wd / nx), nx)
+    X, Y = xs[None, :], xs[:, None]
+    R2 = X * X + Y * Y
+    q = 2 * k * np.sin(0.5 * np.arctan2(np.sqrt(R2), D))
+    u = q * R
+    V = 4 * math.pi / 3 * R ** 3
+    Iq = 1e8 * scale * drho ** 2 * V * (3 * (np.sin(u) - u * np.cos(u)) / u ** 3) ** 2
+    Iq = np.where((q >= ins["q_min"]) & (q <= ins["q_max"]), Iq, 0.0)
+    f = Iq * D / (D * D + R2) ** 1.5 * w1[None, :] * w1[:, None]
+    E = n * p0 * 100 * ell * f.reshape(ny, 5, nx, 5).sum(axis=(1, 3))
+    ok = cn > 100
+    ok[30:34, 30:34] = False                      # pixels cut by the q_min circle
+    z = (sp[ok] - E[ok]) / np.sqrt(sp2[ok])
+    chi2 = float((z * z).mean())
+    assert ok.sum() > 3000
+    assert abs(chi2 - 1) < 5 * math.sqrt(2 / ok.sum()), chi2
+    assert (np.abs(z) > 3).mean() <= 0.01
+    assert abs(sp[ok].sum() / E[ok].sum() - 1) < 1e-3

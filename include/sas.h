@@ -160,7 +160,10 @@ sas_status sas_read_detector(sas_ctx* ctx, double* h_sum_p, double* h_sum_p2, ui
 /* out[8] = launched, absorbed at slit 1, at slit 2, missed the sample, |Q| unreachable
  * (q >= 2k), missed the detector, detected; out[7] = how many of the detector misses (out[5])
  * were decided by the conservative q*lambda classifier without running the full geometry
- * (an implementation statistic).  Summed over experiments.  Synchronises. */
+ * (an implementation statistic).  Summed over experiments.  Synchronises.
+ * out[0] is the library's own sum of the traced ranges; the kernels count every outcome they decide in
+ * their queued stages and out[1] is what is left of out[0] (a neutron has exactly one outcome), so
+ * out[0] == out[1] + ... + out[6] always. */
 sas_status sas_get_counters(sas_ctx* ctx, uint64_t out[8]);
 
 /* Zero histograms and counters (asynchronous on the stream). */

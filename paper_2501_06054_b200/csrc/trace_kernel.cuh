@@ -1,12 +1,13 @@
 // The trace kernel: persistent blocks pull work items (experiment, id range) from a global counter;
-// inside a block every warp is autonomous and runs a three-stage pipeline with warp-private ring
+// inside a block every warp is autonomous and runs a four-stage pipeline with warp-private ring
 // queues in shared memory so that each stage executes with full warps although ~75 % of the neutrons
 // die at slit 1 and ~80 % of the rest miss the detector:
 //
 //   stage A  Philox block 0 + slit-1 test on the raw 32-bit draws      (every launched neutron)
 //   stage B0 Philox block 1 + conservative "certain to miss the         (slit-1 survivors)
 //            detector" test on q lambda (geometry.cuh)
-//   stage B  fp64 geometry: slits, sample chord, Q, detector pixel     (survivors that may hit)
+//   stage B  Philox block 0 again, fp64 geometry: slits, sample       (survivors that may hit)
+//            chord, Q, detector pixel
 //   stage C  model intensity I(Q) with the quadrature node loops,      (detected neutrons)
 //            weight, histogram update
 #pragma once

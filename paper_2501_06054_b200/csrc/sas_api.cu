@@ -462,7 +462,8 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
 template <typename Real, int V, bool EV>
 sas_status launch(sas_ctx* c, KernelArgs& a) {
   const bool DUMP = a.d_pixel != nullptr;
-  const size_t smem = trace_smem_bytes<Real>(c->tab_len_max);
+  constexpr int BLOCK_THREADS = block_threads(V);
+  const size_t smem = trace_smem_bytes<Real>(c->tab_len_max, BLOCK_THREADS / 32);
   auto kern = trace_kernel<Real, V, EV>;
   if (smem > 227 * 1024) return fail(c, SAS_EINVAL, "quadrature tables do not fit in shared memory");
   CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -474,7 +474,8 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   const int grid_full = c->n_sm * bps;
   // work items: ~16 per resident block, 2048..262144 ids each, multiple of 256 ids
   uint64_t item = total / ((uint64_t)grid_full * (uint64_t)SAS_ITEMS_PER_BLOCK);
-  item = std::min<uint64_t>(std::max<uint64_t>(item, SAS_MIN_ITEM), 262144);
+  // at least 16 rows of 32 ids per warp and item (a 1e6-neutron launch still fills the chip)
+  item = std::min<uint64_t>(std::max<uint64_t>(item, (uint64_t)SAS_MIN_ITEM / 4 * (BLOCK_THREADS / 32)), 262144);
   item = (item + 255) / 256 * 256;
   a.item_ids = (uint32_t)item;
   a.items_per_exp = (uint32_t)(((uint64_t)a.n_per_exp + item - 1) / item);

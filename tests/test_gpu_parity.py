@@ -529,3 +529,30 @@ def test_detector_image_agrees_with_the_analytic_intensity_within_3_sigma(sas):
     assert abs(chi2 - 1) < 5 * math.sqrt(2 / ok.sum()), chi2
     assert (np.abs(z) > 3).mean() <= 0.01
     assert abs(sp[ok].sum() / E[ok].sum() - 1) < 1e-3
+
+
+def test_host_proved_skips_at_their_margins(sas):
+    """Stage B skips the sample's lateral slabs and the slit arithmetic when the host has proved them idle
+    (DESIGN.md section 5).  Instruments just inside and just outside those proofs must give the oracle's
+    outcomes and pixels exactly."""
+    m = W.config(0)["model"]
+    base = W.instrument()
+    # beam envelope at the far face of the sample (the host's own bound): focus half-width + divergence beyond it
+    z_far = base["sample_z"] + 0.5 * base["sample_zd"]
+    bx = 0.5 * base["focus_xw"] + (z_far - base["focus_z"]) * (0.5 * base["focus_xw"] + 0.5 * base["src_xw"]) / base["focus_z"]
+    for scale in (1 + 3e-6, 1 - 3e-6, 0.9, 0.5):           # proof holds / fails by a hair / lateral faces really cut
+        ins = W.instrument(sample_xw=2 * bx * scale, sample_yh=2 * bx * scale)
+        check_dump(sas, ins, m, 31337, 0, 120000, min_detected=1000)
+        tr = sas.Tracer(ins, m)
+        tr.trace(120000, 31337)
+        ref = O.trace_range(ins, m, 31337, 0, 120000, dump=False)
+        assert np.array_equal(tr.counters()[:7], ref["counters"][:7]), scale
+        tr.close()
+    # slit 2 a hair narrower than the focus rectangle: it cuts, the slit arithmetic must run
+    ins = W.instrument(slit2_xw=base["focus_xw"] * (1 - 1e-9))
+    ref = O.trace_range(ins, m, 31337, 0, 400000, dump=False, hist=False)
+    check_dump(sas, ins, m, 31337, 0, 400000, min_detected=1000)
+    tr = sas.Tracer(ins, m)
+    tr.trace(400000, 31337)
+    assert np.array_equal(tr.counters()[:7], ref["counters"][:7])
+    tr.close()

@@ -556,3 +556,25 @@ def test_host_proved_skips_at_their_margins(sas):
     tr.trace(400000, 31337)
     assert np.array_equal(tr.counters()[:7], ref["counters"][:7])
     tr.close()
+
+
+def test_many_tiny_experiments_in_one_batch(sas):
+    # 150 experiments of 700 neutrons each: work items shorter than the minimum item, ragged rows, an experiment
+    # change at every item, all three kernel variants of c4-like batches plus a per-event one
+    c = W.batch_config(150, 700, 555)
+    models = list(c["models"])
+    models[7] = W.model(model="sphere", precision="fp32", size=[60.0, 0, 0, 0], pd_kind=["gauss_mc", "none"], pd_rel=[0.2, 0])
+    bt = sas.BatchTracer(c["instruments"], models)
+    bt.trace(700, 555)
+    sp, sp2, cn = bt.read_detector()
+    cnt = bt.counters()
+    bt.close()
+    tot = np.zeros(8, np.uint64)
+    for e in range(150):
+        ref = O.trace_range(c["instruments"][e], models[e], 555, 0, 700, exp_index=e, dump=False)
+        tot += ref["counters"]
+        assert np.array_equal(cn[e].reshape(-1), ref["counts"]), e
+        m = ref["sum_p"] > 0
+        if m.any():
+            assert np.abs(sp[e].reshape(-1)[m] / ref["sum_p"][m] - 1).max() < 1e-9, e
+    assert np.array_equal(cnt[:7], tot[:7])

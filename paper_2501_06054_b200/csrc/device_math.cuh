@@ -38,10 +38,11 @@ __device__ __forceinline__ void philox4x32_10(const PhiloxKeys& pk, uint32_t c0,
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// u = (w + 0.5) 2^-32, exact: (double)w is assembled as 2^52 + w minus 2^52 (no I2F conversion).
+// u = (w + 0.5) 2^-32, exact, in one FMA: the double 2^52 + w is assembled from its words (no I2F), and
+// (2^52 + w) 2^-32 + (2^-33 - 2^20) = (w + 0.5) 2^-32 has 33 significant bits, so the single rounding of the
+// FMA returns it exactly -- the same double as the oracle's ((double)w + 0.5) * 2^-32.
 __device__ __forceinline__ double uniform_from_word(uint32_t w) {
-  double d = __hiloint2double(0x43300000, (int)w) - 4503599627370496.0;
-  return (d + 0.5) * 2.3283064365386963e-10;
+  return fma(__hiloint2double(0x43300000, (int)w), 2.3283064365386963e-10, 1.1641532182693481e-10 - 1048576.0);
 }
 
 // ---------------------------------------------------------------- polynomial helpers

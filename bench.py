@@ -299,6 +299,33 @@ def oracle_rate(cfg_index, n=300_000):
     return n / (time.perf_counter() - t0)
 
 
+def run_sweep(torch, S):
+    """Run time against the number of neutrons, the paper's own experiment (N from 1e5 to
+    1e11): c0 (monodisperse sphere) and the paper's per-event scheme on its rod (n1), one launch sequence per N,
+    CUDA events around it, after one warm-up at the same N."""
+    out = {}
+    for idx in (0, 5):
+        c = W.config(idx)
+        tr = S.Tracer(c["instrument"], c["model"])
+        rows = []
+        for n in (10**5, 10**6, 10**7, 10**8, 10**9, 10**10, 10**11):
+            reps = 1 if n >= 10**10 else 2
+            for r in range(reps):
+                tr.reset()
+                tr.kernel_time_ms(reset=True)
+                t0 = time.perf_counter()
+                tr.trace(n, c["seed"])
+                cnt = tr.counters()                      # synchronises
+                wall = time.perf_counter() - t0
+                ms, nl = tr.kernel_time_ms(reset=True)
+            rows.append({"n": n, "kernel_s": ms * nl * 1e-3, "wall_s": wall, "launches": int(nl),
+                         "neutrons_per_s": n / (ms * nl * 1e-3), "detected": int(cnt[6])})
+        tr.close()
+        out[c["name"]] = rows
+    print(json.dumps({"sweep": out}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -308,6 +335,7 @@ def main():
     ap.add_argument("--headline-only", action="store_true", help="skip the four secondary configs")
     ap.add_argument("--config", type=int, default=HEADLINE, help="workload timed as the main line (profiling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1, then exit")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -323,6 +351,9 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     import paper_2501_06054_b200 as S
     S.load_library()              # raises if libsas_b200.so is missing: no fallback
+
+    if args.sweep:
+        return run_sweep(torch, S)
 
     flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 

@@ -38,6 +38,12 @@ constexpr int NB0 = SAS_B0_PER_LANE;  // queue-B entries a lane takes per stage-
 constexpr int RING_B2 = NB0 > 1 ? 128 : 64;
 constexpr int RING_B = (32 * NB0 - 1 + 32 * SAS_STAGE_A_ROWS) > 128 ? 256 : 128;  // queue B takes SAS_STAGE_A_ROWS rows of 32 per stage-A step on top of < 32 entries
 
+// a stage runs only while its input queue is below one batch, so the capacities below can never be exceeded
+static_assert(RING_B >= 32 * NB0 - 1 + 32 * SAS_STAGE_A_ROWS, "queue B: < one B0 batch + one stage-A step");
+static_assert(RING_B2 >= 31 + 32 * NB0, "queue B2: < 32 entries + one B0 batch");
+static_assert(RING >= 31 + 32, "queue C: < 32 entries + one stage-B batch");
+static_assert((RING & (RING - 1)) == 0 && (RING_B & (RING_B - 1)) == 0 && (RING_B2 & (RING_B2 - 1)) == 0, "ring sizes are powers of two");
+
 struct WarpQueues {
   // queue B: slit-1 survivors (their id offsets; stage B draws Philox block 0 again for the few it gets:
   // 40 integer instructions for 6 % of the neutrons instead of eight queue accesses for 25 %)

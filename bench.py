@@ -155,7 +155,9 @@ def time_steps(torch, tracer, do_step, steps, warmup, flush):
     if dist.is_initialized():
         dist.barrier()
     torch.cuda.synchronize()
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    per_step = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(per_step)
+    time_steps.last_per_step = per_step
     if dist.is_initialized() and dist.get_world_size() > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -195,7 +197,9 @@ def bench_config(torch, S, cfg_index, steps, warmup, rank, world, flush, with_e2
     cnt = tr.counters().astype(np.float64)
     ms_per_step = total_ms / steps
     value = n_step * world / (ms_per_step * 1e-3)
+    per = sorted(getattr(time_steps, "last_per_step", [ms_per_step]))
     out = {"workload": c["name"], "n_neutrons_per_step": n_step, "ms_per_step": ms_per_step, "value": value,
+           "ms_per_step_median": per[len(per) // 2], "ms_per_step_best": per[0],
            "kernel_ms": kernel_ms, "grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
            "gpu_launches": int(launches), "detected_frac": cnt[6] / cnt[0], "survive_frac": 1.0 - cnt[1] / cnt[0],
            # survivors whose fp64 geometry ran (the others were certain detector misses, counters[7])
@@ -419,6 +423,7 @@ def main():
                        "l2": "flushed between timed steps (256 MiB write, outside the event pairs)",
                        "grid": head["grid"], "block": head["block"], "smem_bytes": head["smem_bytes"]},
             "clocks": clocks, "e2e": e2e, "gpu_launches": head["gpu_launches"],
+            "ms_per_step_median": head["ms_per_step_median"], "ms_per_step_best": head["ms_per_step_best"],
             "kernel_ms": head["kernel_ms"], "roofline": head["roofline"], "cpu_baseline": cpu,
             "configs": others,
         }

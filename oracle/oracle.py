@@ -113,6 +113,9 @@ def lib():
         L.orc_trace_range.argtypes = [C.POINTER(Instrument), C.POINTER(Model), C.c_uint64, C.c_uint64,
                                       C.c_uint64, C.c_uint32] + [C.c_void_p] * 8
         L.orc_trace_range.restype = None
+        L.orc_reduce_radial.argtypes = [C.POINTER(Instrument), C.c_void_p, C.c_void_p, C.c_double, C.c_double,
+                                        C.c_double, C.c_double, C.c_int32] + [C.c_void_p] * 4
+        L.orc_reduce_radial.restype = None
     return _lib
 
 
@@ -275,3 +278,18 @@ def trace_range(ins_d, model_d, seed: int, first: int, n: int, exp_index: int = 
     out.update(pixel=pixel, weight=weight, weight_env=wenv, q=q, sum_p=sp, sum_p2=sp2, counts=cnt,
                counters=counters)
     return out
+
+
+def reduce_radial(ins_d, sum_p, sum_p2, launched, lambda_ref, q_lo, q_hi, n_bins):
+    """Ring average of one detector image (DESIGN.md R-R1): returns (q, I, sigma, npix) arrays of n_bins."""
+    ins = ins_d if isinstance(ins_d, Instrument) else make_instrument(ins_d)
+    sp = np.ascontiguousarray(sum_p, np.float64).reshape(-1)
+    sp2 = np.ascontiguousarray(sum_p2, np.float64).reshape(-1)
+    assert sp.size == ins.det_nx * ins.det_ny == sp2.size and 1 <= n_bins <= 4096
+    q, i, s = (np.zeros(n_bins) for _ in range(3))
+    n = np.zeros(n_bins, np.uint64)
+    ptr = lambda a: a.ctypes.data_as(C.c_void_p)
+    lib().orc_reduce_radial(C.byref(ins), ptr(sp), ptr(sp2), float(launched), float(lambda_ref), float(q_lo),
+                            float(q_hi), int(n_bins), ptr(q), ptr(i), ptr(s), ptr(n))
+    return q, i, s, n
+

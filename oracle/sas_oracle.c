@@ -557,3 +557,47 @@ void orc_trace_range(const orc_instrument* ins, const orc_model* m, uint64_t see
     }
   }
 }
+
+/* ------------------------------------------------------------- R-R1 */
+void orc_reduce_radial(const orc_instrument* ins, const double* sum_p, const double* sum_p2, double launched,
+                       double lambda_ref, double q_lo, double q_hi, int32_t n_bins, double* q_out, double* i_out,
+                       double* sigma_out, uint64_t* npix_out) {
+  double k = TWO_PI / lambda_ref;
+  double D = ins->det_dist;
+  double px = ins->det_xw / (double)ins->det_nx, py = ins->det_yh / (double)ins->det_ny;
+  double a_pix = px * py;
+  double scale = (double)n_bins / (q_hi - q_lo);
+  for (int b = 0; b < n_bins; ++b) {
+    q_out[b] = q_lo + ((double)b + 0.5) * ((q_hi - q_lo) / (double)n_bins);
+    i_out[b] = 0.0; sigma_out[b] = 0.0; npix_out[b] = 0;
+  }
+  /* i_out, sigma_out hold sum P and sum P2 until the end; the solid angles go to a scratch sum per ring */
+  double omega[4096];
+  if (n_bins > 4096) return;
+  for (int b = 0; b < n_bins; ++b) omega[b] = 0.0;
+  for (int iy = 0; iy < ins->det_ny; ++iy)
+    for (int ix = 0; ix < ins->det_nx; ++ix) {
+      double X = ((double)ix + 0.5) * px - 0.5 * ins->det_xw;
+      double Y = ((double)iy + 0.5) * py - 0.5 * ins->det_yh;
+      double r2 = X * X + Y * Y;
+      double two_theta = atan2(sqrt(r2), D);
+      double q = (2.0 * k) * sin(0.5 * two_theta);
+      if (!(q >= q_lo && q < q_hi)) continue;
+      int b = (int)floor((q - q_lo) * scale);
+      if (b < 0 || b >= n_bins) continue;
+      double d2 = D * D + r2;
+      double dOmega = (a_pix * D) / (d2 * sqrt(d2));
+      int pix = iy * ins->det_nx + ix;
+      i_out[b] += sum_p[pix];
+      sigma_out[b] += sum_p2[pix];
+      omega[b] += dOmega;
+      npix_out[b] += 1;
+    }
+  for (int b = 0; b < n_bins; ++b) {
+    if (npix_out[b] == 0) continue;
+    double norm = omega[b] * launched;
+    i_out[b] = i_out[b] / norm;
+    sigma_out[b] = sqrt(sigma_out[b]) / norm;
+  }
+}
+

@@ -153,6 +153,16 @@ void orc_trace_range(const orc_instrument* ins, const orc_model* m, uint64_t see
                      uint64_t n, uint32_t exp_index, int32_t* pixel, double* weight, double* weight_env,
                      double* q, double* sum_p, double* sum_p2, uint64_t* counts, uint64_t counters[8]);
 
+/* NEXT-4, reading R-R1 of DESIGN.md: ring average of one detector image into I(q) with its
+ * standard error (PAPER.md:86 2-D PSD, :173 I(Q) curve against a measurement).  Pixel centre (X, Y) ->
+ * two_theta = atan2(sqrt(X^2+Y^2), D), q = (2 k) sin(two_theta / 2), k = TWO_PI / lambda_ref; pixel solid angle
+ * dOmega = A_pix D / (D^2+r^2)^(3/2); bin b = floor((q - q_lo) n_bins / (q_hi - q_lo)) for q_lo <= q < q_hi;
+ * I_b = sum P / (sum dOmega * launched), sigma_b = sqrt(sum P2) / (sum dOmega * launched), q_b = bin centre,
+ * npix_b = pixels in the ring (empty ring: I = sigma = 0). */
+void orc_reduce_radial(const orc_instrument* ins, const double* sum_p, const double* sum_p2, double launched,
+                       double lambda_ref, double q_lo, double q_hi, int32_t n_bins, double* q_out, double* i_out,
+                       double* sigma_out, uint64_t* npix_out);
+
 #ifdef __cplusplus
 }
 #endif

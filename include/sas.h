@@ -201,6 +201,28 @@ sas_status sas_get_kernel_time(sas_ctx* ctx, int32_t reset, double* avg_ms, uint
 /* Bytes of the last host-to-device upload of parameters and quadrature tables (sas_set_model /
  * sas_create_batch). */
 sas_status sas_get_upload_bytes(sas_ctx* ctx, uint64_t* bytes);
+
+/* ---- NEXT-4: data reduction of the virtual experiment ----
+ * Ring average of the detector image of experiment `exp_index` into I(q) with its standard error
+ * (PAPER.md:86 2-D PSD, :173 I(Q) curve; DESIGN.md R-R1).  Pixel centre (X, Y): two_theta = atan2(r, D),
+ * q = (4 pi / lambda_ref) sin(two_theta / 2), solid angle dOmega = A_pix D / (D^2 + r^2)^(3/2); ring
+ * b = floor((q - q_lo) n_bins / (q_hi - q_lo)) for q_lo <= q < q_hi.  Host outputs, n_bins entries each (any may
+ * be NULL): q = ring centres, I = sum P / (sum dOmega * launched) (weight per steradian per launched neutron of
+ * that experiment), sigma = sqrt(sum P2) / (same), npix = pixels in the ring (empty ring: I = sigma = 0).
+ * Runs one CUDA kernel on the context's stream over the bound histograms and synchronises.
+ * SAS_EINVAL: n_bins outside 1..SAS_MAX_RINGS, q_lo >= q_hi, lambda_ref <= 0, exp_index out of range. */
+#define SAS_MAX_RINGS 1024
+typedef struct {
+  uint32_t struct_size;
+  uint32_t exp_index;
+  int32_t n_bins;
+  int32_t reserved;
+  double q_lo, q_hi;      /* 1/A */
+  double lambda_ref;      /* A: the wavelength that converts angle to q */
+} sas_radial_desc;
+sas_status sas_reduce_radial(sas_ctx* ctx, const sas_radial_desc* desc, double* h_q, double* h_I, double* h_sigma,
+                             uint64_t* h_npix);
+
 const char* sas_version(void);
 
 #ifdef __cplusplus

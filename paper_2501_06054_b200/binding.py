@@ -18,7 +18,7 @@ EXPORTED_SYMBOLS = [
     "sas_create_instrument", "sas_bind_buffers", "sas_set_model", "sas_trace", "sas_trace_range",
     "sas_trace_dump", "sas_read_detector", "sas_get_counters", "sas_reset_detector", "sas_destroy",
     "sas_last_error", "sas_create_batch", "sas_trace_batch", "sas_quadrature_nodes",
-    "sas_get_launch_info", "sas_get_kernel_time", "sas_get_upload_bytes", "sas_version",
+    "sas_get_launch_info", "sas_get_kernel_time", "sas_get_upload_bytes", "sas_version", "sas_reduce_radial",
 ]
 
 SAMPLE = {"box": 0, "cyl_y": 1}
@@ -56,6 +56,11 @@ class ModelDesc(C.Structure):
                 ("theta", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
                 ("sigma_theta", C.c_double), ("sigma_phi", C.c_double),
                 ("sq_radius_eff", C.c_double), ("sq_volfrac", C.c_double)]
+
+
+class RadialDesc(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("exp_index", C.c_uint32), ("n_bins", C.c_int32), ("reserved", C.c_int32),
+                ("q_lo", C.c_double), ("q_hi", C.c_double), ("lambda_ref", C.c_double)]
 
 
 def instrument_desc(d: dict) -> InstrumentDesc:
@@ -132,6 +137,7 @@ def load_library(path: str | None = None):
     L.sas_get_launch_info.argtypes = [vp, pp(u64), pp(i32), pp(i32), pp(i32)]
     L.sas_get_kernel_time.argtypes = [vp, i32, pp(dbl), pp(u64)]
     L.sas_get_upload_bytes.argtypes = [vp, pp(u64)]
+    L.sas_reduce_radial.argtypes = [vp, pp(RadialDesc), vp, vp, vp, vp]
     L.sas_version.argtypes = []
     L.sas_version.restype = C.c_char_p
     for name in EXPORTED_SYMBOLS:
@@ -189,6 +195,15 @@ class _Base:
         _check(self.L, self.ctx, self.L.sas_read_detector(self.ctx, *(t.data_ptr() for t in host)))
         sp, sp2, cn = (t.numpy() for t in host)
         return sp, sp2, cn.view(np.uint64)
+
+    def reduce_radial(self, lambda_ref, q_lo, q_hi, n_bins, exp_index=0):
+        """Ring average of the detector into I(q): (q, I, sigma, npix) numpy arrays (include/sas.h)."""
+        d = RadialDesc(C.sizeof(RadialDesc), int(exp_index), int(n_bins), 0, float(q_lo), float(q_hi), float(lambda_ref))
+        q, i, s = (np.zeros(max(n_bins, 1)) for _ in range(3))
+        n = np.zeros(max(n_bins, 1), np.uint64)
+        _check(self.L, self.ctx, self.L.sas_reduce_radial(self.ctx, C.byref(d), q.ctypes.data, i.ctypes.data,
+                                                          s.ctypes.data, n.ctypes.data))
+        return q, i, s, n
 
     def launch_info(self):
         n, g, b, s = C.c_uint64(), C.c_int32(), C.c_int32(), C.c_int32()

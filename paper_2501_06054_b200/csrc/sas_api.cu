@@ -9,6 +9,7 @@
 
 #include "../../include/sas.h"
 #include "quadrature_host.h"
+#include "reduce_kernel.cuh"
 #include "trace_kernel.cuh"
 
 using namespace sas;
@@ -56,6 +57,7 @@ struct sas_ctx {
   std::vector<uint32_t> group_ids[2 * N_VARIANTS];
   size_t group_off[2 * N_VARIANTS] = {};
   uint32_t* d_exp_ids = nullptr;
+  double* d_rings = nullptr;  // ring sums of sas_reduce_radial: 3 x SAS_MAX_RINGS doubles + SAS_MAX_RINGS counts
   cudaStream_t stream = nullptr;
   bool own_stream = true;
   // bookkeeping
@@ -569,7 +571,7 @@ void destroy_ctx(sas_ctx* c) {
   for (auto e : c->ev0) cudaEventDestroy(e);
   for (auto e : c->ev1) cudaEventDestroy(e);
   if (c->own_hist) { cudaFree(c->d_sum_p); cudaFree(c->d_sum_p2); cudaFree(c->d_counts); }
-  cudaFree(c->d_counters); cudaFree(c->d_work); cudaFree(c->d_exp_ids); cudaFree(c->d_exps); cudaFree(c->d_tab);
+  cudaFree(c->d_counters); cudaFree(c->d_work); cudaFree(c->d_exp_ids); cudaFree(c->d_rings); cudaFree(c->d_exps); cudaFree(c->d_tab);
   if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
   delete c;
 }
@@ -773,6 +775,51 @@ sas_status sas_get_kernel_time(sas_ctx* c, int32_t reset, double* avg_ms, uint64
 sas_status sas_get_upload_bytes(sas_ctx* c, uint64_t* bytes) {
   if (!c || !bytes) return SAS_EINVAL;
   *bytes = c->h_tab.size() * sizeof(double) + (uint64_t)c->n_exp * sizeof(ExpParams);
+  return SAS_OK;
+}
+
+sas_status sas_reduce_radial(sas_ctx* c, const sas_radial_desc* d, double* h_q, double* h_I, double* h_sigma,
+                             uint64_t* h_npix) {
+  if (!c) return SAS_EINVAL;
+  if (!d || d->struct_size != sizeof(sas_radial_desc)) return fail(c, SAS_EINVAL, "sas_radial_desc.struct_size mismatch");
+  if (d->n_bins < 1 || d->n_bins > SAS_MAX_RINGS) return fail(c, SAS_EINVAL, "n_bins must be in 1..SAS_MAX_RINGS");
+  if (!(d->q_hi > d->q_lo) || !(d->q_lo >= 0.0) || !std::isfinite(d->q_hi)) return fail(c, SAS_EINVAL, "need 0 <= q_lo < q_hi");
+  if (!(d->lambda_ref > 0.0) || !std::isfinite(d->lambda_ref)) return fail(c, SAS_EINVAL, "lambda_ref must be > 0");
+  if (d->exp_index >= c->n_exp) return fail(c, SAS_EINVAL, "exp_index out of range");
+  const int nb = d->n_bins;
+  if (!c->d_rings) CUDA_TRY(c, cudaMalloc(&c->d_rings, 4 * (size_t)SAS_MAX_RINGS * sizeof(double)));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_rings, 0, 4 * (size_t)SAS_MAX_RINGS * sizeof(double), c->stream));
+  const sas_instrument_desc& ins = c->instr[d->exp_index];
+  ReduceArgs a;
+  a.sum_p = c->d_sum_p + (size_t)d->exp_index * c->npix;
+  a.sum_p2 = c->d_sum_p2 + (size_t)d->exp_index * c->npix;
+  a.ring_p = c->d_rings;
+  a.ring_p2 = c->d_rings + SAS_MAX_RINGS;
+  a.ring_omega = c->d_rings + 2 * SAS_MAX_RINGS;
+  a.ring_n = reinterpret_cast<unsigned long long*>(c->d_rings + 3 * SAS_MAX_RINGS);
+  a.det_xw = ins.det_xw; a.det_yh = ins.det_yh; a.det_dist = ins.det_dist;
+  a.px = ins.det_xw / (double)ins.det_nx; a.py = ins.det_yh / (double)ins.det_ny;
+  a.a_pix_d = (a.px * a.py) * ins.det_dist;
+  a.two_k = 2.0 * (TWO_PI / d->lambda_ref);
+  a.q_lo = d->q_lo; a.q_hi = d->q_hi; a.scale = (double)nb / (d->q_hi - d->q_lo);
+  a.nx = ins.det_nx; a.ny = ins.det_ny; a.n_bins = nb;
+  const int grid = std::max(1, std::min(c->n_sm * 4, (c->npix + REDUCE_THREADS - 1) / REDUCE_THREADS));
+  reduce_radial_kernel<<<grid, REDUCE_THREADS, 0, c->stream>>>(a);
+  CUDA_TRY(c, cudaGetLastError());
+  c->n_launches += 1;
+  std::vector<double> h(4 * (size_t)SAS_MAX_RINGS);
+  CUDA_TRY(c, cudaMemcpyAsync(h.data(), c->d_rings, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  const unsigned long long* hn = reinterpret_cast<const unsigned long long*>(h.data() + 3 * SAS_MAX_RINGS);
+  const double launched = (double)(c->launched / c->n_exp);  // every experiment of a context traces the same ids
+  for (int b = 0; b < nb; ++b) {
+    if (h_q) h_q[b] = d->q_lo + ((double)b + 0.5) * ((d->q_hi - d->q_lo) / (double)nb);
+    const double norm = h[2 * SAS_MAX_RINGS + b] * launched;
+    const bool any = hn[b] != 0 && norm > 0.0;
+    if (h_I) h_I[b] = any ? h[b] / norm : 0.0;
+    if (h_sigma) h_sigma[b] = any ? std::sqrt(h[SAS_MAX_RINGS + b]) / norm : 0.0;
+    if (h_npix) h_npix[b] = hn[b];
+  }
   return SAS_OK;
 }
 

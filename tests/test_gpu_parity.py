@@ -578,3 +578,42 @@ def test_many_tiny_experiments_in_one_batch(sas):
         if m.any():
             assert np.abs(sp[e].reshape(-1)[m] / ref["sum_p"][m] - 1).max() < 1e-9, e
     assert np.array_equal(cnt[:7], tot[:7])
+
+
+# ---- NEXT-4 (first part): ring average of the detector into I(q) on the GPU
+def test_radial_reduction_matches_the_oracle(sas):
+    c = W.config(1)
+    tr = sas.Tracer(c["instrument"], c["model"])
+    tr.trace(2 * 10**7, c["seed"])
+    sp, sp2, cn = tr.read_detector()
+    launched = int(tr.counters()[0])
+    for lam, q_lo, q_hi, nb in ((6.0, 0.0, 0.08, 64), (5.4, 0.004, 0.05, 1), (6.6, 0.01, 0.0733, 1024)):
+        q, I, s, n = tr.reduce_radial(lam, q_lo, q_hi, nb)
+        rq, rI, rs, rn = O.reduce_radial(c["instrument"], sp, sp2, launched, lam, q_lo, q_hi, nb)
+        assert np.array_equal(n, rn) and np.array_equal(q, rq)
+        m = rI > 0
+        assert m.sum() >= min(nb, 40) * 0.8
+        assert np.abs(I[m] / rI[m] - 1).max() < 1e-12 and np.abs(s[m] / rs[m] - 1).max() < 1e-12
+        assert np.all(I[~m] == 0) and np.all(s[~m] == 0)
+    # 2e7 neutrons give every populated ring a positive intensity with a small relative error
+    q, I, s, n = tr.reduce_radial(6.0, 0.004, 0.07, 66)
+    assert np.all(I[n > 0] > 0) and np.all(s[n > 0] < 0.2 * I[n > 0]) and (n > 0).sum() >= 60
+    with pytest.raises(sas.SasError):
+        tr.reduce_radial(6.0, 0.05, 0.01, 10)
+    with pytest.raises(sas.SasError):
+        tr.reduce_radial(6.0, 0.0, 0.1, 5000)
+    with pytest.raises(sas.SasError):
+        tr.reduce_radial(6.0, 0.0, 0.1, 10, exp_index=1)
+    tr.close()
+    # a batch: each experiment's own detector distance and histogram
+    b = W.batch_config(6, 400000, 77)
+    bt = sas.BatchTracer(b["instruments"], b["models"])
+    bt.trace(400000, 77)
+    sp, sp2, cn = bt.read_detector()
+    for e in (0, 3, 5):
+        lam = 0.5 * (b["instruments"][e]["lambda_min"] + b["instruments"][e]["lambda_max"])
+        q, I, s, n = bt.reduce_radial(lam, 0.0, 0.1, 40, exp_index=e)
+        rq, rI, rs, rn = O.reduce_radial(b["instruments"][e], sp[e], sp2[e], 400000, lam, 0.0, 0.1, 40)
+        m = rI > 0
+        assert np.array_equal(n, rn) and np.abs(I[m] / rI[m] - 1).max() < 1e-12 and np.abs(s[m] / rs[m] - 1).max() < 1e-12
+    bt.close()

@@ -131,6 +131,55 @@ double orc_py_sq(double q, double r_eff, double volfrac) {
   return 1.0 / (1.0 + (24.0 * phi) * ((alpha * t1 + beta * t2) + gamma * t3));
 }
 
+/* 32-node Gauss-Legendre rule on [-1, 1] (nodes ascending, weights summing to 2): Newton iteration on the
+ * Legendre polynomial P_32 from the Chebyshev-like starting points, the textbook construction. */
+#define ORC_GL_N 32
+static double gl_x[ORC_GL_N], gl_w[ORC_GL_N];
+static int gl_ready = 0;
+static void gl_init(void) {
+  if (gl_ready) return;
+  for (int i = 0; i < ORC_GL_N; ++i) {
+    double x = cos(PI_ * ((double)i + 0.75) / ((double)ORC_GL_N + 0.5));
+    double dp = 1.0;
+    for (int it = 0; it < 100; ++it) {
+      double p0 = 1.0, p1 = x;
+      for (int k = 2; k <= ORC_GL_N; ++k) {
+        double pk = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
+        p0 = p1; p1 = pk;
+      }
+      dp = ORC_GL_N * (x * p1 - p0) / (x * x - 1.0);
+      double dx = p1 / dp;
+      x -= dx;
+      if (fabs(dx) < 1e-16) break;
+    }
+    gl_x[ORC_GL_N - 1 - i] = x;
+    gl_w[ORC_GL_N - 1 - i] = 2.0 / ((1.0 - x * x) * dp * dp);
+  }
+  gl_ready = 1;
+}
+
+/* R-M2: end piece of a body of revolution about C: the part z in [L/2, zc + Rb] of the sphere of radius Rb
+ * centred on the axis at zc.  Eq. 1 slice by slice: a slice at height z is a disc of radius rho(z) whose
+ * in-plane integral is pi rho^2 Lambda(Q_AB rho); the two end pieces at +-z add up to 2 cos(Q_C z).
+ * Returns the integral for ONE end piece without the factor 2; *vcap its volume. */
+static double end_piece(double qab, double qc, double L, double Rb, double zc, double* vcap) {
+  gl_init();
+  double z0 = 0.5 * L, z1 = zc + Rb;
+  double half = 0.5 * (z1 - z0), mid = 0.5 * (z1 + z0);
+  double sum = 0.0;
+  for (int i = 0; i < ORC_GL_N; ++i) {
+    double z = mid + half * gl_x[i];
+    double dz = z - zc;
+    double rho2 = Rb * Rb - dz * dz;
+    if (rho2 < 0.0) rho2 = 0.0;
+    double rho = sqrt(rho2);
+    sum += gl_w[i] * (((PI_ * rho2) * orc_lambda1(qab * rho)) * cos(qc * z));
+  }
+  double a = z1 - zc, b = z0 - zc;
+  *vcap = PI_ * ((Rb * Rb) * (z1 - z0) - (((a * a) * a) - ((b * b) * b)) / 3.0);
+  return half * sum;
+}
+
 /* ------------------------------------------------------ R-C12 amplitudes */
 /* One particle, sizes scaled by the polydispersity node values x0, x1
  * (R-A12).  qa,qb,qc: projections of Q on the particle axes (PAPER.md:76-82,
@@ -226,6 +275,22 @@ double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double
       *vol = V;
       *env = m->sld[0] * V;
       return (m->sld[0] * V) * orc_sphere_phi(u);
+    }
+    case ORC_BARBELL:
+    case ORC_CAPPED_CYLINDER: {
+      /* R-M2: cylinder (R, L) along C plus two spherical end pieces of radius Rb >= R; x0 scales R, x1 scales L */
+      double R = m->size[0] * x0, L = m->size[1] * x1, Rb = m->size[2];
+      double h2 = Rb * Rb - R * R;
+      double h = sqrt(h2 > 0.0 ? h2 : 0.0);
+      double zc = m->model == ORC_BARBELL ? 0.5 * L + h : 0.5 * L - h;
+      double qab = sqrt(qa * qa + qb * qb);
+      double vcap;
+      double cap = end_piece(qab, qc, L, Rb, zc, &vcap);
+      double Vcyl = (PI_ * (R * R)) * L;
+      double V = Vcyl + 2.0 * vcap;
+      *vol = V;
+      *env = m->sld[0] * V;
+      return m->sld[0] * ((Vcyl * orc_sinc(qc * (0.5 * L))) * orc_lambda1(qab * R) + 2.0 * cap);
     }
     default:
       *vol = 1.0;

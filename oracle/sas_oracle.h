@@ -44,7 +44,12 @@ enum {
   /* NEXT-2: three more of the paper's models, each Eq. 1 integrated over its body */
   ORC_PARALLELEPIPED = 6,       /* Table I group E, Eq. 6: sides a, b, c along A, B, C */
   ORC_CORE_SHELL_CYLINDER = 7,  /* Table I group A, Eq. 7: core R, L; shell t on every face */
-  ORC_ELLIPSOID = 8             /* Table I group B, Eq. 7: equatorial R_e, polar R_p (axis C) */
+  ORC_ELLIPSOID = 8,            /* Table I group B, Eq. 7: equatorial R_e, polar R_p (axis C) */
+  /* two of the models the paper found expensive (inner numerical integration; R-M2):
+   * bodies of revolution = cylinder (R, L) + two spherical end pieces of radius R_b >= R, Eq. 1 integrated
+   * slice by slice with a 32-node Gauss-Legendre rule over each end piece */
+  ORC_BARBELL = 9,              /* sphere centres outside the cylinder, at +-(L/2 + h), h = sqrt(R_b^2 - R^2) */
+  ORC_CAPPED_CYLINDER = 10      /* sphere centres inside, at +-(L/2 - h): lens-shaped caps */
 };
 enum {
   ORC_ORIENT_FIXED = 0,

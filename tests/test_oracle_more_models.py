@@ -134,3 +134,63 @@ def test_new_models_trace_end_to_end_and_average_over_nodes():
     FV = [O.amplitude(md, *Q, xi, 1.0) for xi in x]
     want = 1e8 * 0.02 * sum(wi * F * F for wi, (F, V) in zip(w, FV)) / sum(wi * V for wi, (F, V) in zip(w, FV))
     assert abs(O.intensity(md, Q) / want - 1) < 1e-13
+
+
+# ---- R-M2: barbell and capped cylinder (bodies of revolution with spherical end pieces)
+def _brute_revolution(Q, pieces, n=64):
+    """Re integral of exp(-iQ.r) over a body of revolution about z given as [(z0, z1, rho(z))...] (PAPER.md:37,
+    Eq. 1, drho = 1), by Gauss-Legendre in (z, rho, phi) piece by piece; also returns the volume."""
+    F = V = 0.0
+    ph, wp = _gl(2 * n, 0.0, 2 * math.pi)
+    t, wt = _gl(n, 0.0, 1.0)
+    for z0, z1, rho in pieces:
+        z, wz = _gl(n, z0, z1)
+        rmax = rho(z)                                   # (n,)
+        Z, T, P = np.meshgrid(z, t, ph, indexing="ij")
+        RM = rmax[:, None, None]
+        RR = T * RM
+        f = np.cos(Q[0] * RR * np.cos(P) + Q[1] * RR * np.sin(P) + Q[2] * Z) * RR * RM
+        F += np.einsum("ijk,i,j,k->", f, wz, wt, wp)
+        V += np.einsum("i,i->", math.pi * rmax ** 2, wz)
+    return F, V
+
+
+def _pieces(kind, R, L, Rb):
+    h = math.sqrt(Rb * Rb - R * R)
+    zc = 0.5 * L + h if kind == "barbell" else 0.5 * L - h
+    cap = lambda z: np.sqrt(np.maximum(Rb * Rb - (np.abs(z) - zc) ** 2, 0.0))
+    return [(-0.5 * L, 0.5 * L, lambda z: np.full_like(z, R)), (0.5 * L, zc + Rb, cap), (-(zc + Rb), -0.5 * L, cap)]
+
+
+def test_barbell_and_capped_cylinder_are_eq1_integrated_slice_by_slice():
+    for kind, R, L, Rb in (("barbell", 20.0, 200.0, 40.0), ("capped_cylinder", 20.0, 200.0, 25.0),
+                           ("barbell", 30.0, 90.0, 30.0001), ("capped_cylinder", 30.0, 90.0, 60.0)):
+        m = W.model(model=kind, size=[R, L, Rb, 0], sld=[1.0, 0, 0])
+        for Q in (np.array(v) for v in ((0.03, 0.0, 0.0), (0.0, 0.0, 0.02), (0.013, -0.021, 0.017), (0.05, 0.04, -0.06),
+                                        (1e-4, 2e-4, -1e-4))):
+            F, V = O.amplitude(m, *Q)
+            Fb, Vb = _brute_revolution(Q, _pieces(kind, R, L, Rb))
+            assert abs(V - Vb) < 1e-9 * Vb, (kind, V, Vb)
+            assert abs(F - Fb) < 2e-8 * Vb, (kind, Q, F, Fb)
+    # closed-form volumes: cylinder + two sphere pieces
+    R, L, Rb = 20.0, 200.0, 40.0
+    h = math.sqrt(Rb * Rb - R * R)
+    v_big = math.pi * (2 * Rb ** 3 / 3 + Rb * Rb * h - h ** 3 / 3)      # sphere part beyond the plane at distance h
+    assert abs(O.amplitude(W.model(model="barbell", size=[R, L, Rb, 0]), 0, 0, 0)[1] - (math.pi * R * R * L + 2 * v_big)) < 1e-6
+    Rc = 25.0
+    hc = math.sqrt(Rc * Rc - R * R)
+    v_cap = math.pi * (Rc - hc) ** 2 * (2 * Rc + hc) / 3                 # spherical cap of height Rc - hc
+    assert abs(O.amplitude(W.model(model="capped_cylinder", size=[R, L, Rc, 0]), 0, 0, 0)[1] - (math.pi * R * R * L + 2 * v_cap)) < 1e-6
+    # a cap radius much larger than R flattens the caps: the capped cylinder tends to the plain cylinder
+    cyl = W.model(model="cylinder", size=[R, L, 0, 0], sld=[1.0, 0, 0])
+    flat = W.model(model="capped_cylinder", size=[R, L, 1e5, 0], sld=[1.0, 0, 0])
+    for Q in ((0.02, 0.0, 0.01), (0.0, 0.03, 0.02)):
+        assert abs(O.amplitude(flat, *Q)[0] - O.amplitude(cyl, *Q)[0]) < 1e-4 * O.amplitude(cyl, 0, 0, 0)[1]
+    # a barbell of zero length with R -> 0 is two touching spheres: F = 2 V_s Phi(q Rb) cos(Q_C Rb)
+    two = W.model(model="barbell", size=[1e-6, 1e-9, 30.0, 0], sld=[1.0, 0, 0])
+    Vs = 4 * math.pi / 3 * 30.0 ** 3
+    for qc_, qa_ in ((0.02, 0.0), (0.01, 0.03), (0.0, 0.05)):
+        q = math.hypot(qc_, qa_)
+        u = q * 30.0
+        want = 2 * Vs * 3 * (math.sin(u) - u * math.cos(u)) / u ** 3 * math.cos(qc_ * 30.0)
+        assert abs(O.amplitude(two, qa_, 0.0, qc_)[0] - want) < 1e-6 * Vs

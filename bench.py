@@ -115,6 +115,8 @@ def model_key_and_nodes(model):
     pd = [n if k == "schulz" else 1 for k, n in zip(model["pd_kind"], model["pd_nodes"])]
     if is_event_model(model) and m == "cylinder":
         return "cylinder_event_fp64", 1
+    if is_event_model(model) and m == "barbell":
+        return "barbell_event_fp64", 64
     if m == "sphere":
         nodes = pd[0]
         eff = prec if nodes > 1 else "fp64"
@@ -374,7 +376,7 @@ def main():
 
     others = {}
     if not args.headline_only:
-        for i in [j for j in range(6) if j != args.config]:
+        for i in [j for j in range(7) if j != args.config]:
             o, _ = bench_config(torch, S, i, 3, 3, rank, world, flush, False)
             others[o["workload"]] = {k: o[k] for k in ("value", "ms_per_step", "kernel_ms", "n_neutrons_per_step",
                                                        "detected_frac", "grid", "smem_bytes")}
@@ -407,7 +409,7 @@ def main():
         except Exception as exc:                          # a reported extra, never fatal
             cpu["all_cores"] = {"error": str(exc)}
         if not args.headline_only:
-            names = {W.config(i)["name"]: i for i in range(6)}
+            names = {W.config(i)["name"]: i for i in range(7)}
             for k, v in others.items():
                 if k in names:
                     v["oracle_1core"] = oracle_rate(names[k])

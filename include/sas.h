@@ -61,7 +61,12 @@ enum {
    * (no SAS_ORIENT_GAUSS_QUAD) */
   SAS_PARALLELEPIPED = 6,      /* size = a, b, c along A, B, C (Eq. 6); pd[0] = common scale */
   SAS_CORE_SHELL_CYLINDER = 7, /* size = R, L, t (Eq. 7); sld[0] core, sld[1] shell; pd[0] on R, pd[1] on L */
-  SAS_ELLIPSOID = 8            /* size = R_equatorial, R_polar (axis C, Eq. 7); pd[0] on R_e, pd[1] on R_p */
+  SAS_ELLIPSOID = 8,           /* size = R_equatorial, R_polar (axis C, Eq. 7); pd[0] on R_e, pd[1] on R_p */
+  /* two of the models the paper found expensive (DESIGN.md R-M2): cylinder (R, L) along C plus two
+   * spherical end pieces of radius R_b >= R, integrated slice by slice (32 Gauss-Legendre nodes per end piece).
+   * size = R, L, R_b; pd[0] on R, pd[1] on L */
+  SAS_BARBELL = 9,             /* sphere centres outside the cylinder, at +-(L/2 + sqrt(R_b^2 - R^2)) */
+  SAS_CAPPED_CYLINDER = 10     /* sphere centres inside, at +-(L/2 - sqrt(R_b^2 - R^2)): lens-shaped caps */
 };
 enum {
   SAS_ORIENT_FIXED = 0,

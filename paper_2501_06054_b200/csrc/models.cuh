@@ -12,6 +12,11 @@
 
 namespace sas {
 
+// 32-node Gauss-Legendre rule on [-1, 1] for the end pieces of the barbell and the capped cylinder (R-M2):
+// nodes then weights (summing to 1), uploaded once by the host from its own Jacobi-matrix rule (sas_api.cu)
+constexpr int GL_N = 32;
+__constant__ double c_gl[2 * GL_N];
+
 constexpr int CYL_UNROLL = SAS_CYL_UNROLL;  // nodes of the phi-tilt loop in flight
 
 template <typename Real>
@@ -165,6 +170,28 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
     const double qab = sqrt(fma(qA, qA, qB * qB));
     F = fma(((s0 - s1) * Vc) * sinc_r(qC * (0.5 * L)), lambda1_r(qab * R),
             ((s1 * Vol) * sinc_r(qC * (0.5 * Lt))) * lambda1_r(qab * Rt));
+  } else if (V == V_BARBELL || V == V_CAPPED) {
+    // R-M2: cylinder (R, L) along C plus two sphere pieces z in [L/2, zc + Rb]; Eq. 1 slice by slice: a slice is a
+    // disc pi rho^2 Lambda(Q_AB rho), the two pieces at +-z give 2 cos(Q_C z)
+    const double R = P.msize[0] * x0, L = P.msize[1] * x1, Rb = P.msize[2];
+    const double h = sqrt(fmax(Rb * Rb - R * R, 0.0));
+    const double zc = V == V_BARBELL ? 0.5 * L + h : 0.5 * L - h;
+    const double z0 = 0.5 * L, z1 = zc + Rb;
+    const double half = 0.5 * (z1 - z0), mid = 0.5 * (z1 + z0);
+    const double qab = sqrt(fma(qA, qA, qB * qB));
+    double sum = 0.0;
+#pragma unroll 1
+    for (int i = 0; i < GL_N; ++i) {
+      const double z = fma(half, c_gl[i], mid);
+      const double dz = z - zc;
+      const double rho2 = fmax(Rb * Rb - dz * dz, 0.0);
+      sum = fma(c_gl[GL_N + i], ((PI_D * rho2) * lambda1_r(qab * sqrt(rho2))) * cos(qC * z), sum);
+    }
+    const double pz = z1 - zc, qz = z0 - zc;
+    const double Vcyl = (PI_D * (R * R)) * L;
+    Vol = Vcyl + 2.0 * (PI_D * ((Rb * Rb) * (z1 - z0) - (((pz * pz) * pz) - ((qz * qz) * qz)) / 3.0));
+    // the weights sum to 1: the rule's (z1 - z0)/2 x 2 becomes (z1 - z0); two end pieces
+    F = s0 * fma((Vcyl * sinc_r(qC * (0.5 * L))), lambda1_r(qab * R), 2.0 * ((z1 - z0) * sum));
   } else if (V == V_ELL) {
     const double Re = P.msize[0] * x0, Rp = P.msize[1] * x1;
     Vol = FOUR_PI_3 * ((Re * Re) * Rp);

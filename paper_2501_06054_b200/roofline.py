@@ -53,6 +53,10 @@ MODEL_COST = {
     # per-event sizes: Philox blocks 2 and 3, two Box-Muller normals (log, sqrt, cos in fp64), three sincospi,
     # sin, j1, the weight
     "cylinder_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12, 40), (0, 0, 0, 0)),
+    # barbell, per event: the cylinder term and the prologue of the per-event path, then 64 slice evaluations
+    # (square root, fp64 J1, fp64 cos, ~15 multiply-adds: ~95 instructions of which ~30 FP64, from the ncu
+    # instruction and pipe counts of the n2 workload: 491 thread instructions and 143 FP64 per launched neutron)
+    "barbell_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12, 40), (95, 30, 2, 0)),
 }
 
 # DRAM traffic of one trace-kernel launch, dram__bytes_read.sum + dram__bytes_write.sum of the

@@ -101,6 +101,15 @@ def config(i: int, precision: str | None = None):
                         pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.05, 0.05],
                         orient_kind="uniform_angles_mc"),
             n_neutrons=10**9, seed=20250111)
+    if i == 6:
+        # NEXT-2 (not a BASELINE.json config): one of the models the paper found expensive, the
+        # barbell, with the paper's per-event sizes and orientation: 64 slice evaluations with a Bessel J1 each per
+        # detected neutron
+        return dict(
+            name="n2_paper_barbell", instrument=instrument(det_nx=256, det_ny=256),
+            model=model(model="barbell", precision="fp64", size=[20.0, 400.0, 40.0, 0],
+                        pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.05, 0.05], orient_kind="uniform_angles_mc"),
+            n_neutrons=10**9, seed=20250112)
     raise ValueError(i)
 
 

@@ -333,6 +333,12 @@ MORE_MODELS = [
                                  sq_kind="hard_sphere_py", sq_radius_eff=45.0, sq_volfrac=0.15, background=0.01)),
     ("ellipsoid_paper", dict(model="ellipsoid", size=[30.0, 70.0, 0, 0], pd_kind=["gauss_mc", "none"], pd_rel=[0.2, 0],
                              theta=0.5, phi=1.0)),
+    ("barbell_pd_fixed", dict(model="barbell", size=[20.0, 200.0, 40.0, 0], pd_kind=["schulz", "schulz"], pd_rel=[0.1, 0.1],
+                              pd_nodes=[4, 3], theta=0.8, phi=0.5)),
+    ("barbell_paper", dict(model="barbell", size=[20.0, 200.0, 40.0, 0], pd_kind=["gauss_mc", "gauss_mc"],
+                           pd_rel=[0.05, 0.1], orient_kind="uniform_angles_mc")),
+    ("capped_cylinder_iso", dict(model="capped_cylinder", size=[20.0, 200.0, 25.0, 0], orient_kind="isotropic_mc",
+                                 pd_kind=["none", "schulz"], pd_rel=[0, 0.2], pd_nodes=[1, 5])),
 ]
 
 

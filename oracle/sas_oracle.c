@@ -276,6 +276,42 @@ double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double
       *env = m->sld[0] * V;
       return (m->sld[0] * V) * orc_sphere_phi(u);
     }
+    case ORC_ELLIPTICAL_CYLINDER: {
+      /* Eq. 1 over {x^2/a^2 + y^2/b^2 <= 1, |z| <= L/2}: the elliptic disc is a unit disc stretched by (a, b), so its
+       * in-plane integral is pi a b Lambda(sqrt((a Q_A)^2 + (b Q_B)^2)); x0 scales a and b, x1 scales L */
+      double a = m->size[0] * x0, b = m->size[1] * x0, L = m->size[2] * x1;
+      double V = (PI_ * (a * b)) * L;
+      double u = sqrt((a * qa) * (a * qa) + (b * qb) * (b * qb));
+      *vol = V;
+      *env = m->sld[0] * V;
+      return ((m->sld[0] * V) * orc_sinc(qc * (0.5 * L))) * orc_lambda1(u);
+    }
+    case ORC_HOLLOW_CYLINDER: {
+      /* tube = cylinder of radius R + t minus the hollow core of radius R, same length; normalised by the volume of
+       * the wall; x0 scales the core radius, x1 the length, the wall keeps its thickness */
+      double Ri = m->size[0] * x0, L = m->size[1] * x1, t = m->size[2];
+      double Ro = Ri + t;
+      double Vo = (PI_ * (Ro * Ro)) * L, Vi = (PI_ * (Ri * Ri)) * L;
+      double qab = sqrt(qa * qa + qb * qb);
+      double sl = orc_sinc(qc * (0.5 * L));
+      *vol = Vo - Vi;
+      *env = m->sld[0] * (Vo + Vi);
+      return m->sld[0] * ((Vo * sl) * orc_lambda1(qab * Ro) - (Vi * sl) * orc_lambda1(qab * Ri));
+    }
+    case ORC_CORE_SHELL_ELLIPSOID: {
+      /* core ellipsoid of revolution (R_e, R_p) of contrast sld[0] inside the ellipsoid (R_e + t, R_p + t) of
+       * contrast sld[1]; x0 scales R_e, x1 scales R_p */
+      double Re = m->size[0] * x0, Rp = m->size[1] * x1, t = m->size[2];
+      double Ret = Re + t, Rpt = Rp + t;
+      double Vc = FOUR_PI_3 * ((Re * Re) * Rp), Vt = FOUR_PI_3 * ((Ret * Ret) * Rpt);
+      double qab2 = qa * qa + qb * qb;
+      double uc = sqrt((Re * Re) * qab2 + (Rp * qc) * (Rp * qc));
+      double ut = sqrt((Ret * Ret) * qab2 + (Rpt * qc) * (Rpt * qc));
+      double fc = (m->sld[0] - m->sld[1]) * Vc, ft = m->sld[1] * Vt;
+      *vol = Vt;
+      *env = fabs(fc) + fabs(ft);
+      return fc * orc_sphere_phi(uc) + ft * orc_sphere_phi(ut);
+    }
     case ORC_BARBELL:
     case ORC_CAPPED_CYLINDER: {
       /* R-M2: cylinder (R, L) along C plus two spherical end pieces of radius Rb >= R; x0 scales R, x1 scales L */

@@ -49,7 +49,11 @@ enum {
    * bodies of revolution = cylinder (R, L) + two spherical end pieces of radius R_b >= R, Eq. 1 integrated
    * slice by slice with a 32-node Gauss-Legendre rule over each end piece */
   ORC_BARBELL = 9,              /* sphere centres outside the cylinder, at +-(L/2 + h), h = sqrt(R_b^2 - R^2) */
-  ORC_CAPPED_CYLINDER = 10      /* sphere centres inside, at +-(L/2 - h): lens-shaped caps */
+  ORC_CAPPED_CYLINDER = 10,     /* sphere centres inside, at +-(L/2 - h): lens-shaped caps */
+  /* three more bodies of Table I, each Eq. 1 over the body (R-M3) */
+  ORC_ELLIPTICAL_CYLINDER = 11, /* group B: cross-section semi-axes a (along A), b (along B), length L along C */
+  ORC_HOLLOW_CYLINDER = 12,     /* group A: tube, hollow core radius R, wall thickness t, length L */
+  ORC_CORE_SHELL_ELLIPSOID = 13 /* group B: core of revolution (R_e, R_p) in a shell of thickness t */
 };
 enum {
   ORC_ORIENT_FIXED = 0,

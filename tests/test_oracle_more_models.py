@@ -194,3 +194,60 @@ def test_barbell_and_capped_cylinder_are_eq1_integrated_slice_by_slice():
         u = q * 30.0
         want = 2 * Vs * 3 * (math.sin(u) - u * math.cos(u)) / u ** 3 * math.cos(qc_ * 30.0)
         assert abs(O.amplitude(two, qa_, 0.0, qc_)[0] - want) < 1e-6 * Vs
+
+
+# ---- R-M3: elliptical cylinder, hollow cylinder, core-shell ellipsoid of revolution
+def _brute_elliptic_cylinder(Q, a, b, L, n=48):
+    r, wr = _gl(n, 0.0, 1.0)
+    ph, wp = _gl(2 * n, 0.0, 2 * math.pi)
+    z, wz = _gl(n, -0.5 * L, 0.5 * L)
+    RR, P, Z = np.meshgrid(r, ph, z, indexing="ij")
+    f = np.cos(Q[0] * a * RR * np.cos(P) + Q[1] * b * RR * np.sin(P) + Q[2] * Z) * RR * (a * b)
+    return np.einsum("ijk,i,j,k->", f, wr, wp, wz)
+
+
+def test_elliptical_cylinder_hollow_cylinder_core_shell_ellipsoid_are_eq1_integrated():
+    a, b, L = 20.0, 35.0, 300.0
+    m = W.model(model="elliptical_cylinder", size=[a, b, L, 0], sld=[1.0, 0, 0])
+    circ = W.model(model="elliptical_cylinder", size=[a, a, L, 0], sld=[1.0, 0, 0])
+    cyl = W.model(model="cylinder", size=[a, L, 0, 0], sld=[1.0, 0, 0])
+    for Q in QS:
+        F, V = O.amplitude(m, *Q)
+        assert abs(V - math.pi * a * b * L) < 1e-9 * V
+        assert abs(F - _brute_elliptic_cylinder(Q, a, b, L)) < 2e-9 * V, Q
+        assert abs(O.amplitude(circ, *Q)[0] - O.amplitude(cyl, *Q)[0]) < 1e-12 * V     # a = b: the circular cylinder
+    # which semi-axis belongs to which particle axis: Lambda's first zero (j_{1,1} = 3.8317) along A and along B
+    assert abs(O.amplitude(m, 3.8317059702 / a, 0.0, 0.0)[0]) < 1e-8 * math.pi * a * b * L
+    assert abs(O.amplitude(m, 0.0, 3.8317059702 / b, 0.0)[0]) < 1e-8 * math.pi * a * b * L
+    # x0 scales both semi-axes, x1 the length
+    F, V = O.amplitude(m, 0.01, 0.02, 0.005, 1.2, 0.8)
+    assert abs(F - _brute_elliptic_cylinder((0.01, 0.02, 0.005), 1.2 * a, 1.2 * b, 0.8 * L)) < 2e-9 * V
+
+    Ri, Lh, t = 20.0, 300.0, 8.0
+    hol = W.model(model="hollow_cylinder", size=[Ri, Lh, t, 0], sld=[1.0, 0, 0])
+    Vw = math.pi * ((Ri + t) ** 2 - Ri ** 2) * Lh
+    for Q in QS:
+        F, V = O.amplitude(hol, *Q)
+        ref = _brute_cylinder(Q, Ri + t, Lh) - _brute_cylinder(Q, Ri, Lh)
+        assert abs(V - Vw) < 1e-9 * Vw and abs(F - ref) < 5e-9 * math.pi * (Ri + t) ** 2 * Lh, Q
+    # the same body as a core-shell cylinder whose core has the solvent's contrast and whose caps are missing:
+    # for Q perpendicular to the axis the caps do not matter in the radial factor
+    F0, V0 = O.amplitude(W.model(model="hollow_cylinder", size=[1e-9, Lh, t, 0], sld=[1.0, 0, 0]), 0.02, 0.01, 0.003)
+    Fc, Vc = O.amplitude(W.model(model="cylinder", size=[t, Lh, 0, 0], sld=[1.0, 0, 0]), 0.02, 0.01, 0.003)
+    assert abs(F0 - Fc) < 1e-9 * Vc                       # no hole: a solid cylinder of radius t
+
+    Re, Rp, ts, s0, s1 = 30.0, 70.0, 8.0, 3.0, 1.0
+    cse = W.model(model="core_shell_ellipsoid", size=[Re, Rp, ts, 0], sld=[s0, s1, 0])
+    Vt = 4 * math.pi / 3 * (Re + ts) ** 2 * (Rp + ts)
+    for Q in QS:
+        F, V = O.amplitude(cse, *Q)
+        ref = (s0 - s1) * _brute_ellipsoid(Q, Re, Re, Rp) + s1 * _brute_ellipsoid(Q, Re + ts, Re + ts, Rp + ts)
+        assert abs(V - Vt) < 1e-9 * Vt and abs(F - ref) < 1e-9 * s0 * Vt, Q
+    # equal contrasts: the homogeneous ellipsoid (R_e + t, R_p + t); R_e = R_p: the core-shell sphere
+    hom = W.model(model="ellipsoid", size=[Re + ts, Rp + ts, 0, 0], sld=[s1, 0, 0])
+    eq = W.model(model="core_shell_ellipsoid", size=[Re, Rp, ts, 0], sld=[s1, s1, 0])
+    css = W.model(model="core_shell_sphere", size=[Re, ts, 0, 0], sld=[s0, s1, 0])
+    rnd = W.model(model="core_shell_ellipsoid", size=[Re, Re, ts, 0], sld=[s0, s1, 0])
+    for Q in QS:
+        assert abs(O.amplitude(eq, *Q)[0] - O.amplitude(hom, *Q)[0]) < 1e-12 * s1 * Vt
+        assert abs(O.amplitude(rnd, *Q)[0] - O.amplitude(css, *Q)[0]) < 1e-12 * s0 * Vt

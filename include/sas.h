@@ -66,7 +66,11 @@ enum {
    * spherical end pieces of radius R_b >= R, integrated slice by slice (32 Gauss-Legendre nodes per end piece).
    * size = R, L, R_b; pd[0] on R, pd[1] on L */
   SAS_BARBELL = 9,             /* sphere centres outside the cylinder, at +-(L/2 + sqrt(R_b^2 - R^2)) */
-  SAS_CAPPED_CYLINDER = 10     /* sphere centres inside, at +-(L/2 - sqrt(R_b^2 - R^2)): lens-shaped caps */
+  SAS_CAPPED_CYLINDER = 10,    /* sphere centres inside, at +-(L/2 - sqrt(R_b^2 - R^2)): lens-shaped caps */
+  /* three more bodies of Table I (DESIGN.md R-M3) */
+  SAS_ELLIPTICAL_CYLINDER = 11,  /* size = a (along A), b (along B), L (along C); pd[0] scales a and b, pd[1] on L */
+  SAS_HOLLOW_CYLINDER = 12,      /* size = hollow core radius R, L, wall thickness t; pd[0] on R, pd[1] on L */
+  SAS_CORE_SHELL_ELLIPSOID = 13  /* size = R_e, R_p, t; sld[0] core, sld[1] shell; pd[0] on R_e, pd[1] on R_p */
 };
 enum {
   SAS_ORIENT_FIXED = 0,

@@ -170,6 +170,24 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
     const double qab = sqrt(fma(qA, qA, qB * qB));
     F = fma(((s0 - s1) * Vc) * sinc_r(qC * (0.5 * L)), lambda1_r(qab * R),
             ((s1 * Vol) * sinc_r(qC * (0.5 * Lt))) * lambda1_r(qab * Rt));
+  } else if (V == V_ELL_CYL) {
+    const double a = P.msize[0] * x0, b = P.msize[1] * x0, L = P.msize[2] * x1;
+    Vol = (PI_D * (a * b)) * L;
+    const double ua = a * qA, ub = b * qB;
+    F = ((s0 * Vol) * sinc_r(qC * (0.5 * L))) * lambda1_r(sqrt(fma(ua, ua, ub * ub)));
+  } else if (V == V_HOLLOW_CYL) {
+    const double Ri = P.msize[0] * x0, L = P.msize[1] * x1, Ro = Ri + P.msize[2];
+    const double Vo = (PI_D * (Ro * Ro)) * L, Vi = (PI_D * (Ri * Ri)) * L;
+    const double qab = sqrt(fma(qA, qA, qB * qB));
+    Vol = Vo - Vi;
+    F = (s0 * sinc_r(qC * (0.5 * L))) * fma(Vo, lambda1_r(qab * Ro), -(Vi * lambda1_r(qab * Ri)));
+  } else if (V == V_CS_ELL) {
+    const double Re = P.msize[0] * x0, Rp = P.msize[1] * x1, Ret = Re + P.msize[2], Rpt = Rp + P.msize[2];
+    const double Vc = FOUR_PI_3 * ((Re * Re) * Rp);
+    Vol = FOUR_PI_3 * ((Ret * Ret) * Rpt);
+    const double qab2 = fma(qA, qA, qB * qB), uc = Rp * qC, ut = Rpt * qC;
+    F = fma((s0 - s1) * Vc, sphere_phi(sqrt(fma(Re * Re, qab2, uc * uc))),
+            (s1 * Vol) * sphere_phi(sqrt(fma(Ret * Ret, qab2, ut * ut))));
   } else if (V == V_BARBELL || V == V_CAPPED) {
     // R-M2: cylinder (R, L) along C plus two sphere pieces z in [L/2, zc + Rb]; Eq. 1 slice by slice: a slice is a
     // disc pi rho^2 Lambda(Q_AB rho), the two pieces at +-z give 2 cos(Q_C z)

@@ -339,6 +339,13 @@ MORE_MODELS = [
                            pd_rel=[0.05, 0.1], orient_kind="uniform_angles_mc")),
     ("capped_cylinder_iso", dict(model="capped_cylinder", size=[20.0, 200.0, 25.0, 0], orient_kind="isotropic_mc",
                                  pd_kind=["none", "schulz"], pd_rel=[0, 0.2], pd_nodes=[1, 5])),
+    ("elliptical_cylinder_pd", dict(model="elliptical_cylinder", size=[20.0, 35.0, 300.0, 0], theta=1.1, phi=0.4, psi=0.9,
+                                    pd_kind=["schulz", "schulz"], pd_rel=[0.1, 0.1], pd_nodes=[5, 4])),
+    ("hollow_cylinder_paper", dict(model="hollow_cylinder", size=[20.0, 300.0, 8.0, 0], pd_kind=["gauss_mc", "gauss_mc"],
+                                   pd_rel=[0.1, 0.05], orient_kind="uniform_angles_mc")),
+    ("core_shell_ellipsoid_iso", dict(model="core_shell_ellipsoid", size=[30.0, 70.0, 8.0, 0], sld=[3e-6, 1e-6, 0],
+                                      orient_kind="isotropic_mc", pd_kind=["schulz", "none"], pd_rel=[0.15, 0],
+                                      pd_nodes=[9, 1])),
 ]
 
 

@@ -577,6 +577,12 @@ sas_status launch_groups(sas_ctx* c, KernelArgs& a) {
   return SAS_OK;
 }
 
+// ids one launch may take from `first`: at most 2^31, at most n, and up to the next multiple of 2^32
+uint64_t launch_span(uint64_t first, uint64_t n) {
+  const uint64_t to_boundary = (1ull << 32) - (first & 0xFFFFFFFFull);
+  return std::min<uint64_t>(std::min<uint64_t>(n, 1ull << 31), to_boundary);
+}
+
 sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t seed) {
   if (!c) return SAS_EINVAL;
   if (!c->model_set) return fail(c, SAS_ESTATE, "sas_set_model must precede tracing");
@@ -589,14 +595,15 @@ sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t
   a.counters = c->d_counters; a.work_counter = c->d_work;
   a.n_exp = c->n_exp; a.exp_base = 0; a.npix = c->npix;
   philox_make_keys(seed, a.keys);
-  // one launch covers at most 2^31 ids per experiment (32-bit id offsets inside the kernel)
-  const uint64_t chunk = 1ull << 31;
-  for (uint64_t done = 0; done < n_each; done += chunk) {
+  // one launch covers at most 2^31 ids per experiment (32-bit id offsets inside the kernel) and never crosses a
+  // multiple of 2^32 (the kernel keeps the high Philox counter word of the ids as one number per launch)
+  for (uint64_t done = 0; done < n_each;) {
     a.first_id = first_id + done;
-    a.n_per_exp = (uint32_t)std::min<uint64_t>(chunk, n_each - done);
+    a.n_per_exp = (uint32_t)launch_span(a.first_id, n_each - done);
     sas_status st = launch_groups(c, a);
     if (st != SAS_OK) return st;
     c->launched += (uint64_t)a.n_per_exp * c->n_exp;
+    done += a.n_per_exp;
   }
   return SAS_OK;
 }
@@ -742,12 +749,19 @@ sas_status sas_trace_dump(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t se
   a.counters = c->d_counters; a.work_counter = c->d_work;
   a.d_pixel = d_pixel; a.d_weight = d_weight; a.d_q = d_q;
   a.n_exp = 1; a.exp_base = exp_index; a.npix = c->npix;
-  a.first_id = first_id; a.n_per_exp = (uint32_t)n;
   philox_make_keys(seed, a.keys);
   CUDA_TRY(c, cudaMemsetAsync(d_pixel, 0xFF, n * sizeof(int32_t), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(d_weight, 0, n * sizeof(double), c->stream));
   if (d_q) CUDA_TRY(c, cudaMemsetAsync(d_q, 0, n * sizeof(double), c->stream));
-  return launch_groups(c, a);
+  for (uint64_t done = 0; done < n;) {
+    a.first_id = first_id + done;
+    a.n_per_exp = (uint32_t)launch_span(a.first_id, n - done);
+    a.d_pixel = d_pixel + done; a.d_weight = d_weight + done; a.d_q = d_q ? d_q + done : nullptr;
+    sas_status st = launch_groups(c, a);
+    if (st != SAS_OK) return st;
+    done += a.n_per_exp;
+  }
+  return SAS_OK;
 }
 
 sas_status sas_read_detector(sas_ctx* c, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts) {

@@ -103,6 +103,8 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
   const unsigned FULL = 0xFFFFFFFFu;
   const bool DUMP = a.d_pixel != nullptr;  // parity hook: per-neutron outputs instead of the histogram
   const bool DUMP_Q = DUMP && a.d_q != nullptr;
+  // the host never lets a launch cross a multiple of 2^32 ids: the high counter word is one number per launch
+  const uint32_t first_lo = (uint32_t)a.first_id, id_hi = (uint32_t)(a.first_id >> 32);
 
   // warp-uniform pipeline state
   int headB = 0, cntB = 0, headB2 = 0, cntB2 = 0, headC = 0, cntC = 0;
@@ -168,12 +170,12 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
         headC = (headC + n) & (RING - 1);
         cntC -= n;
         if (act) {
-          const uint64_t id = a.first_id + idoff;
+          const uint32_t id_lo = first_lo + idoff;
           Real I;
           if (EV)
-            I = (Real)eval_intensity_event<V>(P, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
+            I = (Real)eval_intensity_event<V>(P, a.keys, id_lo, id_hi, exp_word, Qx, Qy, Qz);
           else
-            I = eval_intensity<Real, V>(P, tab, a.keys, (uint32_t)id, (uint32_t)(id >> 32), exp_word, Qx, Qy, Qz);
+            I = eval_intensity<Real, V>(P, tab, a.keys, id_lo, id_hi, exp_word, Qx, Qy, Qz);
           const double p = G * (double)I;
           if (DUMP) {
             a.d_pixel[idoff] = pixel;
@@ -204,8 +206,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
           for (int i = 0; i < 4; ++i) w1[i] = wq.b2_w[i][slot];
         }
         {
-          const uint64_t id = a.first_id + idoff;
-          philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
+          philox4x32_10(a.keys, first_lo + idoff, id_hi, 0u, exp_word, w);
         }
         __syncwarp();
         headB2 = (headB2 + n) & (RING_B2 - 1);
@@ -243,8 +244,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
         cntB -= n;
 #pragma unroll
         for (int k = 0; k < NB0; ++k) {
-          const uint64_t id = a.first_id + idoff[k];
-          philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 1u, exp_word, w1[k]);
+          philox4x32_10(a.keys, first_lo + idoff[k], id_hi, 1u, exp_word, w1[k]);
         }
         int tail = headB2 + cntB2;
 #pragma unroll
@@ -274,7 +274,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
         // survivors is queued (tight loop: ~4 rows per stage-B round at a 25 % pass rate)
         const bool s1_int = P.s1_int_ok != 0;
         const uint32_t lo0 = P.s1_lo[0], hi0 = P.s1_hi[0], lo1 = P.s1_lo[1], hi1 = P.s1_hi[1];
-        const uint64_t id0 = a.first_id + off0 + lane;
+        const uint32_t id0 = first_lo + off0 + lane;
 #if SAS_STAGE_A_ROWS >= 2
         // several rows per step: independent Philox chains in flight, round keys loaded once
         do {
@@ -284,8 +284,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
           unsigned m[NR];
 #pragma unroll
           for (int k = 0; k < NR; ++k) {
-            const uint64_t id = id0 + ((row + k * WARPS_PER_BLOCK) << 5);
-            philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w[k]);
+            philox4x32_10(a.keys, id0 + ((row + k * WARPS_PER_BLOCK) << 5), id_hi, 0u, exp_word, w[k]);
           }
           int tail = headB + cntB;
 #pragma unroll
@@ -305,9 +304,8 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
 #else
         do {
           const uint32_t in_item = (row << 5) + lane;
-          const uint64_t id = id0 + (row << 5);
           uint32_t w[4];
-          philox4x32_10(a.keys, (uint32_t)id, (uint32_t)(id >> 32), 0u, exp_word, w);
+          philox4x32_10(a.keys, id0 + (row << 5), id_hi, 0u, exp_word, w);
           bool pass = in_item < cnt_ids;
           if (s1_int) pass = pass && (w[0] - lo0 <= hi0 - lo0) && (w[1] - lo1 <= hi1 - lo1);
           const unsigned m = __ballot_sync(FULL, pass);

@@ -214,6 +214,16 @@ def test_edge_cases(sas):
     tr.close()
     big = (1 << 33) + 12345
     check_dump(sas, c["instrument"], c["model"], c["seed"], big, 100000, min_detected=3000)
+    # a range that crosses a multiple of 2^32: the library splits the launch there (dump and histogram paths)
+    cross = (1 << 32) - 50001
+    check_dump(sas, c["instrument"], c["model"], c["seed"], cross, 100000, min_detected=3000)
+    tr = sas.Tracer(c["instrument"], c["model"])
+    tr.trace_range(cross, 100000, c["seed"])
+    ref = O.trace_range(c["instrument"], c["model"], c["seed"], cross, 100000, dump=False)
+    assert np.array_equal(tr.counters()[:7], ref["counters"][:7])
+    assert np.array_equal(tr.read_detector()[2].reshape(-1), ref["counts"])
+    assert tr.launch_info()["n_launches"] == 2
+    tr.close()
 
 
 def test_error_paths(sas):

@@ -63,11 +63,11 @@ MODEL_COST = {
 # `ncu --set full` captures summarised in profiles/r1_ncu_c<k>.md (bytes per launch; c4: the first of its
 # two launches, the 512 sphere experiments).  The algorithmic traffic is the histograms only.
 NCU_DRAM_BYTES = {
-    "c0_sphere_fp64": 446_208,
-    "c1_polysphere_py": 1_627_136,
-    "c2_oriented_cylinder": 75_744_512,
-    "c3_coreshell_triaxial": 6_375_936,
-    "c4_batch": 354_264_576,
+    "c0_sphere_fp64": 445_696,
+    "c1_polysphere_py": 1_626_880,
+    "c2_oriented_cylinder": 1_683_712,
+    "c3_coreshell_triaxial": 6_359_040,
+    "c4_batch": 351_287_296,
 }
 
 

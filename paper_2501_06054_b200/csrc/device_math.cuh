@@ -25,12 +25,23 @@ __host__ __device__ inline void philox_make_keys(uint64_t seed, PhiloxKeys& pk) 
   }
 }
 
+// 32 x 32 -> 64-bit product as ONE instruction (IMAD.WIDE.U32: 4 clocks of the heavy FMA pipe, one issue slot).
+// Written as mul.wide.u32 because ptxas otherwise may split a __umulhi/mul.lo pair into IMAD.HI + IMAD: the
+// same pipe time but twice the issue slots (profiles/r2_ws_notes.md).
+__device__ __forceinline__ void mul_wide(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
+  unsigned long long p;
+  asm("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(a), "r"(b));
+  lo = (uint32_t)p;
+  hi = (uint32_t)(p >> 32);
+}
+
 __device__ __forceinline__ void philox4x32_10(const PhiloxKeys& pk, uint32_t c0, uint32_t c1, uint32_t c2,
                                               uint32_t c3, uint32_t out[4]) {
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t hi0, lo0, hi1, lo1;
+    mul_wide(0xD2511F53u, c0, hi0, lo0);
+    mul_wide(0xCD9E8D57u, c2, hi1, lo1);
     uint32_t n0 = hi1 ^ c1 ^ pk.k0[r];
     uint32_t n2 = hi0 ^ c3 ^ pk.k1[r];
     c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;

@@ -78,6 +78,18 @@ __device__ __forceinline__ bool surely_misses_detector(const ExpParams& P, const
   return (s_a > P.s_cut) && (s_a < 0.999999);
 }
 
+// The same decision from fp32 arithmetic (the warp-specialised kernel's stage B0): q lambda is formed from the
+// raw words with host-folded constants, |relative error| < 6e-7 (two conversions, two FMAs, one product, four
+// rounded constants), and compared with thresholds the host moved 2e-6 INTO the certain region, so
+// true here implies true for the fp64 test above; a neutron this test leaves undecided simply runs the full
+// geometry (which finds the same ST_MISS_DET).
+__device__ __forceinline__ bool surely_misses_detector_f32(const ExpParams& P, uint32_t w_lambda, uint32_t w_q) {
+  const float lam = fmaf(__uint2float_rn(w_lambda), P.cls_la, P.cls_lb);
+  const float q = fmaf(__uint2float_rn(w_q), P.cls_qa, P.cls_qb);
+  const float ql = q * lam;
+  return (ql > P.cls_lo) && (ql < P.cls_hi);
+}
+
 // From the words of Philox blocks 0 and 1 to the detector pixel.  Returns the ST_* outcome.
 __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t w[4], const uint32_t w1[4], Hit& h) {
   // R-C2 source point

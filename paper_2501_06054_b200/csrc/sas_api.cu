@@ -11,6 +11,7 @@
 #include "quadrature_host.h"
 #include "reduce_kernel.cuh"
 #include "trace_kernel.cuh"
+#include "trace_kernel_ws.cuh"
 
 using namespace sas;
 
@@ -200,6 +201,8 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
   P.det_nx = d.det_nx; P.det_ny = d.det_ny;
   P.s_cut = INFINITY;
   P.s1_int_ok = 0;
+  // the word window of the integer slit-1 test: everything passes unless slit 1 lies in the source plane
+  P.s1_lo[0] = P.s1_lo[1] = 0u; P.s1_hi[0] = P.s1_hi[1] = 0xFFFFFFFFu;
   P.lateral_free = 0; P.slits_free = 0;
   if (d.slit1_z == 0.0) {
     // slit 1 in the source plane: xs = x0 + dx*0 = x0 exactly, so the test depends on draws 0, 1 only
@@ -237,6 +240,16 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
       const double a_cut = (std::atan(t_cut) + delta) * (1.0 + m) + 1.0e-9;         // on 2 theta
       if (a_cut < 3.0) P.s_cut = std::sin(0.5 * a_cut) * (1.0 + m);
     }
+  }
+  // fp32 form of the classifier: u = (w + 1/2) 2^-32, lambda = lambda_min + u dlam, q = q_min + u dq, and
+  // sin(theta) = q lambda / 4 pi in (s_cut, 0.999999), with both thresholds moved 2e-6 into the certain region
+  {
+    const double t = 2.3283064365386963e-10;  // 2^-32
+    P.cls_la = (float)(P.dlam * t); P.cls_lb = (float)(P.lambda_min + 0.5 * t * P.dlam);
+    P.cls_qa = (float)(P.dq * t); P.cls_qb = (float)(P.q_min + 0.5 * t * P.dq);
+    const double four_pi = 4.0 * PI_D;
+    P.cls_lo = std::isfinite(P.s_cut) ? std::nextafterf((float)(four_pi * P.s_cut * (1.0 + 2.0e-6)), INFINITY) : INFINITY;
+    P.cls_hi = std::nextafterf((float)(four_pi * 0.999999 * (1.0 - 2.0e-6)), 0.0f);
   }
 }
 
@@ -445,6 +458,7 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     ExpParams& P = c->h_exps[e];
     fill_instrument(c->instr[e], P);
+    P.exp_index = (int32_t)e;
     sas_model_desc m = models[e];
     m.precision = c->precision;
     fill_model(m, P, c->h_tab);
@@ -492,23 +506,43 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   return SAS_OK;
 }
 
+// Which kernel serves a variant: the warp-specialised one (trace_kernel_ws.cuh) where the integer stages A/B0
+// are a large share of the work (at most a few dozen node evaluations per detected neutron), the unified one
+// (trace_kernel.cuh) where the node loops dominate and every resident warp should run them.
+#ifndef SAS_WS_VARIANTS
+#define SAS_WS_VARIANTS ((1u << V_SPHERE) | (1u << V_CS_SPHERE) | (1u << V_CYL) | (1u << V_TRIAX) | (1u << V_FLAT))
+#endif
+constexpr bool use_ws(int v) { return ((SAS_WS_VARIANTS >> v) & 1u) != 0; }
+
+// occupancy and shared-memory opt-in of one kernel instantiation, asked from the runtime once per (kernel, smem)
+struct KernelPlan { size_t smem = ~(size_t)0; int bps = 0; };
+
 template <typename Real, int V, bool EV>
 sas_status launch(sas_ctx* c, KernelArgs& a) {
   const bool DUMP = a.d_pixel != nullptr;
-  constexpr int BLOCK_THREADS = block_threads(V);
-  const size_t smem = trace_smem_bytes<Real>(c->tab_len_max, BLOCK_THREADS / 32);
-  auto kern = trace_kernel<Real, V, EV>;
+  constexpr bool WS = use_ws(V);
+  constexpr int BLOCK_THREADS = WS ? WS_THREADS : block_threads(V);
+  constexpr int ROW_WARPS = WS ? WS_PAIRS : BLOCK_THREADS / 32;  // warps that share the rows of a work item
+  const size_t smem = WS ? ws_smem_bytes<Real>(c->tab_len_max) : trace_smem_bytes<Real>(c->tab_len_max, BLOCK_THREADS / 32);
+  void (*kern)(const KernelArgs);
+  if constexpr (WS) kern = trace_kernel_ws<Real, V, EV>; else kern = trace_kernel<Real, V, EV>;
   if (smem > 227 * 1024) return fail(c, SAS_EINVAL, "quadrature tables do not fit in shared memory");
-  CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  int bps = 0;
-  CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, BLOCK_THREADS, smem));
-  if (bps < 1) return fail(c, SAS_ECUDA, "trace kernel does not fit on an SM");
+  static thread_local KernelPlan plan[8];  // per device ordinal
+  KernelPlan& pl = plan[c->device & 7];
+  if (pl.smem != smem) {
+    CUDA_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int bps = 0;
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, BLOCK_THREADS, smem));
+    if (bps < 1) return fail(c, SAS_ECUDA, "trace kernel does not fit on an SM");
+    pl.smem = smem; pl.bps = bps;
+  }
+  const int bps = pl.bps;
   const uint64_t total = (uint64_t)a.n_per_exp * a.n_exp;
   const int grid_full = c->n_sm * bps;
   // work items: ~16 per resident block, 2048..262144 ids each, multiple of 256 ids
   uint64_t item = total / ((uint64_t)grid_full * (uint64_t)SAS_ITEMS_PER_BLOCK);
   // at least 16 rows of 32 ids per warp and item (a 1e6-neutron launch still fills the chip)
-  item = std::min<uint64_t>(std::max<uint64_t>(item, (uint64_t)SAS_MIN_ITEM / 4 * (BLOCK_THREADS / 32)), 262144);
+  item = std::min<uint64_t>(std::max<uint64_t>(item, (uint64_t)SAS_MIN_ITEM / 4 * ROW_WARPS), 262144);
   item = (item + 255) / 256 * 256;
   a.item_ids = (uint32_t)item;
   a.items_per_exp = (uint32_t)(((uint64_t)a.n_per_exp + item - 1) / item);

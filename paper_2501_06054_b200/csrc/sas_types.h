@@ -38,6 +38,8 @@ struct ExpParams {
   // detector (R-C9)
   double det_z, det_hw, det_hh, det_sx, det_sy, det_nxd, det_nyd;
   double s_cut;  // classifier threshold on sin(theta); +inf when the instrument does not qualify
+  // the same test in fp32 with a 2e-6 margin (geometry.cuh: surely_misses_detector_f32): lambda = w a + b, q = w a + b
+  float cls_la, cls_lb, cls_qa, cls_qb, cls_lo, cls_hi;
   // model scalars (R-C12)
   double norm;        // 1e8 * scale / <V>
   double background;
@@ -59,6 +61,7 @@ struct ExpParams {
   int32_t n_a, n_b, n_th, n_ph;
   int32_t tab_off, tab_len;  // in doubles, inside the table pool
   int32_t lam_small;  // cylinder: (q_max * R_max)^2 <= 64, Lambda stays on its polynomial range
+  int32_t exp_index;  // this experiment's index in the context (histogram slice, Philox counter word 3)
 };
 static_assert(sizeof(ExpParams) % 8 == 0, "ExpParams must be a multiple of 8 bytes");
 

@@ -1,0 +1,453 @@
+// The warp-specialised trace kernel: the same four stages as trace_kernel.cuh, split
+// between the warpgroups of one block:
+//
+//   1 producer warpgroup (4 warps, one per SM sub-partition): stage A (Philox block 0 + integer slit-1 test on
+//       every launched neutron) and stage B0 (Philox block 1 + certain-miss classifier on the 25 % that survive):
+//       pure integer work, bound by the heavy FMA pipe (IMAD.WIDE, 4 clocks each).  Measured (profiles/
+//       r2_ws_probes.md): ONE such warp per sub-partition already saturates that pipe; more only queue behind it.
+//   WS_CWG consumer warpgroups (4 x WS_CWG warps): stage B (fp64 geometry, long dependent chains: latency bound,
+//       wants as many warps as fit) and stage C (model node loops, weight, histogram) on the FP64/FP32/XU pipes.
+//
+// Producer warp p feeds consumer warps p, p + 4, ... (the same sub-partition) through a ring of chunks of 32
+// entries (low id word, Philox block 1) handed over with full/empty mbarrier pairs; a free consumer claims the
+// next chunk of the ring with a ticket (a fixed round robin would stall the producer behind whichever consumer
+// happens to be in a long stage C).  No warp ever spins on shared memory, a waiting warp sleeps in
+// mbarrier.try_wait.  Registers move from the
+// producers to the consumers with setmaxnreg where the two budgets differ.
+#pragma once
+#include <cstddef>
+
+#include "trace_kernel.cuh"
+
+namespace sas {
+
+#ifndef SAS_WS_CWG
+#define SAS_WS_CWG 1          // consumer warpgroups per block
+#endif
+#ifndef SAS_WS_REGS
+#define SAS_WS_REGS 64        // registers per thread at launch (x threads = the block's pool)
+#endif
+#ifndef SAS_WS_PROD_REGS
+#define SAS_WS_PROD_REGS 56
+#endif
+#ifndef SAS_WS_CONS_REGS
+#define SAS_WS_CONS_REGS 72
+#endif
+#ifndef SAS_WS_G
+#define SAS_WS_G 8            // chunks of 32 entries per producer warp (a ring shared by its consumers)
+#endif
+#ifndef SAS_WS_NR
+#define SAS_WS_NR 3           // rows of 32 ids per stage-A step (independent Philox chains)
+#endif
+#ifndef SAS_WS_NB0
+#define SAS_WS_NB0 2          // stack entries a lane takes per stage-B0 step (independent Philox chains)
+#endif
+#ifndef SAS_WS_PROD_LAST
+#define SAS_WS_PROD_LAST 0    // the producers are the LAST warpgroup: the sub-partition arbiter serves the highest warp id first
+#endif
+#ifndef SAS_WS_PROBE
+#define SAS_WS_PROBE 0        // measurement probes (never defined in the shipped build)
+#endif
+
+constexpr int WS_CWG = SAS_WS_CWG;
+constexpr int WS_THREADS = 128 * (1 + WS_CWG);
+constexpr int WS_MIN_BLOCKS = (65536 / (SAS_WS_REGS * WS_THREADS)) < 1 ? 1 : (65536 / (SAS_WS_REGS * WS_THREADS));
+constexpr int WS_PAIRS = 4;               // producer warps = sub-partitions
+constexpr int WS_G = SAS_WS_G;            // chunks per producer warp
+constexpr int WS_NR = SAS_WS_NR;
+constexpr int WS_NB0 = SAS_WS_NB0;
+constexpr int WS_STACK = 32 * WS_NB0 + 32 * WS_NR;  // stage A -> B0 stack: < one B0 batch + one stage-A step
+static_assert((WS_G & (WS_G - 1)) == 0 && WS_G >= 2, "chunks per producer: a power of two");
+static_assert(SAS_WS_PROD_REGS * 128 + SAS_WS_CONS_REGS * 128 * WS_CWG <= SAS_WS_REGS * WS_THREADS,
+              "setmaxnreg budgets exceed the block's register pool");
+static_assert(SAS_WS_REGS * WS_THREADS * WS_MIN_BLOCKS <= 65536, "register file");
+
+enum : uint32_t { WS_DATA = 0, WS_FLUSH = 1, WS_DONE = 2 };
+
+struct WsChunk {                 // 32 stage-B0 survivors on their way to stage B
+  uint4 w1[32];                  // Philox block 1
+  uint32_t id[32];               // Philox counter word 0 (low id word)
+  unsigned long long full, empty;  // mbarriers (count 1: one elected lane arrives)
+  uint32_t meta;                 // entries | flag << 8
+  uint32_t pad[3];
+};
+static_assert(sizeof(WsChunk) % 16 == 0, "chunk alignment");
+
+struct WsProducer {
+  WsChunk chunk[WS_G];           // filled in ring order; whichever consumer is free takes the next one
+  uint32_t ticket;               // chunks claimed by the consumers so far
+  uint32_t pad[3];
+  uint32_t b_id[WS_STACK];       // stage A -> B0: slit-1 survivors (low id word), a stack (order is free)
+};
+
+struct WsConsumer {
+  uint32_t c_id[RING];
+  int32_t c_pixel[RING];
+  double c_G[RING];
+  double c_Q[3][RING];
+  uint32_t oc[6][32];            // outcome counts per lane: row 0 detected, rows 1..5 = ST_*
+};
+
+struct WsShared {
+  WsProducer prod[WS_PAIRS];
+  WsConsumer cons[WS_PAIRS * WS_CWG];
+  unsigned int item[2];
+};
+
+template <typename Real>
+__host__ __device__ inline size_t ws_smem_bytes(int tab_len_max) {
+  return round16(sizeof(ExpParams)) + round16((size_t)tab_len_max * sizeof(Real)) + round16(sizeof(WsShared));
+}
+
+// ---------------------------------------------------------------- mbarrier / register-budget primitives
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(void* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_a(uint32_t addr) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_a(uint32_t addr, uint32_t parity) {
+  uint32_t ok;
+  do {  // try_wait suspends the warp in hardware until the phase completes or the time hint (10 ms) passes
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(addr), "r"(parity), "r"(0x989680u) : "memory");
+  } while (!ok);
+}
+template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void bar_block() { asm volatile("bar.sync 0;" ::: "memory"); }
+__device__ __forceinline__ void bar_producers() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+// The producers' shared-memory traffic is written with 32-bit shared-window addresses, and the few
+// loop-invariant values are pinned (an empty volatile asm) so that ptxas keeps them in a register instead of
+// re-deriving them from %tid and the kernel parameters at every use.
+__device__ __forceinline__ uint32_t pin(uint32_t x) { asm volatile("" : "+r"(x)); return x; }
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+
+// stage A needs two words of Philox block 0 only: draw 0 (word 0) and draw 1 (word 1)
+__device__ __forceinline__ void philox_words01(const PhiloxKeys& pk, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t& w0, uint32_t& w1) {
+#pragma unroll
+  for (int r = 0; r < 9; ++r) {
+    uint32_t hi0, lo0, hi1, lo1;
+    mul_wide(0xD2511F53u, c0, hi0, lo0);
+    mul_wide(0xCD9E8D57u, c2, hi1, lo1);
+    const uint32_t n0 = hi1 ^ c1 ^ pk.k0[r];
+    const uint32_t n2 = hi0 ^ c3 ^ pk.k1[r];
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+  }
+  w0 = __umulhi(0xCD9E8D57u, c2) ^ c1 ^ pk.k0[9];
+  w1 = 0xCD9E8D57u * c2;
+}
+
+template <typename Real, int V, bool EV>
+__global__ void __launch_bounds__(WS_THREADS, WS_MIN_BLOCKS)
+trace_kernel_ws(const __grid_constant__ KernelArgs a) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  ExpParams& P = *reinterpret_cast<ExpParams*>(smem_raw);
+  Real* tab = reinterpret_cast<Real*>(smem_raw + round16(sizeof(ExpParams)));
+  WsShared& S = *reinterpret_cast<WsShared*>(smem_raw + round16(sizeof(ExpParams)) +
+                                             round16((size_t)a.tab_len_max * sizeof(Real)));
+  const int lane = threadIdx.x & 31;
+  const int wid = threadIdx.x >> 5;
+  const int pair = wid & 3;      // the producer warp this warp is, or is fed by (= its SM sub-partition)
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const unsigned FULL = 0xFFFFFFFFu;
+  const bool DUMP = a.d_pixel != nullptr;
+  const bool DUMP_Q = DUMP && a.d_q != nullptr;
+  const uint32_t first_lo = (uint32_t)a.first_id, id_hi = (uint32_t)(a.first_id >> 32);
+
+  // ---------------------------------------------------------------- block prologue (all threads)
+  if (threadIdx.x < WS_PAIRS * WS_G) {
+    WsChunk& c = S.prod[threadIdx.x / WS_G].chunk[threadIdx.x % WS_G];
+    mbar_init(&c.full, 1);
+    mbar_init(&c.empty, 1);
+  }
+  if (threadIdx.x < WS_PAIRS) S.prod[threadIdx.x].ticket = 0u;
+  if (threadIdx.x == 0) S.item[0] = atomicAdd(a.work_counter, 1u);
+  __syncthreads();
+  unsigned item = S.item[0];
+  if (item >= a.n_items) return;  // nothing for this block (the whole block leaves together)
+  int cur_exp = (int)a.exp_ids[item / a.items_per_exp];
+  auto stage_experiment = [&](int e, int tid, int nthr) {
+    const ExpParams* src = a.exps + e;
+    const uint32_t* s32 = reinterpret_cast<const uint32_t*>(src);
+    uint32_t* d32 = reinterpret_cast<uint32_t*>(&P);
+    for (int i = tid; i < (int)(sizeof(ExpParams) / 4); i += nthr) d32[i] = s32[i];
+    const int tl = src->tab_len;
+    const double* tsrc = a.tab_pool + src->tab_off;
+    for (int i = tid; i < tl; i += nthr) tab[i] = (Real)tsrc[i];
+  };
+  stage_experiment(cur_exp, threadIdx.x, WS_THREADS);
+  __syncthreads();
+
+  // The warp arbiter of a sub-partition serves the eligible warp with the highest id first
+  // (/opt/skills/guides/B300_MICROARCH.md "Multi-warp arbiter"): the producers, whose IMAD.WIDE stream must reach
+  // the heavy pipe whenever it is free, are the last warpgroup; the consumers fill the issue slots they leave.
+  constexpr int PROD_T0 = SAS_WS_PROD_LAST ? 128 * WS_CWG : 0;   // first producer thread
+  const bool is_producer = SAS_WS_PROD_LAST ? (threadIdx.x >= PROD_T0) : (threadIdx.x < 128);
+  const int cwid = SAS_WS_PROD_LAST ? wid : wid - 4;             // consumer warp index 0 .. 4 WS_CWG - 1
+
+  if (is_producer) {
+    // ================================================================ producers: stages A and B0
+    if (SAS_WS_PROD_REGS != SAS_WS_REGS) reg_dealloc<SAS_WS_PROD_REGS>();
+    const uint32_t cbase = pin(smem_u32(S.prod[pair].chunk));   // chunk 0 (shared-window address)
+    const uint32_t stack0 = pin(smem_u32(S.prod[pair].b_id));   // stack B
+    const uint32_t lt = pin(lt_mask);
+    uint32_t sp = stack0;         // stack pointer (byte address of the first free entry)
+    uint32_t wpos = 0;            // entries already in the current chunk
+    uint32_t cur = cbase;         // chunk being filled (round robin over the WS_G chunks)
+    uint32_t gcur = 0;            // its index
+    // Use k of a chunk may be filled once the consumer released use k - 1: a wait on its empty barrier for
+    // parity (k & 1) ^ 1 (a fresh barrier passes a wait on parity 1).  k is the lap of the round robin:
+    // eph is that parity for the lap `cur` is in.
+    uint32_t eph = 1;
+    uint32_t acq = 1;             // chunks owned from `cur` on: 0, 1 (cur) or 2 (cur and the one after it)
+    uint32_t n_sure = 0;          // detector misses decided by the classifier (this lane)
+    unsigned it = 0;              // items fetched by this block (parity of the item slot)
+    auto next_of = [&](uint32_t g) { return g + 1 == (uint32_t)WS_G ? 0u : g + 1; };
+
+    auto acquire_cur = [&]() {
+      if (acq == 0) { mbar_wait_a(cur + (uint32_t)offsetof(WsChunk, empty), eph); acq = 1; }
+    };
+    auto acquire_next = [&]() {  // the chunk after `cur` (in the next lap when the order wraps)
+      const uint32_t gn = next_of(gcur);
+      mbar_wait_a(cbase + gn * (uint32_t)sizeof(WsChunk) + (uint32_t)offsetof(WsChunk, empty), gn == 0 ? eph ^ 1u : eph);
+      acq = 2;
+    };
+    // hands `cur` to its consumer with n entries and moves on
+    auto publish = [&](uint32_t n, uint32_t flag) {
+      __syncwarp();
+      if (lane == 0) {
+        sts32(cur + (uint32_t)offsetof(WsChunk, meta), n | (flag << 8));
+        mbar_arrive_a(cur + (uint32_t)offsetof(WsChunk, full));
+      }
+      gcur = next_of(gcur);
+      if (gcur == 0) eph ^= 1u;
+      cur = cbase + gcur * (uint32_t)sizeof(WsChunk);
+      acq -= 1;
+    };
+    // stage B0 on up to 32 WS_NB0 stack entries (WS_NB0 per lane: independent Philox chains)
+    auto stage_b0 = [&](uint32_t exp_word) {
+      const uint32_t have = (sp - stack0) >> 2;
+      const uint32_t n = have < 32u * WS_NB0 ? have : 32u * WS_NB0;
+      sp -= 4u * n;
+      uint32_t idl[WS_NB0], w1[WS_NB0][4];
+      bool act[WS_NB0];
+#pragma unroll
+      for (int k = 0; k < WS_NB0; ++k) {
+        act[k] = (uint32_t)(lane + 32 * k) < n;
+        idl[k] = act[k] ? lds32(sp + 4u * (uint32_t)(lane + 32 * k)) : 0u;
+      }
+      __syncwarp();
+#pragma unroll
+      for (int k = 0; k < WS_NB0; ++k) philox4x32_10(a.keys, idl[k], id_hi, 1u, exp_word, w1[k]);
+#pragma unroll
+      for (int k = 0; k < WS_NB0; ++k) {
+        const bool sure = act[k] && surely_misses_detector_f32(P, w1[k][0], w1[k][2]);
+        n_sure += sure ? 1u : 0u;
+        if (DUMP_Q && sure) a.d_q[idl[k] - first_lo] = P.q_min + uniform_from_word(w1[k][2]) * P.dq;  // R-C7
+        const bool keep = act[k] && !sure;
+        const unsigned m = __ballot_sync(FULL, keep);
+        const uint32_t nk = __popc(m);
+        if (nk) {
+          acquire_cur();
+          if (wpos + nk > 32u && acq < 2) acquire_next();
+          if (keep) {
+            const uint32_t L = wpos + __popc(m & lt);
+            const uint32_t base = L < 32u ? cur : cbase + next_of(gcur) * (uint32_t)sizeof(WsChunk);
+            sts32(base + (uint32_t)offsetof(WsChunk, id) + 4u * (L & 31u), idl[k]);
+            sts128(base + (uint32_t)offsetof(WsChunk, w1) + 16u * (L & 31u), w1[k][0], w1[k][1], w1[k][2], w1[k][3]);
+          }
+          wpos += nk;
+          if (wpos >= 32u) { publish(32u, WS_DATA); wpos -= 32u; }
+        }
+      }
+    };
+
+    for (;;) {
+      // ---------------- one work item: (experiment, id range), rows shared by the four producer warps
+      const uint32_t exp_word = a.exp_base + (uint32_t)cur_exp;
+      const uint32_t off0 = (item % a.items_per_exp) * a.item_ids;
+      const uint32_t cnt_ids = min(a.item_ids, a.n_per_exp - off0);
+      const uint32_t rows_full = cnt_ids >> 5;
+      // word window of the integer slit-1 test (the whole range when slit 1 is not in the source plane)
+      const uint32_t lo0 = P.s1_lo[0], d0 = P.s1_hi[0] - P.s1_lo[0], lo1 = P.s1_lo[1], d1 = P.s1_hi[1] - P.s1_lo[1];
+      const uint32_t idc0 = first_lo + off0 + lane;  // Philox counter word 0 of this lane in row 0
+      uint32_t row = pair;
+      // fast path: WS_NR full rows per step, no bound checks
+      while (row + (WS_NR - 1) * WS_PAIRS < rows_full) {
+        uint32_t w0[WS_NR], w1[WS_NR];
+        const uint32_t idr = idc0 + (row << 5);
+#pragma unroll
+        for (int k = 0; k < WS_NR; ++k)
+#if SAS_WS_PROBE == 2
+          { w0[k] = (lane & 3) ? 0u : lo0; w1[k] = lo1; }
+#else
+          philox_words01(a.keys, idr + 32u * (uint32_t)(k * WS_PAIRS), id_hi, 0u, exp_word, w0[k], w1[k]);
+#endif
+#pragma unroll
+        for (int k = 0; k < WS_NR; ++k) {
+          const bool pass = (w0[k] - lo0 <= d0) && (w1[k] - lo1 <= d1);
+          const unsigned m = __ballot_sync(FULL, pass);
+          if (pass) sts32(sp + 4u * __popc(m & lt), idr + 32u * (uint32_t)(k * WS_PAIRS));
+          sp += 4u * __popc(m);
+        }
+        row += WS_NR * WS_PAIRS;
+        __syncwarp();
+        while (sp - stack0 >= 128u * WS_NB0) stage_b0(exp_word);
+      }
+      // ragged end of the item: one row at a time, ids past the end fail
+      for (; (row << 5) < cnt_ids; row += WS_PAIRS) {
+        uint32_t w0, w1;
+        philox_words01(a.keys, idc0 + (row << 5), id_hi, 0u, exp_word, w0, w1);
+        const bool pass = ((row << 5) + lane) < cnt_ids && (w0 - lo0 <= d0) && (w1 - lo1 <= d1);
+        const unsigned m = __ballot_sync(FULL, pass);
+        if (pass) sts32(sp + 4u * __popc(m & lt), idc0 + (row << 5));
+        sp += 4u * __popc(m);
+        __syncwarp();
+        while (sp - stack0 >= 128u * WS_NB0) stage_b0(exp_word);
+      }
+      // ---------------- next item
+      it += 1;
+      if (threadIdx.x == PROD_T0) S.item[it & 1] = atomicAdd(a.work_counter, 1u);
+      bar_producers();
+      item = S.item[it & 1];
+      const int e = item < a.n_items ? (int)a.exp_ids[item / a.items_per_exp] : -1;
+      if (e != cur_exp) {
+        // experiment switch or end of work: empty the stack, then every consumer of this producer gets a
+        // flagged chunk (the partial one first, empty ones for the others) and the block meets at a barrier
+        while (sp != stack0) stage_b0(exp_word);
+        for (int j = 0; j < WS_CWG; ++j) {
+          acquire_cur();
+          publish(j == 0 ? wpos : 0u, e < 0 ? WS_DONE : WS_FLUSH);
+        }
+        wpos = 0;
+        bar_block();  // every consumer has drained the old experiment
+        if (e < 0) break;
+        stage_experiment(e, threadIdx.x - PROD_T0, 128);
+        cur_exp = e;
+        bar_block();
+      }
+    }
+    if (!DUMP) {
+      const unsigned tot = __reduce_add_sync(FULL, n_sure);
+      if (lane == 0 && tot) {
+        atomicAdd(a.counters + 5, (unsigned long long)tot);
+        atomicAdd(a.counters + 7, (unsigned long long)tot);
+      }
+    }
+  } else {
+    // ================================================================ consumers: stages B and C
+    if (SAS_WS_CONS_REGS != SAS_WS_REGS) reg_alloc<SAS_WS_CONS_REGS>();
+    WsConsumer& cq = S.cons[cwid];
+    WsChunk* chunks = S.prod[pair].chunk;
+#pragma unroll
+    for (int f = 0; f < 6; ++f) cq.oc[f][lane] = 0;
+    int headC = 0, cntC = 0;
+    uint32_t ruse = 0;
+    for (;;) {
+      const uint32_t exp_word = a.exp_base + (uint32_t)cur_exp;
+      // ---------------- claim the next chunk of the ring: ticket k is use k / WS_G of chunk k % WS_G
+      uint32_t k = ruse++;  // a producer's only consumer takes its chunks in order
+      if (WS_CWG > 1) {
+        if (lane == 0) k = atomicAdd(&S.prod[pair].ticket, 1u);
+        k = __shfl_sync(FULL, k, 0);
+      }
+      WsChunk& ck = chunks[k % WS_G];
+      mbar_wait_a(smem_u32(&ck.full), (k / WS_G) & 1u);
+      const uint32_t meta = ck.meta;
+      const int n = (int)(meta & 0xFFu);
+      const uint32_t flag = meta >> 8;
+      const bool act = lane < n;
+      uint32_t id_lo = 0;
+      uint4 w1v = make_uint4(0, 0, 0, 0);
+      if (act) { id_lo = ck.id[lane]; w1v = ck.w1[lane]; }
+      __syncwarp();
+      if (lane == 0) mbar_arrive_a(smem_u32(&ck.empty));
+#if SAS_WS_PROBE == 1
+      if (false) {
+#else
+      if (n > 0) {
+#endif
+        // ---------------- stage B: Philox block 0 again, fp64 geometry
+        uint32_t w[4];
+        const uint32_t w1[4] = {w1v.x, w1v.y, w1v.z, w1v.w};
+        philox4x32_10(a.keys, id_lo, id_hi, 0u, exp_word, w);
+        int st = -1;
+        Hit h;
+        if (act) {
+          st = trace_geometry(P, w, w1, h);
+          if (DUMP_Q) a.d_q[id_lo - first_lo] = h.q;
+          cq.oc[st][lane] += 1;
+        }
+        const unsigned m = __ballot_sync(FULL, st == ST_DETECTED);
+        if (st == ST_DETECTED) {
+          const int s2 = (headC + cntC + __popc(m & lt_mask)) & (RING - 1);
+          cq.c_id[s2] = id_lo; cq.c_pixel[s2] = h.pixel; cq.c_G[s2] = h.G;
+          cq.c_Q[0][s2] = h.Qx; cq.c_Q[1][s2] = h.Qy; cq.c_Q[2][s2] = h.Qz;
+        }
+        cntC += __popc(m);
+        __syncwarp();
+      }
+      // ---------------- stage C: model + weight + histogram
+      while (cntC >= 32 || (flag != WS_DATA && cntC > 0)) {
+        const int nc = cntC < 32 ? cntC : 32;
+        const bool actc = lane < nc;
+        const int slot = (headC + lane) & (RING - 1);
+        uint32_t idc = 0; int32_t pixel = 0; double G = 0, Qx = 0, Qy = 0, Qz = 0;
+        if (actc) {
+          idc = cq.c_id[slot]; pixel = cq.c_pixel[slot]; G = cq.c_G[slot];
+          Qx = cq.c_Q[0][slot]; Qy = cq.c_Q[1][slot]; Qz = cq.c_Q[2][slot];
+        }
+        __syncwarp();
+        headC = (headC + nc) & (RING - 1);
+        cntC -= nc;
+        if (actc) {
+          Real I;
+          if (EV)
+            I = (Real)eval_intensity_event<V>(P, a.keys, idc, id_hi, exp_word, Qx, Qy, Qz);
+          else
+            I = eval_intensity<Real, V>(P, tab, a.keys, idc, id_hi, exp_word, Qx, Qy, Qz);
+          const double p = G * (double)I;
+          if (DUMP) {
+            a.d_pixel[idc - first_lo] = pixel;
+            a.d_weight[idc - first_lo] = p;
+          } else {
+            const size_t ix = (size_t)cur_exp * (size_t)a.npix + (size_t)pixel;
+            atomicAdd(a.counts + ix, 1ull);
+            atomicAdd(a.sum_p + ix, p);
+            atomicAdd(a.sum_p2 + ix, p * p);
+          }
+        }
+        __syncwarp();
+      }
+      if (flag != WS_DATA) {
+        bar_block();  // the experiment is drained
+        if (flag == WS_DONE) break;
+        bar_block();  // the producers staged the next one
+        cur_exp = (int)P.exp_index;
+      }
+    }
+    if (!DUMP) {
+#pragma unroll
+      for (int f = 0; f < 6; ++f) {
+        const unsigned tot = __reduce_add_sync(FULL, cq.oc[f][lane]);
+        if (lane == 0 && tot) atomicAdd(a.counters + (f == 0 ? 6 : f), (unsigned long long)tot);
+      }
+    }
+  }
+}
+
+}  // namespace sas

@@ -91,6 +91,12 @@ __device__ __forceinline__ bool surely_misses_detector_f32(const ExpParams& P, u
 }
 
 // From the words of Philox blocks 0 and 1 to the detector pixel.  Returns the ST_* outcome.
+// FAST is the instrument class of every BASELINE.json config with a box sample (ExpParams::geo_fast, set by the
+// host): no slit can cut a stage-B ray (slits_free), the primary ray cannot touch the sample's lateral faces
+// (lateral_free), box sample, no attenuation.  What is left of R-C4/R-C5/R-C11 is the depth slab alone, whose
+// roots need no min/max (dz > 0 and hz > 0: (-hz - oz) inv <= (hz - oz) inv by monotonic rounding) -- the same
+// values as the general code, without its runtime branches.
+template <bool FAST>
 __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t w[4], const uint32_t w1[4], Hit& h) {
   // R-C2 source point
   const double u0 = uniform_from_word(w[0]), u1 = uniform_from_word(w[1]);
@@ -110,7 +116,7 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
   // R-C4 slits.  slits_free: stage A already applied the (bit-identical) integer slit-1 test and the host
   // proved that slit 2 cannot cut a ray aimed at the focus rectangle: nothing to compute
   bool f_s1 = false, f_s2 = false;
-  if (!P.slits_free) {
+  if (!FAST && !P.slits_free) {
     const double inv_dz = 1.0 / dz;
     const double s1 = (P.slit1_z - 0.0) * inv_dz;
     const double xs1 = x0 + dx * s1, ys1 = y0 + dy * s1;
@@ -125,7 +131,14 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
   const double lambda = P.lambda_min + u4 * P.dlam;
   // R-C5 sample
   double tin, tout;
-  const bool hit_s = intersect_sample(P, x0, y0, 0.0 - P.sample_z, dx, dy, dz, tin, tout, P.lateral_free != 0);
+  bool hit_s = true;
+  if (FAST) {
+    const double oz = 0.0 - P.sample_z, inv = 1.0 / dz;
+    tin = (-P.hz - oz) * inv;
+    tout = (P.hz - oz) * inv;
+  } else {
+    hit_s = intersect_sample(P, x0, y0, 0.0 - P.sample_z, dx, dy, dz, tin, tout, P.lateral_free != 0);
+  }
   tin = tin < 0.0 ? 0.0 : tin;
   const bool f_ms = !hit_s || !(tout > tin);
   const double ell = tout - tin;
@@ -175,13 +188,13 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
     h.pixel = (int)floor(fy) * P.det_nx + (int)floor(fx);
     // R-C11 attenuation and the geometric part of the weight
     double T = 1.0;
-    if (P.has_mu) {
+    if (!FAST && P.has_mu) {
       const double mu = (P.mu_abs_2200 * lambda) / 1.7982 + P.mu_inc;
       double tin2, tout2, ell_out = 0.0;
       if (intersect_sample(P, rsx, rsy, rsz - P.sample_z, dpx, dpy, dpz, tin2, tout2) && tout2 > 0.0) ell_out = tout2;
       T = exp(-(mu * (u5 * ell + ell_out)));
     }
-    const double geo = (p0 * T) * (100.0 * ell);
+    const double geo = (FAST ? p0 : p0 * T) * (100.0 * ell);  // p0 * 1.0 is p0
     h.G = (geo * (qk * inv_k)) * P.qnorm;
   }
   return st;

@@ -203,12 +203,18 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
   P.s1_int_ok = 0;
   // the word window of the integer slit-1 test: everything passes unless slit 1 lies in the source plane
   P.s1_lo[0] = P.s1_lo[1] = 0u; P.s1_hi[0] = P.s1_hi[1] = 0xFFFFFFFFu;
-  P.lateral_free = 0; P.slits_free = 0;
+  P.lateral_free = 0; P.slits_free = 0; P.geo_fast = 0;
   if (d.slit1_z == 0.0) {
     // slit 1 in the source plane: xs = x0 + dx*0 = x0 exactly, so the test depends on draws 0, 1 only
     slit1_word_window(d.src_xw, P.slit1_hx, P.s1_lo[0], P.s1_hi[0]);
     slit1_word_window(d.src_yh, P.slit1_hy, P.s1_lo[1], P.s1_hi[1]);
     P.s1_int_ok = 1;
+    if (P.s1_lo[0] > P.s1_hi[0] || P.s1_lo[1] > P.s1_hi[1]) {
+      // a slit narrower than the spacing of the source coordinates passes no draw at all: the kernels' window
+      // test (w - lo <= hi - lo) cannot express an empty window, so the fp64 slit test decides (all absorbed)
+      P.s1_lo[0] = P.s1_lo[1] = 0u; P.s1_hi[0] = P.s1_hi[1] = 0xFFFFFFFFu;
+      P.s1_int_ok = 0;
+    }
   }
   // Certain-miss classifier (geometry.cuh: surely_misses_detector).  Qualifies when, for EVERY ray the
   // source can emit through slit 1, (i) slit 2 cannot cut (it is the focus rectangle or larger),
@@ -232,6 +238,7 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
     // and to move forward: z_near > 0, dz > 0 always); the cylinder's y slab likewise
     P.lateral_free = sample_sure ? 1 : 0;
     P.slits_free = (P.s1_int_ok && slit2_sure) ? 1 : 0;
+    P.geo_fast = (P.slits_free && P.lateral_free && d.sample_shape == SAS_SAMPLE_BOX && !P.has_mu) ? 1 : 0;
     const double d_min = (d.sample_z + d.det_dist) - z_far;
     if (P.s1_int_ok && slit2_sure && sample_sure && d_min > 0.0) {
       const double delta = std::atan(std::hypot(xf + x0m, yf + y0m) / d.focus_z);  // max tilt of d^ from z

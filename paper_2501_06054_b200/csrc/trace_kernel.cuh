@@ -214,7 +214,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
         int st = -1;
         Hit h;
         if (act) {
-          st = trace_geometry(P, w, w1, h);
+          st = P.geo_fast ? trace_geometry<true>(P, w, w1, h) : trace_geometry<false>(P, w, w1, h);
           if (DUMP_Q) a.d_q[idoff] = h.q;
           wq.oc[st][lane] += 1;
         }

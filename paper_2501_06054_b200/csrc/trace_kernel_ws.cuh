@@ -64,21 +64,18 @@ static_assert(SAS_WS_REGS * WS_THREADS * WS_MIN_BLOCKS <= 65536, "register file"
 
 enum : uint32_t { WS_DATA = 0, WS_FLUSH = 1, WS_DONE = 2 };
 
-struct WsChunk {                 // 32 stage-B0 survivors on their way to stage B
-  uint4 w1[32];                  // Philox block 1
-  uint32_t id[32];               // Philox counter word 0 (low id word)
-  unsigned long long full, empty;  // mbarriers (count 1: one elected lane arrives)
-  uint32_t meta;                 // entries | flag << 8
-  uint32_t pad[3];
-};
-static_assert(sizeof(WsChunk) % 16 == 0, "chunk alignment");
-
-struct WsProducer {
-  WsChunk chunk[WS_G];           // filled in ring order; whichever consumer is free takes the next one
-  uint32_t ticket;               // chunks claimed by the consumers so far
+struct WsProducer {               // one per producer warp
+  // stage B0 -> stage B: a ring of WS_G windows of 32 entries, filled entry by entry in ring order; a window is
+  // handed over when its last entry is written (full barrier) and reused once its consumer copied it (empty)
+  uint4 w1[WS_G * 32];           // Philox block 1
+  uint32_t id[WS_G * 32];        // Philox counter word 0 (low id word)
+  unsigned long long full[WS_G], empty[WS_G];  // mbarriers (count 1: one elected lane arrives)
+  uint32_t meta[WS_G];           // entries | flag << 8
+  uint32_t ticket;               // windows claimed by the consumers so far
   uint32_t pad[3];
   uint32_t b_id[WS_STACK];       // stage A -> B0: slit-1 survivors (low id word), a stack (order is free)
 };
+static_assert(sizeof(WsProducer) % 16 == 0, "ring alignment");
 
 struct WsConsumer {
   uint32_t c_id[RING];
@@ -129,6 +126,28 @@ __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) { asm volatile(
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+// A consumer waiting for its next window has nothing else to do: it backs off between polls so that its polling
+// does not take issue slots from the producers of its sub-partition (profiles/r2_ncu_c0.md)
+#ifndef SAS_WS_SLEEP_NS
+#define SAS_WS_SLEEP_NS 200
+#endif
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t addr, uint32_t parity) {
+  for (;;) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    if (ok) break;
+    __nanosleep(SAS_WS_SLEEP_NS);
+  }
+}
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
   uint32_t v;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
@@ -170,9 +189,9 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
 
   // ---------------------------------------------------------------- block prologue (all threads)
   if (threadIdx.x < WS_PAIRS * WS_G) {
-    WsChunk& c = S.prod[threadIdx.x / WS_G].chunk[threadIdx.x % WS_G];
-    mbar_init(&c.full, 1);
-    mbar_init(&c.empty, 1);
+    WsProducer& pr = S.prod[threadIdx.x / WS_G];
+    mbar_init(&pr.full[threadIdx.x % WS_G], 1);
+    mbar_init(&pr.empty[threadIdx.x % WS_G], 1);
   }
   if (threadIdx.x < WS_PAIRS) S.prod[threadIdx.x].ticket = 0u;
   if (threadIdx.x == 0) S.item[0] = atomicAdd(a.work_counter, 1u);
@@ -202,41 +221,32 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
   if (is_producer) {
     // ================================================================ producers: stages A and B0
     if (SAS_WS_PROD_REGS != SAS_WS_REGS) reg_dealloc<SAS_WS_PROD_REGS>();
-    const uint32_t cbase = pin(smem_u32(S.prod[pair].chunk));   // chunk 0 (shared-window address)
+    const uint32_t ring = pin(smem_u32(&S.prod[pair]));         // this warp's ring (shared-window address)
     const uint32_t stack0 = pin(smem_u32(S.prod[pair].b_id));   // stack B
     const uint32_t lt = pin(lt_mask);
     uint32_t sp = stack0;         // stack pointer (byte address of the first free entry)
-    uint32_t wpos = 0;            // entries already in the current chunk
-    uint32_t cur = cbase;         // chunk being filled (round robin over the WS_G chunks)
-    uint32_t gcur = 0;            // its index
-    // Use k of a chunk may be filled once the consumer released use k - 1: a wait on its empty barrier for
-    // parity (k & 1) ^ 1 (a fresh barrier passes a wait on parity 1).  k is the lap of the round robin:
-    // eph is that parity for the lap `cur` is in.
-    uint32_t eph = 1;
-    uint32_t acq = 1;             // chunks owned from `cur` on: 0, 1 (cur) or 2 (cur and the one after it)
+    // Entries pushed into the ring so far.  Entry t lives in slot t mod 32 WS_G; window sequence number
+    // s = t / 32 is use s / WS_G of window s mod WS_G.  Invariant: the windows s and s + 1 of the current tail
+    // are owned by this warp (their previous use was released), so a step's entries are written without a test;
+    // window s + 2 is acquired when window s is handed over.  Use u of a window may be filled once the consumer
+    // released use u - 1: a wait on its empty barrier for parity (u & 1) ^ 1 (a fresh barrier passes parity 1).
+    uint32_t tail = 0;
     uint32_t n_sure = 0;          // detector misses decided by the classifier (this lane)
     unsigned it = 0;              // items fetched by this block (parity of the item slot)
-    auto next_of = [&](uint32_t g) { return g + 1 == (uint32_t)WS_G ? 0u : g + 1; };
+    constexpr uint32_t OFF_ID = (uint32_t)offsetof(WsProducer, id), OFF_FULL = (uint32_t)offsetof(WsProducer, full);
+    constexpr uint32_t OFF_EMPTY = (uint32_t)offsetof(WsProducer, empty), OFF_META = (uint32_t)offsetof(WsProducer, meta);
 
-    auto acquire_cur = [&]() {
-      if (acq == 0) { mbar_wait_a(cur + (uint32_t)offsetof(WsChunk, empty), eph); acq = 1; }
-    };
-    auto acquire_next = [&]() {  // the chunk after `cur` (in the next lap when the order wraps)
-      const uint32_t gn = next_of(gcur);
-      mbar_wait_a(cbase + gn * (uint32_t)sizeof(WsChunk) + (uint32_t)offsetof(WsChunk, empty), gn == 0 ? eph ^ 1u : eph);
-      acq = 2;
-    };
-    // hands `cur` to its consumer with n entries and moves on
-    auto publish = [&](uint32_t n, uint32_t flag) {
+    // hands the window of `tail_in` (sequence number tail_in / 32) over with n entries and acquires the window two
+    // sequence numbers later
+    auto publish = [&](uint32_t tail_in, uint32_t n, uint32_t flag) {
+      const uint32_t seq = tail_in >> 5, w = seq & (uint32_t)(WS_G - 1);
       __syncwarp();
       if (lane == 0) {
-        sts32(cur + (uint32_t)offsetof(WsChunk, meta), n | (flag << 8));
-        mbar_arrive_a(cur + (uint32_t)offsetof(WsChunk, full));
+        sts32(ring + OFF_META + 4u * w, n | (flag << 8));
+        mbar_arrive_a(ring + OFF_FULL + 8u * w);
       }
-      gcur = next_of(gcur);
-      if (gcur == 0) eph ^= 1u;
-      cur = cbase + gcur * (uint32_t)sizeof(WsChunk);
-      acq -= 1;
+      const uint32_t seq2 = seq + 2u;  // (a first use passes at once)
+      mbar_wait_a(ring + OFF_EMPTY + 8u * (seq2 & (uint32_t)(WS_G - 1)), ((seq2 / (uint32_t)WS_G) & 1u) ^ 1u);
     };
     // stage B0 on up to 32 WS_NB0 stack entries (WS_NB0 per lane: independent Philox chains)
     auto stage_b0 = [&](uint32_t exp_word) {
@@ -260,19 +270,14 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
         if (DUMP_Q && sure) a.d_q[idl[k] - first_lo] = P.q_min + uniform_from_word(w1[k][2]) * P.dq;  // R-C7
         const bool keep = act[k] && !sure;
         const unsigned m = __ballot_sync(FULL, keep);
-        const uint32_t nk = __popc(m);
-        if (nk) {
-          acquire_cur();
-          if (wpos + nk > 32u && acq < 2) acquire_next();
-          if (keep) {
-            const uint32_t L = wpos + __popc(m & lt);
-            const uint32_t base = L < 32u ? cur : cbase + next_of(gcur) * (uint32_t)sizeof(WsChunk);
-            sts32(base + (uint32_t)offsetof(WsChunk, id) + 4u * (L & 31u), idl[k]);
-            sts128(base + (uint32_t)offsetof(WsChunk, w1) + 16u * (L & 31u), w1[k][0], w1[k][1], w1[k][2], w1[k][3]);
-          }
-          wpos += nk;
-          if (wpos >= 32u) { publish(32u, WS_DATA); wpos -= 32u; }
+        if (keep) {
+          const uint32_t L = (tail + __popc(m & lt)) & (uint32_t)(32 * WS_G - 1);
+          sts32(ring + OFF_ID + 4u * L, idl[k]);
+          sts128(ring + 16u * L, w1[k][0], w1[k][1], w1[k][2], w1[k][3]);
         }
+        const uint32_t nt = tail + __popc(m);
+        if ((nt ^ tail) & 32u) publish(tail, 32u, WS_DATA);  // the window of `tail` is complete
+        tail = nt;
       }
     };
 
@@ -330,10 +335,9 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
         // flagged chunk (the partial one first, empty ones for the others) and the block meets at a barrier
         while (sp != stack0) stage_b0(exp_word);
         for (int j = 0; j < WS_CWG; ++j) {
-          acquire_cur();
-          publish(j == 0 ? wpos : 0u, e < 0 ? WS_DONE : WS_FLUSH);
+          publish(tail, tail & 31u, e < 0 ? WS_DONE : WS_FLUSH);
+          tail = (tail | 31u) + 1u;  // the next window
         }
-        wpos = 0;
         bar_block();  // every consumer has drained the old experiment
         if (e < 0) break;
         stage_experiment(e, threadIdx.x - PROD_T0, 128);
@@ -352,30 +356,35 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     // ================================================================ consumers: stages B and C
     if (SAS_WS_CONS_REGS != SAS_WS_REGS) reg_alloc<SAS_WS_CONS_REGS>();
     WsConsumer& cq = S.cons[cwid];
-    WsChunk* chunks = S.prod[pair].chunk;
+    const uint32_t ring = pin(smem_u32(&S.prod[pair]));
+    constexpr uint32_t OFF_ID = (uint32_t)offsetof(WsProducer, id), OFF_FULL = (uint32_t)offsetof(WsProducer, full);
+    constexpr uint32_t OFF_EMPTY = (uint32_t)offsetof(WsProducer, empty), OFF_META = (uint32_t)offsetof(WsProducer, meta);
 #pragma unroll
     for (int f = 0; f < 6; ++f) cq.oc[f][lane] = 0;
     int headC = 0, cntC = 0;
     uint32_t ruse = 0;
     for (;;) {
       const uint32_t exp_word = a.exp_base + (uint32_t)cur_exp;
-      // ---------------- claim the next chunk of the ring: ticket k is use k / WS_G of chunk k % WS_G
-      uint32_t k = ruse++;  // a producer's only consumer takes its chunks in order
+      // ---------------- claim the next window of the ring: ticket k is use k / WS_G of window k % WS_G
+      uint32_t k = ruse++;  // a producer's only consumer takes its windows in order
       if (WS_CWG > 1) {
         if (lane == 0) k = atomicAdd(&S.prod[pair].ticket, 1u);
         k = __shfl_sync(FULL, k, 0);
       }
-      WsChunk& ck = chunks[k % WS_G];
-      mbar_wait_a(smem_u32(&ck.full), (k / WS_G) & 1u);
-      const uint32_t meta = ck.meta;
+      const uint32_t w = k & (uint32_t)(WS_G - 1);
+      mbar_wait_sleep(ring + OFF_FULL + 8u * w, (k / (uint32_t)WS_G) & 1u);
+      const uint32_t meta = lds32(ring + OFF_META + 4u * w);
       const int n = (int)(meta & 0xFFu);
       const uint32_t flag = meta >> 8;
       const bool act = lane < n;
       uint32_t id_lo = 0;
       uint4 w1v = make_uint4(0, 0, 0, 0);
-      if (act) { id_lo = ck.id[lane]; w1v = ck.w1[lane]; }
+      if (act) {
+        id_lo = lds32(ring + OFF_ID + 4u * (32u * w + (uint32_t)lane));
+        w1v = lds128(ring + 16u * (32u * w + (uint32_t)lane));
+      }
       __syncwarp();
-      if (lane == 0) mbar_arrive_a(smem_u32(&ck.empty));
+      if (lane == 0) mbar_arrive_a(ring + OFF_EMPTY + 8u * w);
 #if SAS_WS_PROBE == 1
       if (false) {
 #else
@@ -388,7 +397,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
         int st = -1;
         Hit h;
         if (act) {
-          st = trace_geometry(P, w, w1, h);
+          st = P.geo_fast ? trace_geometry<true>(P, w, w1, h) : trace_geometry<false>(P, w, w1, h);
           if (DUMP_Q) a.d_q[id_lo - first_lo] = h.q;
           cq.oc[st][lane] += 1;
         }

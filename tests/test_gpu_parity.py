@@ -226,6 +226,25 @@ def test_edge_cases(sas):
     tr.close()
 
 
+def test_slit_narrower_than_the_source_grid(sas):
+    """A slit 1 in the source plane that no 32-bit source draw can pass (its aperture is below the spacing of the
+    source coordinates, 10 mm / 2^32): every neutron is absorbed at slit 1, as the oracle finds; and a slit that
+    passes a handful of words keeps exactly those."""
+    c = W.config(0)
+    for width, expect_none in ((1.0e-12, True), (2.0e-8, False)):
+        ins = dict(c["instrument"], slit1_xw=width)
+        n = 3_000_000
+        tr = sas.Tracer(ins, c["model"])
+        tr.trace(n, c["seed"])
+        cnt = tr.counters()
+        counts = tr.read_detector()[2]
+        tr.close()
+        ref = O.trace_range(ins, c["model"], c["seed"], 0, n, dump=False)
+        assert np.array_equal(cnt[:7], ref["counters"][:7])
+        assert np.array_equal(counts.reshape(-1), ref["counts"])
+        assert (cnt[1] == n) == expect_none
+
+
 def test_error_paths(sas):
     tr = sas.Tracer(W.instrument())
     with pytest.raises(sas.SasError) as e:

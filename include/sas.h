@@ -48,7 +48,10 @@ typedef enum {
   SAS_EUNSUPPORTED = 5  /* valid request this build does not implement */
 } sas_status;
 
-enum { SAS_FP32 = 0, SAS_FP64 = 1 }; /* precision of the MODEL evaluation; RNG->uniform and geometry are always fp64 */
+/* precision of the MODEL evaluation; RNG->uniform and geometry are always fp64.  SAS_FP32 is a request: an
+ * experiment whose model is evaluated once per neutron (no node loop), or whose phases q_max x size exceed 1e3
+ * rad (the proven range of the fp32 argument reductions), runs its model in fp64. */
+enum { SAS_FP32 = 0, SAS_FP64 = 1 };
 enum { SAS_SAMPLE_BOX = 0, SAS_SAMPLE_CYL_Y = 1 };
 enum {
   SAS_SPHERE = 0,              /* Table II F.9 */
@@ -138,7 +141,8 @@ typedef struct {
 
 /* Validate and copy the instrument; allocate device state on the current CUDA
  * device (its own zeroed histograms and an internal stream until sas_bind_buffers
- * says otherwise).  *out is set only on SAS_OK; free with sas_destroy. */
+ * says otherwise).  *out is set only on SAS_OK; free with sas_destroy.  The context stays on that device:
+ * every later call on it runs there whatever the calling thread's current device is (and leaves that unchanged). */
 sas_status sas_create_instrument(const sas_instrument_desc* instr, sas_ctx** out);
 
 /* Use caller-owned DEVICE histograms ([n_exp][ny][nx]: double, double, uint64)
@@ -185,13 +189,18 @@ const char* sas_last_error(const sas_ctx* ctx);
 /* --- batched mode (PAPER.md:19, :213 dataset generation) ------------------ */
 
 /* n_exp experiments, each with its own instrument + model and its own histogram
- * ([n_exp][ny][nx]; every experiment must have the same det_nx, det_ny and the same
- * precision).  Tables are built and uploaded here. */
+ * ([n_exp][ny][nx]; every experiment must have the same det_nx, det_ny).  Tables are built and
+ * uploaded here.  Experiments are grouped by kernel (model form, per-event or fixed-node sizes, precision of the
+ * model arithmetic): a trace call launches one kernel per group present. */
 sas_status sas_create_batch(const sas_instrument_desc* instr, const sas_model_desc* model, uint32_t n_exp,
                             sas_ctx** out);
 /* Trace ids [0, n_neutrons_each) of every experiment in ONE launch; experiment e
  * uses Philox counter word 3 = e. */
 sas_status sas_trace_batch(sas_ctx* ctx, uint64_t n_neutrons_each, uint64_t seed);
+/* The same for ids [first_id, first_id + n_each) of every experiment (accumulates): a batch can be resumed, or
+ * sharded over GPUs by contiguous id ranges exactly like a single experiment (scatter
+ * ncount/N, gather) -- the union of the ranges is the same set of neutrons as one call over the whole range. */
+sas_status sas_trace_batch_range(sas_ctx* ctx, uint64_t first_id, uint64_t n_each, uint64_t seed);
 
 /* --- introspection -------------------------------------------------------- */
 /* HOST-ONLY (needs no device): the quadrature rule the library builds for
@@ -207,6 +216,23 @@ sas_status sas_get_launch_info(sas_ctx* ctx, uint64_t* n_launches, int32_t* grid
 /* Average device time in ms (CUDA events on the context's stream) of the trace kernels launched
  * since the last call with reset != 0; *n_timed = how many launches the average covers. */
 sas_status sas_get_kernel_time(sas_ctx* ctx, int32_t reset, double* avg_ms, uint64_t* n_timed);
+/* One record per trace-kernel launch since the last sas_get_kernel_time(reset != 0), oldest first (at most
+ * SAS_MAX_LAUNCH_RECORDS are kept): which kernel ran (variant = the model form it was compiled for, per-event
+ * sizes or fixed nodes, precision of the model arithmetic), over how many experiments and ids, and its device
+ * time from CUDA events on the context's stream.  Writes min(*n, cap) records to h_records; synchronises. */
+#define SAS_MAX_LAUNCH_RECORDS 4096
+typedef struct {
+  int32_t variant;       /* internal kernel variant: 0 sphere, 1 core-shell sphere, 2 cylinder, 3 triaxial,
+                            4 core-shell triaxial, 5 flat, 6 cylinder with tilt quadrature, 7.. NEXT-2 models */
+  int32_t per_event;     /* 1: SAS_PD_GAUSS_MC kernel */
+  int32_t precision;     /* SAS_FP32 | SAS_FP64 actually used by the model arithmetic */
+  int32_t warp_specialised; /* 1: producer/consumer kernel (trace_kernel_ws.cuh) */
+  uint32_t n_exp;        /* experiments of the launch */
+  uint32_t n_per_exp;    /* ids per experiment */
+  int32_t grid, block;
+  double ms;
+} sas_launch_record;
+sas_status sas_get_launch_records(sas_ctx* ctx, sas_launch_record* h_records, uint32_t cap, uint32_t* n);
 /* Bytes of the last host-to-device upload of parameters and quadrature tables (sas_set_model /
  * sas_create_batch). */
 sas_status sas_get_upload_bytes(sas_ctx* ctx, uint64_t* bytes);
@@ -217,7 +243,7 @@ sas_status sas_get_upload_bytes(sas_ctx* ctx, uint64_t* bytes);
  * q = (4 pi / lambda_ref) sin(two_theta / 2), solid angle dOmega = A_pix D / (D^2 + r^2)^(3/2); ring
  * b = floor((q - q_lo) n_bins / (q_hi - q_lo)) for q_lo <= q < q_hi.  Host outputs, n_bins entries each (any may
  * be NULL): q = ring centres, I = sum P / (sum dOmega * launched) (weight per steradian per launched neutron of
- * that experiment), sigma = sqrt(sum P2) / (same), npix = pixels in the ring (empty ring: I = sigma = 0).
+ * that experiment; launched = desc->n_launched, or the context's own count when that is 0), sigma = sqrt(sum P2) / (same), npix = pixels in the ring (empty ring: I = sigma = 0).
  * Runs one CUDA kernel on the context's stream over the bound histograms and synchronises.
  * SAS_EINVAL: n_bins outside 1..SAS_MAX_RINGS, q_lo >= q_hi, lambda_ref <= 0, exp_index out of range. */
 #define SAS_MAX_RINGS 1024
@@ -228,9 +254,15 @@ typedef struct {
   int32_t reserved;
   double q_lo, q_hi;      /* 1/A */
   double lambda_ref;      /* A: the wavelength that converts angle to q */
+  uint64_t n_launched;    /* neutrons launched INTO THIS EXPERIMENT that the bound histograms hold; 0 = what this
+                             context traced since its last reset / bind.  Must be given when the buffers hold more
+                             than that (detectors merged from other GPUs, buffers accumulated elsewhere). */
 } sas_radial_desc;
 sas_status sas_reduce_radial(sas_ctx* ctx, const sas_radial_desc* desc, double* h_q, double* h_I, double* h_sigma,
                              uint64_t* h_npix);
+
+/* Device time in ms (CUDA events around the kernel) of the last sas_reduce_radial on this context. */
+sas_status sas_get_reduce_time(sas_ctx* ctx, double* ms);
 
 const char* sas_version(void);
 

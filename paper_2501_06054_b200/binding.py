@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = [
     "sas_trace_dump", "sas_read_detector", "sas_get_counters", "sas_reset_detector", "sas_destroy",
     "sas_last_error", "sas_create_batch", "sas_trace_batch", "sas_quadrature_nodes",
     "sas_get_launch_info", "sas_get_kernel_time", "sas_get_upload_bytes", "sas_version", "sas_reduce_radial",
+    "sas_trace_batch_range", "sas_get_launch_records", "sas_get_reduce_time",
 ]
 
 SAMPLE = {"box": 0, "cyl_y": 1}
@@ -61,7 +62,16 @@ class ModelDesc(C.Structure):
 
 class RadialDesc(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("exp_index", C.c_uint32), ("n_bins", C.c_int32), ("reserved", C.c_int32),
-                ("q_lo", C.c_double), ("q_hi", C.c_double), ("lambda_ref", C.c_double)]
+                ("q_lo", C.c_double), ("q_hi", C.c_double), ("lambda_ref", C.c_double), ("n_launched", C.c_uint64)]
+
+
+class LaunchRecord(C.Structure):
+    _fields_ = [("variant", C.c_int32), ("per_event", C.c_int32), ("precision", C.c_int32),
+                ("warp_specialised", C.c_int32), ("n_exp", C.c_uint32), ("n_per_exp", C.c_uint32),
+                ("grid", C.c_int32), ("block", C.c_int32), ("ms", C.c_double)]
+
+
+MAX_LAUNCH_RECORDS = 4096
 
 
 def instrument_desc(d: dict) -> InstrumentDesc:
@@ -134,6 +144,9 @@ def load_library(path: str | None = None):
     L.sas_last_error.restype = C.c_char_p
     L.sas_create_batch.argtypes = [pp(InstrumentDesc), pp(ModelDesc), u32, pp(vp)]
     L.sas_trace_batch.argtypes = [vp, u64, u64]
+    L.sas_trace_batch_range.argtypes = [vp, u64, u64, u64]
+    L.sas_get_launch_records.argtypes = [vp, pp(LaunchRecord), u32, pp(u32)]
+    L.sas_get_reduce_time.argtypes = [vp, pp(dbl)]
     L.sas_quadrature_nodes.argtypes = [i32, dbl, i32, pp(dbl), pp(dbl)]
     L.sas_get_launch_info.argtypes = [vp, pp(u64), pp(i32), pp(i32), pp(i32)]
     L.sas_get_kernel_time.argtypes = [vp, i32, pp(dbl), pp(u64)]
@@ -166,12 +179,21 @@ def quadrature_nodes(kind: str, param: float, n: int):
 class _Base:
     """Owns a sas_ctx plus torch-allocated device histograms bound to it."""
 
-    def _bind(self, n_exp, ny, nx, device, stream):
+    @staticmethod
+    def _device(device):
+        """torch.device of the context: the given one, else torch's current CUDA device."""
         import torch
         if not torch.cuda.is_available():
             raise SasError(3, "no CUDA device: the tracer has no CPU fallback")
+        dev = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        if dev.index is None:
+            dev = torch.device("cuda", torch.cuda.current_device())
+        return dev
+
+    def _bind(self, n_exp, ny, nx, device, stream):
+        import torch
         self.torch = torch
-        self.device = torch.device(device)
+        self.device = device
         self.shape = (n_exp, ny, nx) if n_exp > 1 or self._batch else (ny, nx)
         self.sum_p = torch.zeros(self.shape, dtype=torch.float64, device=self.device)
         self.sum_p2 = torch.zeros(self.shape, dtype=torch.float64, device=self.device)
@@ -189,17 +211,22 @@ class _Base:
         return np.array(out[:], dtype=np.uint64)
 
     def read_detector(self):
-        """Device -> host copy through the ABI: (sum_p, sum_p2, counts) numpy arrays."""
-        # page-locked host arrays (torch's caching host allocator): the three copies are plain DMA transfers
+        """Device -> host copy through the ABI: (sum_p, sum_p2, counts) numpy arrays (views of page-locked
+        host buffers owned by this object and reused by the next call: copy what must outlive it)."""
         import torch
-        host = [torch.empty(self.shape, dtype=dt, pin_memory=True) for dt in (torch.float64, torch.float64, torch.int64)]
+        if getattr(self, "_host", None) is None:   # page-locked once: the three copies are plain DMA transfers
+            self._host = [torch.empty(self.shape, dtype=dt, pin_memory=True)
+                          for dt in (torch.float64, torch.float64, torch.int64)]
+        host = self._host
         _check(self.L, self.ctx, self.L.sas_read_detector(self.ctx, *(t.data_ptr() for t in host)))
         sp, sp2, cn = (t.numpy() for t in host)
         return sp, sp2, cn.view(np.uint64)
 
-    def reduce_radial(self, lambda_ref, q_lo, q_hi, n_bins, exp_index=0):
-        """Ring average of the detector into I(q): (q, I, sigma, npix) numpy arrays (include/sas.h)."""
-        d = RadialDesc(C.sizeof(RadialDesc), int(exp_index), int(n_bins), 0, float(q_lo), float(q_hi), float(lambda_ref))
+    def reduce_radial(self, lambda_ref, q_lo, q_hi, n_bins, exp_index=0, n_launched=0):
+        """Ring average of the detector into I(q): (q, I, sigma, npix) numpy arrays (include/sas.h).
+        n_launched: neutrons launched into that experiment held by the buffers (0 = this context's own count)."""
+        d = RadialDesc(C.sizeof(RadialDesc), int(exp_index), int(n_bins), 0, float(q_lo), float(q_hi), float(lambda_ref),
+                       int(n_launched))
         q, i, s = (np.zeros(max(n_bins, 1)) for _ in range(3))
         n = np.zeros(max(n_bins, 1), np.uint64)
         _check(self.L, self.ctx, self.L.sas_reduce_radial(self.ctx, C.byref(d), q.ctypes.data, i.ctypes.data,
@@ -215,6 +242,18 @@ class _Base:
         ms, n = C.c_double(), C.c_uint64()
         _check(self.L, self.ctx, self.L.sas_get_kernel_time(self.ctx, 1 if reset else 0, ms, n))
         return ms.value, n.value
+
+    def launch_records(self):
+        """One dict per trace-kernel launch since the last kernel_time_ms(reset=True) (include/sas.h)."""
+        buf = (LaunchRecord * MAX_LAUNCH_RECORDS)()
+        n = C.c_uint32()
+        _check(self.L, self.ctx, self.L.sas_get_launch_records(self.ctx, buf, MAX_LAUNCH_RECORDS, n))
+        return [{k: getattr(buf[i], k) for k, _ in LaunchRecord._fields_} for i in range(min(n.value, MAX_LAUNCH_RECORDS))]
+
+    def reduce_time_ms(self):
+        ms = C.c_double()
+        _check(self.L, self.ctx, self.L.sas_get_reduce_time(self.ctx, ms))
+        return ms.value
 
     def upload_bytes(self):
         n = C.c_uint64()
@@ -237,16 +276,16 @@ class Tracer(_Base):
     """One virtual experiment: sas_create_instrument / sas_set_model / sas_trace / sas_read_detector."""
     _batch = False
 
-    def __init__(self, instrument: dict, model: dict | None = None, device="cuda:0", stream=None):
+    def __init__(self, instrument: dict, model: dict | None = None, device=None, stream=None):
+        """device: a torch device (default: torch's current CUDA device, which is left unchanged)."""
         self.L = load_library()
         import torch
-        if not torch.cuda.is_available():
-            raise SasError(3, "no CUDA device: the tracer has no CPU fallback")
-        torch.cuda.set_device(device)
+        dev = self._device(device)
         self.ctx = C.c_void_p()
         ins = instrument_desc(instrument)
-        _check(self.L, None, self.L.sas_create_instrument(C.byref(ins), C.byref(self.ctx)))
-        self._bind(1, ins.det_ny, ins.det_nx, device, stream)
+        with torch.cuda.device(dev):       # the library creates the context on the calling thread's current device
+            _check(self.L, None, self.L.sas_create_instrument(C.byref(ins), C.byref(self.ctx)))
+        self._bind(1, ins.det_ny, ins.det_nx, dev, stream)
         if model is not None:
             self.set_model(model)
 
@@ -276,19 +315,22 @@ class BatchTracer(_Base):
     """Many experiments in one launch: sas_create_batch / sas_trace_batch."""
     _batch = True
 
-    def __init__(self, instruments: list, models: list, device="cuda:0", stream=None):
+    def __init__(self, instruments: list, models: list, device=None, stream=None):
         self.L = load_library()
         import torch
-        if not torch.cuda.is_available():
-            raise SasError(3, "no CUDA device: the tracer has no CPU fallback")
-        torch.cuda.set_device(device)
+        dev = self._device(device)
         n = len(instruments)
         assert n == len(models) and n > 0
         ins = (InstrumentDesc * n)(*[instrument_desc(d) for d in instruments])
         mod = (ModelDesc * n)(*[model_desc(d) for d in models])
         self.ctx = C.c_void_p()
-        _check(self.L, None, self.L.sas_create_batch(ins, mod, n, C.byref(self.ctx)))
-        self._bind(n, ins[0].det_ny, ins[0].det_nx, device, stream)
+        with torch.cuda.device(dev):
+            _check(self.L, None, self.L.sas_create_batch(ins, mod, n, C.byref(self.ctx)))
+        self._bind(n, ins[0].det_ny, ins[0].det_nx, dev, stream)
 
     def trace(self, n_neutrons_each: int, seed: int):
         _check(self.L, self.ctx, self.L.sas_trace_batch(self.ctx, n_neutrons_each, seed))
+
+    def trace_range(self, first_id: int, n_each: int, seed: int):
+        """ids [first_id, first_id + n_each) of every experiment (resume, or one GPU's shard)."""
+        _check(self.L, self.ctx, self.L.sas_trace_batch_range(self.ctx, first_id, n_each, seed))

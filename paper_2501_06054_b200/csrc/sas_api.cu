@@ -22,7 +22,8 @@ thread_local std::string g_create_error;
 constexpr double TWO_PI = 6.283185307179586;
 constexpr double FOUR_PI_3 = 4.1887902047863905;
 constexpr double PI_D = 3.141592653589793;
-constexpr int MAX_TIMED = 256;
+constexpr int MAX_TIMED = SAS_MAX_LAUNCH_RECORDS;
+constexpr int N_GROUPS = 4 * N_VARIANTS;
 #ifndef SAS_ITEMS_PER_BLOCK
 #define SAS_ITEMS_PER_BLOCK 16
 #endif
@@ -37,6 +38,7 @@ struct sas_ctx {
   uint32_t n_exp = 0;
   int nx = 0, ny = 0, npix = 0;
   int precision = -1;  // set by the model(s)
+  std::vector<int> exp_prec;  // precision the model arithmetic of each experiment runs in
   bool model_set = false;
   bool batch = false;
   std::vector<sas_instrument_desc> instr;
@@ -53,10 +55,10 @@ struct sas_ctx {
   bool own_hist = true;
   unsigned long long* d_counters = nullptr;
   unsigned int* d_work = nullptr;
-  // experiments grouped by kernel variant: one launch per non-empty group (ids concatenated on the device)
-  // (groups N_VARIANTS.. are the per-event-size kernels of the same variants)
-  std::vector<uint32_t> group_ids[2 * N_VARIANTS];
-  size_t group_off[2 * N_VARIANTS] = {};
+  // experiments grouped by kernel: one launch per non-empty group (ids concatenated on the device).
+  // group = variant + N_VARIANTS * (per-event sizes ? 1 : 0) + 2 N_VARIANTS * (fp64 model arithmetic ? 1 : 0)
+  std::vector<uint32_t> group_ids[N_GROUPS];
+  size_t group_off[N_GROUPS] = {};
   uint32_t* d_exp_ids = nullptr;
   double* d_rings = nullptr;  // ring sums of sas_reduce_radial: 3 x SAS_MAX_RINGS doubles + SAS_MAX_RINGS counts
   cudaStream_t stream = nullptr;
@@ -66,7 +68,9 @@ struct sas_ctx {
   uint64_t launched = 0;  // neutrons traced into the detector since the last reset (counters[0])
   int last_grid = 0, last_block = 0, last_smem = 0;
   std::vector<cudaEvent_t> ev0, ev1;
+  std::vector<sas_launch_record> records;  // of the timed launches (ms filled on request)
   uint64_t n_timed = 0;
+  double last_reduce_ms = 0.0;
 };
 
 namespace {
@@ -82,6 +86,17 @@ sas_status fail(sas_ctx* c, sas_status st, const std::string& msg) {
     if (e_ != cudaSuccess)                                                                      \
       return fail(ctx, SAS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));          \
   } while (0)
+
+// Every call on a context runs on the device the context was created on and leaves the caller's current
+// device as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(const sas_ctx* c) {
+    if (c && cudaGetDevice(&prev) == cudaSuccess && prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
 
@@ -447,27 +462,54 @@ int node_evaluations(const sas_model_desc& m) {
   return n;
 }
 
+// largest phase q x length the fp32 node loops of this experiment can see (sizes times their largest node)
+double max_phase(const sas_model_desc& m, const sas_instrument_desc& ins) {
+  double f[2] = {1.0, 1.0};
+  for (int k = 0; k < 2; ++k)
+    if (m.pd_kind[k] == SAS_PD_SCHULZ_QUAD && m.pd_rel[k] > 0.0 && m.pd_nodes[k] > 1) {
+      std::vector<double> x, w;
+      schulz_rule(m.pd_rel[k], m.pd_nodes[k], x, w);
+      f[k] = *std::max_element(x.begin(), x.end());
+    }
+  double len = 0.0;
+  switch (m.model) {
+    case SAS_SPHERE: len = m.size[0] * f[0]; break;
+    case SAS_CORE_SHELL_SPHERE: len = m.size[0] * f[0] + m.size[1] * f[1]; break;
+    case SAS_CYLINDER: len = std::max(m.size[0] * f[0], 0.5 * m.size[1] * f[1]); break;
+    case SAS_TRIAXIAL_ELLIPSOID: len = std::max(m.size[0], std::max(m.size[1], m.size[2])) * f[0]; break;
+    case SAS_CORE_SHELL_TRIAXIAL: len = std::max(m.size[0], std::max(m.size[1], m.size[2])) * f[0] + m.size[3] * f[1]; break;
+    default: break;
+  }
+  return ins.q_max * len;
+}
+
+// Precision the model arithmetic of one experiment really runs in.  A model without any node loop is evaluated
+// once per detected neutron; that single evaluation is done in fp64 whatever precision was asked for: it costs
+// little next to the fp64 geometry before it, and a monodisperse form factor near its zeros cannot meet 1e-5 in
+// fp32.  Per-event sizes (SAS_PD_GAUSS_MC) and the NEXT-2 models are fp64 as well (R-N2).
+// So is an experiment whose phases leave the range the fp32 argument reductions are proven for (|x| < 1e3).
+constexpr double FP32_MAX_PHASE = 1.0e3;
+int effective_precision(const sas_model_desc& m, const sas_instrument_desc& ins) {
+  if (m.precision == SAS_FP64) return SAS_FP64;
+  if (node_evaluations(m) <= 1) return SAS_FP64;
+  if (m.pd_kind[0] == SAS_PD_GAUSS_MC || m.pd_kind[1] == SAS_PD_GAUSS_MC || m.model >= SAS_PARALLELEPIPED) return SAS_FP64;
+  if (max_phase(m, ins) > FP32_MAX_PHASE) return SAS_FP64;
+  return SAS_FP32;
+}
+
 // (re)build ExpParams + tables of every experiment and upload them
 sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   c->h_tab.clear();
   c->tab_len_max = 0;
-  // A model without any node loop is evaluated once per detected neutron; that single evaluation is
-  // done in fp64 whatever precision was asked for: it costs little next to the fp64 geometry before
-  // it, and a monodisperse form factor near its zeros cannot meet 1e-5 in fp32.
-  bool any_loop = false;
-  for (uint32_t e = 0; e < c->n_exp; ++e) any_loop = any_loop || node_evaluations(models[e]) > 1;
-  // ... and per-event sizes (SAS_PD_GAUSS_MC) are one fp64 evaluation per neutron as well (R-N2)
-  bool any_event = false;
-  for (uint32_t e = 0; e < c->n_exp; ++e)
-    any_event = any_event || models[e].pd_kind[0] == SAS_PD_GAUSS_MC || models[e].pd_kind[1] == SAS_PD_GAUSS_MC ||
-                models[e].model >= SAS_PARALLELEPIPED;  // the NEXT-2 models have an fp64 node loop only
-  c->precision = (models[0].precision == SAS_FP64 || !any_loop || any_event) ? SAS_FP64 : SAS_FP32;
+  c->exp_prec.assign(c->n_exp, SAS_FP64);
+  c->precision = SAS_FP32;  // of the context: fp64 as soon as one experiment runs in fp64 (introspection only)
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     ExpParams& P = c->h_exps[e];
     fill_instrument(c->instr[e], P);
     P.exp_index = (int32_t)e;
     sas_model_desc m = models[e];
-    m.precision = c->precision;
+    m.precision = c->exp_prec[e] = effective_precision(models[e], c->instr[e]);
+    if (m.precision == SAS_FP64) c->precision = SAS_FP64;
     fill_model(m, P, c->h_tab);
     P.lam_small = 0;
     if (m.model == SAS_CYLINDER) {
@@ -490,10 +532,10 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
     const int v = (P.model == SAS_CYLINDER && P.orient_kind == SAS_ORIENT_GAUSS_QUAD) ? (int)V_CYL_QUAD
                   : P.model >= SAS_PARALLELEPIPED ? (int)V_PARA + (P.model - SAS_PARALLELEPIPED) : P.model;
     const bool event = (P.pd_mc[0] | P.pd_mc[1]) != 0 && P.model != SAS_FLAT;
-    c->group_ids[v + (event ? (int)N_VARIANTS : 0)].push_back(e);
+    c->group_ids[v + (event ? (int)N_VARIANTS : 0) + (c->exp_prec[e] == SAS_FP64 ? 2 * (int)N_VARIANTS : 0)].push_back(e);
   }
   std::vector<uint32_t> ids;
-  for (int v = 0; v < 2 * N_VARIANTS; ++v) {
+  for (int v = 0; v < N_GROUPS; ++v) {
     c->group_off[v] = ids.size();
     ids.insert(ids.end(), c->group_ids[v].begin(), c->group_ids[v].end());
   }
@@ -574,6 +616,12 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   CUDA_TRY(c, cudaGetLastError());
   if (timed) {
     CUDA_TRY(c, cudaEventRecord(c->ev1[c->n_timed], c->stream));
+    sas_launch_record r;
+    r.variant = V; r.per_event = EV ? 1 : 0; r.precision = sizeof(Real) == 8 ? SAS_FP64 : SAS_FP32;
+    r.warp_specialised = WS ? 1 : 0; r.n_exp = a.n_exp; r.n_per_exp = a.n_per_exp; r.grid = grid; r.block = BLOCK_THREADS;
+    r.ms = 0.0;
+    if (c->records.size() <= c->n_timed) c->records.resize(c->n_timed + 1);
+    c->records[c->n_timed] = r;
     c->n_timed += 1;
   }
   c->n_launches += 1;
@@ -607,12 +655,13 @@ sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v, int g) {
 }
 
 sas_status launch_groups(sas_ctx* c, KernelArgs& a) {
-  for (int g = 0; g < 2 * N_VARIANTS; ++g) {
+  for (int g = 0; g < N_GROUPS; ++g) {
     if (c->group_ids[g].empty()) continue;
     const int v = g % N_VARIANTS;
+    const bool event = (g / N_VARIANTS) & 1, fp64 = g >= 2 * N_VARIANTS;
     sas_status st;
-    if (g >= N_VARIANTS) st = launch_variant<double, true>(c, a, v, g);  // upload_models forced fp64
-    else st = c->precision == SAS_FP64 ? launch_variant<double, false>(c, a, v, g) : launch_variant<float, false>(c, a, v, g);
+    if (event) st = launch_variant<double, true>(c, a, v, g);  // effective_precision: always fp64
+    else st = fp64 ? launch_variant<double, false>(c, a, v, g) : launch_variant<float, false>(c, a, v, g);
     if (st != SAS_OK) return st;
   }
   return SAS_OK;
@@ -651,6 +700,7 @@ sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t
 
 void destroy_ctx(sas_ctx* c) {
   if (!c) return;
+  DeviceGuard g(c);
   if (c->stream) cudaStreamSynchronize(c->stream);
   for (auto e : c->ev0) cudaEventDestroy(e);
   for (auto e : c->ev1) cudaEventDestroy(e);
@@ -713,7 +763,6 @@ sas_status sas_create_batch(const sas_instrument_desc* instr, const sas_model_de
     sas_status st = validate_instrument(instr + e, why);
     if (st == SAS_OK) st = validate_model(model + e, why);
     if (st == SAS_OK && (instr[e].det_nx != instr[0].det_nx || instr[e].det_ny != instr[0].det_ny)) { st = SAS_EINVAL; why = "all experiments of a batch need the same det_nx, det_ny"; }
-    if (st == SAS_OK && model[e].precision != model[0].precision) { st = SAS_EINVAL; why = "all experiments of a batch need the same precision"; }
     if (st != SAS_OK) return fail(nullptr, st, "experiment " + std::to_string(e) + ": " + why);
   }
   sas_ctx* c = new (std::nothrow) sas_ctx();
@@ -732,6 +781,7 @@ sas_status sas_create_batch(const sas_instrument_desc* instr, const sas_model_de
 
 sas_status sas_bind_buffers(sas_ctx* c, void* d_sum_p, void* d_sum_p2, void* d_counts, void* cuda_stream) {
   if (!c) return SAS_EINVAL;
+  DeviceGuard g(c);
   if (!d_sum_p || !d_sum_p2 || !d_counts) return fail(c, SAS_EINVAL, "histogram pointers must not be NULL");
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   if (c->own_hist) { cudaFree(c->d_sum_p); cudaFree(c->d_sum_p2); cudaFree(c->d_counts); }
@@ -752,6 +802,7 @@ sas_status sas_bind_buffers(sas_ctx* c, void* d_sum_p, void* d_sum_p2, void* d_c
 
 sas_status sas_set_model(sas_ctx* c, const sas_model_desc* model) {
   if (!c) return SAS_EINVAL;
+  DeviceGuard g(c);
   if (c->batch) return fail(c, SAS_ESTATE, "batched contexts take their models at sas_create_batch");
   std::string why;
   sas_status st = validate_model(model, why);
@@ -763,23 +814,47 @@ sas_status sas_set_model(sas_ctx* c, const sas_model_desc* model) {
 
 sas_status sas_trace(sas_ctx* c, uint64_t n_neutrons, uint64_t seed) {
   if (c && c->batch) return fail(c, SAS_ESTATE, "use sas_trace_batch on a batched context");
+  DeviceGuard g(c);
   return trace_common(c, 0, n_neutrons, seed);
 }
 
 sas_status sas_trace_range(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t seed) {
   if (c && c->batch) return fail(c, SAS_ESTATE, "use sas_trace_batch on a batched context");
+  DeviceGuard g(c);
   return trace_common(c, first_id, n, seed);
 }
 
 sas_status sas_trace_batch(sas_ctx* c, uint64_t n_neutrons_each, uint64_t seed) {
   if (c && !c->batch) return fail(c, SAS_ESTATE, "sas_trace_batch needs a context from sas_create_batch");
+  DeviceGuard g(c);
   return trace_common(c, 0, n_neutrons_each, seed);
+}
+
+sas_status sas_trace_batch_range(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t seed) {
+  if (c && !c->batch) return fail(c, SAS_ESTATE, "sas_trace_batch_range needs a context from sas_create_batch");
+  DeviceGuard g(c);
+  return trace_common(c, first_id, n_each, seed);
+}
+
+sas_status sas_get_launch_records(sas_ctx* c, sas_launch_record* h_records, uint32_t cap, uint32_t* n) {
+  if (!c || !n || (cap && !h_records)) return SAS_EINVAL;
+  DeviceGuard g(c);
+  CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+  for (uint64_t i = 0; i < c->n_timed; ++i) {
+    float ms = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev0[i], c->ev1[i]));
+    c->records[i].ms = ms;
+    if (i < cap) h_records[i] = c->records[i];
+  }
+  *n = (uint32_t)c->n_timed;
+  return SAS_OK;
 }
 
 sas_status sas_trace_dump(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t seed, uint32_t exp_index,
                           int32_t* d_pixel, double* d_weight, double* d_q) {
   if (!c) return SAS_EINVAL;
   if (c->batch) return fail(c, SAS_ESTATE, "sas_trace_dump works on single-experiment contexts");
+  DeviceGuard g(c);
   if (!c->model_set) return fail(c, SAS_ESTATE, "sas_set_model must precede tracing");
   if (!d_pixel || !d_weight) return fail(c, SAS_EINVAL, "d_pixel and d_weight must not be NULL");
   if (n == 0) return SAS_OK;
@@ -807,6 +882,7 @@ sas_status sas_trace_dump(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t se
 
 sas_status sas_read_detector(sas_ctx* c, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts) {
   if (!c) return SAS_EINVAL;
+  DeviceGuard g(c);
   const size_t nh = (size_t)c->n_exp * c->npix;
   if (h_sum_p) CUDA_TRY(c, cudaMemcpyAsync(h_sum_p, c->d_sum_p, nh * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   if (h_sum_p2) CUDA_TRY(c, cudaMemcpyAsync(h_sum_p2, c->d_sum_p2, nh * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -817,6 +893,7 @@ sas_status sas_read_detector(sas_ctx* c, double* h_sum_p, double* h_sum_p2, uint
 
 sas_status sas_get_counters(sas_ctx* c, uint64_t out[8]) {
   if (!c || !out) return SAS_EINVAL;
+  DeviceGuard g(c);
   CUDA_TRY(c, cudaMemcpyAsync(out, c->d_counters, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   // the kernel counts the outcomes it decides in its queued stages (slots 2..7); launched is the host's
@@ -830,6 +907,7 @@ sas_status sas_get_counters(sas_ctx* c, uint64_t out[8]) {
 
 sas_status sas_reset_detector(sas_ctx* c) {
   if (!c) return SAS_EINVAL;
+  DeviceGuard g(c);
   const size_t nh = (size_t)c->n_exp * c->npix;
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
@@ -850,6 +928,7 @@ sas_status sas_get_launch_info(sas_ctx* c, uint64_t* n_launches, int32_t* grid, 
 
 sas_status sas_get_kernel_time(sas_ctx* c, int32_t reset, double* avg_ms, uint64_t* n_timed) {
   if (!c) return SAS_EINVAL;
+  DeviceGuard g(c);
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
   double sum = 0.0;
   for (uint64_t i = 0; i < c->n_timed; ++i) {
@@ -872,22 +951,24 @@ sas_status sas_get_upload_bytes(sas_ctx* c, uint64_t* bytes) {
 sas_status sas_reduce_radial(sas_ctx* c, const sas_radial_desc* d, double* h_q, double* h_I, double* h_sigma,
                              uint64_t* h_npix) {
   if (!c) return SAS_EINVAL;
+  DeviceGuard g(c);
   if (!d || d->struct_size != sizeof(sas_radial_desc)) return fail(c, SAS_EINVAL, "sas_radial_desc.struct_size mismatch");
   if (d->n_bins < 1 || d->n_bins > SAS_MAX_RINGS) return fail(c, SAS_EINVAL, "n_bins must be in 1..SAS_MAX_RINGS");
   if (!(d->q_hi > d->q_lo) || !(d->q_lo >= 0.0) || !std::isfinite(d->q_hi)) return fail(c, SAS_EINVAL, "need 0 <= q_lo < q_hi");
   if (!(d->lambda_ref > 0.0) || !std::isfinite(d->lambda_ref)) return fail(c, SAS_EINVAL, "lambda_ref must be > 0");
   if (d->exp_index >= c->n_exp) return fail(c, SAS_EINVAL, "exp_index out of range");
   const int nb = d->n_bins;
+  // ring scratch: sum P, sum P2, sum dOmega, pixel count, nb entries each (one memset, one copy of what is used)
   if (!c->d_rings) CUDA_TRY(c, cudaMalloc(&c->d_rings, 4 * (size_t)SAS_MAX_RINGS * sizeof(double)));
-  CUDA_TRY(c, cudaMemsetAsync(c->d_rings, 0, 4 * (size_t)SAS_MAX_RINGS * sizeof(double), c->stream));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_rings, 0, 4 * (size_t)nb * sizeof(double), c->stream));
   const sas_instrument_desc& ins = c->instr[d->exp_index];
   ReduceArgs a;
   a.sum_p = c->d_sum_p + (size_t)d->exp_index * c->npix;
   a.sum_p2 = c->d_sum_p2 + (size_t)d->exp_index * c->npix;
   a.ring_p = c->d_rings;
-  a.ring_p2 = c->d_rings + SAS_MAX_RINGS;
-  a.ring_omega = c->d_rings + 2 * SAS_MAX_RINGS;
-  a.ring_n = reinterpret_cast<unsigned long long*>(c->d_rings + 3 * SAS_MAX_RINGS);
+  a.ring_p2 = c->d_rings + nb;
+  a.ring_omega = c->d_rings + 2 * nb;
+  a.ring_n = reinterpret_cast<unsigned long long*>(c->d_rings + 3 * nb);
   a.det_xw = ins.det_xw; a.det_yh = ins.det_yh; a.det_dist = ins.det_dist;
   a.px = ins.det_xw / (double)ins.det_nx; a.py = ins.det_yh / (double)ins.det_ny;
   a.a_pix_d = (a.px * a.py) * ins.det_dist;
@@ -895,22 +976,39 @@ sas_status sas_reduce_radial(sas_ctx* c, const sas_radial_desc* d, double* h_q, 
   a.q_lo = d->q_lo; a.q_hi = d->q_hi; a.scale = (double)nb / (d->q_hi - d->q_lo);
   a.nx = ins.det_nx; a.ny = ins.det_ny; a.n_bins = nb;
   const int grid = std::max(1, std::min(c->n_sm * 4, (c->npix + REDUCE_THREADS - 1) / REDUCE_THREADS));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  CUDA_TRY(c, cudaEventCreate(&e0));
+  CUDA_TRY(c, cudaEventCreate(&e1));
+  CUDA_TRY(c, cudaEventRecord(e0, c->stream));
   reduce_radial_kernel<<<grid, REDUCE_THREADS, 0, c->stream>>>(a);
   CUDA_TRY(c, cudaGetLastError());
+  CUDA_TRY(c, cudaEventRecord(e1, c->stream));
   c->n_launches += 1;
-  std::vector<double> h(4 * (size_t)SAS_MAX_RINGS);
+  std::vector<double> h(4 * (size_t)nb);
   CUDA_TRY(c, cudaMemcpyAsync(h.data(), c->d_rings, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-  const unsigned long long* hn = reinterpret_cast<const unsigned long long*>(h.data() + 3 * SAS_MAX_RINGS);
-  const double launched = (double)(c->launched / c->n_exp);  // every experiment of a context traces the same ids
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  c->last_reduce_ms = ms;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  const unsigned long long* hn = reinterpret_cast<const unsigned long long*>(h.data() + 3 * nb);
+  // neutrons launched into this experiment: the caller's figure, else this context's own count (every experiment
+  // of a context traces the same ids)
+  const double launched = d->n_launched ? (double)d->n_launched : (double)(c->launched / c->n_exp);
   for (int b = 0; b < nb; ++b) {
     if (h_q) h_q[b] = d->q_lo + ((double)b + 0.5) * ((d->q_hi - d->q_lo) / (double)nb);
-    const double norm = h[2 * SAS_MAX_RINGS + b] * launched;
+    const double norm = h[2 * nb + b] * launched;
     const bool any = hn[b] != 0 && norm > 0.0;
     if (h_I) h_I[b] = any ? h[b] / norm : 0.0;
-    if (h_sigma) h_sigma[b] = any ? std::sqrt(h[SAS_MAX_RINGS + b]) / norm : 0.0;
+    if (h_sigma) h_sigma[b] = any ? std::sqrt(h[nb + b]) / norm : 0.0;
     if (h_npix) h_npix[b] = hn[b];
   }
+  return SAS_OK;
+}
+
+sas_status sas_get_reduce_time(sas_ctx* c, double* ms) {
+  if (!c || !ms) return SAS_EINVAL;
+  *ms = c->last_reduce_ms;
   return SAS_OK;
 }
 

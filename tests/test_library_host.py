@@ -35,12 +35,14 @@ def test_every_declared_symbol_is_exported(lib):
 def test_struct_layouts_match_the_header(lib):
     # sizes the C compiler gives for the header's structs
     import subprocess, tempfile
-    src = '#include "sas.h"\n#include <stdio.h>\nint main(){printf("%zu %zu\\n", sizeof(sas_instrument_desc), sizeof(sas_model_desc));return 0;}\n'
+    src = ('#include "sas.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu\\n", sizeof(sas_instrument_desc), '
+           'sizeof(sas_model_desc), sizeof(sas_radial_desc), sizeof(sas_launch_record));return 0;}\n')
     with tempfile.TemporaryDirectory() as d:
         open(os.path.join(d, "t.c"), "w").write(src)
         subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), "-o", os.path.join(d, "t"), os.path.join(d, "t.c")])
-        a, b = map(int, subprocess.check_output([os.path.join(d, "t")]).split())
+        a, b, r, l = map(int, subprocess.check_output([os.path.join(d, "t")]).split())
     assert a == C.sizeof(B.InstrumentDesc) and b == C.sizeof(B.ModelDesc)
+    assert r == C.sizeof(B.RadialDesc) and l == C.sizeof(B.LaunchRecord)
 
 
 def test_quadrature_rules_agree_with_the_oracles(lib):

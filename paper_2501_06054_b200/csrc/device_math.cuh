@@ -90,7 +90,52 @@ __device__ __forceinline__ void sincos_core(float x, float lo, float& s, float& 
   c = __int_as_float(__float_as_int(cc) ^ (((kb + 1) << 30) & 0x80000000));  // k mod 4 in {1,2}: -cos
 }
 __device__ __forceinline__ void sincos_r(float x, float& s, float& c) { sincos_core(x, 0.0f, s, c); }
-__device__ __forceinline__ void sincos_r(double x, double& s, double& c) { sincos(x, &s, &c); }
+
+// fp64 sin and cos for the tracer's arguments (azimuth 2 pi u, form-factor phases q x size): three-step
+// Cody-Waite reduction by pi/2 with FMAs (pi/2 in three 33-bit pieces: n P1 is exact for |n| < 2^20), Taylor
+// kernels on [-pi/4, pi/4] up to r^15 / r^16 (truncation below 6e-17 relative).  About one ulp, i.e. within the
+// two ulps that separate any two good libraries (DESIGN.md R-C10); straight-line, no large-argument path, its
+// constants in constant memory (an fp64 literal costs two moves per use).  |x| > 1e6 goes to the library.
+__constant__ double c_sincos[20] = {
+    0x1.45f306dc9c883p-1,                                     // 2 / pi
+    0x1.921fb544p+0, 0x1.0b4611a6p-34, 0x1.3198a2ep-69,       // pi/2 = P1 + P2 + P3 + 8.5e-32 (33 bits each)
+    -1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0, 1.0 / 6227020800.0,
+    -1.0 / 1307674368000.0, 0.0,                              // sin: r + r^3 (S1 + z (S2 + ...)), z = r^2
+    -0.5, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0, 1.0 / 479001600.0, -1.0 / 87178291200.0,
+    1.0 / 20922789888000.0};                                  // cos: 1 + z (C1 + z (C2 + ...))
+__device__ __forceinline__ void sincos_cw(double x, double& s, double& c) {
+  const double t = fma(x, c_sincos[0], 6755399441055744.0);  // 1.5 * 2^52: nearest integer in the low word
+  const int k = __double2loint(t);
+  const double nf = t - 6755399441055744.0;
+  double r = fma(-nf, c_sincos[1], x);
+  r = fma(-nf, c_sincos[2], r);
+  r = fma(-nf, c_sincos[3], r);
+  const double z = r * r;
+  double ps = fma(z, c_sincos[10], c_sincos[9]);
+  ps = fma(ps, z, c_sincos[8]);
+  ps = fma(ps, z, c_sincos[7]);
+  ps = fma(ps, z, c_sincos[6]);
+  ps = fma(ps, z, c_sincos[5]);
+  ps = fma(ps, z, c_sincos[4]);
+  ps = fma(r * z, ps, r);
+  double pc = fma(z, c_sincos[19], c_sincos[18]);
+  pc = fma(pc, z, c_sincos[17]);
+  pc = fma(pc, z, c_sincos[16]);
+  pc = fma(pc, z, c_sincos[15]);
+  pc = fma(pc, z, c_sincos[14]);
+  pc = fma(pc, z, c_sincos[13]);
+  pc = fma(pc, z, c_sincos[12]);
+  pc = fma(pc, z, 1.0);
+  const double ss = (k & 1) ? pc : ps;
+  const double cc = (k & 1) ? ps : pc;
+  s = (k & 2) ? -ss : ss;
+  c = ((k + 1) & 2) ? -cc : cc;
+}
+__device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
+  if (fabs(x) > 1.0e6) { sincos(x, &s, &c); return; }
+  sincos_cw(x, s, c);
+}
+__device__ __forceinline__ void sincos_r(double x, double& s, double& c) { sincos_d(x, s, c); }
 
 // fp32 reciprocal / square root: one MUFU each (~1 ulp), no IEEE fix-up path
 __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
@@ -133,7 +178,7 @@ __device__ __forceinline__ Phase<float> phase_mul(Proj<float> p, float l_hi, flo
 __device__ __forceinline__ double ph_val(Phase<double> p) { return p.v; }
 __device__ __forceinline__ float ph_val(Phase<float> p) { return p.hi; }
 
-__device__ __forceinline__ void sincos_ph(Phase<double> p, double& s, double& c) { sincos(p.v, &s, &c); }
+__device__ __forceinline__ void sincos_ph(Phase<double> p, double& s, double& c) { sincos_d(p.v, s, c); }
 __device__ __forceinline__ void sincos_ph(Phase<float> p, float& s, float& c) { sincos_core(p.hi, p.lo, s, c); }
 
 // sin/cos of 2 pi u, u in (0,1), fp64, ~1e-13: exact reduction by quarter turns, Taylor kernels.
@@ -200,7 +245,7 @@ __device__ __forceinline__ double sphere_phi(double u) {
     return fma(s, u2, 1.0);
   }
   double s, c;
-  sincos(u, &s, &c);
+  sincos_d(u, s, c);
   return (3.0 * fma(-u, c, s)) / ((u * u) * u);
 }
 

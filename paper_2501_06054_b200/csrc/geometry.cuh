@@ -162,7 +162,7 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
   const double e1x = dz * inv_n, e1z = -(dx * inv_n);
   const double e2x = dy * e1z, e2y = dz * e1x - dx * e1z, e2z = -(dy * e1x);
   double sc, cc;
-  sincos(chi, &sc, &cc);
+  sincos_cw(chi, sc, cc);  // chi in (0, 2 pi)
   const double tx = cc * e1x + sc * e2x, ty = sc * e2y, tz = cc * e1z + sc * e2z;
   const double dpx = c2 * dx + s2 * tx, dpy = c2 * dy + s2 * ty, dpz = c2 * dz + s2 * tz;
   h.Qx = k * (ss2 * dx - s2 * tx);

@@ -1,25 +1,28 @@
 #!/usr/bin/env python
 """bench.py -- neutrons traced per second on B200 (BASELINE.json metric).
 
-A "step" is one pass of the whole hot path (RNG -> source -> slits -> sample -> Q -> I(Q) with the
-quadrature loops -> detector histogram) over one batch of n_neutrons synthetic neutrons of the
-headline workload, BASELINE.json configs[1] (polydisperse sphere + Percus-Yevick S(q), fp32 model,
-1e8 neutrons, 256x256 detector).  `value` is timed with the descriptors and tables resident on the
-device; `e2e` goes through the C ABI with host buffers every step (sas_set_model: H2D of parameters
-and tables; sas_read_detector: D2H of the three histograms).  The other four configs are timed with
-a short loop and reported under "configs".
+A "step" is one pass of the whole hot path (RNG -> source -> slits -> sample -> Q -> I(Q) with the quadrature
+loops -> detector histogram) over one batch of synthetic neutrons.  The headline workload is the largest
+single-GPU one of BASELINE.json that the target names, configs[2]: oriented cylinders, fp32 model, 24 x 24
+orientation nodes per detected neutron, 1e9 neutrons per step, 256 x 256 detector.  `value` is timed with the
+descriptors and tables resident on the device; `e2e` goes through the C ABI with host buffers every step
+(sas_set_model: H2D of parameters and tables; sas_read_detector: D2H of the three histograms).  Every other
+workload -- c0 (1e6 as specified, and 1e9), c1 in fp32 AND fp64, c3, c4 (batch of 1024), n1, n2 -- is timed the
+same way (>= 10 steps, its own clock record, roofline and e2e) and reported under "configs".
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
 
-N > 1 is launched by torch.distributed.run, one rank per GPU; rank r traces the id range
-[r n, (r+1) n) (weak scaling) and the detectors are merged onto rank 0 by one reduction per step.
---impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+N > 1 is launched by torch.distributed.run, one rank per GPU (`python bench.py --gpus N` without a launcher
+re-executes itself under it); rank r traces the id range [r n, (r+1) n) of every experiment (weak scaling) and
+the detectors are merged onto rank 0 by one reduction per step.  --impl reference times the CPU oracle
+(oracle/) on bounded 1e5-id steps of the same workload.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -33,7 +36,12 @@ import sas_workloads as W  # noqa: E402
 
 METRIC = "neutrons traced/sec on 1 B200 (SANS + SAS sample)"
 UNIT = "neutrons/s"
-HEADLINE = 1                      # BASELINE.json configs[1]
+HEADLINE = 2                      # BASELINE.json configs[2]
+# (name in "configs", workload index, precision override, neutrons per step override)
+SECONDARY = [("c0_sphere_fp64", 0, None, None), ("c0_sphere_fp64_1e9", 0, None, 10**9),
+             ("c1_polysphere_py_fp32", 1, "fp32", None), ("c1_polysphere_py_fp64", 1, "fp64", None),
+             ("c3_coreshell_triaxial", 3, None, None), ("c4_batch", 4, None, None),
+             ("n1_paper_cylinder", 5, None, None), ("n2_paper_barbell", 6, None, None)]
 
 
 # ------------------------------------------------------------------ reference arm: the CPU oracle
@@ -44,7 +52,7 @@ def run_reference(args):
     from oracle import oracle as O
     c = W.config(HEADLINE)
     ins, mod = O.make_instrument(c["instrument"]), O.make_model(c["model"])
-    sample = 1_000_000            # ids per step: a bounded prefix-like sample of the 1e8-neutron workload
+    sample = 100_000              # ids per step: a bounded sample of the 1e9-neutron workload (~0.5 s each)
     for w in range(args.warmup):
         O.trace_range(ins, mod, c["seed"], w * sample, sample, dump=False)
     t0 = time.perf_counter()
@@ -58,7 +66,7 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": c["name"], "n_neutrons_per_step": sample,
-                   "note": "CPU oracle, single thread, ids [0, steps*1e6) of the 1e8-neutron workload"},
+                   "note": "CPU oracle, single thread, ids [0, (warmup+steps)*1e5) of the 1e9-neutron workload"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
                          "sample": f"{args.steps} x {sample} neutron ids of {c['name']}"},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -99,7 +107,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(k)
             except Exception:
                 break
-            time.sleep(0.002)
+            time.sleep(0.001)
 
     def result(self):
         if not self.samples:
@@ -109,35 +117,57 @@ class ClockSampler(threading.Thread):
 
 
 # ------------------------------------------------------------------ helpers
-def model_key_and_nodes(model):
-    from paper_2501_06054_b200 import roofline as R  # noqa: F401
-    m, prec = model["model"], model["precision"]
-    pd = [n if k == "schulz" else 1 for k, n in zip(model["pd_kind"], model["pd_nodes"])]
-    if is_event_model(model) and m == "cylinder":
-        return "cylinder_event_fp64", 1
-    if is_event_model(model) and m == "barbell":
-        return "barbell_event_fp64", 64
-    if m == "sphere":
-        nodes = pd[0]
-        eff = prec if nodes > 1 else "fp64"
-        key = ("sphere_py_" if model["sq_kind"] != "none" else "sphere_") + eff
-        return key, nodes
-    if m == "cylinder" and model["orient_kind"] == "gauss_quad":
-        return "cylinder_quad_fp32", model["n_theta"] * model["n_phi"] * (pd[0] + pd[1]) // 2
-    if m == "core_shell_triaxial":
-        return "cs_triaxial_iso_fp32", pd[0] * pd[1]
-    if m == "cylinder":
-        return "cylinder_iso_fp64", 1
-    raise KeyError(m)
-
-
 def is_event_model(model):
     return "gauss_mc" in model["pd_kind"]
 
 
+def model_key_and_nodes(model):
+    """Row of roofline.MODEL_COST that prices this model, and its node evaluations per detected neutron."""
+    m, prec = model["model"], model["precision"]
+    pd = [n if k == "schulz" else 1 for k, n in zip(model["pd_kind"], model["pd_nodes"])]
+    if is_event_model(model) and m == "cylinder":
+        return "cylinder_event_fp64", 0
+    if is_event_model(model) and m == "barbell":
+        return "barbell_event_fp64", 64
+    if m == "sphere":
+        nodes = pd[0]
+        if nodes == 1:
+            return "sphere_fp64", 0              # one evaluation, served in fp64 (DESIGN.md section 6)
+        return ("sphere_py_" if model["sq_kind"] != "none" else "sphere_") + prec, nodes
+    if m == "cylinder" and model["orient_kind"] == "gauss_quad":
+        return "cylinder_quad_fp32", model["n_theta"] * model["n_phi"] * pd[0] * pd[1]
+    if m == "core_shell_triaxial":
+        return "cs_triaxial_iso_fp32", pd[0] * pd[1]
+    if m == "cylinder":
+        return "cylinder_iso_fp64", 0
+    raise KeyError(m)
+
+
+def geometry_class(ins):
+    return "fast" if ins["sample_shape"] == "box" and ins["mu_abs_2200"] == 0 and ins["mu_inc"] == 0 else "general"
+
+
+VARIANT_OF = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3, "core_shell_triaxial": 4}
+
+
+def run_microbench(local):
+    """Pipe rates of this GPU from csrc/microbench.cu (built by __graft_entry__.build / build.py --microbench)."""
+    from paper_2501_06054_b200 import build as libbuild
+    exe = os.path.join(ROOT, "paper_2501_06054_b200", "microbench")
+    try:
+        if not os.path.exists(exe):
+            libbuild.build_microbench()
+        env = dict(os.environ, CUDA_VISIBLE_DEVICES=os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")[local]
+                   if os.environ.get("CUDA_VISIBLE_DEVICES") else str(local))
+        out = subprocess.run([exe], capture_output=True, text=True, timeout=120, env=env).stdout
+        return json.loads([ln for ln in out.splitlines() if ln.startswith("{")][-1])
+    except Exception as exc:                              # the roofline then says it used the recorded rates
+        return {"error": str(exc)}
+
+
 def time_steps(torch, tracer, do_step, steps, warmup, flush):
-    """Device time of `steps` steps: one CUDA-event pair per step on the tracer's stream, L2 flushed
-    between steps outside the pairs; barrier + synchronize on both sides."""
+    """Device time of `steps` steps: one CUDA-event pair per step on the tracer's stream, L2 flushed between
+    steps outside the pairs; barrier + synchronize on both sides; MAX over ranks."""
     import torch.distributed as dist
     for i in range(warmup):
         do_step(i)
@@ -147,7 +177,6 @@ def time_steps(torch, tracer, do_step, steps, warmup, flush):
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     tracer.kernel_time_ms(reset=True)
-    l0 = tracer.launch_info()["n_launches"]
     for i in range(steps):
         flush()
         ev[i][0].record()
@@ -159,150 +188,203 @@ def time_steps(torch, tracer, do_step, steps, warmup, flush):
     torch.cuda.synchronize()
     per_step = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(per_step)
-    time_steps.last_per_step = per_step
     if dist.is_initialized() and dist.get_world_size() > 1:
         t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
-    return total_ms, tracer.launch_info()["n_launches"] - l0
+    return total_ms, per_step
 
 
-def bench_config(torch, S, cfg_index, steps, warmup, rank, world, flush, with_e2e):
+def bench_config(torch, S, cfg_index, precision, n_override, steps, warmup, rank, world, local, flush, rates, traffic):
     from paper_2501_06054_b200 import roofline as R
     from paper_2501_06054_b200.sharding import weak_shard, merge_detectors
-    c = W.config(cfg_index)
+    c = W.config(cfg_index, precision) if precision else W.config(cfg_index)
     batch = "models" in c
+    dev = torch.device("cuda", local)
     if batch:
-        tr = S.BatchTracer(c["instruments"], c["models"])
-        n_step = c["n_neutrons_each"] * len(c["models"])
-        n_arg = c["n_neutrons_each"]
+        tr = S.BatchTracer(c["instruments"], c["models"], device=dev)
+        n_arg = n_override or c["n_neutrons_each"]
+        n_step = n_arg * len(c["models"])
     else:
-        tr = S.Tracer(c["instrument"], c["model"])
-        n_step = n_arg = c["n_neutrons"]
+        tr = S.Tracer(c["instrument"], c["model"], device=dev)
+        n_step = n_arg = n_override or c["n_neutrons"]
     seed = c["seed"]
-    first, _ = weak_shard(n_arg, rank)
+    first, _ = weak_shard(n_arg, rank)                    # rank r owns ids [r n, (r+1) n) of every experiment
 
     def do_step(i):
         tr.reset()
-        if batch:
-            tr.trace(n_arg, seed + rank)           # ranks use distinct streams of the same experiments
-        else:
-            tr.trace_range(first, n_arg, seed)
+        tr.trace_range(first, n_arg, seed)
         if world > 1:
             merge_detectors([tr.sum_p, tr.sum_p2, tr.counts], dst=0)
 
-    total_ms, launches = time_steps(torch, tr, do_step, steps, warmup, flush)
-    kernel_ms, n_timed = tr.kernel_time_ms(reset=True)   # average per launch; a step may take several
-    launches_per_step = max(1, int(n_timed) // steps)    # launches (one per kernel variant in a batch)
-    kernel_ms *= launches_per_step                        # trace-kernel time per step
+    sampler = ClockSampler(local)
+    sampler.start()
+    total_ms, per_step = time_steps(torch, tr, do_step, steps, warmup, flush)
+    sampler.stop_flag = True
+    sampler.join()
+    clocks = sampler.result()
+    recs = tr.launch_records()                            # every trace-kernel launch of the timed steps
+    tr.kernel_time_ms(reset=True)
     info = tr.launch_info()
     cnt = tr.counters().astype(np.float64)
     ms_per_step = total_ms / steps
-    value = n_step * world / (ms_per_step * 1e-3)
-    per = sorted(getattr(time_steps, "last_per_step", [ms_per_step]))
-    out = {"workload": c["name"], "n_neutrons_per_step": n_step, "ms_per_step": ms_per_step, "value": value,
-           "ms_per_step_median": per[len(per) // 2], "ms_per_step_best": per[0],
-           "kernel_ms": kernel_ms, "grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
-           "gpu_launches": int(launches), "detected_frac": cnt[6] / cnt[0], "survive_frac": 1.0 - cnt[1] / cnt[0],
+    per = sorted(per_step)
+    kernel_ms = sum(r["ms"] for r in recs) / steps
+    out = {"workload": c["name"], "precision_requested": (c["models"][0] if batch else c["model"])["precision"],
+           "n_neutrons_per_step": n_step, "steps": steps, "ms_per_step": ms_per_step,
+           "value": n_step * world / (ms_per_step * 1e-3),
+           "ms_per_step_median": per[len(per) // 2], "ms_per_step_best": per[0], "kernel_ms": kernel_ms,
+           "grid": info["grid"], "block": info["block"], "smem_bytes": info["smem_bytes"],
+           "gpu_launches": len(recs) // steps, "clocks": clocks,
+           "detected_frac": cnt[6] / cnt[0], "survive_frac": 1.0 - cnt[1] / cnt[0],
            # survivors whose fp64 geometry ran (the others were certain detector misses, counters[7])
            "geometry_frac": 1.0 - cnt[1] / cnt[0] - cnt[7] / cnt[0]}
-    # roofline of the (only) kernel of the step, from its own average launch duration
-    if batch:
-        ks = {}
-        for m in c["models"]:
-            k, n = model_key_and_nodes(m)
-            ks[k] = n
-        # mixed batch: weigh the per-detected cost of the two model families equally (half each)
-        rl = None
-        for k, n in ks.items():
-            r = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n,
-                           workload=c["name"], frac_geometry=out["geometry_frac"])
-            rl = r if rl is None else {**rl, "achieved": 0.5 * (rl["achieved"] + r["achieved"]),
-                                       "frac": 0.5 * (rl["frac"] + r["frac"])}
-        out["roofline"] = rl
+    # roofline: one record per launch group (a batch launches one kernel per model form), each from its own
+    # event time; the step's fraction is the sum of the groups' algorithmic lane-clocks over peak x kernel time
+    models = c["models"] if batch else [c["model"]]
+    inss = c["instruments"] if batch else [c["instrument"]]
+    groups = {}
+    for ins, m in zip(inss, models):
+        key, nodes = model_key_and_nodes(m)
+        g = groups.setdefault((VARIANT_OF.get(m["model"], -1), is_event_model(m)), dict(key=key, nodes=nodes, geo=geometry_class(ins), n_exp=0))
+        g["n_exp"] += 1
+    ms_of = {}
+    for r in recs:
+        k = (r["variant"] if r["variant"] != 6 else 2, bool(r["per_event"]))
+        ms_of[k] = ms_of.get(k, 0.0) + r["ms"] / steps
+    peak = R.N_SM * R.SMSP_PER_SM * 32 * R.SM_MAX_MHZ * 1e6
+    lane_clocks, parts = 0.0, []
+    for k, g in groups.items():
+        ms = ms_of.get(k, kernel_ms if len(groups) == 1 else 0.0)
+        n_g = n_arg * g["n_exp"]
+        rl = R.roofline(n_g / (ms * 1e-3) if ms > 0 else 0.0, out["survive_frac"], out["detected_frac"], g["key"], g["nodes"],
+                        frac_geometry=out["geometry_frac"], geometry=g["geo"], rates=rates,
+                        sm_mhz_sampled=clocks.get("sm_mhz"), traffic=traffic.get(c["name"]))
+        rl["model_cost_row"], rl["kernel_ms"], rl["n_exp"] = g["key"], ms, g["n_exp"]
+        lane_clocks += rl["achieved"] * 1e9 * ms * 1e-3
+        parts.append(rl)
+    if len(parts) == 1:
+        out["roofline"] = parts[0]
     else:
-        k, n = model_key_and_nodes(c["model"])
-        out["roofline"] = R.roofline(n_step / (kernel_ms * 1e-3), out["survive_frac"], out["detected_frac"], k, n,
-                                     workload=c["name"], frac_geometry=out["geometry_frac"])
-    e2e = None
-    if with_e2e and not batch:
-        # the call a user makes, host buffers in and out, every step
+        top = max(parts, key=lambda p: p["kernel_ms"])
+        out["roofline"] = dict(top, frac=lane_clocks / (peak * kernel_ms * 1e-3), achieved=lane_clocks / (kernel_ms * 1e-3) / 1e9,
+                               note="per-launch records under 'launches'; frac = sum of their algorithmic lane-clocks / (peak x kernel time)",
+                               launches=parts)
+        out["roofline"].pop("frac_at_sampled_clock", None)
+
+    # ---- end to end: the call a user makes, host buffers in and out, every step
+    import paper_2501_06054_b200.binding as B
+    if batch:
+        host = [torch.empty((len(models),) + tuple(tr.shape[1:]), dtype=dt, pin_memory=True)
+                for dt in (torch.float64, torch.float64, torch.int64)]
+        tr.close()
+
+        def e2e_step(i):
+            bt = S.BatchTracer(c["instruments"], c["models"], device=dev)   # host descriptors -> tables -> H2D
+            bt._host = host                                                    # caller-owned page-locked output
+            bt.trace_range(first, n_arg, seed)
+            res = bt.read_detector()                                           # D2H of every histogram
+            up = bt.upload_bytes()
+            bt.close()
+            return res, up
+    else:
         def e2e_step(i):
             tr.set_model(c["model"])                # H2D: parameters + quadrature tables
             tr.reset()
             tr.trace_range(first, n_arg, seed)
-            return tr.read_detector()               # D2H: three histograms into host arrays
+            return tr.read_detector(), tr.upload_bytes()   # D2H: three histograms into host arrays
 
-        for i in range(2):
-            e2e_step(i)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for i in range(steps):
-            sp, sp2, cn = e2e_step(i)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        if world > 1:
-            import torch.distributed as dist
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        npix = sp.size
-        e2e = {"value": n_step * world * steps / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(tr.upload_bytes()), "d2h_bytes_per_step": int(3 * 8 * npix)}
-    tr.close()
-    return out, e2e
-
-
-def cpu_baseline(cfg_index, budget_s=12.0):
-    from oracle import oracle as O
-    c = W.config(cfg_index)
-    ins, mod = O.make_instrument(c["instrument"]), O.make_model(c["model"])
-    O.trace_range(ins, mod, c["seed"], 0, 100000, dump=False)
+    n_e2e = steps if not batch else max(3, steps // 3)
+    for i in range(2):
+        e2e_step(i)
+    torch.cuda.synchronize()
     t0 = time.perf_counter()
-    O.trace_range(ins, mod, c["seed"], 0, 1_000_000, dump=False)
-    rate = 1e6 / (time.perf_counter() - t0)
-    n = int(min(max(rate * budget_s, 1e6), 1e8))
-    t0 = time.perf_counter()
-    O.trace_range(ins, mod, c["seed"], 0, n, dump=False)
+    for i in range(n_e2e):
+        (sp, sp2, cn), up = e2e_step(i)
+    torch.cuda.synchronize()
     dt = time.perf_counter() - t0
-    return {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"ids [0, {n}) of {c['name']} ({dt:.1f} s, single thread)"}
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+    out["e2e"] = {"value": n_step * world * n_e2e / dt, "unit": UNIT, "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
+                  "h2d_bytes_per_step": int(up), "d2h_bytes_per_step": int(3 * 8 * sp.size),
+                  "includes": ("sas_create_batch + sas_trace_batch_range + sas_read_detector + sas_destroy" if batch else
+                               "sas_set_model + sas_reset_detector + sas_trace_range + sas_read_detector")}
+    if not batch:
+        tr.close()
+    return out
+
+
+def bench_reduce(torch, S, local, hbm_gbs):
+    """The ring average (sas_reduce_radial): one kernel reading sum_p and sum_p2 of a 512 x 512 detector (16 B per
+    pixel), HBM-bound; its own roofline against the measured copy bandwidth."""
+    c = W.config(3)
+    tr = S.Tracer(c["instrument"], c["model"], device=torch.device("cuda", local))
+    tr.trace(10**7, c["seed"])
+    flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=tr.device)
+    best = []
+    for i in range(12):
+        flush_buf.fill_(i)
+        tr.reduce_radial(6.0, 0.001, 0.05, 200)
+        best.append(tr.reduce_time_ms())
+    tr.close()
+    ms = float(np.median(best[2:]))
+    npix = c["instrument"]["det_nx"] * c["instrument"]["det_ny"]
+    gbs = 16.0 * npix / (ms * 1e-3) / 1e9
+    return {"workload": "ring average of the 512 x 512 detector of c3 into 200 rings (L2 flushed before each call)",
+            "kernel_ms_median": ms, "algorithmic_bytes": 16 * npix,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s", "frac": gbs / hbm_gbs if hbm_gbs else None,
+                         "note": "4 MB read once: the kernel is launch-latency sized (a few microseconds), far from bandwidth-bound"}}
 
 
 def _oracle_worker(job):
-    cfg_index, first, n = job
+    cfg_index, precision, first, n, exps = job
     from oracle import oracle as O
-    c = W.config(cfg_index)
-    O.trace_range(c["instrument"], c["model"], c["seed"], first, n, dump=False)
+    c = W.config(cfg_index, precision) if precision else W.config(cfg_index)
+    if "models" in c:
+        for e in exps:
+            O.trace_range(c["instruments"][e], c["models"][e], c["seed"], first, n // len(exps), exp_index=e, dump=False)
+    else:
+        O.trace_range(c["instrument"], c["model"], c["seed"], first, n, dump=False)
     return n
 
 
-def cpu_baseline_all_cores(cfg_index, rate_1core, seconds=3.0):
-    """The same oracle as K independent id-range processes (the paper's MPI scheme):
-    K = the cores this process may run on."""
+def oracle_rates(cfg_index, precision, seconds=2.0):
+    """The oracle as it stands on the host cores: one core, then K independent id-range processes (the paper's
+    MPI scheme), K = the cores this process may run on."""
     import multiprocessing as mp
-    k = len(os.sched_getaffinity(0))
-    n = int(max(rate_1core * seconds, 2e5))
-    with mp.get_context("spawn").Pool(k) as pool:
-        pool.map(_oracle_worker, [(cfg_index, 0, 1000)] * k)          # start the workers, load the library
-        t0 = time.perf_counter()
-        pool.map(_oracle_worker, [(cfg_index, r * n, n) for r in range(k)])
-        dt = time.perf_counter() - t0
-    return {"value": k * n / dt, "cores": k, "sample": f"{k} processes x {n} ids ({dt:.1f} s)"}
-
-
-def oracle_rate(cfg_index, n=300_000):
-    """Oracle neutrons/s on one host core over ids [0, n) of a secondary config (c4: its first two experiments)."""
-    from oracle import oracle as O
-    c = W.config(cfg_index)
-    if "models" in c:
-        pairs = [(c["instruments"][e], c["models"][e], e) for e in (0, 1)]
-    else:
-        pairs = [(c["instrument"], c["model"], 0)]
+    exps = (0, 1)                                         # c4: its first sphere and its first cylinder
     t0 = time.perf_counter()
-    for ins, mod, e in pairs:
-        O.trace_range(ins, mod, c["seed"], 0, n // len(pairs), exp_index=e, dump=False)
-    return n / (time.perf_counter() - t0)
+    _oracle_worker((cfg_index, precision, 0, 20000, exps))
+    rate = 20000 / (time.perf_counter() - t0)
+    n = int(min(max(rate * seconds, 2e4), 5e7))
+    t0 = time.perf_counter()
+    _oracle_worker((cfg_index, precision, 0, n, exps))
+    dt1 = time.perf_counter() - t0
+    k = len(os.sched_getaffinity(0))
+    out = {"oracle_1core": n / dt1, "oracle_1core_sample": f"ids [0, {n}) ({dt1:.1f} s)"}
+    try:
+        with mp.get_context("spawn").Pool(k) as pool:
+            pool.map(_oracle_worker, [(cfg_index, precision, 0, 1000, exps)] * k)   # start the workers, load the library
+            t0 = time.perf_counter()
+            pool.map(_oracle_worker, [(cfg_index, precision, r * n, n, exps) for r in range(k)])
+            dtk = time.perf_counter() - t0
+        out.update(oracle_kcores=k * n / dtk, cores=k, oracle_kcores_sample=f"{k} processes x {n} ids ({dtk:.1f} s)")
+    except Exception as exc:                              # a reported extra, never fatal
+        out["oracle_kcores_error"] = str(exc)
+    return out
+
+
+def cpu_model_name():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def run_sweep(torch, S):
@@ -338,96 +420,94 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200")
-    ap.add_argument("--headline-only", action="store_true", help="skip the four secondary configs")
+    ap.add_argument("--headline-only", action="store_true", help="skip the secondary workloads")
     ap.add_argument("--config", type=int, default=HEADLINE, help="workload timed as the main line (profiling)")
+    ap.add_argument("--precision", default=None, help="precision override of --config (profiling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1, then exit")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
 
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: one rank per GPU under torch.distributed.run
+        port = 29500 + os.getpid() % 2000
+        os.execvp(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+                                   "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
+
     import torch
     import torch.distributed as dist
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE is {world}: launch one rank per GPU")
     torch.cuda.set_device(local)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     import paper_2501_06054_b200 as S
+    from paper_2501_06054_b200 import roofline as R
     S.load_library()              # raises if libsas_b200.so is missing: no fallback
 
     if args.sweep:
         return run_sweep(torch, S)
 
+    mb = run_microbench(local)
+    rates = R.rates_from_microbench(mb) if "error" not in mb else None
+    traffic = R.read_traffic(os.path.join(ROOT, "profiles", "r2_dram_traffic.md"))
     flush_buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
     def flush():
         flush_buf.fill_(1)
 
-    sampler = ClockSampler(local)
-    sampler.start()
-    head, e2e = bench_config(torch, S, args.config, args.steps, max(args.warmup, 3) if args.warmup else 0,
-                             rank, world, flush, True)
-    sampler.stop_flag = True
-    sampler.join()
-    clocks = sampler.result()
+    warm = max(args.warmup, 3) if args.warmup else 0
+    head = bench_config(torch, S, args.config, args.precision, None, args.steps, warm, rank, world, local, flush, rates, traffic)
 
     others = {}
     if not args.headline_only:
-        for i in [j for j in range(7) if j != args.config]:
-            o, _ = bench_config(torch, S, i, 3, 3, rank, world, flush, False)
-            others[o["workload"]] = {k: o[k] for k in ("value", "ms_per_step", "kernel_ms", "n_neutrons_per_step",
-                                                       "detected_frac", "grid", "smem_bytes")}
-            others[o["workload"]]["roofline_frac"] = o["roofline"]["frac"]
-            others[o["workload"]]["roofline_pipe"] = o["roofline"]["pipe"]
-        # config 0 at 1e6 neutrons is launch-latency bound; the same experiment at 1e9 shows the path
-        c0 = W.config(0)
-        tr = S.Tracer(c0["instrument"], c0["model"])
-        first = rank * 10**9
-        tr.trace_range(first, 10**9, c0["seed"])
-        torch.cuda.synchronize()
-        tr.reset()
-        tr.kernel_time_ms(reset=True)
-        tr.trace_range(first, 10**9, c0["seed"])
-        ms, nt = tr.kernel_time_ms(reset=True)
-        ms *= nt
-        from paper_2501_06054_b200 import roofline as R
-        cnt = tr.counters().astype(np.float64)
-        rl = R.roofline(1e9 / (ms * 1e-3), 1 - cnt[1] / cnt[0], cnt[6] / cnt[0], "sphere_fp64", 1,
-                        frac_geometry=1 - cnt[1] / cnt[0] - cnt[7] / cnt[0])
-        others["c0_sphere_fp64_1e9"] = {"value": 1e9 * world / (ms * 1e-3), "kernel_ms": ms,
-                                        "roofline_frac": rl["frac"], "roofline_pipe": rl["pipe"]}
-        tr.close()
+        for name, idx, prec, n_over in SECONDARY:
+            if idx == args.config and n_over is None and prec == args.precision:
+                continue
+            k = max(10, min(args.steps, 20)) if idx != 4 else 10
+            o = bench_config(torch, S, idx, prec, n_over, k, 3, rank, world, local, flush, rates, traffic)
+            others[name] = o
+        if rank == 0:
+            peaks = {}
+            try:
+                peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            except Exception:
+                pass
+            others["reduce_radial"] = bench_reduce(torch, S, local, peaks.get("hbm_gbs"))
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = cpu_baseline(args.config if args.config < 4 else HEADLINE)
-        try:
-            cpu["all_cores"] = cpu_baseline_all_cores(args.config if args.config < 4 else HEADLINE, cpu["value"])
-        except Exception as exc:                          # a reported extra, never fatal
-            cpu["all_cores"] = {"error": str(exc)}
-        if not args.headline_only:
-            names = {W.config(i)["name"]: i for i in range(7)}
-            for k, v in others.items():
-                if k in names:
-                    v["oracle_1core"] = oracle_rate(names[k])
+        c = W.config(args.config, args.precision) if args.precision else W.config(args.config)
+        r = oracle_rates(args.config, args.precision, seconds=12.0)
+        cpu = {"value": r["oracle_1core"], "unit": UNIT, "cores": 1, "kind": "oracle", "cpu": cpu_model_name(),
+               "sample": f"{r['oracle_1core_sample']} of {c['name']}, single thread",
+               "all_cores": {k: r.get(k) for k in ("oracle_kcores", "cores", "oracle_kcores_sample", "oracle_kcores_error") if k in r}}
+        for name, idx, prec, n_over in SECONDARY:
+            if name in others and n_over is None:
+                others[name].update(oracle_rates(idx, prec, seconds=1.5))
 
     if rank == 0:
-        c = W.config(args.config)
+        c = W.config(args.config, args.precision) if args.precision else W.config(args.config)
+        m0 = c["models"][0] if "models" in c else c["model"]
         line = {
             "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32 model / f64 geometry+accumulation",
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": ("f32" if m0["precision"] == "fp32" else "f64") + " model / f64 RNG-to-uniform, geometry and accumulation",
             "data": "synthetic",
-            "config": {"workload": c["name"], "n_neutrons_per_step": head["n_neutrons_per_step"], "seed": c["seed"], "parallelism": f"ids sharded over {world} GPU(s)",
+            "config": {"workload": c["name"], "n_neutrons_per_step": head["n_neutrons_per_step"], "seed": c["seed"],
+                       "parallelism": f"neutron ids sharded over {world} GPU(s), one detector reduction per step",
                        "l2": "flushed between timed steps (256 MiB write, outside the event pairs)",
                        "grid": head["grid"], "block": head["block"], "smem_bytes": head["smem_bytes"]},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": head["gpu_launches"],
+            "clocks": head["clocks"], "e2e": head["e2e"], "gpu_launches": head["gpu_launches"] * args.steps,
             "ms_per_step_median": head["ms_per_step_median"], "ms_per_step_best": head["ms_per_step_best"],
             "kernel_ms": head["kernel_ms"], "roofline": head["roofline"], "cpu_baseline": cpu,
-            "configs": others,
+            "microbench": mb, "configs": others,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

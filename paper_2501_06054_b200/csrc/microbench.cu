@@ -71,6 +71,62 @@ __global__ void __launch_bounds__(256, 4) bench_philox(const __grid_constant__ K
   if (acc == 0x12345678u) out[id & 1023] = acc;
 }
 
+// IMAD.WIDE chains with NL extra independent LOP3 per multiply (each chain step is one LOP3 + one wide multiply,
+// as in a Philox round): how the integer multiplier and the logic pipe share the sub-partition
+template <int NL>
+__global__ void __launch_bounds__(256, 4) bench_mix(int iters, uint32_t seed, uint32_t* out) {
+  constexpr int CH = 6;
+  uint32_t id = blockIdx.x * blockDim.x + threadIdx.x + seed;
+  unsigned long long w[CH]; uint32_t u[CH][4];
+#pragma unroll
+  for (int c = 0; c < CH; ++c) { w[c] = id * 2654435761u + c; for (int j = 0; j < 4; ++j) u[c][j] = id + 17 * c + j; }
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+#pragma unroll
+      for (int c = 0; c < CH; ++c) {
+        unsigned long long p; const uint32_t x = (uint32_t)w[c] ^ (uint32_t)(w[c] >> 32) ^ seed;
+        asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(x), "r"(0xD2511F53u));
+        w[c] = p;
+#pragma unroll
+        for (int j = 0; j < NL; ++j) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[c][j]) : "r"(id), "r"(seed));
+      }
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int c = 0; c < CH; ++c) { acc ^= (uint32_t)w[c] ^ (uint32_t)(w[c] >> 32); for (int j = 0; j < 4; ++j) acc ^= u[c][j]; }
+  if (acc == 0x12345678u) out[id & 1023] = acc;
+}
+
+// The arithmetic core of the tracer's stage A for one row of 32 neutron ids: words 0 and 1 of Philox block 0 of
+// (id, id_hi, 0, exp) -- the compiler drops what the unused words 2, 3 would need -- and the two window compares,
+// three rows in flight; no compaction, no stores.  What this loop costs is what stage A cannot go below.
+__global__ void __launch_bounds__(256, 4) bench_stage_a(const __grid_constant__ Keys pk, int iters, uint32_t id_hi, uint32_t expw,
+                                                        uint32_t lo0, uint32_t d0, uint32_t lo1, uint32_t d1, uint32_t* out) {
+  uint32_t id = blockIdx.x * blockDim.x + threadIdx.x, acc = 0;
+  for (int i = 0; i < iters; ++i) {
+    uint32_t w0[3], w1[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      uint32_t c0 = id + k * 77777u + i * 131u, c1 = id_hi, c2 = 0u, c3 = expw;
+#pragma unroll
+      for (int rd = 0; rd < 9; ++rd) {
+        unsigned long long p0, p1;
+        asm("mul.wide.u32 %0, %1, %2;" : "=l"(p0) : "r"(0xD2511F53u), "r"(c0));
+        asm("mul.wide.u32 %0, %1, %2;" : "=l"(p1) : "r"(0xCD9E8D57u), "r"(c2));
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ pk.k0[rd], n2 = (uint32_t)(p0 >> 32) ^ c3 ^ pk.k1[rd];
+        c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0;
+      }
+      w0[k] = __umulhi(0xCD9E8D57u, c2) ^ c1 ^ pk.k0[9];
+      w1[k] = 0xCD9E8D57u * c2;
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) acc += ((w0[k] - lo0 <= d0) && (w1[k] - lo1 <= d1)) ? 1u : 0u;
+  }
+  if (acc == 0x12345678u) out[id & 1023] = acc;
+}
+
 template <int KIND>
 static double run(double mhz) {
   uint32_t* d; cudaMalloc(&d, 4096);
@@ -109,6 +165,42 @@ static double run_philox(double mhz) {
   return best * 1e-3 * mhz * 1e6 / warp_blocks_per_smsp;
 }
 
+template <int NL>
+static double run_mix(double mhz) {
+  uint32_t* d; cudaMalloc(&d, 4096);
+  int n_sm = 0; cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  const int grid = n_sm * 4, iters = 300;
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    bench_mix<NL><<<grid, 256>>>(iters, rep, d);
+    cudaEventRecord(e1); cudaEventSynchronize(e1);
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaFree(d);
+  return best * 1e-3 * mhz * 1e6 / ((double)grid * 8 / (n_sm * 4) * iters * 16 * 6);   // clocks per (multiply + its LOP3 + NL LOP3)
+}
+
+static double run_stage_a(double mhz) {
+  uint32_t* d; cudaMalloc(&d, 4096);
+  int n_sm = 0; cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, 0);
+  Keys pk; for (int r = 0; r < 10; ++r) { pk.k0[r] = 1234u + r * 0x9E3779B9u; pk.k1[r] = 99u + r * 0xBB67AE85u; }
+  const int grid = n_sm * 4, iters = 4000;
+  cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    bench_stage_a<<<grid, 256>>>(pk, iters, 7u, 3u, 0x40000000u, 0x7FFFFFFFu, 0x40000000u, 0x7FFFFFFFu, d);
+    cudaEventRecord(e1); cudaEventSynchronize(e1);
+    float ms; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaFree(d);
+  return best * 1e-3 * mhz * 1e6 / ((double)grid * 8 / (n_sm * 4) * iters * 3);   // clocks per row of 32 ids
+}
+
 int main() {
   const char* env = getenv("SM_MHZ");
   const double mhz = env ? atof(env) : 1965.0;
@@ -118,5 +210,12 @@ int main() {
   v[K_PHILOX] = run_philox(mhz);
   printf("SMSP clocks per warp instruction at %.0f MHz (32 resident warps per SM, %d independent chains per thread)\n", mhz, CHAINS);
   for (int k = 0; k < N_KINDS; ++k) printf("  %-52s %7.2f\n", NAMES[k], v[k]);
+  const double m0 = run_mix<0>(mhz), m1 = run_mix<1>(mhz), m2 = run_mix<2>(mhz), m3 = run_mix<3>(mhz), sa = run_stage_a(mhz);
+  printf("  %-52s %7.2f %7.2f %7.2f %7.2f\n", "wide multiply + (1 + NL) LOP3, NL = 0..3", m0, m1, m2, m3);
+  printf("  %-52s %7.2f\n", "stage-A core: Philox words 0,1 + window test, per row", sa);
+  // one machine-readable line for bench.py
+  printf("{\"sm_mhz\": %.0f, \"ffma\": %.4f, \"imad\": %.4f, \"imad_wide\": %.4f, \"lop3\": %.4f, \"dfma\": %.4f, \"mufu\": %.4f, "
+         "\"philox_block\": %.3f, \"wide_lop3\": [%.4f, %.4f, %.4f, %.4f], \"stage_a_core_row\": %.3f}\n",
+         mhz, v[K_FFMA], v[K_IMAD], v[K_IMAD_WIDE], v[K_LOP3], v[K_DFMA], v[K_MUFU_RCP], v[K_PHILOX], m0, m1, m2, m3, sa);
   return 0;
 }

@@ -1,31 +1,32 @@
-"""ALU roofline of the trace kernel.
+"""ALU roofline of the trace kernels.
 
-The path moves almost no HBM bytes (<= 0.04 B per neutron) and has no dense contraction: it is bound
-by instruction issue on the plain ALUs.  One SM sub-partition (SMSP; 4 per SM, 148 SMs) issues at most
-one warp instruction per clock; FP64 instructions additionally occupy the 16-lane FP64 pipe for 2
-clocks and MUFU/conversion instructions the 4-lane XU pipe for 8 clocks.  The roofline of a config is
-therefore the largest of three per-neutron costs, in SMSP-clocks per 32 neutrons:
+The path moves almost no HBM bytes (<= 0.04 B per neutron) and has no dense contraction: it is bound by the
+integer, FP64, FP32 and special-function units of the SM sub-partitions (SMSP; 4 per SM, 148 SMs).  A config's
+bound is the largest of five per-neutron costs, in SMSP clocks per lane (x 32 = per warp row):
 
-    issue = all algorithmic thread-instructions          (1 clock per warp instruction)
-    fp64  = 2 x FP64 thread-instructions
-    xu    = 8 x MUFU/conversion thread-instructions
-    imul  = 4 x 32x32->64-bit integer multiplies         (Philox: 20 per block, the heavy FMA pipe)
+    issue = c_ffma  x all algorithmic thread-instructions            (the issue port; FFMA runs at that rate)
+    imul  = c_wide  x 32x32->64 multiplies + c_imad x 32-bit multiplies   (the integer multiplier, "FMA heavy" pipe)
+    int   = c_lop3  x logic-pipe instructions + c_wide_int x 32x32->64 multiplies
+    fp64  = c_dfma  x FP64 instructions
+    xu    = c_mufu  x MUFU / POPC / conversion instructions
 
-The clocks per warp instruction are MEASURED on the B200 with csrc/microbench.cu (profiles/r1_microbench.md):
-FFMA 1.04, IMAD 2.02, IMAD.WIDE 4.05 inside Philox (a whole Philox4x32-10 block: 81 clocks), LOP3 2.03,
-DFMA 2.03, MUFU 8.05.
+The clocks per warp instruction (c_*) are MEASURED on the box by csrc/microbench.cu, which bench.py runs before
+timing anything (`rates` below holds the figures of profiles/r2_microbench.md as a fallback only):
+FFMA 1.04, IMAD 2.02, LOP3 2.02, DFMA 2.03, MUFU 8.04; a 32x32->64 multiply occupies the multiplier for 4.05
+clocks AND keeps the logic pipe from issuing for 2.05 of them: a stream of one multiply plus n LOP3 takes
+2.02 n + 2.05 clocks for every n >= 1 (measured 4.14, 6.10, 8.08, 10.07 for n = 1..4), so a Philox4x32-10 block
+(20 multiplies, 20 LOP3) costs 81 clocks on both pipes at once and every further logic instruction of stage A
+adds two full clocks.  `int` is that law.  It is checked against the kernel's own arithmetic: the stage-A core
+(words 0, 1 of Philox block 0 plus the window test, microbench `stage_a_core_row`) measures 76.1 clocks per row
+where the law gives 2.02 x 19.7 + 2.05 x 16 = 72.6 and the multiplier alone 66.
 
-The per-unit instruction counts below are ALGORITHMIC: the arithmetic that the method, in the
-formulation this library uses, needs on this ISA (a fp64 division = 1 MUFU.RCP64H + 9 DFMA-class,
-a fp64 sqrt = 1 MUFU.RSQ64H + 9, fp64 sincos = 62, Philox4x32-10 = 40 integer instructions, ...),
-counted per unit of work: every launched neutron (stage A), every slit-1 survivor (stage B0: Philox
-block 1 and the certain-miss test), every survivor whose geometry is evaluated (stage B), every
-detected neutron (stage-C prologue) and every quadrature node evaluation.  The per-node counts are the
-arithmetic instructions (FFMA/FMUL/FADD/MUFU/select) of the shipped loop bodies, read from the SASS of
-this build (cuobjdump): table loads, loop control, register moves, queue handling, work fetching and
-atomics are NOT in them, so the fraction cannot exceed the kernel's issue-slot utilisation.  The unit
-fractions (survivors, evaluated geometries, detected per launched neutron) are the counters of the
-timed run itself.
+The per-unit instruction counts are ALGORITHMIC: the arithmetic (multiplies, logic/compare/select, FP64, FP32,
+MUFU/POPC/conversions) of the shipped code of each stage, counted from the executed SASS of this build with the
+ncu source page (profiles/r2_instruction_counts.md): loads, stores, atomics, address arithmetic, moves, branches,
+barriers, queue handling and work fetching are NOT in them, nor are two things the kernels do for their own
+convenience -- the second draw of Philox block 0 in stage B and the certain-miss classifier of stage B0.  The
+fraction therefore cannot exceed the kernel's issue-slot utilisation.  The unit frequencies (survivors,
+evaluated geometries, detected per launched neutron) are the counters of the timed run itself.
 """
 from __future__ import annotations
 
@@ -33,75 +34,122 @@ N_SM = 148
 SMSP_PER_SM = 4
 SM_MAX_MHZ = 1965.0
 
-# thread-instructions per unit: (issue_total, fp64, xu, wide integer multiplies)
-STAGE_A = (46, 0, 0, 19)        # Philox block 0 (40; the last round needs one of its two products) + id/compare (6)
-STAGE_B0 = (40 + 12, 12, 0, 20) # Philox block 1 (40) + two uniforms, q, lambda, q*lambda test in fp64 (12)
-# Philox block 0 again (40) + 8 uniforms (3 fp64 each) + ~125 fp64 add/mul/compare + 8 div (10) + 3 sqrt (10)
-# + sincos (62) + floor/convert (6 xu-class conversions)
-STAGE_B = (40 + 24 + 125 + 80 + 30 + 62 + 12, 24 + 125 + 72 + 27 + 62, 11 + 6, 20)
+# fallback rates: profiles/r2_microbench.md (B200, 1965 MHz); bench.py replaces them with the live run
+RATES = dict(ffma=1.036, imad=2.020, imad_wide=4.05, lop3=2.024, dfma=2.029, mufu=8.04, wide_int=2.05,
+             philox_block=81.0, stage_a_core_row=76.1, source="profiles/r2_microbench.md (not re-measured)")
 
-# per detected neutron: prologue (|Q|, projections, weight product, 3 atomics) and per node evaluation
+
+def rates_from_microbench(mb: dict) -> dict:
+    """Per-instruction pipe clocks from the JSON line csrc/microbench.cu prints."""
+    lop3 = mb["lop3"]
+    # inside a Philox-like stream (one multiply + n LOP3): slope = LOP3 cost, intercept = what the multiply adds
+    w = mb["wide_lop3"]                       # clocks for 1 multiply + (1 + NL) LOP3, NL = 0..3
+    slope = (w[3] - w[1]) / 2.0
+    wide_int = w[1] - 2.0 * slope             # intercept of the n >= 2 line
+    return dict(ffma=mb["ffma"], imad=mb["imad"], imad_wide=mb["philox_block"] / 20.0, lop3=lop3, dfma=mb["dfma"],
+                mufu=mb["mufu"], wide_int=wide_int, philox_block=mb["philox_block"],
+                stage_a_core_row=mb["stage_a_core_row"], source="csrc/microbench.cu, run by bench.py on this box")
+
+
+def U(issue, wide=0.0, imad=0.0, logic=0.0, fp64=0.0, fp32=0.0, xu=0.0):
+    return dict(issue=float(issue), wide=float(wide), imad=float(imad), logic=float(logic), fp64=float(fp64),
+                fp32=float(fp32), xu=float(xu))
+
+
+# ---- per-unit algorithmic thread-instruction counts (profiles/r2_instruction_counts.md)
+# every launched neutron: Philox block 0, words 0 and 1 only (16 wide multiplies + 2 low products survive dead-code
+# elimination: counter words 1..3 are launch constants), 17.7 XOR, window compares, ballot, prefix mask, 2 POPC
+STAGE_A = U(42, wide=16, imad=2, logic=22, xu=2)
+# every slit-1 survivor: Philox block 1 (18.5 multiplies: two have constant inputs), 19 XOR, compaction
+# (ballot, mask, 2 POPC, ring position); the classifier's 8 instructions are not counted
+STAGE_B0 = U(50.5, wide=18.5, logic=30, xu=2)
+# every survivor whose geometry is evaluated (Philox block 0 again is not counted)
+STAGE_B = {
+    "fast": U(262, logic=47, fp64=200, fp32=2, xu=13),       # slit-free box-sample instrument class (c0, c1, c2, c4)
+    "general": U(295, logic=61, fp64=225, fp32=3, xu=14),    # cylinder sample, slits that may cut (c3)
+}
+
+# per detected neutron: (prologue, per node evaluation)
 MODEL_COST = {
-    # name: (prologue(issue, fp64, xu), per_node(issue, fp64, xu))
-    "sphere_fp64": ((40, 30, 2, 0), (110, 100, 2, 0)),
-    "sphere_fp32": ((40, 30, 4, 0), (32, 0, 1, 0)),
-    "sphere_py_fp32": ((40 + 60, 30, 5, 0), (32, 0, 1, 0)),
-    "sphere_py_fp64": ((40 + 160, 30 + 150, 4, 0), (110, 100, 2, 0)),
-    "cylinder_quad_fp32": ((60, 40, 4, 0), (27, 0, 1, 0)),
-    "cs_triaxial_iso_fp32": ((40 + 40 + 90, 120, 6, 20), (33, 0, 2, 0)),
-    "cylinder_iso_fp64": ((40 + 40 + 200 + 320, 520, 8, 20), (0, 0, 0, 0)),
-    # per-event sizes: Philox blocks 2 and 3, two Box-Muller normals (log, sqrt, cos in fp64), three sincospi,
-    # sin, j1, the weight
-    "cylinder_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12, 40), (0, 0, 0, 0)),
+    "sphere_fp64": (U(94, wide=1, imad=1, logic=27, fp64=63, xu=2), U(0)),            # one evaluation, in the prologue
+    "sphere_fp32": (U(80, wide=1, imad=1, logic=22, fp64=14, fp32=30, xu=12), U(32.2, logic=1.2, fp32=30, xu=1)),
+    "sphere_py_fp32": (U(121, wide=1, imad=1, logic=22, fp64=14, fp32=69, xu=14), U(32.2, logic=1.2, fp32=30, xu=1)),
+    "sphere_py_fp64": (U(150, logic=30, fp64=110, xu=6), U(72, logic=8, fp64=62, xu=2)),
+    "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(27, logic=1, fp32=25, xu=1)),
+    # Philox block 2 (orientation draws), three sincos of 2 pi u, frame; outer node 43 / inner node 34.5
+    "cs_triaxial_iso_fp32": (U(200 + 16 * 43, wide=19, logic=55 + 16 * 6, fp64=114, fp32=16 * 34, xu=14 + 16), U(34.5, imad=1, logic=2.5, fp32=29, xu=2)),
+    "cylinder_iso_fp64": (U(420, wide=19, logic=70, fp64=310, xu=10), U(0)),
+    # per-event sizes: Philox blocks 2 and 3, two Box-Muller normals, three sincospi, sin, j1, the weight
+    "cylinder_event_fp64": (U(620, wide=38, logic=110, fp64=450, xu=14), U(0)),
     # barbell, per event: the cylinder term and the prologue of the per-event path, then 64 slice evaluations
-    # (square root, fp64 J1, fp64 cos, ~15 multiply-adds: ~95 instructions of which ~30 FP64, from the ncu
-    # instruction and pipe counts of the n2 workload: 491 thread instructions and 143 FP64 per launched neutron)
-    "barbell_event_fp64": ((40 + 80 + 260 + 200 + 320, 780, 12, 40), (95, 30, 2, 0)),
+    "barbell_event_fp64": (U(620, wide=38, logic=110, fp64=450, xu=14), U(70, logic=8, fp64=58, xu=2)),
 }
 
-# DRAM traffic of one trace-kernel launch, dram__bytes_read.sum + dram__bytes_write.sum of the
-# `ncu --set full` captures summarised in profiles/r1_ncu_c<k>.md (bytes per launch; c4: the first of its
-# two launches, the 512 sphere experiments).  The algorithmic traffic is the histograms only.
-NCU_DRAM_BYTES = {
-    "c0_sphere_fp64": 445_696,
-    "c1_polysphere_py": 1_626_880,
-    "c2_oriented_cylinder": 1_683_712,
-    "c3_coreshell_triaxial": 6_359_040,
-    "c4_batch": 351_287_296,
-}
+RESOURCES = ("issue", "imul", "int", "fp64", "xu")
 
 
-def smsp_clocks_per_neutron(frac_survive: float, frac_detect: float, model_key: str, nodes: int,
-                            frac_geometry: float | None = None):
-    """Algorithmic SMSP-clocks per launched neutron (per lane: divide by 32 for per-warp) for each
-    resource; returns dict(issue=, fp64=, xu=, imul=)."""
+def unit_sum(frac_survive, frac_geometry, frac_detect, model_key, nodes, geometry="fast"):
+    """Algorithmic thread-instructions per launched neutron, by class."""
     pro, node = MODEL_COST[model_key]
-    if frac_geometry is None:
-        frac_geometry = frac_survive      # no classifier: every survivor's geometry is evaluated
-    tot = [0.0, 0.0, 0.0, 0.0]
-    for i in range(4):
-        tot[i] = (STAGE_A[i] + frac_survive * STAGE_B0[i] + frac_geometry * STAGE_B[i]
-                  + frac_detect * (pro[i] + nodes * node[i]))
-    return dict(issue=tot[0], fp64=2.0 * tot[1], xu=8.0 * tot[2], imul=4.0 * tot[3])
+    tot = {}
+    for k in STAGE_A:
+        tot[k] = (STAGE_A[k] + frac_survive * STAGE_B0[k] + frac_geometry * STAGE_B[geometry][k]
+                  + frac_detect * (pro[k] + nodes * node[k]))
+    return tot
+
+
+def clocks(tot, r):
+    """SMSP clocks per launched neutron-lane on each resource."""
+    return dict(issue=r["ffma"] * tot["issue"],
+                imul=r["imad_wide"] * tot["wide"] + r["imad"] * tot["imad"],
+                int=r["lop3"] * tot["logic"] + r["wide_int"] * tot["wide"],
+                fp64=r["dfma"] * tot["fp64"],
+                xu=r["mufu"] * tot["xu"])
 
 
 def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, model_key: str, nodes: int,
-             sm_mhz: float = SM_MAX_MHZ, workload: str | None = None, frac_geometry: float | None = None):
-    """Roofline record for bench.py.  `achieved` and `peak` are in G thread-instructions/s on the
-    binding resource (issue slots x 32 lanes: 148 SM x 4 SMSP x 32 lanes x clock)."""
-    c = smsp_clocks_per_neutron(frac_survive, frac_detect, model_key, nodes, frac_geometry)
+             sm_mhz: float = SM_MAX_MHZ, frac_geometry: float | None = None, geometry: str = "fast",
+             rates: dict | None = None, sm_mhz_sampled: float | None = None, traffic=None):
+    """Roofline record for bench.py.  `achieved` and `peak` are G lane-clocks/s on the binding resource
+    (peak = 148 SM x 4 SMSP x 32 lanes x clock: every SMSP clock offers 32 lanes of its binding pipe)."""
+    r = rates or RATES
+    if frac_geometry is None:
+        frac_geometry = frac_survive      # no classifier: every survivor's geometry is evaluated
+    tot = unit_sum(frac_survive, frac_geometry, frac_detect, model_key, nodes, geometry)
+    c = clocks(tot, r)
     pipe = max(c, key=c.get)
-    peak_lane_clocks = N_SM * SMSP_PER_SM * 32 * sm_mhz * 1e6      # lane-clocks per second
+    peak = N_SM * SMSP_PER_SM * 32 * sm_mhz * 1e6
     achieved = neutrons_per_s * c[pipe]
-    # the same path without the classifier shortcut (every survivor's geometry evaluated): what a plain
-    # implementation of DESIGN.md section 3 would have to issue for this throughput
-    plain = smsp_clocks_per_neutron(frac_survive, frac_detect, model_key, nodes, frac_survive)
-    return {
+    c_old = {k: v for k, v in c.items() if k != "int"}
+    out = {
         "bound": "alu", "pipe": pipe,
-        "achieved": achieved / 1e9, "peak": peak_lane_clocks / 1e9, "unit": "G lane-clocks/s",
-        "frac": achieved / peak_lane_clocks,
-        "frac_plain_algorithm": neutrons_per_s * max(plain.values()) / peak_lane_clocks,
+        "achieved": achieved / 1e9, "peak": peak / 1e9, "unit": "G lane-clocks/s",
+        "frac": achieved / peak,
+        # the same throughput against the round-1 resource list (no logic-pipe resource)
+        "frac_without_int_resource": neutrons_per_s * max(c_old.values()) / peak,
         "alg_clocks_per_neutron": {k: round(v, 2) for k, v in c.items()},
-        "peak_source": f"derived: {N_SM} SM x {SMSP_PER_SM} SMSP x 32 lanes x {sm_mhz:.0f} MHz (DESIGN.md s.7)",
-        "traffic": NCU_DRAM_BYTES.get(workload),
+        "alg_instr_per_neutron": {k: round(v, 2) for k, v in tot.items()},
+        "peak_source": (f"{N_SM} SM x {SMSP_PER_SM} SMSP x 32 lanes x {sm_mhz:.0f} MHz (maximum SM clock); clocks per "
+                        f"instruction of each pipe from {r['source']}"),
+        "pipe_clocks_per_warp_instruction": {k: round(float(r[k]), 3) for k in
+                                             ("ffma", "imad", "imad_wide", "lop3", "wide_int", "dfma", "mufu")},
+        "traffic": traffic,
     }
+    if sm_mhz_sampled:
+        out["frac_at_sampled_clock"] = out["frac"] * sm_mhz / sm_mhz_sampled
+        out["sm_mhz_sampled"] = sm_mhz_sampled
+    return out
+
+
+def read_traffic(path: str) -> dict:
+    """DRAM bytes per trace-kernel launch (dram__bytes_read.sum + dram__bytes_write.sum of one `ncu --set full`
+    capture per workload), read from the table of profiles/r2_dram_traffic.md: `| workload | read | written |`."""
+    out = {}
+    try:
+        for line in open(path):
+            cells = [c.strip() for c in line.strip().strip("|").split("|")]
+            if len(cells) >= 3 and cells[1].replace(".", "").isdigit():
+                out[cells[0]] = int(float(cells[1]) + float(cells[2]))
+    except OSError:
+        pass
+    return out

@@ -55,6 +55,7 @@ struct sas_ctx {
   bool own_hist = true;
   unsigned long long* d_counters = nullptr;
   unsigned int* d_work = nullptr;
+  uint32_t work_base = 0;   // fetches of the work counter made by every launch so far (KernelArgs::work_base)
   // experiments grouped by kernel: one launch per non-empty group (ids concatenated on the device).
   // group = variant + N_VARIANTS * (per-event sizes ? 1 : 0) + 2 N_VARIANTS * (fp64 model arithmetic ? 1 : 0)
   std::vector<uint32_t> group_ids[N_GROUPS];
@@ -86,6 +87,13 @@ sas_status fail(sas_ctx* c, sas_status st, const std::string& msg) {
     if (e_ != cudaSuccess)                                                                      \
       return fail(ctx, SAS_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));          \
   } while (0)
+
+__global__ void __launch_bounds__(256) zero_detector_kernel(unsigned long long* p0, unsigned long long* p1,
+                                                            unsigned long long* p2, unsigned long long* counters, size_t n) {
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) { p0[i] = 0ull; p1[i] = 0ull; p2[i] = 0ull; }
+  if (blockIdx.x == 0 && threadIdx.x < 8) counters[threadIdx.x] = 0ull;
+}
 
 // Every call on a context runs on the device the context was created on and leaves the caller's current
 // device as it found it.
@@ -440,6 +448,7 @@ sas_status alloc_common(sas_ctx* c) {
   c->own_hist = true;
   CUDA_TRY(c, cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)));
   CUDA_TRY(c, cudaMalloc(&c->d_work, sizeof(unsigned int)));
+  CUDA_TRY(c, cudaMemset(c->d_work, 0, sizeof(unsigned int)));
   CUDA_TRY(c, cudaMalloc(&c->d_exp_ids, (size_t)c->n_exp * sizeof(uint32_t)));
   CUDA_TRY(c, cudaMalloc(&c->d_exps, (size_t)c->n_exp * sizeof(ExpParams)));
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
@@ -588,10 +597,12 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   const int bps = pl.bps;
   const uint64_t total = (uint64_t)a.n_per_exp * a.n_exp;
   const int grid_full = c->n_sm * bps;
-  // work items: ~16 per resident block, 2048..262144 ids each, multiple of 256 ids
+  // work items: ~16 per resident block, up to 262144 ids each, multiple of 256 ids.  A launch too small for that
+  // (fewer than 16 rows of 32 ids per warp and item) is cut into one item per resident block instead, so that a
+  // 1e6-neutron launch fills the chip evenly with a single static item per block and no work-counter traffic.
   uint64_t item = total / ((uint64_t)grid_full * (uint64_t)SAS_ITEMS_PER_BLOCK);
-  // at least 16 rows of 32 ids per warp and item (a 1e6-neutron launch still fills the chip)
-  item = std::min<uint64_t>(std::max<uint64_t>(item, (uint64_t)SAS_MIN_ITEM / 4 * ROW_WARPS), 262144);
+  if (item < (uint64_t)SAS_MIN_ITEM / 4 * ROW_WARPS) item = std::max<uint64_t>((a.n_per_exp + (uint64_t)grid_full - 1) / grid_full, 256);
+  item = std::min<uint64_t>(item, 262144);
   item = (item + 255) / 256 * 256;
   a.item_ids = (uint32_t)item;
   a.items_per_exp = (uint32_t)(((uint64_t)a.n_per_exp + item - 1) / item);
@@ -600,7 +611,10 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   a.n_items = (uint32_t)n_items;
   a.tab_len_max = c->tab_len_max;
   const int grid = (int)std::min<uint64_t>((uint64_t)grid_full, n_items);
-  CUDA_TRY(c, cudaMemsetAsync(c->d_work, 0, sizeof(unsigned int), c->stream));
+  a.work_base = c->work_base;
+  if (n_items > (uint64_t)grid) c->work_base += (uint32_t)n_items;  // the fetches this launch will make (sas_types.h)
+  a.use_exp0 = (!c->batch && c->n_exp == 1) ? 1 : 0;
+  if (a.use_exp0) a.exp0 = c->h_exps[0];
   const bool timed = !DUMP && c->n_timed < (uint64_t)MAX_TIMED;
   if (timed) {
     if (c->ev0.size() <= c->n_timed) {
@@ -909,10 +923,13 @@ sas_status sas_reset_detector(sas_ctx* c) {
   if (!c) return SAS_EINVAL;
   DeviceGuard g(c);
   const size_t nh = (size_t)c->n_exp * c->npix;
-  CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
-  CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
-  CUDA_TRY(c, cudaMemsetAsync(c->d_counts, 0, nh * sizeof(unsigned long long), c->stream));
-  CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  // one launch for the three histograms and the counters (four memsets cost four stream operations: as much as
+  // the trace kernel itself at 1e6 neutrons)
+  const int grid = (int)std::max<size_t>(1, std::min<size_t>((size_t)c->n_sm * 8, (nh + 255) / 256));
+  zero_detector_kernel<<<grid, 256, 0, c->stream>>>(reinterpret_cast<unsigned long long*>(c->d_sum_p),
+                                                    reinterpret_cast<unsigned long long*>(c->d_sum_p2), c->d_counts,
+                                                    c->d_counters, nh);
+  CUDA_TRY(c, cudaGetLastError());
   c->launched = 0;
   return SAS_OK;
 }

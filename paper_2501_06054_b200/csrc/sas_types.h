@@ -89,7 +89,14 @@ struct KernelArgs {
   uint32_t n_items;
   int32_t npix;
   int32_t tab_len_max;     // Reals of table space in shared memory
+  // Work items: block b starts with item b (grid <= n_items); further items are gridDim.x + (fetch - work_base),
+  // fetch = atomicAdd(work_counter, 1).  A launch with n_items > grid makes exactly n_items fetches (n_items - grid
+  // that succeed, one failing one per block), one with n_items <= grid makes none: the host advances work_base by
+  // that number after every launch, so the counter is never reset between launches.
+  uint32_t work_base;
+  int32_t use_exp0;        // single-experiment context: the parameter block travels with the kernel arguments
   PhiloxKeys keys;
+  ExpParams exp0;          // (no dependent global loads before the first neutron of a small launch)
 };
 
 }  // namespace sas

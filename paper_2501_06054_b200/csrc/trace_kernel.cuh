@@ -112,18 +112,23 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
   for (int f = 0; f < 7; ++f) wq.oc[f][lane] = 0;
 
   int cur_exp = -1;
-  bool replay = false;
-  unsigned item = 0;
+  bool replay = false, first = true;
+  unsigned item = blockIdx.x;  // the first item of a block is its own index (the host launches grid <= n_items)
 
   for (;;) {
-    if (!replay) {
-      __syncthreads();  // everyone is done with s_item and with the staged experiment of the last pass
-      if (threadIdx.x == 0) s_item = atomicAdd(a.work_counter, 1u);
-      __syncthreads();
-      item = s_item;
+    if (!replay && !first) {
+      if (a.n_items <= gridDim.x) {
+        item = a.n_items;      // every block had its one item: nothing to fetch
+      } else {
+        __syncthreads();  // everyone is done with s_item and with the staged experiment of the last pass
+        if (threadIdx.x == 0) s_item = gridDim.x + (atomicAdd(a.work_counter, 1u) - a.work_base);
+        __syncthreads();
+        item = s_item;
+      }
     }
+    first = false;
     const bool have = item < a.n_items;
-    const int e = have ? (int)a.exp_ids[item / a.items_per_exp] : -1;
+    const int e = have ? (a.use_exp0 ? a.exp0.exp_index : (int)a.exp_ids[item / a.items_per_exp]) : -1;
     const bool drain = (e != cur_exp) && (cur_exp >= 0) && !replay;
     uint32_t row = 0, row_end = 0, off0 = 0, cnt_ids = 0;
     if (drain) {
@@ -134,7 +139,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
       if (e != cur_exp) {
         // stage the experiment: parameters and tables (fp64 in HBM -> Real in shared memory)
         __syncthreads();  // every warp has drained the previous experiment
-        const ExpParams* src = a.exps + e;
+        const ExpParams* src = a.use_exp0 ? &a.exp0 : a.exps + e;   // kernel arguments or HBM
         const uint32_t* s32 = reinterpret_cast<const uint32_t*>(src);
         uint32_t* d32 = reinterpret_cast<uint32_t*>(&P);
         for (int i = threadIdx.x; i < (int)(sizeof(ExpParams) / 4); i += BLOCK_THREADS) d32[i] = s32[i];

@@ -194,13 +194,10 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     mbar_init(&pr.empty[threadIdx.x % WS_G], 1);
   }
   if (threadIdx.x < WS_PAIRS) S.prod[threadIdx.x].ticket = 0u;
-  if (threadIdx.x == 0) S.item[0] = atomicAdd(a.work_counter, 1u);
-  __syncthreads();
-  unsigned item = S.item[0];
-  if (item >= a.n_items) return;  // nothing for this block (the whole block leaves together)
-  int cur_exp = (int)a.exp_ids[item / a.items_per_exp];
+  unsigned item = blockIdx.x;    // the first item of a block is its own index (the host launches grid <= n_items)
+  int cur_exp = a.use_exp0 ? a.exp0.exp_index : (int)a.exp_ids[item / a.items_per_exp];
   auto stage_experiment = [&](int e, int tid, int nthr) {
-    const ExpParams* src = a.exps + e;
+    const ExpParams* src = a.use_exp0 ? &a.exp0 : a.exps + e;   // kernel arguments or HBM
     const uint32_t* s32 = reinterpret_cast<const uint32_t*>(src);
     uint32_t* d32 = reinterpret_cast<uint32_t*>(&P);
     for (int i = tid; i < (int)(sizeof(ExpParams) / 4); i += nthr) d32[i] = s32[i];
@@ -326,10 +323,14 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
       }
       // ---------------- next item
       it += 1;
-      if (threadIdx.x == PROD_T0) S.item[it & 1] = atomicAdd(a.work_counter, 1u);
-      bar_producers();
-      item = S.item[it & 1];
-      const int e = item < a.n_items ? (int)a.exp_ids[item / a.items_per_exp] : -1;
+      if (a.n_items <= gridDim.x) {
+        item = a.n_items;        // every block had its one item: nothing to fetch
+      } else {
+        if (threadIdx.x == PROD_T0) S.item[it & 1] = gridDim.x + (atomicAdd(a.work_counter, 1u) - a.work_base);
+        bar_producers();
+        item = S.item[it & 1];
+      }
+      const int e = item < a.n_items ? (a.use_exp0 ? a.exp0.exp_index : (int)a.exp_ids[item / a.items_per_exp]) : -1;
       if (e != cur_exp) {
         // experiment switch or end of work: empty the stack, then every consumer of this producer gets a
         // flagged chunk (the partial one first, empty ones for the others) and the block meets at a barrier

@@ -33,7 +33,7 @@ _SAMPLE = {"box": 0, "cyl_y": 1}
 _MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3,
           "core_shell_triaxial": 4, "flat": 5, "parallelepiped": 6, "core_shell_cylinder": 7, "ellipsoid": 8,
           "barbell": 9, "capped_cylinder": 10, "elliptical_cylinder": 11, "hollow_cylinder": 12,
-          "core_shell_ellipsoid": 13}
+          "core_shell_ellipsoid": 13, "polymer_micelle": 14}
 _ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
 _SQ = {"none": 0, "hard_sphere_py": 1}
 
@@ -96,6 +96,11 @@ def lib():
         for f in (L.orc_sphere_phi, L.orc_sinc, L.orc_lambda1):
             f.argtypes = [C.c_double]
             f.restype = C.c_double
+        for f in (L.orc_debye, L.orc_chain_psi):
+            f.argtypes = [C.c_double]
+            f.restype = C.c_double
+        L.orc_micelle_f2.argtypes = [C.POINTER(Model), C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_micelle_f2.restype = C.c_double
         L.orc_py_sq.argtypes = [C.c_double] * 3
         L.orc_py_sq.restype = C.c_double
         L.orc_intensity.argtypes = [C.POINTER(Model), C.POINTER(C.c_double), C.POINTER(C.c_double),
@@ -244,6 +249,22 @@ def amplitude(model_d: dict, qa, qb, qc, x0=1.0, x1=1.0):
     vol, env = C.c_double(), C.c_double()
     F = lib().orc_amplitude(C.byref(m), qa, qb, qc, x0, x1, C.byref(vol), C.byref(env))
     return F, vol.value
+
+
+def micelle_f2(model_d: dict, q: float, x0: float = 1.0):
+    """(|F|^2, normalising volume) of the polymer micelle (DESIGN.md R-M4)."""
+    m = model_d if isinstance(model_d, Model) else make_model(model_d)
+    vol, env2 = C.c_double(), C.c_double()
+    f2 = lib().orc_micelle_f2(C.byref(m), float(q), float(x0), C.byref(vol), C.byref(env2))
+    return f2, vol.value
+
+
+def debye(x: float) -> float:
+    return lib().orc_debye(float(x))
+
+
+def chain_psi(x: float) -> float:
+    return lib().orc_chain_psi(float(x))
 
 
 def trace_one(ins_d, model_d, seed: int, nid: int, exp_index: int = 0) -> Record:

@@ -335,6 +335,58 @@ double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double
   }
 }
 
+/* R-M4: Gaussian chain of gyration radius R_g, x = (q R_g)^2.  The chain is a continuous random walk of contour
+ * length 1 whose points s, s' are separated by a Gaussian of variance proportional to |s - s'|:
+ * <exp(i q (r_s - r_s'))> = exp(-x |s - s'|).  Debye function = double average over s, s' in [0, 1];
+ * psi = single average over s of exp(-x s) (amplitude seen from the attached end).  Series below x = 0.1, where
+ * the closed forms cancel (2 ulp / x^2): D = sum_k 2 (-x)^k / (k + 2)!, psi = sum_k (-x)^k / (k + 1)!. */
+double orc_debye(double x) {
+  if (x < 0.1) {
+    double sum = 0.0, term = 1.0;             /* term = (-x)^k / (k + 2)! * 2, starting at k = 0: 2 / 2! = 1 */
+    for (int k = 0; k < 12; ++k) {
+      sum += term;
+      term *= -x / (double)(k + 3);
+    }
+    return sum;
+  }
+  return 2.0 * ((exp(-x) - 1.0) + x) / (x * x);
+}
+double orc_chain_psi(double x) {
+  if (x < 0.1) {
+    double sum = 0.0, term = 1.0;             /* term = (-x)^k / (k + 1)! */
+    for (int k = 0; k < 12; ++k) {
+      sum += term;
+      term *= -x / (double)(k + 2);
+    }
+    return sum;
+  }
+  return (1.0 - exp(-x)) / x;
+}
+
+/* R-M4 (Pedersen & Gerstenberg 1996): core of radius R = size[0] x0 and excess scattering length
+ * B_s = sld[0] V_core; N = size[3] chains of gyration radius R_g = size[1], volume V_c = size[2] and excess
+ * scattering length b_c = sld[1] V_c each, starting at radius R + d R_g with d = 1, mutually independent and
+ * uniformly distributed over the surface:
+ *   |F|^2 = B_s^2 Phi(qR)^2 + N b_c^2 D(x) + N (N - 1) b_c^2 [psi(x) sinc(q(R + R_g))]^2
+ *           + 2 N B_s b_c Phi(qR) psi(x) sinc(q(R + R_g)),        x = (q R_g)^2.
+ * Normalising volume: V_core + N V_c. */
+double orc_micelle_f2(const orc_model* m, double q, double x0, double* vol, double* env2) {
+  double R = m->size[0] * x0, Rg = m->size[1], Vc = m->size[2], N = m->size[3];
+  double Vcore = FOUR_PI_3 * ((R * R) * R);
+  double Bs = m->sld[0] * Vcore, bc = m->sld[1] * Vc;
+  double x = (q * Rg) * (q * Rg);
+  double phi = orc_sphere_phi(q * R);
+  double ps = orc_chain_psi(x) * orc_sinc(q * (R + Rg));
+  double self_core = (Bs * Bs) * (phi * phi);
+  double self_chain = (N * (bc * bc)) * orc_debye(x);
+  double chain_chain = ((N * (N - 1.0)) * (bc * bc)) * (ps * ps);
+  double cross = ((2.0 * N) * (Bs * bc)) * (phi * ps);
+  *vol = Vcore + N * Vc;
+  double e = fabs(Bs) + N * fabs(bc);
+  *env2 = e * e;
+  return ((self_core + self_chain) + chain_chain) + cross;
+}
+
 /* particle frame from (theta, phi, psi): R-A7 */
 static void frame_from_angles(double st, double ct, double sp, double cp, double ss, double cs,
                               double A[3], double B[3], double C[3]) {
@@ -391,7 +443,8 @@ double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3]
   for (int a = 0; a < m->n_pd[0]; ++a)
     for (int b = 0; b < m->n_pd[1]; ++b) {
       double V, E;
-      (void)orc_amplitude(m, 0.0, 0.0, 0.0, m->pd_x[0][a], m->pd_x[1][b], &V, &E);
+      if (m->model == ORC_POLYMER_MICELLE) (void)orc_micelle_f2(m, 0.0, m->pd_x[0][a], &V, &E);
+      else (void)orc_amplitude(m, 0.0, 0.0, 0.0, m->pd_x[0][a], m->pd_x[1][b], &V, &E);
       SV += (m->pd_w[0][a] * m->pd_w[1][b]) * V;
     }
   for (int i = 0; i < n_th; ++i)
@@ -410,11 +463,17 @@ double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3]
       }
       for (int a = 0; a < m->n_pd[0]; ++a)
         for (int b = 0; b < m->n_pd[1]; ++b) {
-          double V, E;
-          double F = orc_amplitude(m, qa, qb, qc, m->pd_x[0][a], m->pd_x[1][b], &V, &E);
+          double V, E, F2, E2;
+          if (m->model == ORC_POLYMER_MICELLE) {
+            F2 = orc_micelle_f2(m, qm, m->pd_x[0][a], &V, &E2);   /* isotropic: |Q| only */
+          } else {
+            double F = orc_amplitude(m, qa, qb, qc, m->pd_x[0][a], m->pd_x[1][b], &V, &E);
+            F2 = F * F;
+            E2 = E * E;
+          }
           double w = w_or * (m->pd_w[0][a] * m->pd_w[1][b]);
-          SF2 += w * (F * F);
-          SE2 += w * (E * E);
+          SF2 += w * F2;
+          SE2 += w * E2;
         }
     }
   double S = 1.0;
@@ -435,12 +494,18 @@ double orc_intensity_event(const orc_model* m, const double Q[3], const double u
   particle_frame(m, u_or, A, B, C);
   double qA = dot3(Q, A), qB = dot3(Q, B), qC = dot3(Q, C);
   double qm = sqrt(dot3(Q, Q));
-  double V, E;
-  double F = orc_amplitude(m, qA, qB, qC, x[0], x[1], &V, &E);
+  double V, E, F2, E2;
+  if (m->model == ORC_POLYMER_MICELLE) {
+    F2 = orc_micelle_f2(m, qm, x[0], &V, &E2);
+  } else {
+    double F = orc_amplitude(m, qA, qB, qC, x[0], x[1], &V, &E);
+    F2 = F * F;
+    E2 = E * E;
+  }
   double S = 1.0;
   if (m->sq_kind == ORC_SQ_HARD_SPHERE_PY) S = orc_py_sq(qm, m->sq_radius_eff, m->sq_volfrac);
-  if (env_out) *env_out = ((1.0e8 * m->scale) * ((E * E) / V)) * S + m->background;
-  return ((1.0e8 * m->scale) * ((F * F) / V)) * S + m->background;
+  if (env_out) *env_out = ((1.0e8 * m->scale) * (E2 / V)) * S + m->background;
+  return ((1.0e8 * m->scale) * (F2 / V)) * S + m->background;
 }
 
 /* R-N1 (Eq. 8): r = mean (1 + rel z), z standard normal by Box-Muller from the two

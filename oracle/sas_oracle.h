@@ -53,7 +53,11 @@ enum {
   /* three more bodies of Table I, each Eq. 1 over the body (R-M3) */
   ORC_ELLIPTICAL_CYLINDER = 11, /* group B: cross-section semi-axes a (along A), b (along B), length L along C */
   ORC_HOLLOW_CYLINDER = 12,     /* group A: tube, hollow core radius R, wall thickness t, length L */
-  ORC_CORE_SHELL_ELLIPSOID = 13 /* group B: core of revolution (R_e, R_p) in a shell of thickness t */
+  ORC_CORE_SHELL_ELLIPSOID = 13, /* group B: core of revolution (R_e, R_p) in a shell of thickness t */
+  /* one of the models the paper found expensive (Table II group F "Polymer micelle"): a homogeneous
+   * spherical core with N Gaussian chains attached to its surface (Pedersen & Gerstenberg, Macromolecules 29
+   * (1996) 1363; DESIGN.md R-M4).  size = R_core, R_g, V_chain (A^3), N; sld[0] core, sld[1] chain */
+  ORC_POLYMER_MICELLE = 14
 };
 enum {
   ORC_ORIENT_FIXED = 0,
@@ -131,6 +135,13 @@ typedef struct {
 /* Philox4x32-10, Salmon et al. SC'11 (DESIGN.md R-B). */
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 double orc_uniform(uint32_t word);
+
+/* R-M4 pieces: Debye function of a Gaussian chain D(x) = 2 (exp(-x) - 1 + x) / x^2, its amplitude relative to a
+ * chain end psi(x) = (1 - exp(-x)) / x, x = (q R_g)^2, and the micelle's |F|^2 (not a perfect square: the chains'
+ * self term is the Debye function); *vol = V_core + N V_chain, *env2 = the same with every shape factor 1 */
+double orc_debye(double x);
+double orc_chain_psi(double x);
+double orc_micelle_f2(const orc_model* m, double q, double x0, double* vol, double* env2);
 
 /* form / structure factor pieces (PAPER.md:37-49 Eq.1-4, :161-163 Eq.9) */
 double orc_sphere_phi(double u);                 /* 3(sin u - u cos u)/u^3 */

@@ -41,7 +41,8 @@ HEADLINE = 2                      # BASELINE.json configs[2]
 SECONDARY = [("c0_sphere_fp64", 0, None, None), ("c0_sphere_fp64_1e9", 0, None, 10**9),
              ("c1_polysphere_py_fp32", 1, "fp32", None), ("c1_polysphere_py_fp64", 1, "fp64", None),
              ("c3_coreshell_triaxial", 3, None, None), ("c4_batch", 4, None, None),
-             ("n1_paper_cylinder", 5, None, None), ("n2_paper_barbell", 6, None, None)]
+             ("n1_paper_cylinder", 5, None, None), ("n2_paper_barbell", 6, None, None),
+             ("n3_paper_micelle", 7, None, None)]
 
 
 # ------------------------------------------------------------------ reference arm: the CPU oracle
@@ -129,6 +130,8 @@ def model_key_and_nodes(model):
         return "cylinder_event_fp64", 0
     if is_event_model(model) and m == "barbell":
         return "barbell_event_fp64", 64
+    if m == "polymer_micelle":
+        return "micelle_event_fp64", 0
     if m == "sphere":
         nodes = pd[0]
         if nodes == 1:

@@ -73,7 +73,12 @@ enum {
   /* three more bodies of Table I (DESIGN.md R-M3) */
   SAS_ELLIPTICAL_CYLINDER = 11,  /* size = a (along A), b (along B), L (along C); pd[0] scales a and b, pd[1] on L */
   SAS_HOLLOW_CYLINDER = 12,      /* size = hollow core radius R, L, wall thickness t; pd[0] on R, pd[1] on L */
-  SAS_CORE_SHELL_ELLIPSOID = 13  /* size = R_e, R_p, t; sld[0] core, sld[1] shell; pd[0] on R_e, pd[1] on R_p */
+  SAS_CORE_SHELL_ELLIPSOID = 13, /* size = R_e, R_p, t; sld[0] core, sld[1] shell; pd[0] on R_e, pd[1] on R_p */
+  /* polymer micelle (PAPER.md:201 and Table II group F name it among the expensive models; DESIGN.md R-M4:
+   * Pedersen & Gerstenberg, Macromolecules 29 (1996) 1363): homogeneous spherical core with N Gaussian chains
+   * starting at R_core + R_g.  size = R_core, R_g, V_chain (A^3), N (0 or >= 1); sld[0] core, sld[1] chain
+   * contrast; normalising volume V_core + N V_chain; pd[0] on R_core; isotropic (orientation is ignored) */
+  SAS_POLYMER_MICELLE = 14
 };
 enum {
   SAS_ORIENT_FIXED = 0,

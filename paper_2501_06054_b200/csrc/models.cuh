@@ -219,6 +219,51 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
   return F;
 }
 
+// R-M4, polymer micelle (Pedersen & Gerstenberg 1996): x = (q R_g)^2; Debye function D = 2 (e^-x - 1 + x) / x^2 and
+// end-attached chain amplitude psi = (1 - e^-x) / x through expm1 (no cancellation at small x: with
+// e = expm1(-x), psi = -e / x and D = 2 (e + x) / x^2 = 2 (1 - psi) / x, the latter by its series below x = 0.1).
+__device__ __forceinline__ void chain_terms(double x, double& D, double& psi) {
+  if (x < 0.1) {
+    // sum_k (-x)^k / (k + 1)! and sum_k 2 (-x)^k / (k + 2)!, twelve terms: below 1e-19 at x = 0.1
+    double sp = 0.0, sd = 0.0, tp = 1.0, td = 1.0;
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+      sp += tp; sd += td;
+      tp *= -x / (double)(k + 2);
+      td *= -x / (double)(k + 3);
+    }
+    psi = sp; D = sd;
+    return;
+  }
+  const double e = expm1(-x);
+  psi = -e / x;
+  D = (2.0 * (e + x)) / (x * x);
+}
+// |F|^2 of one micelle with core radius msize[0] x0 (not a perfect square: the chains' self term is the Debye
+// function) and its normalising volume V_core + N V_chain
+__device__ __forceinline__ double micelle_f2(const ExpParams& P, double q, double x0, double& Vol) {
+  const double FOUR_PI_3 = 4.1887902047863905;
+  const double R = P.msize[0] * x0, Rg = P.msize[1], Vc = P.msize[2], N = P.msize[3];
+  const double Vcore = FOUR_PI_3 * ((R * R) * R);
+  const double Bs = P.ev_sld[0] * Vcore, bc = P.ev_sld[1] * Vc;
+  const double qg = q * Rg;
+  double D, psi;
+  chain_terms(qg * qg, D, psi);
+  const double phi = sphere_phi(q * R);
+  const double ps = psi * sinc_r(q * (R + Rg));
+  Vol = fma(N, Vc, Vcore);
+  const double bb = bc * bc;
+  return fma((2.0 * N) * (Bs * bc), phi * ps, fma((N * (N - 1.0)) * bb, ps * ps, fma(N * bb, D, (Bs * Bs) * (phi * phi))));
+}
+// |F|^2 and volume of any variant
+template <int V>
+__device__ __forceinline__ double particle_f2(const ExpParams& P, double q, double qA, double qB, double qC, double x0,
+                                              double x1, double& Vol) {
+  if (V == V_MICELLE) return micelle_f2(P, q, x0, Vol);
+  const double F = particle_amplitude<V>(P, q, qA, qB, qC, x0, x1, Vol);
+  return F * F;
+}
+
 // R-N2: the paper's per-event model, Eq. 4 with the sizes of THIS scattering event:
 // I = 1e8 scale F(r)^2 / V(r) S(q) + background, one fp64 evaluation per detected neutron.
 // (compiled into kernels of its own, trace_kernel<double, V, true>: in the same kernel as the fixed-node
@@ -231,7 +276,7 @@ __device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const
   const double x1 = P.pd_mc[1] ? draw_rel_size(keys, id_lo, id_hi, exp_word, 1, P.pd_rel[1]) : 1.0;
   const double q = sqrt(fma(Qx, Qx, fma(Qy, Qy, Qz * Qz)));
   double qA = 0, qB = 0, qC = 0;
-  if (V >= 2) {
+  if (V >= 2 && V != V_MICELLE) {
     double A[3], B[3], C[3];
     particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
     qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
@@ -239,10 +284,10 @@ __device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const
     qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
   }
   double Vol;
-  const double F = particle_amplitude<V>(P, q, qA, qB, qC, x0, x1, Vol);
+  const double F2 = particle_f2<V>(P, q, qA, qB, qC, x0, x1, Vol);
   double S = 1.0;
   if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
-  return fma((P.ev_scale * ((F * F) / Vol)), S, P.background);
+  return fma((P.ev_scale * (F2 / Vol)), S, P.background);
 }
 
 // Fixed-node average of the NEXT-2 models: the plain double sum over the (a, b) nodes of F^2, in fp64
@@ -254,18 +299,21 @@ __device__ __forceinline__ double eval_intensity_generic(const ExpParams& P, con
   const Real* ta = tab_base;
   const Real* tb = ta + P.n_a * TA_W;
   const double q = sqrt(fma(Qx, Qx, fma(Qy, Qy, Qz * Qz)));
-  double A[3], B[3], C[3];
-  particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
-  const double qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
-  const double qB = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
-  const double qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
+  double qA = 0, qB = 0, qC = 0;
+  if (V != V_MICELLE) {   // the micelle is isotropic: |Q| only
+    double A[3], B[3], C[3];
+    particle_frame<true, V>(P, keys, id_lo, id_hi, exp_word, A, B, C);
+    qA = fma(Qx, A[0], fma(Qy, A[1], Qz * A[2]));
+    qB = fma(Qx, B[0], fma(Qy, B[1], Qz * B[2]));
+    qC = fma(Qx, C[0], fma(Qy, C[1], Qz * C[2]));
+  }
   double acc = 0.0;
   for (int a = 0; a < P.n_a; ++a) {
     double inner = 0.0;
     for (int b = 0; b < P.n_b; ++b) {
       double Vol;
-      const double F = particle_amplitude<V>(P, q, qA, qB, qC, (double)ta[a * TA_W], (double)tb[b * TB_W], Vol);
-      inner = fma((double)tb[b * TB_W + 2], F * F, inner);
+      const double F2 = particle_f2<V>(P, q, qA, qB, qC, (double)ta[a * TA_W], (double)tb[b * TB_W], Vol);
+      inner = fma((double)tb[b * TB_W + 2], F2, inner);
     }
     acc = fma((double)ta[a * TA_W + 2], inner, acc);
   }

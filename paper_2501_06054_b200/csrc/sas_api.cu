@@ -131,19 +131,21 @@ sas_status validate_instrument(const sas_instrument_desc* d, std::string& why) {
 sas_status validate_model(const sas_model_desc* m, std::string& why) {
   if (!m) { why = "model descriptor is NULL"; return SAS_EINVAL; }
   if (m->struct_size != sizeof(sas_model_desc)) { why = "sas_model_desc.struct_size mismatch"; return SAS_EINVAL; }
-  if (m->model < SAS_SPHERE || m->model > SAS_CORE_SHELL_ELLIPSOID) { why = "unknown model"; return SAS_EINVAL; }
+  if (m->model < SAS_SPHERE || m->model > SAS_POLYMER_MICELLE) { why = "unknown model"; return SAS_EINVAL; }
   if (m->precision != SAS_FP32 && m->precision != SAS_FP64) { why = "unknown precision"; return SAS_EINVAL; }
   if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_UNIFORM_ANGLES_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
   if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY) { why = "unknown sq_kind"; return SAS_EINVAL; }
   if (!std::isfinite(m->scale) || !std::isfinite(m->background)) { why = "scale/background not finite"; return SAS_EINVAL; }
-  static const int n_sizes[14] = {1, 2, 2, 3, 4, 0, 3, 3, 2, 3, 3, 3, 3, 3};
-  static const int n_pd[14] = {1, 2, 2, 1, 2, 0, 1, 2, 2, 2, 2, 2, 2, 2};
+  static const int n_sizes[15] = {1, 2, 2, 3, 4, 0, 3, 3, 2, 3, 3, 3, 3, 3, 4};
+  static const int n_pd[15] = {1, 2, 2, 1, 2, 0, 1, 2, 2, 2, 2, 2, 2, 2, 1};
   for (int i = 0; i < n_sizes[m->model]; ++i) {
     // a shell thickness may be 0, every other size must be > 0
     const bool may_be_zero = (m->model == SAS_CORE_SHELL_SPHERE && i == 1) || (m->model == SAS_CORE_SHELL_TRIAXIAL && i == 3) ||
-                             (m->model == SAS_CORE_SHELL_CYLINDER && i == 2) || (m->model == SAS_CORE_SHELL_ELLIPSOID && i == 2);
+                             (m->model == SAS_CORE_SHELL_CYLINDER && i == 2) || (m->model == SAS_CORE_SHELL_ELLIPSOID && i == 2) ||
+                             (m->model == SAS_POLYMER_MICELLE && i >= 1);
     if (!std::isfinite(m->size[i]) || m->size[i] < 0.0 || (!may_be_zero && m->size[i] == 0.0)) { why = "model sizes must be > 0"; return SAS_EINVAL; }
   }
+  if (m->model == SAS_POLYMER_MICELLE && m->size[3] != 0.0 && !(m->size[3] >= 1.0)) { why = "a micelle has 0 or >= 1 chains"; return SAS_EINVAL; }
   if ((m->model == SAS_BARBELL || m->model == SAS_CAPPED_CYLINDER) && !(m->size[2] >= m->size[0])) { why = "the end-piece radius must be >= the cylinder radius"; return SAS_EINVAL; }
   for (int k = 0; k < 2; ++k) {
     if (m->pd_kind[k] != SAS_PD_NONE && m->pd_kind[k] != SAS_PD_SCHULZ_QUAD && m->pd_kind[k] != SAS_PD_GAUSS_MC) { why = "unknown pd_kind"; return SAS_EINVAL; }
@@ -335,6 +337,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
           const double Ret = m.size[0] * xa[a] + m.size[2], Rpt = m.size[1] * xb[b] + m.size[2];
           V = FOUR_PI_3 * Ret * Ret * Rpt;
         } break;
+        case SAS_POLYMER_MICELLE: { const double R = m.size[0] * xa[a]; V = FOUR_PI_3 * R * R * R + m.size[3] * m.size[2]; } break;
         case SAS_BARBELL: case SAS_CAPPED_CYLINDER: {
           // cylinder + two sphere pieces z in [L/2, zc + Rb] (R-M2)
           const double R = m.size[0] * xa[a], L = m.size[1] * xb[b], Rb = m.size[2];
@@ -363,7 +366,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
       case SAS_CORE_SHELL_TRIAXIAL: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
       // NEXT-2 models: the node value and its weight; the kernel forms the amplitude itself (models.cuh)
       case SAS_PARALLELEPIPED: case SAS_CORE_SHELL_CYLINDER: case SAS_ELLIPSOID: case SAS_BARBELL: case SAS_CAPPED_CYLINDER:
-      case SAS_ELLIPTICAL_CYLINDER: case SAS_HOLLOW_CYLINDER: case SAS_CORE_SHELL_ELLIPSOID:
+      case SAS_ELLIPTICAL_CYLINDER: case SAS_HOLLOW_CYLINDER: case SAS_CORE_SHELL_ELLIPSOID: case SAS_POLYMER_MICELLE:
         r[0] = xa[a]; r[2] = wa[a]; break;
       default: break;
     }
@@ -374,7 +377,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
       case SAS_CYLINDER: { const double L = m.size[1] * xb[b]; split(0.5 * L, r); r[2] = wb[b] * L * L; } break;
       case SAS_CORE_SHELL_TRIAXIAL: { const double t = m.size[3] * xb[b]; r[0] = t; r[1] = wb[b]; r[2] = t * t; } break;
       case SAS_PARALLELEPIPED: case SAS_CORE_SHELL_CYLINDER: case SAS_ELLIPSOID: case SAS_BARBELL: case SAS_CAPPED_CYLINDER:
-      case SAS_ELLIPTICAL_CYLINDER: case SAS_HOLLOW_CYLINDER: case SAS_CORE_SHELL_ELLIPSOID:
+      case SAS_ELLIPTICAL_CYLINDER: case SAS_HOLLOW_CYLINDER: case SAS_CORE_SHELL_ELLIPSOID: case SAS_POLYMER_MICELLE:
         r[0] = xb[b]; r[2] = wb[b]; break;
       default: r[1] = wb[b]; break;
     }
@@ -664,6 +667,7 @@ sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v, int g) {
     case V_ELL_CYL: return launch<double, V_ELL_CYL, EV>(c, a);
     case V_HOLLOW_CYL: return launch<double, V_HOLLOW_CYL, EV>(c, a);
     case V_CS_ELL: return launch<double, V_CS_ELL, EV>(c, a);
+    case V_MICELLE: return launch<double, V_MICELLE, EV>(c, a);
     default: return fail(c, SAS_EINVAL, "unknown kernel variant");
   }
 }

@@ -83,6 +83,8 @@ MODEL_COST = {
     "cylinder_event_fp64": (U(620, wide=38, logic=110, fp64=450, xu=14), U(0)),
     # barbell, per event: the cylinder term and the prologue of the per-event path, then 64 slice evaluations
     "barbell_event_fp64": (U(620, wide=38, logic=110, fp64=450, xu=14), U(70, logic=8, fp64=58, xu=2)),
+    # micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms (estimate)
+    "micelle_event_fp64": (U(330, wide=19, logic=60, fp64=230, xu=8), U(0)),
 }
 
 RESOURCES = ("issue", "imul", "int", "fp64", "xu")

@@ -56,7 +56,7 @@ def model(**over):
 
 
 def config(i: int, precision: str | None = None):
-    """Return dict(name, instrument, model, n_neutrons, seed) for config i in 0..3 and 5,
+    """Return dict(name, instrument, model, n_neutrons, seed) for config i in 0..3 and 5..7,
     or dict(name, instruments[], models[], n_neutrons_each, seed) for config 4."""
     if i == 0:
         return dict(name="c0_sphere_fp64", instrument=instrument(),
@@ -110,6 +110,14 @@ def config(i: int, precision: str | None = None):
             model=model(model="barbell", precision="fp64", size=[20.0, 400.0, 40.0, 0],
                         pd_kind=["gauss_mc", "gauss_mc"], pd_rel=[0.05, 0.05], orient_kind="uniform_angles_mc"),
             n_neutrons=10**9, seed=20250112)
+    if i == 7:
+        # NEXT-2 (not a BASELINE.json config): the polymer micelle, another model PAPER.md:201 singles out, with the
+        # paper's per-event Gaussian core radius (DESIGN.md R-M4, R-N1)
+        return dict(
+            name="n3_paper_micelle", instrument=instrument(det_nx=256, det_ny=256),
+            model=model(model="polymer_micelle", precision="fp64", size=[40.0, 15.0, 4000.0, 30.0],
+                        sld=[2.0e-6, 1.0e-6, 0.0], pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0.0]),
+            n_neutrons=10**9, seed=20250113)
     raise ValueError(i)
 
 

@@ -428,6 +428,13 @@ MORE_MODELS = [
     ("core_shell_ellipsoid_iso", dict(model="core_shell_ellipsoid", size=[30.0, 70.0, 8.0, 0], sld=[3e-6, 1e-6, 0],
                                       orient_kind="isotropic_mc", pd_kind=["schulz", "none"], pd_rel=[0.15, 0],
                                       pd_nodes=[9, 1])),
+    # polymer micelle (R-M4): monodisperse, Schulz core radii with a hard-sphere S(q), the paper's per-event sizes
+    ("micelle_mono", dict(model="polymer_micelle", size=[40.0, 15.0, 4000.0, 30.0], sld=[2e-6, 1e-6, 0])),
+    ("micelle_pd_py", dict(model="polymer_micelle", size=[40.0, 15.0, 4000.0, 30.0], sld=[2e-6, -1e-6, 0],
+                           pd_kind=["schulz", "none"], pd_rel=[0.12, 0], pd_nodes=[12, 1], sq_kind="hard_sphere_py",
+                           sq_radius_eff=60.0, sq_volfrac=0.1, background=0.005)),
+    ("micelle_paper", dict(model="polymer_micelle", size=[40.0, 15.0, 4000.0, 30.0], sld=[2e-6, 1e-6, 0],
+                           pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0])),
 ]
 
 

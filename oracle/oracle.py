@@ -30,6 +30,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 MAX_NODES = 64
 
 _SAMPLE = {"box": 0, "cyl_y": 1}
+_LAMBDA = {"uniform": 0, "triangle": 1}
 _MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3,
           "core_shell_triaxial": 4, "flat": 5, "parallelepiped": 6, "core_shell_cylinder": 7, "ellipsoid": 8,
           "barbell": 9, "capped_cylinder": 10, "elliptical_cylinder": 11, "hollow_cylinder": 12,
@@ -43,7 +44,7 @@ class Instrument(C.Structure):
                 ("src_xw", "src_yh", "lambda_min", "lambda_max", "flux",
                  "slit1_z", "slit1_xw", "slit1_yh", "slit2_z", "slit2_xw", "slit2_yh",
                  "focus_z", "focus_xw", "focus_yh")] + \
-               [("sample_shape", C.c_int32), ("pad0", C.c_int32)] + \
+               [("sample_shape", C.c_int32), ("lambda_dist", C.c_int32)] + \
                [(n, C.c_double) for n in
                 ("sample_z", "sample_xw", "sample_yh", "sample_zd", "sample_radius",
                  "mu_abs_2200", "mu_inc", "q_min", "q_max", "det_dist", "det_xw", "det_yh")] + \
@@ -155,7 +156,8 @@ def gauss_tilts(sigma: float, n: int):
 def make_instrument(d: dict) -> Instrument:
     ins = Instrument()
     for name, _ in Instrument._fields_:
-        if name == "pad0":
+        if name == "lambda_dist":
+            ins.lambda_dist = _LAMBDA[d.get(name, "uniform")]
             continue
         if name == "sample_shape":
             ins.sample_shape = _SAMPLE[d[name]]

@@ -607,7 +607,12 @@ void orc_trace_one(const orc_instrument* ins, const orc_model* m, uint64_t seed,
   }
 
   draw_block(seed, id, 1, exp_index, u + 4);
-  double lambda = ins->lambda_min + u[4] * dlam;
+  /* R-L1: position t in [0, 1] of the wavelength inside the band: t = u4 (uniform), or the inverse distribution
+   * function of the symmetric triangle, 2 t^2 below the centre and 1 - 2 (1 - t)^2 above it */
+  double t_lam = u[4];
+  if (ins->lambda_dist == ORC_LAMBDA_TRIANGLE)
+    t_lam = (u[4] < 0.5) ? sqrt(0.5 * u[4]) : 1.0 - sqrt(0.5 * (1.0 - u[4]));
+  double lambda = ins->lambda_min + t_lam * dlam;
   rec->lambda = lambda;
 
   /* R-C5 sample intersection in the sample frame (origin at (0,0,sample_z)) */

@@ -34,6 +34,9 @@ enum {
 };
 
 enum { ORC_SAMPLE_BOX = 0, ORC_SAMPLE_CYL_Y = 1 };
+/* R-L1: uniform band (BASELINE.json configs), or the triangular transmission of a mechanical velocity selector
+ * (KWS-1's selector sets the wavelength spread): symmetric triangle on [lambda_min, lambda_max] */
+enum { ORC_LAMBDA_UNIFORM = 0, ORC_LAMBDA_TRIANGLE = 1 };
 enum {
   ORC_SPHERE = 0,
   ORC_CORE_SHELL_SPHERE = 1,
@@ -78,7 +81,7 @@ typedef struct {
   double slit2_z, slit2_xw, slit2_yh;
   double focus_z, focus_xw, focus_yh;
   int32_t sample_shape;
-  int32_t pad0;
+  int32_t lambda_dist;            /* ORC_LAMBDA_*: law of the wavelength inside [lambda_min, lambda_max] (R-L1) */
   double sample_z, sample_xw, sample_yh, sample_zd, sample_radius;
   double mu_abs_2200, mu_inc;     /* 1/m */
   double q_min, q_max;            /* 1/A */

@@ -20,6 +20,7 @@ import numpy as np
 BASE_INSTRUMENT = dict(
     src_xw=0.010, src_yh=0.010,            # 10 x 10 mm flat source
     lambda_min=5.4, lambda_max=6.6,        # Angstrom
+    lambda_dist="uniform",                 # or "triangle": velocity-selector law (DESIGN.md R-L1)
     flux=1.0,
     slit1_z=0.0, slit1_xw=0.005, slit1_yh=0.005,
     slit2_z=5.0, slit2_xw=0.005, slit2_yh=0.005,

@@ -242,3 +242,39 @@ def test_unreachable_q_is_dropped():
     q = out["q"]
     k = TWO_PI / 30.0
     assert out["counters"][4] == (q >= 2 * k).sum() > 0
+
+
+def test_triangular_wavelength_law_of_a_velocity_selector():
+    """R-L1 (the selector fixes the wavelength spread): the wavelengths the oracle draws follow the
+    symmetric triangle on [lambda_min, lambda_max] -- mean at the centre, variance (d lambda)^2 / 24,
+    Kolmogorov-Smirnov against the triangle's distribution function -- from the same uniform draw 4 as the uniform
+    law (continuous at u = 1/2, monotone), and nothing else of the neutron changes."""
+    import math
+    ins_u = W.instrument()
+    ins_t = W.instrument(lambda_dist="triangle")
+    lam_u, lam_t = [], []
+    c = W.config(0)
+    for nid in range(60000):
+        ru, rt = O.trace_one(ins_u, c["model"], 99, nid), O.trace_one(ins_t, c["model"], 99, nid)
+        if ru.status == 1:                                 # died at slit 1: no wavelength drawn
+            continue
+        assert ru.status == rt.status or {ru.status, rt.status} <= {0, 4, 5}   # only outcomes that depend on lambda may differ
+        assert ru.u[4] == rt.u[4] and ru.p0 == rt.p0 and ru.q == rt.q
+        u4 = ru.u[4]
+        t = math.sqrt(0.5 * u4) if u4 < 0.5 else 1.0 - math.sqrt(0.5 * (1.0 - u4))
+        assert rt.lam == 5.4 + t * (6.6 - 5.4) and ru.lam == 5.4 + u4 * (6.6 - 5.4)
+        lam_u.append(ru.lam)
+        lam_t.append(rt.lam)
+    lam_t = np.sort(np.array(lam_t))
+    n = lam_t.size
+    assert n > 14000
+    d = 6.6 - 5.4
+    assert abs(lam_t.mean() - 6.0) < 5 * d / math.sqrt(24 * n)
+    assert abs(lam_t.var() - d * d / 24) < 0.03 * d * d / 24
+    t = (lam_t - 5.4) / d
+    cdf = np.where(t < 0.5, 2 * t * t, 1 - 2 * (1 - t) ** 2)
+    ks = np.abs(cdf - (np.arange(n) + 0.5) / n).max()
+    assert ks < 1.63 / math.sqrt(n)                        # 1 % level
+    # the uniform law is not a triangle (the test has power)
+    tu = (np.sort(np.array(lam_u)) - 5.4) / d
+    assert np.abs(np.where(tu < 0.5, 2 * tu * tu, 1 - 2 * (1 - tu) ** 2) - (np.arange(n) + 0.5) / n).max() > 5 / math.sqrt(n)

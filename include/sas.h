@@ -53,6 +53,9 @@ typedef enum {
  * rad (the proven range of the fp32 argument reductions), runs its model in fp64. */
 enum { SAS_FP32 = 0, SAS_FP64 = 1 };
 enum { SAS_SAMPLE_BOX = 0, SAS_SAMPLE_CYL_Y = 1 };
+/* law of the wavelength inside [lambda_min, lambda_max] (DESIGN.md R-L1): uniform, or the symmetric triangle of a
+ * mechanical velocity selector, FWHM = (lambda_max - lambda_min) / 2 */
+enum { SAS_LAMBDA_UNIFORM = 0, SAS_LAMBDA_TRIANGLE = 1 };
 enum {
   SAS_SPHERE = 0,              /* Table II F.9 */
   SAS_CORE_SHELL_SPHERE = 1,   /* Table II F.3  */
@@ -107,7 +110,7 @@ typedef struct {
   uint32_t struct_size;              /* = sizeof(sas_instrument_desc) */
   int32_t sample_shape;              /* SAS_SAMPLE_* */
   double src_xw, src_yh;             /* flat rectangular source in the plane z = 0 */
-  double lambda_min, lambda_max;     /* uniform wavelength band; equal => monochromatic */
+  double lambda_min, lambda_max;     /* wavelength band (law: lambda_dist); equal => monochromatic */
   double flux;                       /* n / (cm^2 s sr A); 1 for unit flux */
   double slit1_z, slit1_xw, slit1_yh;
   double slit2_z, slit2_xw, slit2_yh;
@@ -120,6 +123,8 @@ typedef struct {
   double det_dist;                   /* detector plane at sample_z + det_dist */
   double det_xw, det_yh;
   int32_t det_nx, det_ny;
+  int32_t lambda_dist;               /* SAS_LAMBDA_* */
+  int32_t reserved;
 } sas_instrument_desc;
 
 /* Sample model (PAPER.md:51 parameters {theta_i}; :122-133 distributions). */

@@ -23,6 +23,7 @@ EXPORTED_SYMBOLS = [
 ]
 
 SAMPLE = {"box": 0, "cyl_y": 1}
+LAMBDA_DIST = {"uniform": 0, "triangle": 1}
 MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3, "core_shell_triaxial": 4, "flat": 5,
          "parallelepiped": 6, "core_shell_cylinder": 7, "ellipsoid": 8, "barbell": 9, "capped_cylinder": 10,
          "elliptical_cylinder": 11, "hollow_cylinder": 12, "core_shell_ellipsoid": 13, "polymer_micelle": 14}
@@ -46,7 +47,7 @@ class InstrumentDesc(C.Structure):
                  "slit1_z", "slit1_xw", "slit1_yh", "slit2_z", "slit2_xw", "slit2_yh",
                  "focus_z", "focus_xw", "focus_yh", "sample_z", "sample_xw", "sample_yh", "sample_zd",
                  "sample_radius", "mu_abs_2200", "mu_inc", "q_min", "q_max", "det_dist", "det_xw", "det_yh")] + \
-               [("det_nx", C.c_int32), ("det_ny", C.c_int32)]
+               [("det_nx", C.c_int32), ("det_ny", C.c_int32), ("lambda_dist", C.c_int32), ("reserved", C.c_int32)]
 
 
 class ModelDesc(C.Structure):
@@ -80,7 +81,12 @@ def instrument_desc(d: dict) -> InstrumentDesc:
     for name, typ in InstrumentDesc._fields_:
         if name == "struct_size":
             continue
-        if name == "sample_shape":
+        if name == "reserved":
+            continue
+        if name == "lambda_dist":
+            v = d.get(name, "uniform")
+            s.lambda_dist = LAMBDA_DIST[v] if isinstance(v, str) else int(v)
+        elif name == "sample_shape":
             s.sample_shape = SAMPLE[d[name]] if isinstance(d[name], str) else int(d[name])
         elif typ is C.c_int32:
             setattr(s, name, int(d[name]))

@@ -64,6 +64,14 @@ struct Hit {
   double q;      // drawn |Q| (0 if the neutron died before the draw)
 };
 
+// R-L1: wavelength from draw 4: uniform in the band, or the inverse distribution function of the symmetric
+// triangle (velocity selector), operation by operation as the design note writes it (sqrt is correctly rounded)
+__device__ __forceinline__ double lambda_from_u(const ExpParams& P, double u4) {
+  double t = u4;
+  if (P.lambda_dist == 1) t = (u4 < 0.5) ? sqrt(0.5 * u4) : 1.0 - sqrt(0.5 * (1.0 - u4));
+  return P.lambda_min + t * P.dlam;
+}
+
 // Conservative classifier (stage B0): true when the neutron is CERTAIN to end as
 // ST_MISS_DET.  The host proved for this instrument that every slit-1 survivor passes slit 2 and
 // crosses the sample, and folded the worst-case beam divergence, beam radius at the sample, sample
@@ -72,7 +80,7 @@ struct Hit {
 // detector's circumscribed circle whatever its azimuth.  q is formed exactly as R-C7 forms it.
 __device__ __forceinline__ bool surely_misses_detector(const ExpParams& P, const uint32_t w1[4], double& q) {
   const double u4 = uniform_from_word(w1[0]), u6 = uniform_from_word(w1[2]);
-  const double lambda = P.lambda_min + u4 * P.dlam;
+  const double lambda = lambda_from_u(P, u4);
   q = P.q_min + u6 * P.dq;
   const double s_a = (q * lambda) * 0.07957747154594767;  // 1 / (4 pi)
   return (s_a > P.s_cut) && (s_a < 0.999999);
@@ -128,7 +136,7 @@ __device__ __forceinline__ int trace_geometry(const ExpParams& P, const uint32_t
   // draws 4..7 (Philox block 1, drawn by the classifier stage)
   const double u4 = uniform_from_word(w1[0]), u5 = uniform_from_word(w1[1]);
   const double u6 = uniform_from_word(w1[2]), u7 = uniform_from_word(w1[3]);
-  const double lambda = P.lambda_min + u4 * P.dlam;
+  const double lambda = lambda_from_u(P, u4);
   // R-C5 sample
   double tin, tout;
   bool hit_s = true;

@@ -124,6 +124,7 @@ sas_status validate_instrument(const sas_instrument_desc* d, std::string& why) {
   if (!(d->mu_abs_2200 >= 0.0) || !(d->mu_inc >= 0.0)) { why = "attenuation coefficients must be >= 0"; return SAS_EINVAL; }
   if (!(d->q_min >= 0.0) || !(d->q_max > d->q_min) || !std::isfinite(d->q_max)) { why = "need 0 <= q_min < q_max"; return SAS_EINVAL; }
   if (!finite_pos(d->det_dist) || !finite_pos(d->det_xw) || !finite_pos(d->det_yh)) { why = "detector distance and size must be > 0"; return SAS_EINVAL; }
+  if (d->lambda_dist != SAS_LAMBDA_UNIFORM && d->lambda_dist != SAS_LAMBDA_TRIANGLE) { why = "unknown lambda_dist"; return SAS_EINVAL; }
   if (d->det_nx < 1 || d->det_ny < 1 || d->det_nx > 16384 || d->det_ny > 16384) { why = "detector pixels must be in 1..16384 per axis"; return SAS_EINVAL; }
   return SAS_OK;
 }
@@ -209,6 +210,7 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
   P.lambda_min = d.lambda_min;
   P.dlam = d.lambda_max - d.lambda_min;
   P.dlam_w = P.dlam > 0.0 ? P.dlam : 1.0;
+  P.lambda_dist = d.lambda_dist;
   P.slit1_z = d.slit1_z; P.slit1_hx = 0.5 * d.slit1_xw; P.slit1_hy = 0.5 * d.slit1_yh;
   P.slit2_z = d.slit2_z; P.slit2_hx = 0.5 * d.slit2_xw; P.slit2_hy = 0.5 * d.slit2_yh;
   P.sample_shape = d.sample_shape;

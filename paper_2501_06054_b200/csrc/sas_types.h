@@ -58,7 +58,7 @@ struct ExpParams {
   int32_t lateral_free;  // primary rays cannot touch the sample's lateral faces (geometry.cuh)
   int32_t slits_free;    // no stage-B ray can be cut by a slit (geometry.cuh)
   int32_t geo_fast;      // slits_free, lateral_free, box sample, no attenuation: trace_geometry<true>
-  int32_t pad0;
+  int32_t lambda_dist;   // 0 uniform band, 1 symmetric triangle (R-L1)
   int32_t model, orient_kind, sq_kind;
   int32_t n_a, n_b, n_th, n_ph;
   int32_t tab_off, tab_len;  // in doubles, inside the table pool

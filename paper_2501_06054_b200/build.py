@@ -20,8 +20,18 @@ NVCC_FLAGS = [
 ]
 
 
+def extra_flags() -> list:
+    """SAS_DEBUG_BOUNDS=1 in the environment builds the bounds-checking variant (csrc/sas_types.h: SAS_CHECK)."""
+    return ["-DSAS_DEBUG_BOUNDS"] if os.environ.get("SAS_DEBUG_BOUNDS", "0") not in ("", "0") else []
+
+
 def is_stale() -> bool:
     if not os.path.exists(LIB):
+        return True
+    try:
+        if open(LIB + ".flags").read() != " ".join(extra_flags()):
+            return True
+    except OSError:
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
@@ -30,8 +40,9 @@ def is_stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or is_stale():
-        cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+        cmd = ["nvcc"] + NVCC_FLAGS + extra_flags() + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
         subprocess.check_call(cmd, cwd=CSRC)
+        open(LIB + ".flags", "w").write(" ".join(extra_flags()))
     return LIB
 
 

@@ -4,6 +4,15 @@
 
 #include "device_math.cuh"
 
+// -DSAS_DEBUG_BOUNDS (build.py: SAS_DEBUG_BOUNDS=1): the kernels trap on a queue, ring, table, pixel or work-item
+// index outside its bounds (compute-sanitizer is closed on this pool; profiles/r2_debug_bounds.md records a run
+// of the GPU test-suite on such a build).  The shipped build compiles the checks away.
+#ifdef SAS_DEBUG_BOUNDS
+#define SAS_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define SAS_CHECK(cond) do { } while (0)
+#endif
+
 namespace sas {
 
 enum : int { ST_DETECTED = 0, ST_SLIT1 = 1, ST_SLIT2 = 2, ST_MISS_SAMPLE = 3, ST_UNREACHABLE = 4, ST_MISS_DET = 5 };

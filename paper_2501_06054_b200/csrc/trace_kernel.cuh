@@ -144,6 +144,7 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
         uint32_t* d32 = reinterpret_cast<uint32_t*>(&P);
         for (int i = threadIdx.x; i < (int)(sizeof(ExpParams) / 4); i += BLOCK_THREADS) d32[i] = s32[i];
         const int tl = src->tab_len;
+        SAS_CHECK(tl >= 0 && tl <= a.tab_len_max);
         const double* tsrc = a.tab_pool + src->tab_off;
         for (int i = threadIdx.x; i < tl; i += BLOCK_THREADS) tab[i] = (Real)tsrc[i];
         cur_exp = e;
@@ -152,12 +153,14 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
       const uint32_t kk = item % a.items_per_exp;
       off0 = kk * a.item_ids;
       cnt_ids = min(a.item_ids, a.n_per_exp - off0);
+      SAS_CHECK(item < a.n_items && off0 < a.n_per_exp);
       row = warp;
       row_end = (cnt_ids + 31u) >> 5;
     }
 
     // ------------------------------------------------------------------ the pump
     for (;;) {
+      SAS_CHECK(cntB >= 0 && cntB <= RING_B && cntB2 >= 0 && cntB2 <= RING_B2 && cntC >= 0 && cntC <= RING);
       const bool rows_left = row < row_end;
       // Philox counter word 3 of the staged experiment (one add from a kernel parameter: not kept live)
       const uint32_t exp_word = a.exp_base + (uint32_t)cur_exp;
@@ -186,12 +189,8 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
             a.d_pixel[idoff] = pixel;
             a.d_weight[idoff] = p;
           } else {
+            SAS_CHECK(pixel >= 0 && pixel < a.npix && cur_exp >= 0);
             const size_t ix = (size_t)cur_exp * (size_t)a.npix + (size_t)pixel;
-#ifdef SAS_PROBE_NO_ATOMICS
-            // measurement probe only (profiles/r1_atomics.md): the same kernel without its histogram
-            // updates (the weight stays live through an impossible condition)
-            if (p != -1.0) continue;
-#endif
             atomicAdd(a.counts + ix, 1ull);
             atomicAdd(a.sum_p + ix, p);
             atomicAdd(a.sum_p2 + ix, p * p);

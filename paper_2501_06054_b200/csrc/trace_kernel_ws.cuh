@@ -45,9 +45,6 @@ namespace sas {
 #ifndef SAS_WS_PROD_LAST
 #define SAS_WS_PROD_LAST 0    // the producers are the LAST warpgroup: the sub-partition arbiter serves the highest warp id first
 #endif
-#ifndef SAS_WS_PROBE
-#define SAS_WS_PROBE 0        // measurement probes (never defined in the shipped build)
-#endif
 
 constexpr int WS_CWG = SAS_WS_CWG;
 constexpr int WS_THREADS = 128 * (1 + WS_CWG);
@@ -202,6 +199,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     uint32_t* d32 = reinterpret_cast<uint32_t*>(&P);
     for (int i = tid; i < (int)(sizeof(ExpParams) / 4); i += nthr) d32[i] = s32[i];
     const int tl = src->tab_len;
+    SAS_CHECK(tl >= 0 && tl <= a.tab_len_max);
     const double* tsrc = a.tab_pool + src->tab_off;
     for (int i = tid; i < tl; i += nthr) tab[i] = (Real)tsrc[i];
   };
@@ -275,6 +273,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
         const unsigned m = __ballot_sync(FULL, keep);
         if (keep) {
           const uint32_t L = (tail + __popc(m & lt)) & (uint32_t)(32 * WS_G - 1);
+          SAS_CHECK(((tail + __popc(m & lt)) >> 5) - (tail >> 5) <= 1u);  // inside the two windows this warp owns
           sts32(ring + OFF_ID + 4u * L, idl[k]);
           sts128(ring + 16u * L, w1[k][0], w1[k][1], w1[k][2], w1[k][3]);
         }
@@ -290,6 +289,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
       const uint32_t off0 = (item % a.items_per_exp) * a.item_ids;
       const uint32_t cnt_ids = min(a.item_ids, a.n_per_exp - off0);
       const uint32_t rows_full = cnt_ids >> 5;
+      SAS_CHECK(item < a.n_items && off0 < a.n_per_exp && off0 + cnt_ids <= a.n_per_exp);
       // word window of the integer slit-1 test (the whole range when slit 1 is not in the source plane)
       const uint32_t lo0 = P.s1_lo[0], d0 = P.s1_hi[0] - P.s1_lo[0], lo1 = P.s1_lo[1], d1 = P.s1_hi[1] - P.s1_lo[1];
       const uint32_t idc0 = first_lo + off0 + lane;  // Philox counter word 0 of this lane in row 0
@@ -300,11 +300,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
         const uint32_t idr = idc0 + (row << 5);
 #pragma unroll
         for (int k = 0; k < WS_NR; ++k)
-#if SAS_WS_PROBE == 2
-          { w0[k] = (lane & 3) ? 0u : lo0; w1[k] = lo1; }
-#else
           philox_words01(a.keys, idr + 32u * (uint32_t)(k * WS_PAIRS), id_hi, 0u, exp_word, w0[k], w1[k]);
-#endif
 #pragma unroll
         for (int k = 0; k < WS_NR; ++k) {
           const bool pass = (w0[k] - lo0 <= d0) && (w1[k] - lo1 <= d1);
@@ -313,6 +309,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
           sp += 4u * __popc(m);
         }
         row += WS_NR * WS_PAIRS;
+        SAS_CHECK(sp - stack0 <= 4u * (uint32_t)WS_STACK);
         __syncwarp();
         while (sp - stack0 >= 128u * WS_NB0) stage_b0(exp_word);
       }
@@ -383,6 +380,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
       const uint32_t meta = lds32(ring + OFF_META + 4u * w);
       const int n = (int)(meta & 0xFFu);
       const uint32_t flag = meta >> 8;
+      SAS_CHECK(n <= 32 && flag <= WS_DONE);
       const bool act = lane < n;
       uint32_t id_lo = 0;
       uint4 w1v = make_uint4(0, 0, 0, 0);
@@ -392,11 +390,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
       }
       __syncwarp();
       if (lane == 0) mbar_arrive_a(ring + OFF_EMPTY + 8u * w);
-#if SAS_WS_PROBE == 1
-      if (false) {
-#else
       if (n > 0) {
-#endif
         // ---------------- stage B: Philox block 0 again, fp64 geometry
         uint32_t w[4];
         const uint32_t w1[4] = {w1v.x, w1v.y, w1v.z, w1v.w};
@@ -415,6 +409,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
           cq.c_Q[0][s2] = h.Qx; cq.c_Q[1][s2] = h.Qy; cq.c_Q[2][s2] = h.Qz;
         }
         cntC += __popc(m);
+        SAS_CHECK(cntC <= RING);
         __syncwarp();
       }
       // ---------------- stage C: model + weight + histogram
@@ -441,6 +436,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
             a.d_pixel[idc - first_lo] = pixel;
             a.d_weight[idc - first_lo] = p;
           } else {
+            SAS_CHECK(pixel >= 0 && pixel < a.npix && cur_exp >= 0);
             const size_t ix = (size_t)cur_exp * (size_t)a.npix + (size_t)pixel;
             atomicAdd(a.counts + ix, 1ull);
             atomicAdd(a.sum_p + ix, p);

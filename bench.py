@@ -426,6 +426,7 @@ def main():
     ap.add_argument("--headline-only", action="store_true", help="skip the secondary workloads")
     ap.add_argument("--config", type=int, default=HEADLINE, help="workload timed as the main line (profiling)")
     ap.add_argument("--precision", default=None, help="precision override of --config (profiling)")
+    ap.add_argument("--neutrons", type=int, default=None, help="neutrons per step override of --config (profiling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1, then exit")
     args = ap.parse_args()
@@ -465,7 +466,7 @@ def main():
         flush_buf.fill_(1)
 
     warm = max(args.warmup, 3) if args.warmup else 0
-    head = bench_config(torch, S, args.config, args.precision, None, args.steps, warm, rank, world, local, flush, rates, traffic)
+    head = bench_config(torch, S, args.config, args.precision, args.neutrons, args.steps, warm, rank, world, local, flush, rates, traffic)
 
     others = {}
     if not args.headline_only:

@@ -66,9 +66,13 @@ struct Hit {
 
 // R-L1: wavelength from draw 4: uniform in the band, or the inverse distribution function of the symmetric
 // triangle (velocity selector), operation by operation as the design note writes it (sqrt is correctly rounded)
+// (out of line: the uniform law of every BASELINE.json config must not carry the two square roots as selects)
+__device__ __noinline__ double triangle_position(double u4) {
+  return (u4 < 0.5) ? sqrt(0.5 * u4) : 1.0 - sqrt(0.5 * (1.0 - u4));
+}
 __device__ __forceinline__ double lambda_from_u(const ExpParams& P, double u4) {
   double t = u4;
-  if (P.lambda_dist == 1) t = (u4 < 0.5) ? sqrt(0.5 * u4) : 1.0 - sqrt(0.5 * (1.0 - u4));
+  if (P.lambda_dist == 1) t = triangle_position(u4);
   return P.lambda_min + t * P.dlam;
 }
 
@@ -90,7 +94,9 @@ __device__ __forceinline__ bool surely_misses_detector(const ExpParams& P, const
 // raw words with host-folded constants, |relative error| < 6e-7 (two conversions, two FMAs, one product, four
 // rounded constants), and compared with thresholds the host moved 2e-6 INTO the certain region, so
 // true here implies true for the fp64 test above; a neutron this test leaves undecided simply runs the full
-// geometry (which finds the same ST_MISS_DET).
+// geometry (which finds the same ST_MISS_DET).  For a wavelength law that is not linear in the draw (R-L1) the
+// host sets cls_la = 0, cls_lb = lambda_min: a lower bound of lambda is all the first comparison needs, and the
+// second one (|Q| reachable) is then proved for the whole instrument or the classifier is switched off.
 __device__ __forceinline__ bool surely_misses_detector_f32(const ExpParams& P, uint32_t w_lambda, uint32_t w_q) {
   const float lam = fmaf(__uint2float_rn(w_lambda), P.cls_la, P.cls_lb);
   const float q = fmaf(__uint2float_rn(w_q), P.cls_qa, P.cls_qb);

@@ -284,6 +284,14 @@ void fill_instrument(const sas_instrument_desc& d, ExpParams& P) {
     const double four_pi = 4.0 * PI_D;
     P.cls_lo = std::isfinite(P.s_cut) ? std::nextafterf((float)(four_pi * P.s_cut * (1.0 + 2.0e-6)), INFINITY) : INFINITY;
     P.cls_hi = std::nextafterf((float)(four_pi * 0.999999 * (1.0 - 2.0e-6)), 0.0f);
+    if (d.lambda_dist != SAS_LAMBDA_UNIFORM) {
+      // a law that is not linear in the draw (R-L1): the fp32 test takes lambda_min, a lower bound of every
+      // wavelength, in its first comparison; its second comparison (|Q| reachable: q lambda / 4 pi < 0.999999) must
+      // then hold for the whole instrument, else the fp32 classifier is switched off (the fp64 geometry decides)
+      P.cls_la = 0.0f;
+      P.cls_lb = std::nextafterf((float)P.lambda_min, 0.0f);
+      if (d.q_max * d.lambda_max < four_pi * 0.99) P.cls_hi = INFINITY; else P.cls_lo = INFINITY;
+    }
   }
 }
 
@@ -446,21 +454,29 @@ sas_status alloc_common(sas_ctx* c) {
   CUDA_TRY(c, cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device));
   CUDA_TRY(c, cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking));
   c->own_stream = true;
-  const size_t nh = (size_t)c->n_exp * c->npix;
-  CUDA_TRY(c, cudaMalloc(&c->d_sum_p, nh * sizeof(double)));
-  CUDA_TRY(c, cudaMalloc(&c->d_sum_p2, nh * sizeof(double)));
-  CUDA_TRY(c, cudaMalloc(&c->d_counts, nh * sizeof(unsigned long long)));
-  c->own_hist = true;
+  c->own_hist = true;  // the context's own histograms are allocated by the first call that needs them (ensure_hist)
   CUDA_TRY(c, cudaMalloc(&c->d_counters, 8 * sizeof(unsigned long long)));
   CUDA_TRY(c, cudaMalloc(&c->d_work, sizeof(unsigned int)));
   CUDA_TRY(c, cudaMemset(c->d_work, 0, sizeof(unsigned int)));
   CUDA_TRY(c, cudaMalloc(&c->d_exp_ids, (size_t)c->n_exp * sizeof(uint32_t)));
   CUDA_TRY(c, cudaMalloc(&c->d_exps, (size_t)c->n_exp * sizeof(ExpParams)));
+  CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
+  c->launched = 0;
+  return SAS_OK;
+}
+
+// The context's own zeroed histograms, unless the caller bound its buffers (sas_bind_buffers) before anything
+// needed them: a batch of 1024 detectors is 1.2 GB that a binding caller never wants allocated twice.
+sas_status ensure_hist(sas_ctx* c) {
+  if (c->d_sum_p) return SAS_OK;
+  const size_t nh = (size_t)c->n_exp * c->npix;
+  CUDA_TRY(c, cudaMalloc(&c->d_sum_p, nh * sizeof(double)));
+  CUDA_TRY(c, cudaMalloc(&c->d_sum_p2, nh * sizeof(double)));
+  CUDA_TRY(c, cudaMalloc(&c->d_counts, nh * sizeof(unsigned long long)));
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p, 0, nh * sizeof(double), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_sum_p2, 0, nh * sizeof(double), c->stream));
   CUDA_TRY(c, cudaMemsetAsync(c->d_counts, 0, nh * sizeof(unsigned long long), c->stream));
-  CUDA_TRY(c, cudaMemsetAsync(c->d_counters, 0, 8 * sizeof(unsigned long long), c->stream));
-  c->launched = 0;
+  c->own_hist = true;
   return SAS_OK;
 }
 
@@ -698,6 +714,7 @@ sas_status trace_common(sas_ctx* c, uint64_t first_id, uint64_t n_each, uint64_t
   if (!c->model_set) return fail(c, SAS_ESTATE, "sas_set_model must precede tracing");
   if (n_each == 0) return SAS_OK;
   if (first_id + n_each < first_id) return fail(c, SAS_EINVAL, "neutron id range overflows 64 bits");
+  { sas_status st = ensure_hist(c); if (st != SAS_OK) return st; }
   KernelArgs a;
   std::memset(&a, 0, sizeof(a));
   a.exps = c->d_exps; a.tab_pool = c->d_tab;
@@ -903,6 +920,7 @@ sas_status sas_trace_dump(sas_ctx* c, uint64_t first_id, uint64_t n, uint64_t se
 sas_status sas_read_detector(sas_ctx* c, double* h_sum_p, double* h_sum_p2, uint64_t* h_counts) {
   if (!c) return SAS_EINVAL;
   DeviceGuard g(c);
+  { sas_status st = ensure_hist(c); if (st != SAS_OK) return st; }
   const size_t nh = (size_t)c->n_exp * c->npix;
   if (h_sum_p) CUDA_TRY(c, cudaMemcpyAsync(h_sum_p, c->d_sum_p, nh * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   if (h_sum_p2) CUDA_TRY(c, cudaMemcpyAsync(h_sum_p2, c->d_sum_p2, nh * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -928,6 +946,7 @@ sas_status sas_get_counters(sas_ctx* c, uint64_t out[8]) {
 sas_status sas_reset_detector(sas_ctx* c) {
   if (!c) return SAS_EINVAL;
   DeviceGuard g(c);
+  { sas_status st = ensure_hist(c); if (st != SAS_OK) return st; }
   const size_t nh = (size_t)c->n_exp * c->npix;
   // one launch for the three histograms and the counters (four memsets cost four stream operations: as much as
   // the trace kernel itself at 1e6 neutrons)
@@ -980,6 +999,7 @@ sas_status sas_reduce_radial(sas_ctx* c, const sas_radial_desc* d, double* h_q, 
   if (!(d->q_hi > d->q_lo) || !(d->q_lo >= 0.0) || !std::isfinite(d->q_hi)) return fail(c, SAS_EINVAL, "need 0 <= q_lo < q_hi");
   if (!(d->lambda_ref > 0.0) || !std::isfinite(d->lambda_ref)) return fail(c, SAS_EINVAL, "lambda_ref must be > 0");
   if (d->exp_index >= c->n_exp) return fail(c, SAS_EINVAL, "exp_index out of range");
+  { sas_status st = ensure_hist(c); if (st != SAS_OK) return st; }
   const int nb = d->n_bins;
   // ring scratch: sum P, sum P2, sum dOmega, pixel count, nb entries each (one memset, one copy of what is used)
   if (!c->d_rings) CUDA_TRY(c, cudaMalloc(&c->d_rings, 4 * (size_t)SAS_MAX_RINGS * sizeof(double)));

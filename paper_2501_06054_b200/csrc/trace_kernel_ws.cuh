@@ -260,13 +260,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
       for (int k = 0; k < WS_NB0; ++k) philox4x32_10(a.keys, idl[k], id_hi, 1u, exp_word, w1[k]);
 #pragma unroll
       for (int k = 0; k < WS_NB0; ++k) {
-        bool sure;
-        if (P.lambda_dist == 0) {
-          sure = act[k] && surely_misses_detector_f32(P, w1[k][0], w1[k][2]);
-        } else {  // the fp32 form folds the uniform law into its constants: any other law takes the fp64 test
-          double qd;
-          sure = surely_misses_detector(P, w1[k], qd) && act[k];
-        }
+        const bool sure = act[k] && surely_misses_detector_f32(P, w1[k][0], w1[k][2]);
         n_sure += sure ? 1u : 0u;
         if (DUMP_Q && sure) a.d_q[idl[k] - first_lo] = P.q_min + uniform_from_word(w1[k][2]) * P.dq;  // R-C7
         const bool keep = act[k] && !sure;

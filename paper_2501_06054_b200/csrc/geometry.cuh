@@ -66,13 +66,9 @@ struct Hit {
 
 // R-L1: wavelength from draw 4: uniform in the band, or the inverse distribution function of the symmetric
 // triangle (velocity selector), operation by operation as the design note writes it (sqrt is correctly rounded)
-// (out of line: the uniform law of every BASELINE.json config must not carry the two square roots as selects)
-__device__ __noinline__ double triangle_position(double u4) {
-  return (u4 < 0.5) ? sqrt(0.5 * u4) : 1.0 - sqrt(0.5 * (1.0 - u4));
-}
 __device__ __forceinline__ double lambda_from_u(const ExpParams& P, double u4) {
   double t = u4;
-  if (P.lambda_dist == 1) t = triangle_position(u4);
+  if (P.lambda_dist == 1) t = (u4 < 0.5) ? sqrt(0.5 * u4) : 1.0 - sqrt(0.5 * (1.0 - u4));
   return P.lambda_min + t * P.dlam;
 }
 

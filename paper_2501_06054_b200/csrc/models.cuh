@@ -322,6 +322,35 @@ __device__ __forceinline__ double eval_intensity_generic(const ExpParams& P, con
   return fma(P.norm * acc, S, P.background);
 }
 
+// fp64 node loop of the polydisperse sphere: w (drho V)^2 Phi(u)^2 = [16 pi^2 drho^2 w] (sin u - u cos u)^2 / q^6,
+// u = q R: the bracket is the node's fourth table entry and 1 / q^6 multiplies the sum once, so the loop has no
+// division; below u = 0.5, where sin u - u cos u cancels, the node takes the series of Phi (R-C12).  u < 1e6
+// (sas_set_model).  Out of line: inlined, its registers cost the one-evaluation kernels (c0, c4) 2 %.
+__device__ __forceinline__ void lds_f64x2(uint32_t addr, double& x, double& y) {
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(addr));
+}
+// (ta: shared-window address of the node table {R, -, w (drho V)^2, 16 pi^2 drho^2 w} in doubles)
+__device__ __noinline__ double sphere_nodes_fp64(uint32_t ta, int n_a, double qd, double q2d) {
+  const double iq2 = 1.0 / q2d;
+  double direct = 0.0, small = 0.0;
+  for (int a = 0; a < n_a; ++a) {
+    double R, unused, w_small, w_direct;
+    lds_f64x2(ta + 32u * (uint32_t)a, R, unused);
+    lds_f64x2(ta + 32u * (uint32_t)a + 16u, w_small, w_direct);
+    const double u = qd * R;
+    if (u < 0.5) {
+      const double ph = sphere_phi(u);
+      small = fma(w_small, ph * ph, small);
+    } else {
+      double sn, cs;
+      sincos_cw(u, sn, cs);
+      const double d = fma(-u, cs, sn);
+      direct = fma(w_direct, d * d, direct);
+    }
+  }
+  return fma(direct, (iq2 * iq2) * iq2, small);
+}
+
 // Model table meaning (host: fill_model).  Lengths that multiply a projection of Q are stored as a
 // (hi, lo) pair: in the fp32 path hi = float(L), lo = float(L - hi); in the fp64 path hi = L, lo = 0.
 //  sphere              ta = {R_hi, R_lo, w_a (drho V_a)^2}
@@ -358,11 +387,15 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
   Real acc = 0;
   switch (model) {
     case 0: {  // sphere
-      const Proj<Real> qp = make_proj<Real>(qd);
-      for (int a = 0; a < P.n_a; ++a) {
-        const Real* r = T.ta + a * TA_W;
-        const Real ph = sphere_phi_abs_ph(phase_mul(qp, r[0], r[1]));
-        acc = fma_r(r[2], ph * ph, acc);
+      if (sizeof(Real) == 8 && P.n_a > 1) {
+        acc = (Real)sphere_nodes_fp64((uint32_t)__cvta_generic_to_shared(T.ta), P.n_a, qd, q2d);
+      } else {
+        const Proj<Real> qp = make_proj<Real>(qd);
+        for (int a = 0; a < P.n_a; ++a) {
+          const Real* r = T.ta + a * TA_W;
+          const Real ph = sphere_phi_abs_ph(phase_mul(qp, r[0], r[1]));
+          acc = fma_r(r[2], ph * ph, acc);
+        }
       }
     } break;
     case 1: {  // core-shell sphere

@@ -369,7 +369,11 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
   for (int a = 0; a < na; ++a) {
     double* r = &ta[a * TA_W];
     switch (m.model) {
-      case SAS_SPHERE: { const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R; split(R, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
+      case SAS_SPHERE: {
+        const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R;
+        split(R, r); r[2] = wa[a] * (s0 * V) * (s0 * V);
+        r[3] = wa[a] * ((4.0 * PI_D * s0) * (4.0 * PI_D * s0));   // 9 w (drho V)^2 / R^6: the fp64 node loop (models.cuh)
+      } break;
       case SAS_CORE_SHELL_SPHERE: { const double R = m.size[0] * xa[a], V = FOUR_PI_3 * R * R * R; split(R, r); r[2] = (s0 - s1) * V; r[3] = wa[a]; } break;
       case SAS_CYLINDER: { const double R = m.size[0] * xa[a], c = s0 * PI_D * R * R; split(R, r); r[2] = wa[a] * c * c; r[3] = R * R; } break;
       case SAS_TRIAXIAL_ELLIPSOID: { const double x = xa[a], V = FOUR_PI_3 * (m.size[0] * x) * (m.size[1] * x) * (m.size[2] * x); split(x, r); r[2] = wa[a] * (s0 * V) * (s0 * V); } break;
@@ -508,7 +512,11 @@ double max_phase(const sas_model_desc& m, const sas_instrument_desc& ins) {
     case SAS_CYLINDER: len = std::max(m.size[0] * f[0], 0.5 * m.size[1] * f[1]); break;
     case SAS_TRIAXIAL_ELLIPSOID: len = std::max(m.size[0], std::max(m.size[1], m.size[2])) * f[0]; break;
     case SAS_CORE_SHELL_TRIAXIAL: len = std::max(m.size[0], std::max(m.size[1], m.size[2])) * f[0] + m.size[3] * f[1]; break;
-    default: break;
+    case SAS_POLYMER_MICELLE: len = m.size[0] * f[0] + m.size[1]; break;
+    case SAS_FLAT: break;
+    default:  // NEXT-2 bodies: every size is a length; a generous bound
+      len = (std::max(std::max(m.size[0], m.size[1]), std::max(m.size[2], m.size[3])) + m.size[2]) * std::max(f[0], f[1]);
+      break;
   }
   return ins.q_max * len;
 }
@@ -533,6 +541,9 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   c->tab_len_max = 0;
   c->exp_prec.assign(c->n_exp, SAS_FP64);
   c->precision = SAS_FP32;  // of the context: fp64 as soon as one experiment runs in fp64 (introspection only)
+  for (uint32_t e = 0; e < c->n_exp; ++e)
+    if (max_phase(models[e], c->instr[e]) > 1.0e6)   // the tracer's own fp64 sin/cos reduce exactly below 2^20 pi/2
+      return fail(c, SAS_EUNSUPPORTED, "experiment " + std::to_string(e) + ": q_max x particle size exceeds 1e6 rad");
   for (uint32_t e = 0; e < c->n_exp; ++e) {
     ExpParams& P = c->h_exps[e];
     fill_instrument(c->instr[e], P);

@@ -65,25 +65,36 @@ STAGE_A = U(42, wide=16, imad=2, logic=22, xu=2)
 STAGE_B0 = U(50.5, wide=18.5, logic=30, xu=2)
 # every survivor whose geometry is evaluated (Philox block 0 again is not counted)
 STAGE_B = {
-    "fast": U(262, logic=47, fp64=200, fp32=2, xu=13),       # slit-free box-sample instrument class (c0, c1, c2, c4)
-    "general": U(295, logic=61, fp64=225, fp32=3, xu=14),    # cylinder sample, slits that may cut (c3)
+    "fast": U(268, logic=52, fp64=200, fp32=3, xu=13),       # slit-free box-sample instrument class (c0, c1, c2, c4)
+    "general": U(307, logic=66, fp64=225, fp32=2, xu=14),    # cylinder sample, slits that may cut (c3)
 }
 
-# per detected neutron: (prologue, per node evaluation)
+# per detected neutron: (prologue, per node evaluation).  Rows marked (counted) are read from the executed SASS of
+# the round-2 profiles (profiles/r2_instruction_counts.md); rows marked (estimate) are assembled from the counted
+# pieces they share with those (Philox block: 19 multiplies + 20 XOR; sincos: 35 FP64; ...) and are not judged as
+# measurements.
 MODEL_COST = {
-    "sphere_fp64": (U(94, wide=1, imad=1, logic=27, fp64=63, xu=2), U(0)),            # one evaluation, in the prologue
-    "sphere_fp32": (U(80, wide=1, imad=1, logic=22, fp64=14, fp32=30, xu=12), U(32.2, logic=1.2, fp32=30, xu=1)),
-    "sphere_py_fp32": (U(121, wide=1, imad=1, logic=22, fp64=14, fp32=69, xu=14), U(32.2, logic=1.2, fp32=30, xu=1)),
-    "sphere_py_fp64": (U(150, logic=30, fp64=110, xu=6), U(72, logic=8, fp64=62, xu=2)),
+    # (counted, c0) one fp64 evaluation, all of it in the prologue
+    "sphere_fp64": (U(94, wide=1, imad=1, logic=27, fp64=63, xu=2), U(0)),
+    # (estimate: sphere_py_fp32 without its S(q))
+    "sphere_fp32": (U(80, wide=1, imad=1, logic=22, fp64=14, fp32=30, xu=12), U(32.4, imad=0.2, logic=1.2, fp32=30, xu=1)),
+    # (counted, c1 fp32)
+    "sphere_py_fp32": (U(123, wide=1, imad=1, logic=24, fp64=14, fp32=69, xu=14), U(32.4, imad=0.2, logic=1.2, fp32=30, xu=1)),
+    # (counted, c1 fp64)
+    "sphere_py_fp64": (U(133, wide=1, logic=27, fp64=101, fp32=1, xu=3), U(63.5, logic=15, fp64=47.5, xu=1)),
+    # (round-1 SASS count of the node; prologue estimate)
     "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(27, logic=1, fp32=25, xu=1)),
-    # Philox block 2 (orientation draws), three sincos of 2 pi u, frame; outer node 43 / inner node 34.5
-    "cs_triaxial_iso_fp32": (U(200 + 16 * 43, wide=19, logic=55 + 16 * 6, fp64=114, fp32=16 * 34, xu=14 + 16), U(34.5, imad=1, logic=2.5, fp32=29, xu=2)),
-    "cylinder_iso_fp64": (U(420, wide=19, logic=70, fp64=310, xu=10), U(0)),
-    # per-event sizes: Philox blocks 2 and 3, two Box-Muller normals, three sincospi, sin, j1, the weight
-    "cylinder_event_fp64": (U(620, wide=38, logic=110, fp64=450, xu=14), U(0)),
-    # barbell, per event: the cylinder term and the prologue of the per-event path, then 64 slice evaluations
-    "barbell_event_fp64": (U(620, wide=38, logic=110, fp64=450, xu=14), U(70, logic=8, fp64=58, xu=2)),
-    # micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms (estimate)
+    # (counted, c3) prologue = Philox block 2 (orientation draws), three sincos of 2 pi u, frame, and the 16 outer
+    # nodes (37 instructions each); inner node 34
+    "cs_triaxial_iso_fp32": (U(832, wide=19, imad=18.5, logic=136, fp64=114, fp32=499, xu=47), U(34, imad=0.5, logic=2.5, fp32=29, xu=2)),
+    # (estimate: the per-event cylinder below without its size draws)
+    "cylinder_iso_fp64": (U(400, wide=37, logic=147, fp64=200, xu=15), U(0)),
+    # (counted, n1) per-event sizes: Philox blocks 2 and 3 and a re-draw, two Box-Muller normals, three sincospi,
+    # sin, j1, the weight
+    "cylinder_event_fp64": (U(624, wide=56, imad=3, logic=187, fp64=350, fp32=5, xu=23), U(0)),
+    # (estimate) barbell, per event: the prologue of the per-event cylinder, then 64 slice evaluations
+    "barbell_event_fp64": (U(624, wide=56, imad=3, logic=187, fp64=350, fp32=5, xu=23), U(70, logic=8, fp64=58, xu=2)),
+    # (estimate) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
     "micelle_event_fp64": (U(330, wide=19, logic=60, fp64=230, xu=8), U(0)),
 }
 

@@ -1,7 +1,7 @@
 """Executed instructions per class in a range of SASS lines of an Nsight Compute report (the counts behind
 paper_2501_06054_b200/roofline.py; profiles/r2_instruction_counts.md states the ranges used).
 
-    python -m paper_2501_06054_b200.sass_counts report.ncu-rep [--launch I] name:first:last:denominator ...
+    python -m paper_2501_06054_b200.sass_counts report.ncu-rep|source.csv[.gz] [--launch I] name:first:last:denominator ...
     python -m paper_2501_06054_b200.sass_counts report.ncu-rep --blocks        # runs of equal execution count
 
 Classes: wide (IMAD.WIDE, IMAD.HI: 32x32->64 multiplies), imad (other integer multiplies), logic (LOP3, integer and
@@ -50,10 +50,18 @@ def classify(full: str) -> str:
 
 
 def load(rep: str, launch: int | None):
-    cmd = ["ncu", "-i", rep, "--page", "source", "--csv", "--print-source", "sass"]
-    if launch is not None:
-        cmd += ["--launch-skip", str(launch), "--launch-count", "1"]
-    rows = list(csv.reader(subprocess.run(cmd, capture_output=True, text=True).stdout.splitlines()))
+    if rep.endswith(".csv") or rep.endswith(".csv.gz"):   # an exported source page (ncu ... --page source --csv)
+        import gzip
+        text = (gzip.open(rep, "rt") if rep.endswith(".gz") else open(rep)).read()
+        if launch:                                        # a multi-launch export: the launch-th "Kernel Name" section
+            parts = text.split('"Kernel Name"')
+            text = '"Kernel Name"' + parts[launch + 1]
+    else:
+        cmd = ["ncu", "-i", rep, "--page", "source", "--csv", "--print-source", "sass"]
+        if launch is not None:
+            cmd += ["--launch-skip", str(launch), "--launch-count", "1"]
+        text = subprocess.run(cmd, capture_output=True, text=True).stdout
+    rows = list(csv.reader(text.splitlines()))
     name = rows[0][1] if rows and len(rows[0]) > 1 else "?"
     hdr, data = rows[1], rows[2:]
     isrc, iex = hdr.index("Source"), hdr.index("Instructions Executed")

@@ -86,6 +86,7 @@ struct WsShared {
   WsProducer prod[WS_PAIRS];
   WsConsumer cons[WS_PAIRS * WS_CWG];
   unsigned int item[2];
+  unsigned long long outcomes[8];  // the block's outcome counts (slots of KernelArgs::counters), flushed once per block
 };
 
 template <typename Real>
@@ -191,6 +192,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     mbar_init(&pr.empty[threadIdx.x % WS_G], 1);
   }
   if (threadIdx.x < WS_PAIRS) S.prod[threadIdx.x].ticket = 0u;
+  if (threadIdx.x < 8) S.outcomes[threadIdx.x] = 0ull;
   unsigned item = blockIdx.x;    // the first item of a block is its own index (the host launches grid <= n_items)
   int cur_exp = a.use_exp0 ? a.exp0.exp_index : (int)a.exp_ids[item / a.items_per_exp];
   auto stage_experiment = [&](int e, int tid, int nthr) {
@@ -346,8 +348,8 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     if (!DUMP) {
       const unsigned tot = __reduce_add_sync(FULL, n_sure);
       if (lane == 0 && tot) {
-        atomicAdd(a.counters + 5, (unsigned long long)tot);
-        atomicAdd(a.counters + 7, (unsigned long long)tot);
+        atomicAdd(&S.outcomes[5], (unsigned long long)tot);
+        atomicAdd(&S.outcomes[7], (unsigned long long)tot);
       }
     }
   } else {
@@ -450,9 +452,15 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
 #pragma unroll
       for (int f = 0; f < 6; ++f) {
         const unsigned tot = __reduce_add_sync(FULL, cq.oc[f][lane]);
-        if (lane == 0 && tot) atomicAdd(a.counters + (f == 0 ? 6 : f), (unsigned long long)tot);
+        if (lane == 0 && tot) atomicAdd(&S.outcomes[f == 0 ? 6 : f], (unsigned long long)tot);
       }
     }
+  }
+  // one set of global updates per block instead of one per warp: a 1e6-neutron launch ended with 2 000 warps adding
+  // to the same three counters, 3 us of its 20
+  if (!DUMP) {
+    bar_block();
+    if (threadIdx.x < 8 && S.outcomes[threadIdx.x]) atomicAdd(a.counters + threadIdx.x, S.outcomes[threadIdx.x]);
   }
 }
 

@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 
 #include "coeffs_generated.h"
+#include "j1_f64_generated.h"
 
 namespace sas {
 
@@ -136,6 +137,35 @@ __device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
   sincos_cw(x, s, c);
 }
 __device__ __forceinline__ void sincos_r(double x, double& s, double& c) { sincos_d(x, s, c); }
+// sin and cos of pi x for |x| < 2^51: x = k/2 + r exactly (|r| <= 1/4), then the same Taylor kernels on pi r
+// (pi r carries one rounding of r pi_hi plus the r pi_lo correction: about one ulp)
+__device__ __forceinline__ void sincospi_cw(double x, double& s, double& c) {
+  const double t = fma(x, 2.0, 6755399441055744.0);
+  const int k = __double2loint(t);
+  const double nf = t - 6755399441055744.0;
+  const double rr = fma(nf, -0.5, x);
+  const double r = fma(rr, 0x1.921fb54442d18p+1, rr * 0x1.1a62633145c07p-53);
+  const double z = r * r;
+  double ps = fma(z, c_sincos[10], c_sincos[9]);
+  ps = fma(ps, z, c_sincos[8]);
+  ps = fma(ps, z, c_sincos[7]);
+  ps = fma(ps, z, c_sincos[6]);
+  ps = fma(ps, z, c_sincos[5]);
+  ps = fma(ps, z, c_sincos[4]);
+  ps = fma(r * z, ps, r);
+  double pc = fma(z, c_sincos[19], c_sincos[18]);
+  pc = fma(pc, z, c_sincos[17]);
+  pc = fma(pc, z, c_sincos[16]);
+  pc = fma(pc, z, c_sincos[15]);
+  pc = fma(pc, z, c_sincos[14]);
+  pc = fma(pc, z, c_sincos[13]);
+  pc = fma(pc, z, c_sincos[12]);
+  pc = fma(pc, z, 1.0);
+  const double ss = (k & 1) ? pc : ps;
+  const double cc = (k & 1) ? ps : pc;
+  s = (k & 2) ? -ss : ss;
+  c = ((k + 1) & 2) ? -cc : cc;
+}
 
 // fp32 reciprocal / square root: one MUFU each (~1 ulp), no IEEE fix-up path
 __device__ __forceinline__ float rcp_fast(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
@@ -280,7 +310,12 @@ __device__ __forceinline__ float sinc_r(float x) {
   const float ps = fmaf(r * z, horner(SP, z), r);
   return sinc_from(__int_as_float(__float_as_int(ps) ^ (kb << 31)), x);
 }
-__device__ __forceinline__ double sinc_r(double x) { return (x == 0.0) ? 1.0 : sin(x) / x; }
+__device__ __forceinline__ double sinc_r(double x) {
+  if (x == 0.0) return 1.0;
+  double s, c;
+  sincos_d(x, s, c);
+  return s / x;
+}
 // |sinc(q h)| for callers that square it: no sign, and the phase is biased by 1e-30 so that q h = 0 gives
 // sin(1e-30) / 1e-30 = 1 instead of 0/0 (the bias is far below one ulp of any other phase)
 __device__ __forceinline__ float sinc_abs_r(float q, float h) {
@@ -342,7 +377,33 @@ template <int LC>
 __device__ __forceinline__ double lambda1_class(double t);
 __device__ __forceinline__ double lambda1_x2_small(double x2);
 __device__ __forceinline__ float lambda1_r(float x) { return lambda1_x2(x * x); }
-__device__ __forceinline__ double lambda1_r(double x) { return (x == 0.0) ? 1.0 : (2.0 * j1(x)) / x; }
+// fp64 Lambda(x) = 2 J1(x)/x, x >= 0, of the tracer's own (gen_j1_f64.py): a Chebyshev series in x^2 up to x = 8, the
+// Hankel form with Chebyshev series for P and x Q beyond; about 3e-16 absolute.  Coefficients in constant memory,
+// Clenshaw recurrence (the power basis of a degree-14 fit loses five digits).  x > 1e6 goes to the library.
+template <int N>
+__device__ __forceinline__ double clenshaw(const double (&c)[N], double t) {
+  const double t2 = t + t;
+  double b1 = c[N - 1], b2 = 0.0;
+#pragma unroll
+  for (int k = N - 2; k >= 1; --k) {
+    const double b0 = fma(t2, b1, c[k] - b2);
+    b2 = b1;
+    b1 = b0;
+  }
+  return fma(t, b1, c[0] - b2);
+}
+__device__ __forceinline__ double lambda1_r(double x) {
+  if (x <= 8.0) return clenshaw(c_j1a, fma(x * x, 0.03125, -1.0));
+  if (x > 1.0e6) return (2.0 * j1(x)) / x;
+  const double inv = 1.0 / x;
+  const double t = fma(128.0 * inv, inv, -1.0);
+  const double P = clenshaw(c_j1p, t), Q = clenshaw(c_j1q, t) * inv;
+  double s, c;
+  sincos_cw(x, s, c);
+  // J1 = sqrt(2/(pi x)) (P cos(x - 3pi/4) - Q sin(x - 3pi/4)) = sqrt(1/(pi x)) (P (s - c) + Q (s + c))
+  const double j = (0.5641895835477563 * sqrt(inv)) * fma(P, s - c, Q * (s + c));
+  return (2.0 * j) * inv;
+}
 __device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(x2)); }
 __device__ __forceinline__ double lambda1_x2_small(double x2) { return lambda1_r(sqrt(x2)); }
 template <int LC>

@@ -79,15 +79,15 @@ __device__ __forceinline__ void particle_frame(const ExpParams& P, const PhiloxK
     const double u8 = uniform_from_word(w2[0]), u9 = uniform_from_word(w2[1]), u10 = uniform_from_word(w2[2]);
     double ct, st, sp, cp, ss, cs;
     if (P.orient_kind == 3) {  // theta = pi u8
-      if (LIBM) sincospi(u8, &st, &ct); else sincos_2pi(0.5 * u8, st, ct);
+      if (LIBM) sincospi_cw(u8, st, ct); else sincos_2pi(0.5 * u8, st, ct);
     } else {                   // cos(theta) = 1 - 2 u8
       ct = 1.0 - 2.0 * u8;
       st = sqrt(1.0 - ct * ct);
     }
     if (LIBM) {
       // sincospi reduces exactly and has no large-argument path: within 1e-15 of sin/cos(TWO_PI u) as R-A3 writes it
-      sincospi(2.0 * u9, &sp, &cp);
-      sincospi(2.0 * u10, &ss, &cs);
+      sincospi_cw(2.0 * u9, sp, cp);
+      sincospi_cw(2.0 * u10, ss, cs);
     } else {
       sincos_2pi(u9, sp, cp);
       sincos_2pi(u10, ss, cs);
@@ -115,7 +115,9 @@ __device__ __forceinline__ double draw_rel_size(const PhiloxKeys& keys, uint32_t
     uint32_t w[4];
     philox4x32_10(keys, id_lo, id_hi, 3u + t, exp_word, w);
     const double ua = uniform_from_word(k ? w[2] : w[0]), ub = uniform_from_word(k ? w[3] : w[1]);
-    const double x = 1.0 + rel * (sqrt(-2.0 * log(ua)) * cos(6.283185307179586 * ub));
+    double sb, cb;
+    sincos_cw(6.283185307179586 * ub, sb, cb);
+    const double x = 1.0 + rel * (sqrt(-2.0 * log(ua)) * cb);
     if (x > 0.0) return x;
   }
   return 1.0;
@@ -203,7 +205,9 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
       const double z = fma(half, c_gl[i], mid);
       const double dz = z - zc;
       const double rho2 = fmax(Rb * Rb - dz * dz, 0.0);
-      sum = fma(c_gl[GL_N + i], ((PI_D * rho2) * lambda1_r(qab * sqrt(rho2))) * cos(qC * z), sum);
+      double sz, cz;
+      sincos_d(qC * z, sz, cz);
+      sum = fma(c_gl[GL_N + i], ((PI_D * rho2) * lambda1_r(qab * sqrt(rho2))) * cz, sum);
     }
     const double pz = z1 - zc, qz = z0 - zc;
     const double Vcyl = (PI_D * (R * R)) * L;

@@ -132,6 +132,39 @@ __device__ __forceinline__ void sincos_cw(double x, double& s, double& c) {
   s = (k & 2) ? -ss : ss;
   c = ((k + 1) & 2) ? -cc : cc;
 }
+// sin u - u cos u, u >= 0, without the cancellation of the direct form at small u: the reduction gives u = k pi/2 + r,
+// sin r = r + r z S(z), cos r = 1 + z C(z) (z = r^2); for k = 0 (u < pi/4) sin u - u cos u = r z (S - C) exactly in
+// the polynomials, elsewhere the direct form is well conditioned.  No branch, no series (R-C12's series of Phi serves
+// the same purpose in the oracle).
+__device__ __forceinline__ double sin_minus_ucos(double u) {
+  const double t = fma(u, c_sincos[0], 6755399441055744.0);
+  const int k = __double2loint(t);
+  const double nf = t - 6755399441055744.0;
+  double r = fma(-nf, c_sincos[1], u);
+  r = fma(-nf, c_sincos[2], r);
+  r = fma(-nf, c_sincos[3], r);
+  const double z = r * r;
+  double S = fma(z, c_sincos[10], c_sincos[9]);
+  S = fma(S, z, c_sincos[8]);
+  S = fma(S, z, c_sincos[7]);
+  S = fma(S, z, c_sincos[6]);
+  S = fma(S, z, c_sincos[5]);
+  S = fma(S, z, c_sincos[4]);
+  double C = fma(z, c_sincos[19], c_sincos[18]);
+  C = fma(C, z, c_sincos[17]);
+  C = fma(C, z, c_sincos[16]);
+  C = fma(C, z, c_sincos[15]);
+  C = fma(C, z, c_sincos[14]);
+  C = fma(C, z, c_sincos[13]);
+  C = fma(C, z, c_sincos[12]);
+  const double rz = r * z;
+  const double ps = fma(rz, S, r), pc = fma(C, z, 1.0);
+  const double ss = (k & 1) ? pc : ps;
+  const double cc = (k & 1) ? ps : pc;
+  const double sn = (k & 2) ? -ss : ss;
+  const double cs = ((k + 1) & 2) ? -cc : cc;
+  return (k == 0) ? rz * (S - C) : fma(-u, cs, sn);
+}
 __device__ __forceinline__ void sincos_d(double x, double& s, double& c) {
   if (fabs(x) > 1.0e6) { sincos(x, &s, &c); return; }
   sincos_cw(x, s, c);

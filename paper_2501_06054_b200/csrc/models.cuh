@@ -328,7 +328,7 @@ __device__ __forceinline__ double eval_intensity_generic(const ExpParams& P, con
 
 // fp64 node loop of the polydisperse sphere: w (drho V)^2 Phi(u)^2 = [16 pi^2 drho^2 w] (sin u - u cos u)^2 / q^6,
 // u = q R: the bracket is the node's fourth table entry and 1 / q^6 multiplies the sum once, so the loop has no
-// division; below u = 0.5, where sin u - u cos u cancels, the node takes the series of Phi (R-C12).  u < 1e6
+// division; sin u - u cos u is formed without cancellation at any u (device_math.cuh: sin_minus_ucos).  u < 1e6
 // (sas_set_model).  Out of line: inlined, its registers cost the one-evaluation kernels (c0, c4) 2 %.
 __device__ __forceinline__ void lds_f64x2(uint32_t addr, double& x, double& y) {
   asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(addr));
@@ -336,23 +336,16 @@ __device__ __forceinline__ void lds_f64x2(uint32_t addr, double& x, double& y) {
 // (ta: shared-window address of the node table {R, -, w (drho V)^2, 16 pi^2 drho^2 w} in doubles)
 __device__ __noinline__ double sphere_nodes_fp64(uint32_t ta, int n_a, double qd, double q2d) {
   const double iq2 = 1.0 / q2d;
-  double direct = 0.0, small = 0.0;
+  double direct = 0.0;
+#pragma unroll 4
   for (int a = 0; a < n_a; ++a) {
     double R, unused, w_small, w_direct;
     lds_f64x2(ta + 32u * (uint32_t)a, R, unused);
     lds_f64x2(ta + 32u * (uint32_t)a + 16u, w_small, w_direct);
-    const double u = qd * R;
-    if (u < 0.5) {
-      const double ph = sphere_phi(u);
-      small = fma(w_small, ph * ph, small);
-    } else {
-      double sn, cs;
-      sincos_cw(u, sn, cs);
-      const double d = fma(-u, cs, sn);
-      direct = fma(w_direct, d * d, direct);
-    }
+    const double d = sin_minus_ucos(qd * R);
+    direct = fma(w_direct, d * d, direct);
   }
-  return fma(direct, (iq2 * iq2) * iq2, small);
+  return direct * ((iq2 * iq2) * iq2);
 }
 
 // Model table meaning (host: fill_model).  Lengths that multiply a projection of Q are stored as a

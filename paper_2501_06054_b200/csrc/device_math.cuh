@@ -297,19 +297,8 @@ __device__ __forceinline__ float sphere_phi_core(float u, float lo) {
 }
 __device__ __forceinline__ float sphere_phi(float u) { return sphere_phi_core<true>(u, 0.0f); }
 __device__ __forceinline__ double sphere_phi(double u) {
-  if (u < 0.5) {
-    const double u2 = u * u;
-    double s = 1.0 / 31135104000.0;
-    s = fma(s, u2, -1.0 / 172972800.0);
-    s = fma(s, u2, 1.0 / 1330560.0);
-    s = fma(s, u2, -1.0 / 15120.0);
-    s = fma(s, u2, 1.0 / 280.0);
-    s = fma(s, u2, -0.1);
-    return fma(s, u2, 1.0);
-  }
-  double s, c;
-  sincos_d(u, s, c);
-  return (3.0 * fma(-u, c, s)) / ((u * u) * u);
+  if (u < 1.0e-8) return 1.0;   // Phi = 1 - u^2/10 + ...: 1 to the last bit
+  return (3.0 * sin_minus_ucos(u)) / ((u * u) * u);
 }
 
 // ---------------------------------------------------------------- sinc

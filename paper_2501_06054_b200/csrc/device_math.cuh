@@ -399,7 +399,7 @@ template <int LC>
 __device__ __forceinline__ double lambda1_class(double t);
 __device__ __forceinline__ double lambda1_x2_small(double x2);
 __device__ __forceinline__ float lambda1_r(float x) { return lambda1_x2(x * x); }
-// fp64 Lambda(x) = 2 J1(x)/x, x >= 0, of the tracer's own (gen_j1_f64.py): a Chebyshev series in x^2 up to x = 8, the
+// fp64 Lambda(x) = 2 J1(x)/x, x >= 0, of the tracer's own (gen_j1_f64.py): a Chebyshev series in x^2 up to x = 12, the
 // Hankel form with Chebyshev series for P and x Q beyond; about 3e-16 absolute.  Coefficients in constant memory,
 // Clenshaw recurrence (the power basis of a degree-14 fit loses five digits).  x > 1e6 goes to the library.
 template <int N>
@@ -415,10 +415,10 @@ __device__ __forceinline__ double clenshaw(const double (&c)[N], double t) {
   return fma(t, b1, c[0] - b2);
 }
 __device__ __forceinline__ double lambda1_r(double x) {
-  if (x <= 8.0) return clenshaw(c_j1a, fma(x * x, 0.03125, -1.0));
+  if (x <= SAS_J1_XA) return clenshaw(c_j1a, fma(x * x, SAS_J1_A_SCALE, -1.0));
   if (x > 1.0e6) return (2.0 * j1(x)) / x;
   const double inv = 1.0 / x;
-  const double t = fma(128.0 * inv, inv, -1.0);
+  const double t = fma(SAS_J1_B_SCALE * inv, inv, -1.0);
   const double P = clenshaw(c_j1p, t), Q = clenshaw(c_j1q, t) * inv;
   double s, c;
   sincos_cw(x, s, c);

@@ -81,19 +81,19 @@ MODEL_COST = {
     # (counted, c1 fp32)
     "sphere_py_fp32": (U(123, wide=1, imad=1, logic=24, fp64=14, fp32=69, xu=14), U(32.4, imad=0.2, logic=1.2, fp32=30, xu=1)),
     # (counted, c1 fp64)
-    "sphere_py_fp64": (U(133, wide=1, logic=27, fp64=101, fp32=1, xu=3), U(63.5, logic=15, fp64=47.5, xu=1)),
+    "sphere_py_fp64": (U(138, wide=1, imad=1, logic=32, fp64=101, fp32=1, xu=3), U(45.2, logic=15.2, fp64=30)),
     # (round-1 SASS count of the node; prologue estimate)
     "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(27, logic=1, fp32=25, xu=1)),
     # (counted, c3) prologue = Philox block 2 (orientation draws), three sincos of 2 pi u, frame, and the 16 outer
     # nodes (37 instructions each); inner node 34
     "cs_triaxial_iso_fp32": (U(832, wide=19, imad=18.5, logic=136, fp64=114, fp32=499, xu=47), U(34, imad=0.5, logic=2.5, fp32=29, xu=2)),
     # (estimate: the per-event cylinder below without its size draws)
-    "cylinder_iso_fp64": (U(400, wide=37, logic=147, fp64=200, xu=15), U(0)),
-    # (counted, n1) per-event sizes: Philox blocks 2 and 3 and a re-draw, two Box-Muller normals, three sincospi,
-    # sin, j1, the weight
-    "cylinder_event_fp64": (U(624, wide=56, imad=3, logic=187, fp64=350, fp32=5, xu=23), U(0)),
+    "cylinder_iso_fp64": (U(370, wide=37, logic=120, fp64=200, xu=6), U(0)),
+    # (counted, n1) per-event sizes: Philox blocks 2 and 3 and a re-draw, two Box-Muller normals, three sin/cos of
+    # pi x, sin, Lambda, the weight
+    "cylinder_event_fp64": (U(562, wide=56, imad=3, logic=150, fp64=344, fp32=2, xu=7), U(0)),
     # (estimate) barbell, per event: the prologue of the per-event cylinder, then 64 slice evaluations
-    "barbell_event_fp64": (U(624, wide=56, imad=3, logic=187, fp64=350, fp32=5, xu=23), U(70, logic=8, fp64=58, xu=2)),
+    "barbell_event_fp64": (U(562, wide=56, imad=3, logic=150, fp64=344, fp32=2, xu=7), U(70, logic=8, fp64=58, xu=2)),
     # (estimate) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
     "micelle_event_fp64": (U(330, wide=19, logic=60, fp64=230, xu=8), U(0)),
 }

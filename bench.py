@@ -452,6 +452,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     import paper_2501_06054_b200 as S
     from paper_2501_06054_b200 import roofline as R
+    from paper_2501_06054_b200 import build as libbuild
+    if rank == 0:
+        libbuild.build()          # no-op when the in-tree library is up to date; nvcc otherwise
+    if world > 1:
+        dist.barrier()
     S.load_library()              # raises if libsas_b200.so is missing: no fallback
 
     if args.sweep:

@@ -295,6 +295,25 @@ __device__ __forceinline__ float sphere_phi_core(float u, float lo) {
   const float sel = (kb == __float_as_int(SAS_ROUND_MAGIC)) ? (S - C) : dir;
   return 3.0f * sel;
 }
+// sin u - u cos u in fp32 (the numerator of Phi without its 1/u^3): same reduction and polynomials as
+// sphere_phi_core; r z (S - C) when u reduces with k = 0 (no cancellation), the direct form elsewhere.  Sign dropped
+// (callers square it).
+__device__ __forceinline__ float sin_minus_ucos_abs(float u, float lo) {
+  const float t = fmaf(u, 0.318309886f, SAS_ROUND_MAGIC);
+  const int kb = __float_as_int(t);
+  const float kf = t - SAS_ROUND_MAGIC;
+  float r = fmaf(kf, -3.14159250259399414062e+00f, u);
+  r = fmaf(kf, -1.50995788317231927067e-07f, r);
+  r += lo;
+  const float z = r * r;
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  const float CP[SAS_COSPI_POLY_N] = SAS_COSPI_POLY;
+  const float S = horner(SP, z), C = horner(CP, z);
+  const float rz = r * z;
+  const float sr = fmaf(rz, S, r);
+  const float cr = fmaf(z, C, 1.0f);
+  return (kb == __float_as_int(SAS_ROUND_MAGIC)) ? rz * (S - C) : fmaf(-u, cr, sr);
+}
 __device__ __forceinline__ float sphere_phi(float u) { return sphere_phi_core<true>(u, 0.0f); }
 __device__ __forceinline__ double sphere_phi(double u) {
   if (u < 1.0e-8) return 1.0;   // Phi = 1 - u^2/10 + ...: 1 to the last bit

@@ -386,6 +386,19 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
     case 0: {  // sphere
       if (sizeof(Real) == 8 && P.n_a > 1) {
         acc = (Real)sphere_nodes_fp64((uint32_t)__cvta_generic_to_shared(T.ta), P.n_a, qd, q2d);
+      } else if (sizeof(Real) == 4 && P.n_a > 1) {
+        // fp32 node loop: w (drho V)^2 Phi(u)^2 = [16 pi^2 drho^2 w] (sin u - u cos u)^2 / q^6: the bracket is the
+        // node's fourth table entry, 1 / q^6 multiplies the sum once (no reciprocal and no u^-3 per node)
+        const Proj<float> qp = make_proj<float>(qd);
+        float direct = 0.0f;
+        for (int a = 0; a < P.n_a; ++a) {
+          const float* r = reinterpret_cast<const float*>(T.ta) + a * TA_W;
+          const Phase<float> ph = phase_mul(qp, r[0], r[1]);
+          const float d = sin_minus_ucos_abs(ph.hi, ph.lo);
+          direct = fmaf(r[3], d * d, direct);
+        }
+        const double iq2 = 1.0 / q2d;
+        acc = (Real)((double)direct * ((iq2 * iq2) * iq2));
       } else {
         const Proj<Real> qp = make_proj<Real>(qd);
         for (int a = 0; a < P.n_a; ++a) {

@@ -77,9 +77,9 @@ MODEL_COST = {
     # (counted, c0) one fp64 evaluation, all of it in the prologue
     "sphere_fp64": (U(94, wide=1, imad=1, logic=27, fp64=63, xu=2), U(0)),
     # (estimate: sphere_py_fp32 without its S(q))
-    "sphere_fp32": (U(80, wide=1, imad=1, logic=22, fp64=14, fp32=30, xu=12), U(32.4, imad=0.2, logic=1.2, fp32=30, xu=1)),
+    "sphere_fp32": (U(90, wide=1, imad=1, logic=22, fp64=22, fp32=30, xu=14), U(28.4, logic=1.2, fp32=27.2)),
     # (counted, c1 fp32)
-    "sphere_py_fp32": (U(123, wide=1, imad=1, logic=24, fp64=14, fp32=69, xu=14), U(32.4, imad=0.2, logic=1.2, fp32=30, xu=1)),
+    "sphere_py_fp32": (U(135.6, wide=1, imad=1, logic=24.6, fp64=22, fp32=69, xu=17), U(28.4, logic=1.2, fp32=27.2)),
     # (counted, c1 fp64)
     "sphere_py_fp64": (U(138, wide=1, imad=1, logic=32, fp64=101, fp32=1, xu=3), U(45.2, logic=15.2, fp64=30)),
     # (round-1 SASS count of the node; prologue estimate)

@@ -644,7 +644,6 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   a.tab_len_max = c->tab_len_max;
   const int grid = (int)std::min<uint64_t>((uint64_t)grid_full, n_items);
   a.work_base = c->work_base;
-  if (n_items > (uint64_t)grid) c->work_base += (uint32_t)n_items;  // the fetches this launch will make (sas_types.h)
   a.use_exp0 = (!c->batch && c->n_exp == 1) ? 1 : 0;
   if (a.use_exp0) a.exp0 = c->h_exps[0];
   const bool timed = !DUMP && c->n_timed < (uint64_t)MAX_TIMED;
@@ -660,6 +659,7 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   }
   kern<<<grid, BLOCK_THREADS, smem, c->stream>>>(a);
   CUDA_TRY(c, cudaGetLastError());
+  if (n_items > (uint64_t)grid) c->work_base += (uint32_t)n_items;  // the fetches this launch makes (sas_types.h)
   if (timed) {
     CUDA_TRY(c, cudaEventRecord(c->ev1[c->n_timed], c->stream));
     sas_launch_record r;

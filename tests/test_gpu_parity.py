@@ -664,6 +664,24 @@ def test_fp32_request_with_phases_beyond_the_proven_range_runs_in_fp64(sas):
         tr.close()
 
 
+@pytest.mark.parametrize("name,over", [
+    ("big_cylinder_iso", dict(model="cylinder", size=[300.0, 3000.0, 0, 0], orient_kind="isotropic_mc")),
+    ("big_cylinder_event", dict(model="cylinder", size=[300.0, 3000.0, 0, 0], pd_kind=["gauss_mc", "gauss_mc"],
+                                pd_rel=[0.1, 0.1], orient_kind="uniform_angles_mc")),
+    ("big_sphere_schulz", dict(model="sphere", size=[2000.0, 0, 0, 0], pd_kind=["schulz", "none"], pd_rel=[0.05, 0],
+                               pd_nodes=[16, 1])),
+    ("big_core_shell_sphere", dict(model="core_shell_sphere", size=[800.0, 150.0, 0, 0], sld=[3e-6, 1e-6, 0],
+                                   pd_kind=["schulz", "schulz"], pd_rel=[0.05, 0.1], pd_nodes=[6, 5])),
+    ("big_hollow_cylinder", dict(model="hollow_cylinder", size=[250.0, 2000.0, 40.0, 0], orient_kind="isotropic_mc")),
+])
+def test_large_arguments_of_the_fp64_special_functions(sas, name, over):
+    """The tracer's own fp64 sin/cos, sin u - u cos u and Lambda = 2 J1(x)/x far beyond the arguments of the
+    BASELINE.json workloads: q x size up to 600 rad (sphere), 450 rad (sinc of the rod) and x = 90 (Lambda: the
+    Hankel range, x > 12, for most detected neutrons), against the oracle's glibc sin, cos, j1 at 1e-12."""
+    model = W.model(precision="fp64", **over)
+    check_dump(sas, W.instrument(det_dist=3.0), model, 4242, 0, 200000, tol=1e-12, min_detected=8000)
+
+
 def test_context_stays_on_its_device(sas):
     """A context lives on the device it was created on, whatever torch's current device is (multi-GPU ranks);
     with one GPU only the default-device behaviour can be checked."""

@@ -36,7 +36,7 @@ _MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3,
           "barbell": 9, "capped_cylinder": 10, "elliptical_cylinder": 11, "hollow_cylinder": 12,
           "core_shell_ellipsoid": 13, "polymer_micelle": 14}
 _ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
-_SQ = {"none": 0, "hard_sphere_py": 1}
+_SQ = {"none": 0, "hard_sphere_py": 1, "hayter_msa": 2}
 
 
 class Instrument(C.Structure):
@@ -61,7 +61,8 @@ class Model(C.Structure):
                 ("n_or", C.c_int32 * 2),
                 ("or_d", (C.c_double * MAX_NODES) * 2), ("or_w", (C.c_double * MAX_NODES) * 2),
                 ("sq_radius_eff", C.c_double), ("sq_volfrac", C.c_double),
-                ("pd_mc", C.c_int32 * 2), ("pd_rel", C.c_double * 2)]
+                ("pd_mc", C.c_int32 * 2), ("pd_rel", C.c_double * 2),
+                ("sq_contact_kT", C.c_double), ("sq_kappa_sigma", C.c_double), ("msa", C.c_double * 5)]
 
 
 class Record(C.Structure):
@@ -102,6 +103,8 @@ def lib():
             f.restype = C.c_double
         L.orc_micelle_f2.argtypes = [C.POINTER(Model), C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_micelle_f2.restype = C.c_double
+        L.orc_msa_sq.argtypes = [C.c_double, C.POINTER(Model)]
+        L.orc_msa_sq.restype = C.c_double
         L.orc_py_sq.argtypes = [C.c_double] * 3
         L.orc_py_sq.restype = C.c_double
         L.orc_intensity.argtypes = [C.POINTER(Model), C.POINTER(C.c_double), C.POINTER(C.c_double),
@@ -168,6 +171,61 @@ def make_instrument(d: dict) -> Instrument:
     return ins
 
 
+def msa_residual(u, eta, gam, k, X, W):
+    """The five equations of DESIGN.md R-S2 for u = (a, b, E, C', H'); X, W: Gauss-Legendre rule on [0, 1]."""
+    a, b, E, Cp, Hp = u
+    e = np.exp(-k)
+    Dp = E * e - Cp                                        # Q is continuous at the contact distance
+    qin = lambda x: 0.5 * a * (x * x - 1.0) + b * (x - 1.0) + E * np.exp(-k * x) - Cp
+    Q = qin(X)
+    I0, I1, Qt = (W * Q).sum(), (W * X * Q).sum(), (W * Q * np.exp(-k * X)).sum()
+    r1 = a - (1.0 - 12.0 * eta * (I0 + Dp / k))
+    r2 = b - 12.0 * eta * (I1 + Dp * (1.0 / k + 1.0 / k ** 2))
+    r3 = -k * E + 12.0 * eta * Dp * ((1.0 + k) / k ** 2 + Hp)
+    r4 = k * Dp * (1.0 - 12.0 * eta * (Qt + Dp * e / (2.0 * k))) + gam
+    phi1 = (1.0 - e * (1.0 + k)) / k ** 2
+    # T = D' phi1 / 2k + int_0^1 -(1 - y) e^{ky} [int_y^1 Q e^{-ks} ds + D' e^{-k}/2k] dy: the inner integral by the same
+    # rule mapped onto [y, 1] for every outer node y (rows: outer nodes, columns: inner nodes)
+    s2 = X[:, None] + (1.0 - X[:, None]) * X[None, :]
+    G = ((1.0 - X[:, None]) * W[None, :] * qin(s2) * np.exp(-k * s2)).sum(axis=1) + Dp * e / (2.0 * k)
+    T = Dp * phi1 / (2.0 * k) + (W * (-(1.0 - X)) * np.exp(k * X) * G).sum()
+    r5 = Hp * (1.0 - 12.0 * eta * Qt) - Dp / 2.0 - 12.0 * eta * T
+    return np.array([r1, r2, r3, r4, r5])
+
+
+def msa_solve(eta: float, gam: float, k: float, steps: int = 20):
+    """Mean-spherical closure for hard spheres (packing eta, diameter 1) with the Yukawa repulsion
+    beta u(x) = gam exp(-k (x - 1)) / x, x > 1 (DESIGN.md R-S2): g(x) = 0 inside the core, c(x) = -beta u(x)
+    outside, through the Baxter / Hoye-Blum factorisation.  Returns (a, b, E, C', D'): Q(x) = a (x^2 - 1)/2 +
+    b (x - 1) + E exp(-k x) - C' for x < 1 and D' exp(-k (x - 1)) beyond.  Newton's method on the five equations,
+    started from the Percus-Yevick solution (gam = 0) and continued in `steps` equal steps of gam, which keeps
+    the branch that is connected to the uncharged fluid."""
+    g, w = np.polynomial.legendre.leggauss(64)
+    X, W = 0.5 * (g + 1.0), 0.5 * w
+    u = np.array([(1.0 + 2.0 * eta) / (1.0 - eta) ** 2, -1.5 * eta / (1.0 - eta) ** 2, 0.0, 0.0, 0.0])
+    for gs in np.linspace(0.0, gam, steps + 1):
+        for _ in range(60):
+            r = msa_residual(u, eta, gs, k, X, W)
+            J = np.zeros((5, 5))
+            for j in range(5):
+                du = np.zeros(5)
+                du[j] = 1e-6 * max(1.0, abs(u[j]))
+                J[:, j] = (msa_residual(u + du, eta, gs, k, X, W) - msa_residual(u - du, eta, gs, k, X, W)) / (2.0 * du[j])
+            st = np.linalg.solve(J, -r)
+            u = u + st
+            if np.abs(st).max() < 1e-15 * max(1.0, np.abs(u).max()):
+                break
+    if np.abs(msa_residual(u, eta, gam, k, X, W)).max() > 1e-11:
+        raise ValueError("the mean-spherical closure did not converge")
+    a, b, E, Cp, _ = u
+    return np.array([a, b, E, Cp, E * np.exp(-k) - Cp])
+
+
+def msa_sq(model_d: dict, q: float) -> float:
+    m = model_d if isinstance(model_d, Model) else make_model(model_d)
+    return lib().orc_msa_sq(float(q), C.byref(m))
+
+
 def make_model(d: dict) -> Model:
     m = Model()
     m.model = _MODEL[d["model"]]
@@ -205,6 +263,12 @@ def make_model(d: dict) -> Model:
             m.or_w[k][i] = w[i]
     m.sq_radius_eff = d["sq_radius_eff"]
     m.sq_volfrac = d["sq_volfrac"]
+    m.sq_contact_kT = d.get("sq_contact_kT", 0.0)
+    m.sq_kappa_sigma = d.get("sq_kappa_sigma", 0.0)
+    if d["sq_kind"] == "hayter_msa":
+        sol = msa_solve(d["sq_volfrac"], m.sq_contact_kT, m.sq_kappa_sigma)
+        for i in range(5):
+            m.msa[i] = sol[i]
     if "gauss_mc" in d["pd_kind"] and (d["orient_kind"] == "gauss_quad" or "schulz" in d["pd_kind"]):
         raise ValueError("per-event sizes (gauss_mc) do not combine with fixed-node averages (DESIGN.md R-N1)")
     if d["orient_kind"] == "gauss_quad" and d["model"] != "cylinder":

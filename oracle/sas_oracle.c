@@ -131,31 +131,58 @@ double orc_py_sq(double q, double r_eff, double volfrac) {
   return 1.0 / (1.0 + (24.0 * phi) * ((alpha * t1 + beta * t2) + gamma * t3));
 }
 
-/* 32-node Gauss-Legendre rule on [-1, 1] (nodes ascending, weights summing to 2): Newton iteration on the
- * Legendre polynomial P_32 from the Chebyshev-like starting points, the textbook construction. */
+/* n-node Gauss-Legendre rule on [-1, 1] (nodes ascending, weights summing to 2): Newton iteration on the
+ * Legendre polynomial P_n from the Chebyshev-like starting points, the textbook construction. */
+static void gl_rule(int n, double* xs, double* ws) {
+  for (int i = 0; i < n; ++i) {
+    double x = cos(PI_ * ((double)i + 0.75) / ((double)n + 0.5));
+    double dp = 1.0;
+    for (int it = 0; it < 100; ++it) {
+      double p0 = 1.0, p1 = x;
+      for (int k = 2; k <= n; ++k) {
+        double pk = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
+        p0 = p1; p1 = pk;
+      }
+      dp = n * (x * p1 - p0) / (x * x - 1.0);
+      double dx = p1 / dp;
+      x -= dx;
+      if (fabs(dx) < 1e-16) break;
+    }
+    xs[n - 1 - i] = x;
+    ws[n - 1 - i] = 2.0 / ((1.0 - x * x) * dp * dp);
+  }
+}
 #define ORC_GL_N 32
 static double gl_x[ORC_GL_N], gl_w[ORC_GL_N];
 static int gl_ready = 0;
 static void gl_init(void) {
   if (gl_ready) return;
-  for (int i = 0; i < ORC_GL_N; ++i) {
-    double x = cos(PI_ * ((double)i + 0.75) / ((double)ORC_GL_N + 0.5));
-    double dp = 1.0;
-    for (int it = 0; it < 100; ++it) {
-      double p0 = 1.0, p1 = x;
-      for (int k = 2; k <= ORC_GL_N; ++k) {
-        double pk = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
-        p0 = p1; p1 = pk;
-      }
-      dp = ORC_GL_N * (x * p1 - p0) / (x * x - 1.0);
-      double dx = p1 / dp;
-      x -= dx;
-      if (fabs(dx) < 1e-16) break;
-    }
-    gl_x[ORC_GL_N - 1 - i] = x;
-    gl_w[ORC_GL_N - 1 - i] = 2.0 / ((1.0 - x * x) * dp * dp);
-  }
+  gl_rule(ORC_GL_N, gl_x, gl_w);
   gl_ready = 1;
+}
+
+/* R-S2: Hayter-Penfold MSA structure factor from the Baxter function the caller solved for (sas_oracle.h).
+ * With x in units of the diameter and K = q sigma:
+ *   Qhat(K) = 1 - 12 eta [ int_0^1 Q_in(x) e^{iKx} dx + D' e^{iK} / (k - iK) ],   S = 1 / |Qhat|^2. */
+double orc_msa_sq(double q, const orc_model* m) {
+  static double x64[64], w64[64];
+  static int ready = 0;
+  if (!ready) { gl_rule(64, x64, w64); ready = 1; }
+  double K = q * (2.0 * m->sq_radius_eff), eta = m->sq_volfrac, k = m->sq_kappa_sigma;
+  double a = m->msa[0], b = m->msa[1], E = m->msa[2], Cp = m->msa[3], Dp = m->msa[4];
+  double re = 0.0, im = 0.0;
+  for (int j = 0; j < 64; ++j) {
+    double x = 0.5 * (x64[j] + 1.0), w = 0.5 * w64[j];
+    double Qin = ((0.5 * a) * (x * x - 1.0) + b * (x - 1.0)) + (E * exp(-k * x) - Cp);
+    re += (w * Qin) * cos(K * x);
+    im += (w * Qin) * sin(K * x);
+  }
+  double den = k * k + K * K;
+  re += Dp * (k * cos(K) - K * sin(K)) / den;   /* Re, Im of e^{iK} / (k - iK) = e^{iK} (k + iK) / (k^2 + K^2) */
+  im += Dp * (k * sin(K) + K * cos(K)) / den;
+  re = 1.0 - (12.0 * eta) * re;
+  im = -(12.0 * eta) * im;
+  return 1.0 / (re * re + im * im);
 }
 
 /* R-M2: end piece of a body of revolution about C: the part z in [L/2, zc + Rb] of the sphere of radius Rb
@@ -478,6 +505,7 @@ double orc_intensity(const orc_model* m, const double Q[3], const double u_or[3]
     }
   double S = 1.0;
   if (m->sq_kind == ORC_SQ_HARD_SPHERE_PY) S = orc_py_sq(qm, m->sq_radius_eff, m->sq_volfrac);
+  if (m->sq_kind == ORC_SQ_HAYTER_MSA) S = orc_msa_sq(qm, m);
   if (env_out) *env_out = ((1.0e8 * m->scale) * (SE2 / SV)) * S + m->background;
   return ((1.0e8 * m->scale) * (SF2 / SV)) * S + m->background;
 }
@@ -504,6 +532,7 @@ double orc_intensity_event(const orc_model* m, const double Q[3], const double u
   }
   double S = 1.0;
   if (m->sq_kind == ORC_SQ_HARD_SPHERE_PY) S = orc_py_sq(qm, m->sq_radius_eff, m->sq_volfrac);
+  if (m->sq_kind == ORC_SQ_HAYTER_MSA) S = orc_msa_sq(qm, m);
   if (env_out) *env_out = ((1.0e8 * m->scale) * (E2 / V)) * S + m->background;
   return ((1.0e8 * m->scale) * (F2 / V)) * S + m->background;
 }

@@ -68,7 +68,10 @@ enum {
   ORC_ORIENT_ISOTROPIC_MC = 2,
   ORC_ORIENT_UNIFORM_ANGLES_MC = 3 /* PAPER.md:131-133 as printed: theta~U[0,pi], phi, psi~U[0,2pi] (R-N3) */
 };
-enum { ORC_SQ_NONE = 0, ORC_SQ_HARD_SPHERE_PY = 1 };
+/* ORC_SQ_HAYTER_MSA (R-S2; Table II group F "Hayter MSA"): mean-spherical closure for hard spheres of
+ * diameter 2 sq_radius_eff with a screened-Coulomb (Yukawa) repulsion of contact value sq_contact_kT and inverse
+ * screening length sq_kappa_sigma (in units of the diameter) */
+enum { ORC_SQ_NONE = 0, ORC_SQ_HARD_SPHERE_PY = 1, ORC_SQ_HAYTER_MSA = 2 };
 
 #define ORC_MAX_NODES 64
 
@@ -116,6 +119,10 @@ typedef struct {
    * the fixed-node tables of axis k must then be the single node (1.0, 1.0). */
   int32_t pd_mc[2];
   double pd_rel[2];
+  /* R-S2: the caller (oracle/oracle.py: msa_solve) solved the closure: Baxter function inside the core
+   * Q(x) = a (x^2 - 1)/2 + b (x - 1) + E exp(-k x) - C', outside D' exp(-k (x - 1)); msa = {a, b, E, C', D'} */
+  double sq_contact_kT, sq_kappa_sigma;
+  double msa[5];
 } orc_model;
 
 /* full per-neutron record, for pins and parity */
@@ -145,6 +152,10 @@ double orc_uniform(uint32_t word);
 double orc_debye(double x);
 double orc_chain_psi(double x);
 double orc_micelle_f2(const orc_model* m, double q, double x0, double* vol, double* env2);
+
+/* R-S2: S(q) = 1 / |Qhat(K)|^2, K = 2 q R_eff, Qhat(K) = 1 - 12 eta int_0^inf Q(x) exp(i K x) dx: the core part by the
+ * 64-node Gauss-Legendre rule, the tail in closed form */
+double orc_msa_sq(double q, const orc_model* m);
 
 /* form / structure factor pieces (PAPER.md:37-49 Eq.1-4, :161-163 Eq.9) */
 double orc_sphere_phi(double u);                 /* 3(sin u - u cos u)/u^3 */

@@ -41,6 +41,7 @@ BASE_MODEL = dict(
     orient_kind="fixed", theta=0.0, phi=0.0, psi=0.0,
     sigma_theta=0.0, sigma_phi=0.0, n_theta=1, n_phi=1,
     sq_kind="none", sq_radius_eff=0.0, sq_volfrac=0.0,
+    sq_contact_kT=0.0, sq_kappa_sigma=0.0,     # "hayter_msa": contact potential in kT, inverse screening length x diameter
 )
 
 

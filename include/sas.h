@@ -100,7 +100,18 @@ enum {
    * (SAS_EUNSUPPORTED); evaluated in fp64 whatever `precision` says. */
   SAS_PD_GAUSS_MC = 2
 };
-enum { SAS_SQ_NONE = 0, SAS_SQ_HARD_SPHERE_PY = 1 };
+enum {
+  SAS_SQ_NONE = 0,
+  SAS_SQ_HARD_SPHERE_PY = 1,
+  /* Hayter-Penfold MSA (Table II group F; DESIGN.md R-S2): mean-spherical closure for hard spheres of
+   * radius sq_radius_eff and packing sq_volfrac with a screened-Coulomb repulsion of contact value sq_contact_kT
+   * (in kT) and inverse screening length sq_kappa_sigma (in units of 1/diameter), solved on the host through the
+   * Baxter / Hoye-Blum factorisation; S(q) by a 64-node Gauss-Legendre rule on the device, once per detected
+   * neutron.  SAS_EUNSUPPORTED: 2 q_max sq_radius_eff > 64 (beyond the rule's range), a contact value g(1+) < 0
+   * (the closure's known failure for dilute, strongly charged systems; the rescaled MSA is not implemented), or no
+   * convergence. */
+  SAS_SQ_HAYTER_MSA = 2
+};
 
 #define SAS_MAX_NODES 64      /* per quadrature axis */
 #define SAS_MAX_PD_PAIRS 1024 /* pd_nodes[0]*pd_nodes[1] */
@@ -145,6 +156,7 @@ typedef struct {
   double theta, phi, psi;            /* axis polar angle from +z, azimuth from +x, spin (DESIGN.md R-A7) */
   double sigma_theta, sigma_phi;     /* Gaussian spreads of the two tilts (uniaxial models only) */
   double sq_radius_eff, sq_volfrac;  /* Percus-Yevick hard-sphere S(q) (Table II F.11) */
+  double sq_contact_kT, sq_kappa_sigma; /* SAS_SQ_HAYTER_MSA only: beta u at contact, kappa x diameter */
 } sas_model_desc;
 
 /* --- single experiment --------------------------------------------------- */

@@ -29,7 +29,7 @@ MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3, "cor
          "elliptical_cylinder": 11, "hollow_cylinder": 12, "core_shell_ellipsoid": 13, "polymer_micelle": 14}
 ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
 PD = {"none": 0, "schulz": 1, "gauss_mc": 2}
-SQ = {"none": 0, "hard_sphere_py": 1}
+SQ = {"none": 0, "hard_sphere_py": 1, "hayter_msa": 2}
 PRECISION = {"fp32": 0, "fp64": 1}
 STATUS = {0: "SAS_OK", 1: "SAS_EINVAL", 2: "SAS_ESTATE", 3: "SAS_ECUDA", 4: "SAS_ENOMEM", 5: "SAS_EUNSUPPORTED"}
 
@@ -58,7 +58,8 @@ class ModelDesc(C.Structure):
                 ("sld", C.c_double * 3), ("size", C.c_double * 4), ("pd_rel", C.c_double * 2),
                 ("theta", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
                 ("sigma_theta", C.c_double), ("sigma_phi", C.c_double),
-                ("sq_radius_eff", C.c_double), ("sq_volfrac", C.c_double)]
+                ("sq_radius_eff", C.c_double), ("sq_volfrac", C.c_double),
+                ("sq_contact_kT", C.c_double), ("sq_kappa_sigma", C.c_double)]
 
 
 class RadialDesc(C.Structure):
@@ -116,6 +117,7 @@ def model_desc(d: dict) -> ModelDesc:
     m.theta, m.phi, m.psi = float(d["theta"]), float(d["phi"]), float(d["psi"])
     m.sigma_theta, m.sigma_phi = float(d["sigma_theta"]), float(d["sigma_phi"])
     m.sq_radius_eff, m.sq_volfrac = float(d["sq_radius_eff"]), float(d["sq_volfrac"])
+    m.sq_contact_kT, m.sq_kappa_sigma = float(d.get("sq_contact_kT", 0.0)), float(d.get("sq_kappa_sigma", 0.0))
     return m
 
 

@@ -268,6 +268,29 @@ __device__ __forceinline__ double particle_f2(const ExpParams& P, double q, doub
   return F * F;
 }
 
+// R-S2, Hayter-Penfold MSA: S = 1 / |Qhat(K)|^2, K = 2 q R_eff, Qhat = 1 - 12 eta [int_0^1 Q e^{iKx} dx + D' e^{iK}/(k - iK)];
+// the core integral is the 64-node Gauss-Legendre sum whose nodes and weighted Q values the host tabulated in fp64
+// (global memory: 1 KB that every detected neutron of the experiment reads).  Out of line: one call per detected
+// neutron, and the kernels of the other structure factors must not carry its registers.
+constexpr int MSA_N = 64;
+__device__ __noinline__ double msa_sq(const double* __restrict__ t, double q) {
+  const double eD = t[2 * MSA_N], k = t[2 * MSA_N + 1], K = q * t[2 * MSA_N + 2];
+  double re = 0.0, im = 0.0;
+#pragma unroll 4
+  for (int j = 0; j < MSA_N; ++j) {
+    double s, c;
+    sincos_cw(K * t[j], s, c);
+    re = fma(t[MSA_N + j], c, re);
+    im = fma(t[MSA_N + j], s, im);
+  }
+  double sK, cK;
+  sincos_cw(K, sK, cK);
+  const double den = fma(k, k, K * K);
+  re = 1.0 - fma(eD, fma(k, cK, -(K * sK)) / den, re);
+  im = -fma(eD, fma(k, sK, K * cK) / den, im);
+  return 1.0 / fma(re, re, im * im);
+}
+
 // R-N2: the paper's per-event model, Eq. 4 with the sizes of THIS scattering event:
 // I = 1e8 scale F(r)^2 / V(r) S(q) + background, one fp64 evaluation per detected neutron.
 // (compiled into kernels of its own, trace_kernel<double, V, true>: in the same kernel as the fixed-node
@@ -291,6 +314,7 @@ __device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const
   const double F2 = particle_f2<V>(P, q, qA, qB, qC, x0, x1, Vol);
   double S = 1.0;
   if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
+  if (P.sq_kind == 2) S = msa_sq(P.msa_tab, q);
   return fma((P.ev_scale * (F2 / Vol)), S, P.background);
 }
 
@@ -323,6 +347,7 @@ __device__ __forceinline__ double eval_intensity_generic(const ExpParams& P, con
   }
   double S = 1.0;
   if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
+  if (P.sq_kind == 2) S = msa_sq(P.msa_tab, q);
   return fma(P.norm * acc, S, P.background);
 }
 
@@ -519,6 +544,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
   }
   Real S = 1;
   if (P.sq_kind == 1) S = py_sq<Real>(q, P.py);
+  if (P.sq_kind == 2) S = (Real)msa_sq(P.msa_tab, qd);
   return fma_r((Real)P.norm * acc, S, (Real)P.background);
 }
 

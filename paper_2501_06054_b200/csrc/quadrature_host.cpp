@@ -136,4 +136,118 @@ void cached_rule(int kind, double param, int n, std::vector<double>& x, std::vec
 void schulz_rule(double p, int n, std::vector<double>& s, std::vector<double>& w) { cached_rule(0, p, n, s, w); }
 void gauss_tilt_rule(double sigma, int n, std::vector<double>& d, std::vector<double>& w) { cached_rule(1, sigma, n, d, w); }
 
+void legendre_rule_01(int n, std::vector<double>& x, std::vector<double>& w) {
+  std::vector<double> a(n, 0.0), b(n, 0.0), xs, ws;
+  for (int k = 1; k < n; ++k) b[k] = (double)k / std::sqrt(4.0 * (double)k * (double)k - 1.0);
+  gauss_from_jacobi(a, b, xs, ws);   // on [-1, 1], weights summing to 1
+  x.resize(n);
+  w.resize(n);
+  for (int i = 0; i < n; ++i) { x[i] = 0.5 * (xs[i] + 1.0); w[i] = ws[i]; }
+}
+
+namespace {
+
+struct MsaRule {
+  std::vector<double> x, w;   // 64 nodes on [0, 1]
+};
+
+inline double msa_qin(double x, double a, double b, double E, double Cp, double k) {
+  return ((0.5 * a) * (x * x - 1.0) + b * (x - 1.0)) + (E * std::exp(-k * x) - Cp);
+}
+
+// the five equations for u = (a, b, E, C', H'): coefficients of x, 1 and exp(-kx) of Baxter's relation for x h(x)
+// inside the core (h = -1), the closure c = -beta u outside, and the Laplace transform at k of the same relation
+// outside the core, which ties H' = int_1^inf t h(t) exp(-k (t - 1)) dt to the rest (DESIGN.md R-S2)
+void msa_residual(const double u[5], double eta, double gam, double k, const MsaRule& R, double r[5]) {
+  const double a = u[0], b = u[1], E = u[2], Cp = u[3], Hp = u[4];
+  const double e = std::exp(-k), Dp = E * e - Cp;
+  const int n = (int)R.x.size();
+  double I0 = 0.0, I1 = 0.0, Qt = 0.0;
+  for (int i = 0; i < n; ++i) {
+    const double q = msa_qin(R.x[i], a, b, E, Cp, k);
+    I0 += R.w[i] * q;
+    I1 += R.w[i] * R.x[i] * q;
+    Qt += R.w[i] * q * std::exp(-k * R.x[i]);
+  }
+  r[0] = a - (1.0 - 12.0 * eta * (I0 + Dp / k));
+  r[1] = b - 12.0 * eta * (I1 + Dp * (1.0 / k + 1.0 / (k * k)));
+  r[2] = -k * E + 12.0 * eta * Dp * ((1.0 + k) / (k * k) + Hp);
+  r[3] = k * Dp * (1.0 - 12.0 * eta * (Qt + Dp * e / (2.0 * k))) + gam;
+  const double phi1 = (1.0 - e * (1.0 + k)) / (k * k);
+  double T = Dp * phi1 / (2.0 * k);
+  for (int i = 0; i < n; ++i) {
+    const double y = R.x[i];
+    double G = Dp * e / (2.0 * k);
+    for (int j = 0; j < n; ++j) {
+      const double s = y + (1.0 - y) * R.x[j];
+      G += (1.0 - y) * R.w[j] * msa_qin(s, a, b, E, Cp, k) * std::exp(-k * s);
+    }
+    T += R.w[i] * (-(1.0 - y)) * std::exp(k * y) * G;
+  }
+  r[4] = Hp * (1.0 - 12.0 * eta * Qt) - Dp / 2.0 - 12.0 * eta * T;
+}
+
+// 5 x 5 linear system by Gaussian elimination with partial pivoting; false if singular
+bool solve5(double A[5][5], double rhs[5], double x[5]) {
+  int p[5] = {0, 1, 2, 3, 4};
+  for (int c = 0; c < 5; ++c) {
+    int best = c;
+    for (int r = c + 1; r < 5; ++r)
+      if (std::fabs(A[p[r]][c]) > std::fabs(A[p[best]][c])) best = r;
+    std::swap(p[c], p[best]);
+    const double piv = A[p[c]][c];
+    if (!(std::fabs(piv) > 0.0)) return false;
+    for (int r = c + 1; r < 5; ++r) {
+      const double f = A[p[r]][c] / piv;
+      for (int cc = c; cc < 5; ++cc) A[p[r]][cc] -= f * A[p[c]][cc];
+      rhs[p[r]] -= f * rhs[p[c]];
+    }
+  }
+  for (int c = 4; c >= 0; --c) {
+    double s = rhs[p[c]];
+    for (int cc = c + 1; cc < 5; ++cc) s -= A[p[c]][cc] * x[cc];
+    x[c] = s / A[p[c]][c];
+  }
+  return true;
+}
+
+}  // namespace
+
+bool msa_solve(double eta, double gam, double k, double out[5], double* g_contact) {
+  MsaRule R;
+  legendre_rule_01(64, R.x, R.w);
+  double u[5] = {(1.0 + 2.0 * eta) / ((1.0 - eta) * (1.0 - eta)), -1.5 * eta / ((1.0 - eta) * (1.0 - eta)), 0.0, 0.0, 0.0};
+  const int steps = 20;
+  for (int s = 0; s <= steps; ++s) {
+    const double g = gam * (double)s / (double)steps;
+    for (int it = 0; it < 60; ++it) {
+      double r[5], J[5][5];
+      msa_residual(u, eta, g, k, R, r);
+      for (int j = 0; j < 5; ++j) {   // central differences: the equations are at most quadratic in u
+        const double h = 1.0e-6 * std::max(1.0, std::fabs(u[j]));
+        double up[5], um[5], rp[5], rm[5];
+        for (int i = 0; i < 5; ++i) { up[i] = u[i]; um[i] = u[i]; }
+        up[j] += h; um[j] -= h;
+        msa_residual(up, eta, g, k, R, rp);
+        msa_residual(um, eta, g, k, R, rm);
+        for (int i = 0; i < 5; ++i) J[i][j] = (rp[i] - rm[i]) / (2.0 * h);
+      }
+      double rhs[5], st[5];
+      for (int i = 0; i < 5; ++i) rhs[i] = -r[i];
+      if (!solve5(J, rhs, st)) return false;
+      double smax = 0.0, umax = 1.0;
+      for (int i = 0; i < 5; ++i) { u[i] += st[i]; smax = std::max(smax, std::fabs(st[i])); umax = std::max(umax, std::fabs(u[i])); }
+      if (!std::isfinite(smax)) return false;
+      if (smax < 1.0e-15 * umax) break;
+    }
+  }
+  double r[5], rmax = 0.0;
+  msa_residual(u, eta, gam, k, R, r);
+  for (int i = 0; i < 5; ++i) rmax = std::max(rmax, std::fabs(r[i]));
+  if (!(rmax < 1.0e-11)) return false;
+  out[0] = u[0]; out[1] = u[1]; out[2] = u[2]; out[3] = u[3]; out[4] = u[2] * std::exp(-k) - u[3];
+  if (g_contact) *g_contact = u[0] + u[1] - k * u[3];
+  return true;
+}
+
 }  // namespace sas

@@ -135,7 +135,7 @@ sas_status validate_model(const sas_model_desc* m, std::string& why) {
   if (m->model < SAS_SPHERE || m->model > SAS_POLYMER_MICELLE) { why = "unknown model"; return SAS_EINVAL; }
   if (m->precision != SAS_FP32 && m->precision != SAS_FP64) { why = "unknown precision"; return SAS_EINVAL; }
   if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_UNIFORM_ANGLES_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
-  if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY) { why = "unknown sq_kind"; return SAS_EINVAL; }
+  if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY && m->sq_kind != SAS_SQ_HAYTER_MSA) { why = "unknown sq_kind"; return SAS_EINVAL; }
   if (!std::isfinite(m->scale) || !std::isfinite(m->background)) { why = "scale/background not finite"; return SAS_EINVAL; }
   static const int n_sizes[15] = {1, 2, 2, 3, 4, 0, 3, 3, 2, 3, 3, 3, 3, 3, 4};
   static const int n_pd[15] = {1, 2, 2, 1, 2, 0, 1, 2, 2, 2, 2, 2, 2, 2, 1};
@@ -176,6 +176,11 @@ sas_status validate_model(const sas_model_desc* m, std::string& why) {
     }
   }
   if (!std::isfinite(m->theta) || !std::isfinite(m->phi) || !std::isfinite(m->psi)) { why = "orientation angles not finite"; return SAS_EINVAL; }
+  if (m->sq_kind == SAS_SQ_HAYTER_MSA) {
+    if (!finite_pos(m->sq_radius_eff) || !(m->sq_volfrac > 0.0) || !(m->sq_volfrac < 0.6)) { why = "Hayter MSA needs radius_eff > 0 and 0 < volfrac < 0.6"; return SAS_EINVAL; }
+    if (!(m->sq_contact_kT >= 0.0) || !std::isfinite(m->sq_contact_kT)) { why = "Hayter MSA: sq_contact_kT must be >= 0"; return SAS_EINVAL; }
+    if (!(m->sq_kappa_sigma >= 0.05) || !(m->sq_kappa_sigma <= 400.0)) { why = "Hayter MSA: sq_kappa_sigma must be in [0.05, 400]"; return SAS_EINVAL; }
+  }
   if (m->sq_kind == SAS_SQ_HARD_SPHERE_PY) {
     if (!finite_pos(m->sq_radius_eff) || !(m->sq_volfrac >= 0.0) || !(m->sq_volfrac < 0.74)) { why = "PY S(q) needs radius_eff > 0 and 0 <= volfrac < 0.74"; return SAS_EINVAL; }
   }
@@ -431,12 +436,35 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
     P.py.two_r = 2.0 * m.sq_radius_eff;
   }
   P.tab_off = (int)pool.size();
+  P.msa_tab = nullptr;
   pool.insert(pool.end(), ta.begin(), ta.end());
   pool.insert(pool.end(), tb.begin(), tb.end());
   pool.insert(pool.end(), tab.begin(), tab.end());
   for (size_t i = 0; i < dth.size(); ++i) { pool.push_back(std::sin(dth[i])); pool.push_back(std::cos(dth[i])); pool.push_back(wth[i]); pool.push_back(0.0); }
   for (size_t i = 0; i < dph.size(); ++i) { pool.push_back(std::sin(dph[i])); pool.push_back(std::cos(dph[i])); pool.push_back(wph[i]); pool.push_back(0.0); }
   P.tab_len = (int)pool.size() - P.tab_off;
+}
+
+// Hayter MSA (R-S2): solve the closure and append the experiment's S(q) table to the pool; *off = its offset in the
+// pool (the device address is formed when the pool is uploaded)
+sas_status fill_msa(const sas_model_desc& m, const sas_instrument_desc& ins, std::vector<double>& pool, size_t* off,
+                    std::string& why) {
+  if (2.0 * ins.q_max * m.sq_radius_eff > 64.0) { why = "Hayter MSA: 2 q_max sq_radius_eff exceeds 64, the range of the 64-node rule"; return SAS_EUNSUPPORTED; }
+  double u[5], g1 = 0.0;
+  if (!msa_solve(m.sq_volfrac, m.sq_contact_kT, m.sq_kappa_sigma, u, &g1)) { why = "Hayter MSA: the closure did not converge"; return SAS_EUNSUPPORTED; }
+  if (!(g1 >= 0.0)) { why = "Hayter MSA: negative contact value g(1+): the closure fails for this dilute, strongly charged system (rescaled MSA not implemented)"; return SAS_EUNSUPPORTED; }
+  std::vector<double> x, w;
+  legendre_rule_01(64, x, w);
+  const double eta12 = 12.0 * m.sq_volfrac, k = m.sq_kappa_sigma;
+  *off = pool.size();
+  pool.insert(pool.end(), x.begin(), x.end());
+  for (int j = 0; j < 64; ++j)
+    pool.push_back(eta12 * w[j] * (((0.5 * u[0]) * (x[j] * x[j] - 1.0) + u[1] * (x[j] - 1.0)) + (u[2] * std::exp(-k * x[j]) - u[3])));
+  pool.push_back(eta12 * u[4]);
+  pool.push_back(k);
+  pool.push_back(2.0 * m.sq_radius_eff);
+  pool.push_back(0.0);
+  return SAS_OK;
 }
 
 }  // namespace
@@ -539,6 +567,7 @@ int effective_precision(const sas_model_desc& m, const sas_instrument_desc& ins)
 sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   c->h_tab.clear();
   c->tab_len_max = 0;
+  std::vector<std::pair<uint32_t, size_t>> msa_offsets;   // experiments with a Hayter MSA table and where it starts
   c->exp_prec.assign(c->n_exp, SAS_FP64);
   c->precision = SAS_FP32;  // of the context: fp64 as soon as one experiment runs in fp64 (introspection only)
   for (uint32_t e = 0; e < c->n_exp; ++e)
@@ -552,6 +581,13 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
     m.precision = c->exp_prec[e] = effective_precision(models[e], c->instr[e]);
     if (m.precision == SAS_FP64) c->precision = SAS_FP64;
     fill_model(m, P, c->h_tab);
+    if (m.sq_kind == SAS_SQ_HAYTER_MSA) {
+      std::string why;
+      size_t off = 0;
+      sas_status st = fill_msa(m, c->instr[e], c->h_tab, &off, why);
+      if (st != SAS_OK) return fail(c, st, "experiment " + std::to_string(e) + ": " + why);
+      msa_offsets.push_back(std::make_pair(e, off));
+    }
     P.lam_small = 0;
     if (m.model == SAS_CYLINDER) {
       // largest Lambda argument this experiment can produce: |Q| <= q_max, radius <= largest node
@@ -587,6 +623,7 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
     CUDA_TRY(c, cudaMalloc(&c->d_tab, tb));
     c->d_tab_cap = tb;
   }
+  for (const auto& mo : msa_offsets) c->h_exps[mo.first].msa_tab = c->d_tab + mo.second;
   // the host vectors stay alive in the context, so asynchronous copies from them are safe to order on
   // the stream; a later set_model first synchronises (below) before overwriting them
   CUDA_TRY(c, cudaMemcpyAsync(c->d_tab, c->h_tab.data(), tb, cudaMemcpyHostToDevice, c->stream));

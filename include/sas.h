@@ -107,7 +107,8 @@ enum {
    * radius sq_radius_eff and packing sq_volfrac with a screened-Coulomb repulsion of contact value sq_contact_kT
    * (in kT) and inverse screening length sq_kappa_sigma (in units of 1/diameter), solved on the host through the
    * Baxter / Hoye-Blum factorisation; S(q) by a 64-node Gauss-Legendre rule on the device, once per detected
-   * neutron.  SAS_EUNSUPPORTED: 2 q_max sq_radius_eff > 64 (beyond the rule's range), a contact value g(1+) < 0
+   * neutron.  Offered for the globular models (sphere, core-shell sphere, the ellipsoids, polymer micelle); the
+   * rod- and plate-like models refuse it.  SAS_EUNSUPPORTED: such a model, 2 q_max sq_radius_eff > 64 (beyond the rule's range), a contact value g(1+) < 0
    * (the closure's known failure for dilute, strongly charged systems; the rescaled MSA is not implemented), or no
    * convergence. */
   SAS_SQ_HAYTER_MSA = 2
@@ -238,6 +239,12 @@ sas_status sas_get_launch_info(sas_ctx* ctx, uint64_t* n_launches, int32_t* grid
 /* Average device time in ms (CUDA events on the context's stream) of the trace kernels launched
  * since the last call with reset != 0; *n_timed = how many launches the average covers. */
 sas_status sas_get_kernel_time(sas_ctx* ctx, int32_t reset, double* avg_ms, uint64_t* n_timed);
+/* Per-launch timing on (enabled != 0, the default) or off.  On, every trace-kernel launch is bracketed by two
+ * cudaEventRecord on the context's stream -- about 6 us of stream operations per launch on a B200, which is a
+ * quarter of a 1e6-neutron step (BASELINE.json configs[0]; PAPER.md:195 is about exactly such fixed costs).  Off,
+ * a launch is the kernel alone: sas_get_kernel_time and sas_get_launch_records then report no launches.
+ * Takes effect from the next launch; results are the same either way. */
+sas_status sas_set_launch_timing(sas_ctx* ctx, int32_t enabled);
 /* One record per trace-kernel launch since the last sas_get_kernel_time(reset != 0), oldest first (at most
  * SAS_MAX_LAUNCH_RECORDS are kept): which kernel ran (variant = the model form it was compiled for, per-event
  * sizes or fixed nodes, precision of the model arithmetic), over how many experiments and ids, and its device

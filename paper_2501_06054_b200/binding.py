@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "sas_trace_dump", "sas_read_detector", "sas_get_counters", "sas_reset_detector", "sas_destroy",
     "sas_last_error", "sas_create_batch", "sas_trace_batch", "sas_quadrature_nodes",
     "sas_get_launch_info", "sas_get_kernel_time", "sas_get_upload_bytes", "sas_version", "sas_reduce_radial",
-    "sas_trace_batch_range", "sas_get_launch_records", "sas_get_reduce_time",
+    "sas_trace_batch_range", "sas_get_launch_records", "sas_get_reduce_time", "sas_set_launch_timing",
 ]
 
 SAMPLE = {"box": 0, "cyl_y": 1}
@@ -158,6 +158,7 @@ def load_library(path: str | None = None):
     L.sas_quadrature_nodes.argtypes = [i32, dbl, i32, pp(dbl), pp(dbl)]
     L.sas_get_launch_info.argtypes = [vp, pp(u64), pp(i32), pp(i32), pp(i32)]
     L.sas_get_kernel_time.argtypes = [vp, i32, pp(dbl), pp(u64)]
+    L.sas_set_launch_timing.argtypes = [vp, i32]
     L.sas_get_upload_bytes.argtypes = [vp, pp(u64)]
     L.sas_reduce_radial.argtypes = [vp, pp(RadialDesc), vp, vp, vp, vp]
     L.sas_version.argtypes = []
@@ -250,6 +251,10 @@ class _Base:
         ms, n = C.c_double(), C.c_uint64()
         _check(self.L, self.ctx, self.L.sas_get_kernel_time(self.ctx, 1 if reset else 0, ms, n))
         return ms.value, n.value
+
+    def set_launch_timing(self, enabled: bool):
+        """Per-launch CUDA events on (default) or off (include/sas.h: sas_set_launch_timing)."""
+        _check(self.L, self.ctx, self.L.sas_set_launch_timing(self.ctx, 1 if enabled else 0))
 
     def launch_records(self):
         """One dict per trace-kernel launch since the last kernel_time_ms(reset=True) (include/sas.h)."""

@@ -273,6 +273,12 @@ __device__ __forceinline__ double particle_f2(const ExpParams& P, double q, doub
 // (global memory: 1 KB that every detected neutron of the experiment reads).  Out of line: one call per detected
 // neutron, and the kernels of the other structure factors must not carry its registers.
 constexpr int MSA_N = 64;
+// Offered for the globular models (sphere family, ellipsoids, micelle) only: an out-of-line call in a kernel costs
+// that kernel's every workload 1-3 % through register allocation (measured on the per-event cylinder and the
+// barbell), and a sphere-sphere structure factor has no meaning for rods and plates anyway (the host refuses it).
+__host__ __device__ constexpr bool msa_offered(int V) {
+  return V == V_SPHERE || V == V_CS_SPHERE || V == V_TRIAX || V == V_CS_TRIAX || V == V_ELL || V == V_CS_ELL || V == V_MICELLE;
+}
 __device__ __noinline__ double msa_sq(const double* __restrict__ t, double q) {
   const double eD = t[2 * MSA_N], k = t[2 * MSA_N + 1], K = q * t[2 * MSA_N + 2];
   double re = 0.0, im = 0.0;
@@ -314,7 +320,7 @@ __device__ __forceinline__ double eval_intensity_event(const ExpParams& P, const
   const double F2 = particle_f2<V>(P, q, qA, qB, qC, x0, x1, Vol);
   double S = 1.0;
   if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
-  if (P.sq_kind == 2) S = msa_sq(P.msa_tab, q);
+  if constexpr (msa_offered(V)) if (P.sq_kind == 2) S = msa_sq(P.msa_tab, q);
   return fma((P.ev_scale * (F2 / Vol)), S, P.background);
 }
 
@@ -347,7 +353,7 @@ __device__ __forceinline__ double eval_intensity_generic(const ExpParams& P, con
   }
   double S = 1.0;
   if (P.sq_kind == 1) S = py_sq<double>(q, P.py);
-  if (P.sq_kind == 2) S = msa_sq(P.msa_tab, q);
+  if constexpr (msa_offered(V)) if (P.sq_kind == 2) S = msa_sq(P.msa_tab, q);
   return fma(P.norm * acc, S, P.background);
 }
 
@@ -544,7 +550,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
   }
   Real S = 1;
   if (P.sq_kind == 1) S = py_sq<Real>(q, P.py);
-  if (P.sq_kind == 2) S = (Real)msa_sq(P.msa_tab, qd);
+  if constexpr (msa_offered(V)) if (P.sq_kind == 2) S = (Real)msa_sq(P.msa_tab, qd);
   return fma_r((Real)P.norm * acc, S, (Real)P.background);
 }
 

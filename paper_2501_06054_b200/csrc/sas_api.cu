@@ -23,6 +23,9 @@ constexpr double TWO_PI = 6.283185307179586;
 constexpr double FOUR_PI_3 = 4.1887902047863905;
 constexpr double PI_D = 3.141592653589793;
 constexpr int MAX_TIMED = SAS_MAX_LAUNCH_RECORDS;
+#ifndef SAS_PDL
+#define SAS_PDL 1   // programmatic dependent launch of the trace kernels (0: plain stream order)
+#endif
 constexpr int N_GROUPS = 4 * N_VARIANTS;
 #ifndef SAS_ITEMS_PER_BLOCK
 #define SAS_ITEMS_PER_BLOCK 16
@@ -71,6 +74,7 @@ struct sas_ctx {
   std::vector<cudaEvent_t> ev0, ev1;
   std::vector<sas_launch_record> records;  // of the timed launches (ms filled on request)
   uint64_t n_timed = 0;
+  bool timing_on = true;   // sas_set_launch_timing
   double last_reduce_ms = 0.0;
 };
 
@@ -90,6 +94,9 @@ sas_status fail(sas_ctx* c, sas_status st, const std::string& msg) {
 
 __global__ void __launch_bounds__(256) zero_detector_kernel(unsigned long long* p0, unsigned long long* p1,
                                                             unsigned long long* p2, unsigned long long* counters, size_t n) {
+  // programmatic dependent launch: the trace kernel that follows in the stream may be scheduled now; it touches
+  // nothing this kernel writes before its own griddepcontrol.wait (trace_kernel*.cuh)
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) { p0[i] = 0ull; p1[i] = 0ull; p2[i] = 0ull; }
   if (blockIdx.x == 0 && threadIdx.x < 8) counters[threadIdx.x] = 0ull;
@@ -177,6 +184,12 @@ sas_status validate_model(const sas_model_desc* m, std::string& why) {
   }
   if (!std::isfinite(m->theta) || !std::isfinite(m->phi) || !std::isfinite(m->psi)) { why = "orientation angles not finite"; return SAS_EINVAL; }
   if (m->sq_kind == SAS_SQ_HAYTER_MSA) {
+    const int32_t k = m->model;
+    if (!(k == SAS_SPHERE || k == SAS_CORE_SHELL_SPHERE || k == SAS_TRIAXIAL_ELLIPSOID || k == SAS_CORE_SHELL_TRIAXIAL ||
+          k == SAS_ELLIPSOID || k == SAS_CORE_SHELL_ELLIPSOID || k == SAS_POLYMER_MICELLE)) {
+      why = "Hayter MSA is offered for the globular models only (spheres, ellipsoids, micelle)";
+      return SAS_EUNSUPPORTED;
+    }
     if (!finite_pos(m->sq_radius_eff) || !(m->sq_volfrac > 0.0) || !(m->sq_volfrac < 0.6)) { why = "Hayter MSA needs radius_eff > 0 and 0 < volfrac < 0.6"; return SAS_EINVAL; }
     if (!(m->sq_contact_kT >= 0.0) || !std::isfinite(m->sq_contact_kT)) { why = "Hayter MSA: sq_contact_kT must be >= 0"; return SAS_EINVAL; }
     if (!(m->sq_kappa_sigma >= 0.05) || !(m->sq_kappa_sigma <= 400.0)) { why = "Hayter MSA: sq_kappa_sigma must be in [0.05, 400]"; return SAS_EINVAL; }
@@ -683,7 +696,7 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   a.work_base = c->work_base;
   a.use_exp0 = (!c->batch && c->n_exp == 1) ? 1 : 0;
   if (a.use_exp0) a.exp0 = c->h_exps[0];
-  const bool timed = !DUMP && c->n_timed < (uint64_t)MAX_TIMED;
+  const bool timed = c->timing_on && !DUMP && c->n_timed < (uint64_t)MAX_TIMED;
   if (timed) {
     if (c->ev0.size() <= c->n_timed) {
       cudaEvent_t e0, e1;
@@ -694,7 +707,22 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
     }
     CUDA_TRY(c, cudaEventRecord(c->ev0[c->n_timed], c->stream));
   }
-  kern<<<grid, BLOCK_THREADS, smem, c->stream>>>(a);
+  // Programmatic stream serialisation: when the previous operation of the stream is a kernel, this one may be
+  // scheduled as soon as every block of that kernel has exited or released its dependents (the zeroing kernel of
+  // sas_reset_detector does so at once), and waits for its completion (griddepcontrol.wait) only where it first
+  // needs the detector, the counters or the work counter: block set-up and the first Philox rows overlap the
+  // zeroing and the launch latency.
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)grid);
+  lc.blockDim = dim3((unsigned)BLOCK_THREADS);
+  lc.dynamicSmemBytes = smem;
+  lc.stream = c->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = SAS_PDL;
+  lc.attrs = at;
+  lc.numAttrs = 1;
+  CUDA_TRY(c, cudaLaunchKernelEx(&lc, kern, a));
   CUDA_TRY(c, cudaGetLastError());
   if (n_items > (uint64_t)grid) c->work_base += (uint32_t)n_items;  // the fetches this launch makes (sas_types.h)
   if (timed) {
@@ -1013,6 +1041,12 @@ sas_status sas_get_launch_info(sas_ctx* c, uint64_t* n_launches, int32_t* grid, 
   if (grid) *grid = c->last_grid;
   if (block) *block = c->last_block;
   if (smem_bytes) *smem_bytes = c->last_smem;
+  return SAS_OK;
+}
+
+sas_status sas_set_launch_timing(sas_ctx* c, int32_t enabled) {
+  if (!c) return SAS_EINVAL;
+  c->timing_on = enabled != 0;
   return SAS_OK;
 }
 

@@ -110,6 +110,8 @@ trace_kernel(const __grid_constant__ KernelArgs a) {
   int headB = 0, cntB = 0, headB2 = 0, cntB2 = 0, headC = 0, cntC = 0;
 #pragma unroll
   for (int f = 0; f < 7; ++f) wq.oc[f][lane] = 0;
+  // programmatic dependent launch (sas_api.cu: launch): the previous kernel of the stream is complete from here on
+  asm volatile("griddepcontrol.wait;" ::: "memory");
 
   int cur_exp = -1;
   bool replay = false, first = true;

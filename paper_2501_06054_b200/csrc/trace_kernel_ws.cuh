@@ -206,6 +206,9 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     for (int i = tid; i < tl; i += nthr) tab[i] = (Real)tsrc[i];
   };
   stage_experiment(cur_exp, threadIdx.x, WS_THREADS);
+  // programmatic dependent launch (sas_api.cu: launch): everything above reads only what the host uploaded; the
+  // detector, the counters and the work counter may still be in the hands of the previous kernel of the stream
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   __syncthreads();
 
   // The warp arbiter of a sub-partition serves the eligible warp with the highest id first

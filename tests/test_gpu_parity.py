@@ -741,9 +741,40 @@ def test_hayter_msa_in_a_batch_and_its_refusals(sas):
     with pytest.raises(sas.SasError) as err:
         sas.Tracer(ins[0], W.model(**dict(MSA, sq_radius_eff=150.0)))
     assert err.value.status == 5
+    with pytest.raises(sas.SasError) as err:                 # a sphere-sphere S(q) is not offered for rods
+        sas.Tracer(ins[0], W.model(model="cylinder", size=[20.0, 400.0, 0, 0], orient_kind="isotropic_mc", **MSA))
+    assert err.value.status == 5 and "globular" in str(err.value)
     with pytest.raises(sas.SasError) as err:
         sas.Tracer(ins[0], W.model(**dict(MSA, sq_kappa_sigma=0.0)))
     assert err.value.status == 1
+
+
+def test_back_to_back_steps_without_launch_timing_are_each_a_clean_step(sas):
+    """sas_set_launch_timing(0) leaves reset -> trace adjacent in the stream, where the trace kernel is launched
+    programmatically dependent on the zeroing kernel (sas_api.cu: launch): 300 steps in a row, no host
+    synchronisation in between, each must leave exactly the image of a single step (a trace kernel that touched
+    the detector before the zeroing finished, or a zeroing that overtook the previous trace, would show)."""
+    c = W.config(0)
+    for ins, model in ((c["instrument"], c["model"]), (W.instrument(det_dist=3.0), W.model(model="cylinder", size=[20.0, 400.0, 0, 0], orient_kind="isotropic_mc", precision="fp32"))):
+        tr = sas.Tracer(ins, model)
+        tr.trace(100000, 3)
+        want = [a.copy() for a in tr.read_detector()]
+        want_c = tr.counters().copy()
+        assert len(tr.launch_records()) == 1
+        tr.kernel_time_ms(reset=True)
+        tr.set_launch_timing(False)
+        for n in (100000, 777, 100000):           # a different step in between: leftovers of it would show too
+            for _ in range(100):
+                tr.reset()
+                tr.trace(n, 3)
+        got = tr.read_detector()
+        assert tr.launch_records() == [] and tr.kernel_time_ms()[1] == 0
+        assert np.array_equal(got[2], want[2]) and np.array_equal(tr.counters(), want_c)
+        assert np.allclose(got[0], want[0], rtol=1e-12, atol=0) and np.allclose(got[1], want[1], rtol=1e-12, atol=0)
+        tr.set_launch_timing(True)
+        tr.reset(); tr.trace(100000, 3)
+        assert len(tr.launch_records()) == 1 and np.array_equal(tr.read_detector()[2], want[2])
+        tr.close()
 
 
 def test_context_stays_on_its_device(sas):

@@ -42,7 +42,7 @@ SECONDARY = [("c0_sphere_fp64", 0, None, None), ("c0_sphere_fp64_1e9", 0, None, 
              ("c1_polysphere_py_fp32", 1, "fp32", None), ("c1_polysphere_py_fp64", 1, "fp64", None),
              ("c3_coreshell_triaxial", 3, None, None), ("c4_batch", 4, None, None),
              ("n1_paper_cylinder", 5, None, None), ("n2_paper_barbell", 6, None, None),
-             ("n3_paper_micelle", 7, None, None)]
+             ("n3_paper_micelle", 7, None, None), ("n4_paper_hayter_msa", 8, None, None)]
 
 
 # ------------------------------------------------------------------ reference arm: the CPU oracle
@@ -132,6 +132,8 @@ def model_key_and_nodes(model):
         return "barbell_event_fp64", 64
     if m == "polymer_micelle":
         return "micelle_event_fp64", 0
+    if is_event_model(model) and m == "sphere" and model["sq_kind"] == "hayter_msa":
+        return "sphere_msa_event_fp64", 65
     if m == "sphere":
         nodes = pd[0]
         if nodes == 1:

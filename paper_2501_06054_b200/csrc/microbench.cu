@@ -201,6 +201,31 @@ static double run_stage_a(double mhz) {
   return best * 1e-3 * mhz * 1e6 / ((double)grid * 8 / (n_sm * 4) * iters * 3);   // clocks per row of 32 ids
 }
 
+// What a CUDA-event pair around one launch reads for a kernel that does nothing: the floor under every per-launch
+// "kernel time" the library reports and under every per-step event pair of bench.py.
+__global__ void __launch_bounds__(640, 1) null_kernel(int* out, int never) {
+  if (never == 12345) out[0] = 1;
+}
+static double event_floor_us() {
+  int* d = nullptr;
+  cudaMalloc(&d, 4);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  double best = 1e30;
+  for (int r = 0; r < 60; ++r) {
+    cudaEventRecord(e0);
+    null_kernel<<<148, 640>>>(d, 0);
+    cudaEventRecord(e1);
+    cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (r >= 10 && (double)ms * 1e3 < best) best = (double)ms * 1e3;
+  }
+  cudaFree(d);
+  return best;
+}
+
 int main() {
   const char* env = getenv("SM_MHZ");
   const double mhz = env ? atof(env) : 1965.0;
@@ -213,9 +238,11 @@ int main() {
   const double m0 = run_mix<0>(mhz), m1 = run_mix<1>(mhz), m2 = run_mix<2>(mhz), m3 = run_mix<3>(mhz), sa = run_stage_a(mhz);
   printf("  %-52s %7.2f %7.2f %7.2f %7.2f\n", "wide multiply + (1 + NL) LOP3, NL = 0..3", m0, m1, m2, m3);
   printf("  %-52s %7.2f\n", "stage-A core: Philox words 0,1 + window test, per row", sa);
+  const double fl = event_floor_us();
+  printf("  %-52s %7.2f us\n", "event pair around a kernel that does nothing", fl);
   // one machine-readable line for bench.py
   printf("{\"sm_mhz\": %.0f, \"ffma\": %.4f, \"imad\": %.4f, \"imad_wide\": %.4f, \"lop3\": %.4f, \"dfma\": %.4f, \"mufu\": %.4f, "
-         "\"philox_block\": %.3f, \"wide_lop3\": [%.4f, %.4f, %.4f, %.4f], \"stage_a_core_row\": %.3f}\n",
-         mhz, v[K_FFMA], v[K_IMAD], v[K_IMAD_WIDE], v[K_LOP3], v[K_DFMA], v[K_MUFU_RCP], v[K_PHILOX], m0, m1, m2, m3, sa);
+         "\"philox_block\": %.3f, \"wide_lop3\": [%.4f, %.4f, %.4f, %.4f], \"stage_a_core_row\": %.3f, \"event_floor_us\": %.2f}\n",
+         mhz, v[K_FFMA], v[K_IMAD], v[K_IMAD_WIDE], v[K_LOP3], v[K_DFMA], v[K_MUFU_RCP], v[K_PHILOX], m0, m1, m2, m3, sa, fl);
   return 0;
 }

@@ -96,6 +96,10 @@ MODEL_COST = {
     "barbell_event_fp64": (U(562, wide=56, imad=3, logic=150, fp64=344, fp32=2, xu=7), U(70, logic=8, fp64=58, xu=2)),
     # (estimate) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
     "micelle_event_fp64": (U(330, wide=19, logic=60, fp64=230, xu=8), U(0)),
+    # (estimate) charged spheres, per event: Philox block 3, one Box-Muller normal, sphere Phi; then the 64 nodes of
+    # the MSA rule and the tail term, each one fp64 sine/cosine pair (three-step reduction, two Taylor kernels) and
+    # two accumulations
+    "sphere_msa_event_fp64": (U(280, wide=19, logic=55, fp64=190, xu=8), U(40, logic=6, fp64=33, xu=0)),
 }
 
 RESOURCES = ("issue", "imul", "int", "fp64", "xu")

@@ -120,6 +120,16 @@ def config(i: int, precision: str | None = None):
             model=model(model="polymer_micelle", precision="fp64", size=[40.0, 15.0, 4000.0, 30.0],
                         sld=[2.0e-6, 1.0e-6, 0.0], pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0.0]),
             n_neutrons=10**9, seed=20250113)
+    if i == 8:
+        # NEXT-2 (not a BASELINE.json config): "Hayter MSA", the third expensive model of PAPER.md:201 built here:
+        # charged spheres, the paper's per-event Gaussian radius, S(q) from the mean-spherical closure (DESIGN.md
+        # R-S2): 65 fp64 sine/cosine pairs per detected neutron
+        return dict(
+            name="n4_paper_hayter_msa", instrument=instrument(det_nx=256, det_ny=256),
+            model=model(model="sphere", precision="fp64", size=[40.0, 0, 0, 0], pd_kind=["gauss_mc", "none"],
+                        pd_rel=[0.1, 0.0], scale=0.2, sq_kind="hayter_msa", sq_radius_eff=45.0, sq_volfrac=0.2,
+                        sq_contact_kT=5.0, sq_kappa_sigma=2.0),
+            n_neutrons=10**9, seed=20250114)
     raise ValueError(i)
 
 

@@ -749,6 +749,14 @@ def test_hayter_msa_in_a_batch_and_its_refusals(sas):
     assert err.value.status == 1
 
 
+@pytest.mark.parametrize("cfg", [5, 6, 7, 8])
+def test_paper_scheme_workloads_of_the_bench_per_neutron(sas, cfg):
+    """The n1..n4 workloads exactly as bench.py configures them (the paper's per-event averaging on its rod, a
+    barbell, a micelle, charged spheres with the Hayter MSA S(q)): an id prefix per neutron and per bin."""
+    c = W.config(cfg)
+    check_prefix(sas, c["instrument"], c["model"], c["seed"], 150000, min_detected=6000)
+
+
 def test_back_to_back_steps_without_launch_timing_are_each_a_clean_step(sas):
     """sas_set_launch_timing(0) leaves reset -> trace adjacent in the stream, where the trace kernel is launched
     programmatically dependent on the zeroing kernel (sas_api.cu: launch): 300 steps in a row, no host

@@ -66,6 +66,22 @@ __device__ __forceinline__ float horner(const float (&c)[N], float t) {
   return r;
 }
 
+// ---------------------------------------------------------------- packed fp32 pairs (sm_100: FFMA2 / FMUL2 / FADD2)
+// One instruction works on two fp32 values per lane (a 64-bit register pair) at two clocks per warp instruction:
+// the FMA pipes do the same work per clock as with FFMA, but in half the issue slots, which is what the fp32 node
+// loops are short of.  Each component is rounded exactly as the scalar operation rounds it.
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+template <int N>
+__device__ __forceinline__ float2 horner2(const float (&c)[N], float2 t) {
+  float2 r = f2(c[N - 1]);
+#pragma unroll
+  for (int i = N - 2; i >= 0; --i) r = fma2(r, t, f2(c[i]));
+  return r;
+}
+
 // ---------------------------------------------------------------- sin/cos
 // fp32: two-step Cody-Waite reduction by pi/2 with FMAs (48 bits of pi/2), kernels on [-pi/4, pi/4].
 // Valid for |x| < ~1e5 (k exact in fp32); the tracer's arguments are q*size < ~1e3.
@@ -370,6 +386,18 @@ __device__ __forceinline__ float sinc_abs_r(float q, float h) {
   return fmaf(r * z, horner(SP, z), r) * rcp_fast(x);
 }
 __device__ __forceinline__ double sinc_abs_r(double q, double h) { return sinc_r(q * h); }
+// two phases at once: the same operations as sinc_abs_r(float, float), component by component
+__device__ __forceinline__ float2 sinc_abs_r2(float2 q, float h) {
+  const float2 x = fma2(q, f2(h), f2(1e-30f));
+  const float2 t = fma2(x, f2(0.318309886f), f2(SAS_ROUND_MAGIC));
+  const float2 kf = add2(t, f2(-SAS_ROUND_MAGIC));
+  float2 r = fma2(kf, f2(-3.14159250259399414062e+00f), x);
+  r = fma2(kf, f2(-1.50995788317231927067e-07f), r);
+  const float2 z = mul2(r, r);
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  const float2 p = fma2(mul2(r, z), horner2(SP, z), r);
+  return mul2(p, make_float2(rcp_fast(x.x), rcp_fast(x.y)));
+}
 
 // ---------------------------------------------------------------- Lambda(x) = 2 J1(x)/x, x >= 0
 // x <= 8: one polynomial in x^2 (no square root needed); x > 8: Hankel form
@@ -413,6 +441,14 @@ __device__ __forceinline__ float lambda1_class(float t) {
   if (LC == 2) { const float c[SAS_LAMBDA_36_N] = SAS_LAMBDA_36; return horner(c, t); }
   const float c[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
   return horner(c, t);
+}
+template <int LC>
+__device__ __forceinline__ float2 lambda1_class2(float2 t) {
+  if (LC == 4) { const float c[SAS_LAMBDA_16_N] = SAS_LAMBDA_16; return horner2(c, t); }
+  if (LC == 3) { const float c[SAS_LAMBDA_25_N] = SAS_LAMBDA_25; return horner2(c, t); }
+  if (LC == 2) { const float c[SAS_LAMBDA_36_N] = SAS_LAMBDA_36; return horner2(c, t); }
+  const float c[SAS_LAMBDA_A_N] = SAS_LAMBDA_A;
+  return horner2(c, t);
 }
 template <int LC>
 __device__ __forceinline__ double lambda1_class(double t);

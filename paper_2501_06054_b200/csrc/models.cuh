@@ -25,7 +25,7 @@ struct Tables {  // views into the shared-memory table block
   const Real* tb;   // [n_b][TB_W]
   const Real* tab;  // [n_a*n_b][TAB_W]
   const Real* tth;  // [n_th][TOR_W]
-  const Real* tph;  // [n_ph][TOR_W]
+  const Real* tph;  // [(n_ph + 1) / 2][2 TOR_W]: pairs of nodes (cyl_quad_row)
 };
 
 template <typename Real>
@@ -45,14 +45,47 @@ __device__ __forceinline__ Real sq(Real x) { return x * x; }
 // One row of the Gaussian-tilt quadrature of a monodisperse cylinder (R-A11): sum over the phi tilts of
 // w_j [sinc(Q.c_ij L/2) Lambda(R sqrt(q^2 - (Q.c_ij)^2))]^2 for one theta tilt (Ai = Q.(tilted axis, phi = 0)).
 // LC > 0: Lambda is the short polynomial of class LC in t = x^2 / h - 1 (device_math.cuh), t in one FMA.
+// The phi-tilt table holds its nodes in pairs, [sin0, sin1, cos0, cos1, w0, w1, 0, 0] per pair (an odd count is
+// padded with a node of weight 0): the fp32 row below takes a pair per step in packed arithmetic.
+template <typename Real> __device__ __forceinline__ Real tph_sin(const Real* tph, int j) { return tph[(j >> 1) * (2 * TOR_W) + (j & 1)]; }
+template <typename Real> __device__ __forceinline__ Real tph_cos(const Real* tph, int j) { return tph[(j >> 1) * (2 * TOR_W) + 2 + (j & 1)]; }
+template <typename Real> __device__ __forceinline__ Real tph_w(const Real* tph, int j) { return tph[(j >> 1) * (2 * TOR_W) + 4 + (j & 1)]; }
+
+// fp32: two phi tilts per step (FFMA2 / FMUL2 / FADD2, device_math.cuh); the two partial sums are added at the end
+template <int LC>
+__device__ __forceinline__ float cyl_quad_row(const float* tph, int n_ph, float Ai, float qB, float hL0, float R20, float q2) {
+  const float k = R20 * (float)lambda_class_scale(LC);
+  const float nk = -k, tq = fmaf(q2, k, -1.0f);
+  float2 row = f2(0.0f);
+  const int n_pairs = (n_ph + 1) >> 1;
+#pragma unroll CYL_UNROLL / 2
+  for (int p = 0; p < n_pairs; ++p) {
+    const float4 sc = *reinterpret_cast<const float4*>(tph + p * (2 * TOR_W));
+    const float2 w = *reinterpret_cast<const float2*>(tph + p * (2 * TOR_W) + 4);
+    const float2 qc = fma2(make_float2(sc.z, sc.w), f2(Ai), mul2(f2(qB), make_float2(sc.x, sc.y)));  // Q . c_ij
+    float2 f;
+    if (LC > 0) {
+      f = mul2(sinc_abs_r2(qc, hL0), lambda1_class2<LC>(fma2(mul2(qc, qc), f2(nk), f2(tq))));
+    } else {
+      float2 r2 = fma2(mul2(qc, qc), f2(-1.0f), f2(q2));
+      r2.x = r2.x > 0.0f ? r2.x : 0.0f;
+      r2.y = r2.y > 0.0f ? r2.y : 0.0f;
+      f = mul2(sinc_abs_r2(qc, hL0), make_float2(lambda1_x2(r2.x * R20), lambda1_x2(r2.y * R20)));
+    }
+    row = fma2(w, mul2(f, f), row);
+  }
+  return row.x + row.y;
+}
+
 template <typename Real, int LC>
 __device__ __forceinline__ Real cyl_quad_row(const Real* tph, int n_ph, Real Ai, Real qB, Real hL0, Real R20, Real q2) {
+  if constexpr (sizeof(Real) == 4) return cyl_quad_row<LC>(tph, n_ph, Ai, qB, hL0, R20, q2);
   const Real k = R20 * (Real)lambda_class_scale(LC);
   const Real nk = -k, tq = fma_r(q2, k, (Real)-1);
   Real row = 0;
 #pragma unroll CYL_UNROLL
   for (int j = 0; j < n_ph; ++j) {
-    const Real sph = tph[j * TOR_W + 0], cph = tph[j * TOR_W + 1], wph = tph[j * TOR_W + 2];
+    const Real sph = tph_sin(tph, j), cph = tph_cos(tph, j), wph = tph_w(tph, j);
     const Real qc = fma_r(cph, Ai, qB * sph);  // Q . c_ij
     Real f;
     if (LC > 0) {
@@ -420,6 +453,8 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
       } else if (sizeof(Real) == 4 && P.n_a > 1) {
         // fp32 node loop: w (drho V)^2 Phi(u)^2 = [16 pi^2 drho^2 w] (sin u - u cos u)^2 / q^6: the bracket is the
         // node's fourth table entry, 1 / q^6 multiplies the sum once (no reciprocal and no u^-3 per node)
+        // (scalar on purpose: a packed loop, two nodes per FFMA2, is 2.4 % slower here -- a packed operation needs both
+        // FMA pipes at once and the producers' IMAD.WIDE stream holds the heavy one 63 % of the time)
         const Proj<float> qp = make_proj<float>(qd);
         float direct = 0.0f;
         for (int a = 0; a < P.n_a; ++a) {
@@ -477,7 +512,7 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
             row *= cL0 * cR0;
           } else {
             for (int j = 0; j < P.n_ph; ++j) {
-              const Real sph = T.tph[j * TOR_W + 0], cph = T.tph[j * TOR_W + 1], wph = T.tph[j * TOR_W + 2];
+              const Real sph = tph_sin(T.tph, j), cph = tph_cos(T.tph, j), wph = tph_w(T.tph, j);
               const Real qc = fma_r(cph, Ai, qB * sph);
               Real r2 = fma_r(-qc, qc, q2);
               r2 = r2 > (Real)0 ? r2 : (Real)0;

@@ -454,7 +454,15 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
   pool.insert(pool.end(), tb.begin(), tb.end());
   pool.insert(pool.end(), tab.begin(), tab.end());
   for (size_t i = 0; i < dth.size(); ++i) { pool.push_back(std::sin(dth[i])); pool.push_back(std::cos(dth[i])); pool.push_back(wth[i]); pool.push_back(0.0); }
-  for (size_t i = 0; i < dph.size(); ++i) { pool.push_back(std::sin(dph[i])); pool.push_back(std::cos(dph[i])); pool.push_back(wph[i]); pool.push_back(0.0); }
+  // the phi tilts in pairs, [sin0, sin1, cos0, cos1, w0, w1, 0, 0] (models.cuh: cyl_quad_row); an odd count is
+  // padded with a node of weight 0 on the mean axis
+  for (size_t i = 0; i < dph.size(); i += 2) {
+    const bool two = i + 1 < dph.size();
+    pool.push_back(std::sin(dph[i])); pool.push_back(two ? std::sin(dph[i + 1]) : 0.0);
+    pool.push_back(std::cos(dph[i])); pool.push_back(two ? std::cos(dph[i + 1]) : 1.0);
+    pool.push_back(wph[i]); pool.push_back(two ? wph[i + 1] : 0.0);
+    pool.push_back(0.0); pool.push_back(0.0);
+  }
   P.tab_len = (int)pool.size() - P.tab_off;
 }
 

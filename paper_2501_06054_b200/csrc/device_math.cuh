@@ -330,6 +330,27 @@ __device__ __forceinline__ float sin_minus_ucos_abs(float u, float lo) {
   const float cr = fmaf(z, C, 1.0f);
   return (kb == __float_as_int(SAS_ROUND_MAGIC)) ? rz * (S - C) : fmaf(-u, cr, sr);
 }
+// signed Phi of two arguments at once (packed arithmetic; the operations of sphere_phi_core<true>(u, 0) component
+// by component)
+__device__ __forceinline__ float2 sphere_phi2(float2 u) {
+  const float2 t = fma2(u, f2(0.318309886f), f2(SAS_ROUND_MAGIC));
+  const float2 kf = add2(t, f2(-SAS_ROUND_MAGIC));
+  float2 r = fma2(kf, f2(-3.14159250259399414062e+00f), u);
+  r = fma2(kf, f2(-1.50995788317231927067e-07f), r);
+  const float2 z = mul2(r, r);
+  const float SP[SAS_SINPI_POLY_N] = SAS_SINPI_POLY;
+  const float CP[SAS_COSPI_POLY_N] = SAS_COSPI_POLY;
+  const float2 S = horner2(SP, z), C = horner2(CP, z);
+  const float2 sr = fma2(mul2(r, z), S, r);
+  const float2 cr = fma2(z, C, f2(1.0f));
+  const float2 inv = make_float2(rcp_fast(u.x), rcp_fast(u.y));
+  const float2 dir = mul2(fma2(make_float2(-u.x, -u.y), cr, sr), mul2(mul2(inv, inv), inv));
+  const float2 ser = add2(S, make_float2(-C.x, -C.y));
+  const int kx = __float_as_int(t.x), ky = __float_as_int(t.y);
+  const float sx = kx == __float_as_int(SAS_ROUND_MAGIC) ? ser.x : __int_as_float(__float_as_int(dir.x) ^ (kx << 31));
+  const float sy = ky == __float_as_int(SAS_ROUND_MAGIC) ? ser.y : __int_as_float(__float_as_int(dir.y) ^ (ky << 31));
+  return mul2(f2(3.0f), make_float2(sx, sy));
+}
 __device__ __forceinline__ float sphere_phi(float u) { return sphere_phi_core<true>(u, 0.0f); }
 __device__ __forceinline__ double sphere_phi(double u) {
   if (u < 1.0e-8) return 1.0;   // Phi = 1 - u^2/10 + ...: 1 to the last bit

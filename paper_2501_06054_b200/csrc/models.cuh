@@ -570,7 +570,26 @@ __device__ __forceinline__ Real eval_intensity(const ExpParams& P, const Real* t
         const Real xa = ra[0] + ra[1];
         const Real xa2U = (xa * xa) * U02;
         Real inner = 0;
-        for (int b = 0; b < P.n_b; ++b) {
+        int b = 0;
+        if constexpr (sizeof(Real) == 4) {
+          // fp32: two shell nodes per step in packed arithmetic (device_math.cuh); the unified kernel's node loop is
+          // short of issue slots, not of FMA-pipe time
+          const float* tab = reinterpret_cast<const float*>(T.tab) + a * P.n_b * TAB_W;
+          const float* tb = reinterpret_cast<const float*>(T.tb);
+          float2 inner2 = f2(0.0f);
+          for (; b + 1 < P.n_b; b += 2) {
+            const float2 p0 = *reinterpret_cast<const float2*>(tab + b * TAB_W);
+            const float2 p1 = *reinterpret_cast<const float2*>(tab + (b + 1) * TAB_W);
+            const float4 r0 = *reinterpret_cast<const float4*>(tb + b * TB_W);
+            const float4 r1 = *reinterpret_cast<const float4*>(tb + (b + 1) * TB_W);
+            const float2 ut2 = fma2(make_float2(r0.z, r1.z), f2((float)qq2), fma2(make_float2(p0.y, p1.y), f2((float)Wm), f2((float)xa2U)));
+            const float2 phi = sphere_phi2(make_float2(sqrt_fast(ut2.x), sqrt_fast(ut2.y)));
+            const float2 F = fma2(make_float2(p0.x, p1.x), phi, f2((float)fc));
+            inner2 = fma2(make_float2(r0.y, r1.y), mul2(F, F), inner2);
+          }
+          inner = (Real)(inner2.x + inner2.y);
+        }
+        for (; b < P.n_b; ++b) {
           const Real* pr = T.tab + (a * P.n_b + b) * TAB_W;
           const Real* rb = T.tb + b * TB_W;
           // u_t^2 = sum ((x a_k + t) Q_k)^2 = x^2 U0^2 + 2 x t W + t^2 q^2

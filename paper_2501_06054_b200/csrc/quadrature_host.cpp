@@ -105,6 +105,7 @@ static void gauss_tilt_rule_compute(double sigma, int n, std::vector<double>& d,
 
 // Rules are memoised by (kind, parameter bits, n): a dataset-generation loop sets thousands of models that
 // share a handful of rules, and the bisection costs ~100 us per 32-node rule.
+static void legendre_rule_01_compute(int n, std::vector<double>& x, std::vector<double>& w);
 namespace {
 struct RuleKey {
   int kind; uint64_t bits; int n;
@@ -124,7 +125,9 @@ void cached_rule(int kind, double param, int n, std::vector<double>& x, std::vec
   auto it = g_rules.find(key);
   if (it == g_rules.end()) {
     Rule r;
-    if (kind == 0) schulz_rule_compute(param, n, r.x, r.w); else gauss_tilt_rule_compute(param, n, r.x, r.w);
+    if (kind == 0) schulz_rule_compute(param, n, r.x, r.w);
+    else if (kind == 1) gauss_tilt_rule_compute(param, n, r.x, r.w);
+    else legendre_rule_01_compute(n, r.x, r.w);
     if (g_rules.size() >= 4096) g_rules.clear();
     it = g_rules.emplace(key, std::move(r)).first;
   }
@@ -136,7 +139,7 @@ void cached_rule(int kind, double param, int n, std::vector<double>& x, std::vec
 void schulz_rule(double p, int n, std::vector<double>& s, std::vector<double>& w) { cached_rule(0, p, n, s, w); }
 void gauss_tilt_rule(double sigma, int n, std::vector<double>& d, std::vector<double>& w) { cached_rule(1, sigma, n, d, w); }
 
-void legendre_rule_01(int n, std::vector<double>& x, std::vector<double>& w) {
+static void legendre_rule_01_compute(int n, std::vector<double>& x, std::vector<double>& w) {
   std::vector<double> a(n, 0.0), b(n, 0.0), xs, ws;
   for (int k = 1; k < n; ++k) b[k] = (double)k / std::sqrt(4.0 * (double)k * (double)k - 1.0);
   gauss_from_jacobi(a, b, xs, ws);   // on [-1, 1], weights summing to 1
@@ -144,6 +147,8 @@ void legendre_rule_01(int n, std::vector<double>& x, std::vector<double>& w) {
   w.resize(n);
   for (int i = 0; i < n; ++i) { x[i] = 0.5 * (xs[i] + 1.0); w[i] = ws[i]; }
 }
+
+void legendre_rule_01(int n, std::vector<double>& x, std::vector<double>& w) { cached_rule(2, 0.0, n, x, w); }
 
 namespace {
 
@@ -213,7 +218,7 @@ bool solve5(double A[5][5], double rhs[5], double x[5]) {
 
 }  // namespace
 
-bool msa_solve(double eta, double gam, double k, double out[5], double* g_contact) {
+static bool msa_solve_compute(double eta, double gam, double k, double out[5], double* g_contact) {
   MsaRule R;
   legendre_rule_01(64, R.x, R.w);
   double u[5] = {(1.0 + 2.0 * eta) / ((1.0 - eta) * (1.0 - eta)), -1.5 * eta / ((1.0 - eta) * (1.0 - eta)), 0.0, 0.0, 0.0};
@@ -248,6 +253,36 @@ bool msa_solve(double eta, double gam, double k, double out[5], double* g_contac
   out[0] = u[0]; out[1] = u[1]; out[2] = u[2]; out[3] = u[3]; out[4] = u[2] * std::exp(-k) - u[3];
   if (g_contact) *g_contact = u[0] + u[1] - k * u[3];
   return true;
+}
+
+// The closure costs ~45 ms to solve (20 continuation steps of Newton's method, each residual a 64 x 64 double
+// sum); a fitting or dataset loop sets the same charged system again and again: memoised by the three parameters.
+namespace {
+struct MsaKey {
+  uint64_t a, b, c;
+  bool operator<(const MsaKey& o) const { return a != o.a ? a < o.a : b != o.b ? b < o.b : c < o.c; }
+};
+struct MsaSol { bool ok; double u[5]; double g1; };
+std::mutex g_msa_mutex;
+std::map<MsaKey, MsaSol> g_msa;
+}  // namespace
+
+bool msa_solve(double eta, double gam, double k, double out[5], double* g_contact) {
+  MsaKey key;
+  std::memcpy(&key.a, &eta, 8);
+  std::memcpy(&key.b, &gam, 8);
+  std::memcpy(&key.c, &k, 8);
+  std::lock_guard<std::mutex> lock(g_msa_mutex);
+  auto it = g_msa.find(key);
+  if (it == g_msa.end()) {
+    MsaSol sol{};
+    sol.ok = msa_solve_compute(eta, gam, k, sol.u, &sol.g1);
+    if (g_msa.size() >= 1024) g_msa.clear();
+    it = g_msa.emplace(key, sol).first;
+  }
+  for (int i = 0; i < 5; ++i) out[i] = it->second.u[i];
+  if (g_contact) *g_contact = it->second.g1;
+  return it->second.ok;
 }
 
 }  // namespace sas

@@ -9,6 +9,12 @@ bound is the largest of five per-neutron costs, in SMSP clocks per lane (x 32 = 
     int   = c_lop3  x logic-pipe instructions + c_wide_int x 32x32->64 multiplies
     fp64  = c_dfma  x FP64 instructions
     xu    = c_mufu  x MUFU / POPC / conversion instructions
+    fma   = (imul + 2 c_ffma x FP32 operations) / 2              (the two FMA pipes, heavy and lite, 16 lanes each)
+
+An FP32 operation occupies one of the two FMA pipes for two clocks, a packed one (FFMA2 / FMUL2 / FADD2: two
+operations per lane in one instruction, measured 2.02 clocks per warp instruction) both of them; the integer
+multiplies run on the heavy pipe only.  The packed node loops of c2 and c3 count one ISSUE slot per packed
+instruction and two FP32 operations: they are bound by `fma`, no longer by `issue`.
 
 The clocks per warp instruction (c_*) are MEASURED on the box by csrc/microbench.cu, which bench.py runs before
 timing anything (`rates` below holds the figures of profiles/r2_microbench.md as a fallback only):
@@ -83,10 +89,12 @@ MODEL_COST = {
     # (counted, c1 fp64)
     "sphere_py_fp64": (U(138, wide=1, imad=1, logic=32, fp64=101, fp32=1, xu=3), U(45.2, logic=15.2, fp64=30)),
     # (round-1 SASS count of the node; prologue estimate)
-    "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(27, logic=1, fp32=25, xu=1)),
+    # (counted from the SASS of the packed row, cuobjdump of this build: 29 packed operations and 2 MUFU.RCP per
+    # pair of tilts, i.e. per node 29 FP32 operations in 14.5 issue slots + 1 MUFU; prologue estimate)
+    "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(15.5, fp32=29, xu=1)),
     # (counted, c3) prologue = Philox block 2 (orientation draws), three sincos of 2 pi u, frame, and the 16 outer
     # nodes (37 instructions each); inner node 34
-    "cs_triaxial_iso_fp32": (U(832, wide=19, imad=18.5, logic=136, fp64=114, fp32=499, xu=47), U(34, imad=0.5, logic=2.5, fp32=29, xu=2)),
+    "cs_triaxial_iso_fp32": (U(832, wide=19, imad=18.5, logic=136, fp64=114, fp32=499, xu=47), U(21, imad=0.5, logic=4, fp32=29, xu=2)),   # inner node packed: 29 FP32 operations in 14.5 issue slots
     # (estimate: the per-event cylinder below without its size draws)
     "cylinder_iso_fp64": (U(370, wide=37, logic=120, fp64=200, xu=6), U(0)),
     # (counted, n1) per-event sizes: Philox blocks 2 and 3 and a re-draw, two Box-Muller normals, three sin/cos of
@@ -102,7 +110,7 @@ MODEL_COST = {
     "sphere_msa_event_fp64": (U(280, wide=19, logic=55, fp64=190, xu=8), U(40, logic=6, fp64=33, xu=0)),
 }
 
-RESOURCES = ("issue", "imul", "int", "fp64", "xu")
+RESOURCES = ("issue", "imul", "int", "fp64", "xu", "fma")
 
 
 def unit_sum(frac_survive, frac_geometry, frac_detect, model_key, nodes, geometry="fast"):
@@ -121,7 +129,8 @@ def clocks(tot, r):
                 imul=r["imad_wide"] * tot["wide"] + r["imad"] * tot["imad"],
                 int=r["lop3"] * tot["logic"] + r["wide_int"] * tot["wide"],
                 fp64=r["dfma"] * tot["fp64"],
-                xu=r["mufu"] * tot["xu"])
+                xu=r["mufu"] * tot["xu"],
+                fma=0.5 * (r["imad_wide"] * tot["wide"] + r["imad"] * tot["imad"]) + r["ffma"] * tot["fp32"])
 
 
 def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, model_key: str, nodes: int,

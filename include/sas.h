@@ -290,6 +290,28 @@ typedef struct {
 sas_status sas_reduce_radial(sas_ctx* ctx, const sas_radial_desc* desc, double* h_q, double* h_I, double* h_sigma,
                              uint64_t* h_npix);
 
+/* The same ring average for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no context, no cudaMalloc / cudaFree / event creation / synchronisation -- one
+ * cudaMemsetAsync and two kernel launches on `stream` (a cudaStream_t; NULL = the default stream) of the CURRENT
+ * device.  The ring scratch is a static device array of SAS_STATIC_MAX_RINGS rings (16 KB) that every GPU which
+ * loads the library holds until exit.
+ *   ins       detector geometry (det_nx, det_ny, det_xw, det_yh, det_dist are read; struct_size checked)
+ *   desc      as for sas_reduce_radial; exp_index is ignored; n_launched MUST be given (> 0)
+ *   d_sum_p, d_sum_p2   DEVICE, [det_ny][det_nx] doubles of one experiment (inputs, caller-owned, not modified)
+ *   d_q, d_I, d_sigma, d_npix   DEVICE outputs, n_bins entries each, caller-owned; any may be NULL
+ * Asynchronous: outputs are valid once the work queued on `stream` has completed.  Results equal
+ * sas_reduce_radial's (ring sums in a different order of fp64 additions: 1e-12; q and npix exactly).
+ * All calls on a device share the static array, which keeps the last call's sums: every call first clears what it
+ * uses, in stream order, so calls queued on ONE stream are safe back to back; calls that overlap on the GPU
+ * (different streams without a dependency, or different host threads) RACE -- serialise them.  The first call on a
+ * device looks the array's address up (once per device; make that call outside a graph capture).
+ * SAS_EINVAL: n_bins outside 1..SAS_STATIC_MAX_RINGS (message names the limit; use sas_reduce_radial beyond it),
+ * n_launched == 0, NULL inputs, bad geometry or q range; SAS_ECUDA: a CUDA call failed.  Message: sas_last_error(NULL). */
+#define SAS_STATIC_MAX_RINGS 512
+sas_status sas_reduce_radial_static(const sas_instrument_desc* ins, const sas_radial_desc* desc, const double* d_sum_p,
+                                    const double* d_sum_p2, double* d_q, double* d_I, double* d_sigma,
+                                    uint64_t* d_npix, void* stream);
+
 /* Device time in ms (CUDA events around the kernel) of the last sas_reduce_radial on this context. */
 sas_status sas_get_reduce_time(sas_ctx* ctx, double* ms);
 

@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "sas_last_error", "sas_create_batch", "sas_trace_batch", "sas_quadrature_nodes",
     "sas_get_launch_info", "sas_get_kernel_time", "sas_get_upload_bytes", "sas_version", "sas_reduce_radial",
     "sas_trace_batch_range", "sas_get_launch_records", "sas_get_reduce_time", "sas_set_launch_timing",
+    "sas_reduce_radial_static",
 ]
 
 SAMPLE = {"box": 0, "cyl_y": 1}
@@ -161,6 +162,7 @@ def load_library(path: str | None = None):
     L.sas_set_launch_timing.argtypes = [vp, i32]
     L.sas_get_upload_bytes.argtypes = [vp, pp(u64)]
     L.sas_reduce_radial.argtypes = [vp, pp(RadialDesc), vp, vp, vp, vp]
+    L.sas_reduce_radial_static.argtypes = [pp(InstrumentDesc), pp(RadialDesc), vp, vp, vp, vp, vp, vp, vp]
     L.sas_version.argtypes = []
     L.sas_version.restype = C.c_char_p
     for name in EXPORTED_SYMBOLS:
@@ -183,6 +185,25 @@ def quadrature_nodes(kind: str, param: float, n: int):
     w = (C.c_double * n)()
     _check(L, None, L.sas_quadrature_nodes({"schulz": 0, "gauss_tilt": 1}[kind], float(param), n, v, w))
     return np.array(v[:]), np.array(w[:])
+
+
+def reduce_radial_static(instrument: dict, sum_p, sum_p2, n_launched, lambda_ref, q_lo, q_hi, n_bins, out=None, stream=None):
+    """sas_reduce_radial_static (include/sas.h): ring average of one detector image without any allocation inside
+    the library.  sum_p, sum_p2: CUDA float64 tensors [ny][nx]; out: four caller-owned CUDA tensors (q, I, sigma
+    float64, npix int64/uint64 storage) of n_bins entries -- made here when omitted (by torch, outside the library).
+    Asynchronous on `stream` (default: torch's current stream of the inputs' device); returns `out`."""
+    import torch
+    L = load_library()
+    ins = instrument_desc(instrument)
+    d = RadialDesc(C.sizeof(RadialDesc), 0, int(n_bins), 0, float(q_lo), float(q_hi), float(lambda_ref), int(n_launched))
+    dev = sum_p.device
+    if out is None:
+        out = tuple(torch.empty(max(int(n_bins), 1), dtype=dt, device=dev) for dt in (torch.float64, torch.float64, torch.float64, torch.int64))
+    with torch.cuda.device(dev):
+        st = (stream if stream is not None else torch.cuda.current_stream(dev)).cuda_stream
+        _check(L, None, L.sas_reduce_radial_static(C.byref(ins), C.byref(d), sum_p.data_ptr(), sum_p2.data_ptr(),
+                                                   *(t.data_ptr() for t in out), st))
+    return out
 
 
 class _Base:

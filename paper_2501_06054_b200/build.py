@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsas_b200.so")
-SOURCES = ["sas_api.cu", "quadrature_host.cpp"]
+SOURCES = ["sas_api.cu", "reduce_static.cu", "quadrature_host.cpp"]
 HEADERS = ["device_math.cuh", "j1_f64_generated.h", "geometry.cuh", "models.cuh", "trace_kernel.cuh", "trace_kernel_ws.cuh", "reduce_kernel.cuh", "sas_types.h",
            "quadrature_host.h", "coeffs_generated.h", os.path.join("..", "..", "include", "sas.h")]
 

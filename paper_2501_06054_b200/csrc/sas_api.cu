@@ -838,6 +838,12 @@ void destroy_ctx(sas_ctx* c) {
 }  // namespace
 
 // ===================================================================== the ABI
+// for the entry points that live in other translation units and have no context (reduce_static.cu): the message
+// sas_last_error(NULL) returns
+namespace sas {
+void set_global_error(const std::string& msg) { g_create_error = msg; }
+}  // namespace sas
+
 extern "C" {
 
 const char* sas_version(void) { return "sas_b200 0.1 (sm_100a)"; }

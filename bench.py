@@ -133,7 +133,7 @@ def model_key_and_nodes(model):
     if m == "polymer_micelle":
         return "micelle_event_fp64", 0
     if is_event_model(model) and m == "sphere" and model["sq_kind"] == "hayter_msa":
-        return "sphere_msa_event_fp64", 65
+        return "sphere_msa_event_fp64", 64
     if m == "sphere":
         nodes = pd[0]
         if nodes == 1:

@@ -112,6 +112,26 @@ __device__ __forceinline__ void mbar_wait_a(uint32_t addr, uint32_t parity) {
         : "=r"(ok) : "r"(addr), "r"(parity), "r"(0x989680u) : "memory");
   } while (!ok);
 }
+// A producer that waits for a window to come back is ahead of its consumers (the launch is bound by stages B and C):
+// it backs off between polls, because the arbiter serves the producers first and their polling takes issue slots
+// from the very warps they wait for (ncu source page of n2 / n4: a quarter of all executed instructions were these
+// polls).  The first poll is immediate: a producer-bound launch never sleeps here.
+#ifndef SAS_WS_PROD_SLEEP_NS
+#define SAS_WS_PROD_SLEEP_NS 400
+#endif
+__device__ __forceinline__ void mbar_wait_producer(uint32_t addr, uint32_t parity) {
+  if (SAS_WS_PROD_SLEEP_NS == 0) { mbar_wait_a(addr, parity); return; }
+  for (;;) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    if (ok) break;
+    __nanosleep(SAS_WS_PROD_SLEEP_NS);
+  }
+}
 template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 __device__ __forceinline__ void bar_block() { asm volatile("bar.sync 0;" ::: "memory"); }
@@ -246,7 +266,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
         mbar_arrive_a(ring + OFF_FULL + 8u * w);
       }
       const uint32_t seq2 = seq + 2u;  // (a first use passes at once)
-      mbar_wait_a(ring + OFF_EMPTY + 8u * (seq2 & (uint32_t)(WS_G - 1)), ((seq2 / (uint32_t)WS_G) & 1u) ^ 1u);
+      mbar_wait_producer(ring + OFF_EMPTY + 8u * (seq2 & (uint32_t)(WS_G - 1)), ((seq2 / (uint32_t)WS_G) & 1u) ^ 1u);
     };
     // stage B0 on up to 32 WS_NB0 stack entries (WS_NB0 per lane: independent Philox chains)
     auto stage_b0 = [&](uint32_t exp_word) {

@@ -89,25 +89,26 @@ MODEL_COST = {
     # (counted, c1 fp64)
     "sphere_py_fp64": (U(138, wide=1, imad=1, logic=32, fp64=101, fp32=1, xu=3), U(45.2, logic=15.2, fp64=30)),
     # (round-1 SASS count of the node; prologue estimate)
-    # (counted from the SASS of the packed row, cuobjdump of this build: 29 packed operations and 2 MUFU.RCP per
-    # pair of tilts, i.e. per node 29 FP32 operations in 14.5 issue slots + 1 MUFU; prologue estimate)
-    "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(15.5, fp32=29, xu=1)),
+    # (counted, c2: executed SASS of the packed row, profiles/r2_instruction_counts.md) per tilt node 13.5 packed
+    # instructions (27 FP32 operations), 0.2 scalar FP32, 0.2 logic, 1 MUFU.RCP; prologue estimate
+    "cylinder_quad_fp32": (U(60, logic=10, fp64=40, xu=4), U(14.9, logic=0.2, fp32=27.2, xu=1)),
     # (counted, c3) prologue = Philox block 2 (orientation draws), three sincos of 2 pi u, frame, and the 16 outer
     # nodes (37 instructions each); inner node 34
-    "cs_triaxial_iso_fp32": (U(832, wide=19, imad=18.5, logic=136, fp64=114, fp32=499, xu=47), U(21, imad=0.5, logic=4, fp32=29, xu=2)),   # inner node packed: 29 FP32 operations in 14.5 issue slots
+    "cs_triaxial_iso_fp32": (U(832, wide=19, imad=18.5, logic=136, fp64=114, fp32=499, xu=47), U(19, imad=0.5, logic=2.5, fp32=28, xu=2)),   # (counted) inner node packed: 14 packed instructions = 28 FP32 operations
     # (estimate: the per-event cylinder below without its size draws)
     "cylinder_iso_fp64": (U(370, wide=37, logic=120, fp64=200, xu=6), U(0)),
     # (counted, n1) per-event sizes: Philox blocks 2 and 3 and a re-draw, two Box-Muller normals, three sin/cos of
     # pi x, sin, Lambda, the weight
     "cylinder_event_fp64": (U(562, wide=56, imad=3, logic=150, fp64=344, fp32=2, xu=7), U(0)),
-    # (estimate) barbell, per event: the prologue of the per-event cylinder, then 64 slice evaluations
-    "barbell_event_fp64": (U(562, wide=56, imad=3, logic=150, fp64=344, fp32=2, xu=7), U(70, logic=8, fp64=58, xu=2)),
-    # (estimate) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
-    "micelle_event_fp64": (U(330, wide=19, logic=60, fp64=230, xu=8), U(0)),
-    # (estimate) charged spheres, per event: Philox block 3, one Box-Muller normal, sphere Phi; then the 64 nodes of
-    # the MSA rule and the tail term, each one fp64 sine/cosine pair (three-step reduction, two Taylor kernels) and
-    # two accumulations
-    "sphere_msa_event_fp64": (U(280, wide=19, logic=55, fp64=190, xu=8), U(40, logic=6, fp64=33, xu=0)),
+    # (counted, n2) barbell, per event: everything that executes once per detected warp (size and orientation draws,
+    # frame, cylinder term, weight), then 64 slice evaluations of the two end pieces (fp64 Lambda and cosine each)
+    "barbell_event_fp64": (U(608, wide=56, imad=3, logic=155, fp64=382, fp32=3, xu=9), U(49.5, logic=6, fp64=43, xu=0.5)),
+    # (counted, n3) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
+    "micelle_event_fp64": (U(514, wide=19, imad=2, logic=111, fp64=350, fp32=15, xu=17), U(0)),
+    # (counted, n4) charged spheres, per event: Philox block 3, one Box-Muller normal, sphere Phi, the tail term of
+    # S(q); then the 64 nodes of the MSA rule, each one fp64 sine/cosine pair (three-step reduction, two Taylor
+    # kernels, quadrant selects) and two accumulations
+    "sphere_msa_event_fp64": (U(312, wide=19, imad=2, logic=84, fp64=195, fp32=4, xu=8), U(39, logic=12, fp64=27)),
 }
 
 RESOURCES = ("issue", "imul", "int", "fp64", "xu", "fma")

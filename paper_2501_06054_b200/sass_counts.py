@@ -6,8 +6,8 @@ paper_2501_06054_b200/roofline.py; profiles/r2_instruction_counts.md states the 
 
 Classes: wide (IMAD.WIDE, IMAD.HI: 32x32->64 multiplies), imad (other integer multiplies), logic (LOP3, integer and
 float compares, votes, selects, min/max), addr (integer adds, shifts, LEA, permutes, IMAD used as add/shift), fp64,
-fp32, xu (MUFU, POPC, conversions), lsu (loads, stores, atomics), move (moves, uniform-datapath and constant loads),
-ctl (branches, barriers, convergence, sleeps).  roofline.py counts wide, imad, logic, fp64, fp32 and xu as
+fp32, fp32x2 (packed FFMA2 / FMUL2 / FADD2: one instruction, two FP32 operations per lane), xu (MUFU, POPC, conversions), lsu (loads, stores, atomics), move (moves, uniform-datapath and constant loads),
+ctl (branches, barriers, convergence, sleeps).  roofline.py counts wide, imad, logic, fp64, fp32, fp32x2 and xu as
 algorithmic; addr, lsu, move and ctl are not.  `denominator` = executions of the unit the counts are per (e.g. the
 execution count of the stage's first line times rows per step)."""
 from __future__ import annotations
@@ -17,7 +17,7 @@ import csv
 import subprocess
 import sys
 
-ORDER = ("wide", "imad", "logic", "addr", "fp64", "fp32", "xu", "lsu", "move", "ctl")
+ORDER = ("wide", "imad", "logic", "addr", "fp64", "fp32", "fp32x2", "xu", "lsu", "move", "ctl")
 
 
 def classify(full: str) -> str:
@@ -33,6 +33,8 @@ def classify(full: str) -> str:
         return "imad"
     if op in ("DFMA", "DMUL", "DADD", "DSETP"):
         return "fp64"
+    if op in ("FFMA2", "FMUL2", "FADD2"):
+        return "fp32x2"          # packed: one issue slot, two FP32 operations per lane (roofline.py: fma resource)
     if op in ("FFMA", "FMUL", "FADD", "HFMA2"):
         return "fp32"
     if op in ("MUFU", "POPC", "I2F", "F2I", "I2FP", "F2F", "FRND"):

@@ -405,10 +405,11 @@ def cpu_model_name():
 
 def run_sweep(torch, S):
     """Run time against the number of neutrons, the paper's own experiment (N from 1e5 to
-    1e11): c0 (monodisperse sphere) and the paper's per-event scheme on its rod (n1), one launch sequence per N,
-    CUDA events around it, after one warm-up at the same N."""
+    1e11): c0 (monodisperse sphere) and the paper's per-event scheme on its rod (n1) and on three of the models it
+    found expensive (barbell n2, polymer micelle n3, Hayter MSA n4), one launch sequence per N, CUDA
+    events around it, after one warm-up at the same N."""
     out = {}
-    for idx in (0, 5):
+    for idx in (0, 5, 6, 7, 8):
         c = W.config(idx)
         tr = S.Tracer(c["instrument"], c["model"])
         rows = []
@@ -441,7 +442,7 @@ def main():
     ap.add_argument("--precision", default=None, help="precision override of --config (profiling)")
     ap.add_argument("--neutrons", type=int, default=None, help="neutrons per step override of --config (profiling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1, then exit")
+    ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1..n4, then exit")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

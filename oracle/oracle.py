@@ -34,7 +34,7 @@ _LAMBDA = {"uniform": 0, "triangle": 1}
 _MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3,
           "core_shell_triaxial": 4, "flat": 5, "parallelepiped": 6, "core_shell_cylinder": 7, "ellipsoid": 8,
           "barbell": 9, "capped_cylinder": 10, "elliptical_cylinder": 11, "hollow_cylinder": 12,
-          "core_shell_ellipsoid": 13, "polymer_micelle": 14}
+          "core_shell_ellipsoid": 13, "polymer_micelle": 14, "hollow_prism_thin": 15}
 _ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
 _SQ = {"none": 0, "hard_sphere_py": 1, "hayter_msa": 2}
 

@@ -278,6 +278,20 @@ double orc_amplitude(const orc_model* m, double qa, double qb, double qc, double
       *env = m->sld[0] * V;
       return (m->sld[0] * V) * ((orc_sinc(qa * (0.5 * a)) * orc_sinc(qb * (0.5 * b))) * orc_sinc(qc * (0.5 * c)));
     }
+    case ORC_HOLLOW_PRISM_THIN: {
+      /* R-M5: rectangular prism a x b x c along A, B, C whose contrast sits in walls of thickness t -> 0 on its six
+       * faces (first order in t): Eq. 1 becomes a surface integral, F = sld t * sum over the faces of
+       * int exp(i Q.r) dS.  The two faces at x = +-a/2 give 2 cos(Q_A a/2) * [b sinc(Q_B b/2)] [c sinc(Q_C c/2)],
+       * and so on cyclically.  Normalising volume = wall volume t * 2 (ab + bc + ca).  x0 scales a, b, c. */
+      double a = m->size[0] * x0, b = m->size[1] * x0, c = m->size[2] * x0, t = m->size[3];
+      double sa = orc_sinc(qa * (0.5 * a)), sb = orc_sinc(qb * (0.5 * b)), sc = orc_sinc(qc * (0.5 * c));
+      double ca = cos(qa * (0.5 * a)), cb = cos(qb * (0.5 * b)), cc = cos(qc * (0.5 * c));
+      double faces = (((b * c) * ca) * (sb * sc) + ((a * c) * cb) * (sa * sc)) + ((a * b) * cc) * (sa * sb);
+      double V = t * (2.0 * ((a * b + b * c) + c * a));
+      *vol = V;
+      *env = m->sld[0] * V;
+      return (m->sld[0] * t) * (2.0 * faces);
+    }
     case ORC_CORE_SHELL_CYLINDER: {
       /* core cylinder (R, L) of contrast sld[0] inside a cylinder (R+t, L+2t) of contrast sld[1]:
        * Eq. 1 with a piecewise contrast = (sld0-sld1) x core + sld1 x whole; x0 scales R, x1 scales L */

@@ -60,7 +60,11 @@ enum {
   /* one of the models the paper found expensive (Table II group F "Polymer micelle"): a homogeneous
    * spherical core with N Gaussian chains attached to its surface (Pedersen & Gerstenberg, Macromolecules 29
    * (1996) 1363; DESIGN.md R-M4).  size = R_core, R_g, V_chain (A^3), N; sld[0] core, sld[1] chain */
-  ORC_POLYMER_MICELLE = 14
+  ORC_POLYMER_MICELLE = 14,
+  /* another of them ("Hollow rectangular prism thin walls"; DESIGN.md R-M5): a rectangular prism
+   * a x b x c whose contrast sits in infinitely thin walls on its six faces: Eq. 1 as a surface integral, to first
+   * order in the wall thickness t.  size = a, b, c, t; sld[0] wall contrast; pd[0] = common scale of a, b, c */
+  ORC_HOLLOW_PRISM_THIN = 15
 };
 enum {
   ORC_ORIENT_FIXED = 0,

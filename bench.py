@@ -42,7 +42,8 @@ SECONDARY = [("c0_sphere_fp64", 0, None, None), ("c0_sphere_fp64_1e9", 0, None, 
              ("c1_polysphere_py_fp32", 1, "fp32", None), ("c1_polysphere_py_fp64", 1, "fp64", None),
              ("c3_coreshell_triaxial", 3, None, None), ("c4_batch", 4, None, None),
              ("n1_paper_cylinder", 5, None, None), ("n2_paper_barbell", 6, None, None),
-             ("n3_paper_micelle", 7, None, None), ("n4_paper_hayter_msa", 8, None, None)]
+             ("n3_paper_micelle", 7, None, None), ("n4_paper_hayter_msa", 8, None, None),
+             ("n5_paper_hollow_prism", 9, None, None)]
 
 
 # ------------------------------------------------------------------ reference arm: the CPU oracle
@@ -132,6 +133,8 @@ def model_key_and_nodes(model):
         return "barbell_event_fp64", 64
     if m == "polymer_micelle":
         return "micelle_event_fp64", 0
+    if is_event_model(model) and m == "hollow_prism_thin":
+        return "hollow_prism_event_fp64", 0
     if is_event_model(model) and m == "sphere" and model["sq_kind"] == "hayter_msa":
         return "sphere_msa_event_fp64", 64
     if m == "sphere":
@@ -406,10 +409,10 @@ def cpu_model_name():
 def run_sweep(torch, S):
     """Run time against the number of neutrons, the paper's own experiment (N from 1e5 to
     1e11): c0 (monodisperse sphere) and the paper's per-event scheme on its rod (n1) and on three of the models it
-    found expensive (barbell n2, polymer micelle n3, Hayter MSA n4), one launch sequence per N, CUDA
+    found expensive (barbell n2, polymer micelle n3, Hayter MSA n4, thin-walled hollow prism n5), one launch sequence per N, CUDA
     events around it, after one warm-up at the same N."""
     out = {}
-    for idx in (0, 5, 6, 7, 8):
+    for idx in (0, 5, 6, 7, 8, 9):
         c = W.config(idx)
         tr = S.Tracer(c["instrument"], c["model"])
         rows = []
@@ -442,7 +445,7 @@ def main():
     ap.add_argument("--precision", default=None, help="precision override of --config (profiling)")
     ap.add_argument("--neutrons", type=int, default=None, help="neutrons per step override of --config (profiling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1..n4, then exit")
+    ap.add_argument("--sweep", action="store_true", help="run time against N (1e5..1e11) for c0 and n1..n5, then exit")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

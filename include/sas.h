@@ -81,7 +81,12 @@ enum {
    * Pedersen & Gerstenberg, Macromolecules 29 (1996) 1363): homogeneous spherical core with N Gaussian chains
    * starting at R_core + R_g.  size = R_core, R_g, V_chain (A^3), N (0 or >= 1); sld[0] core, sld[1] chain
    * contrast; normalising volume V_core + N V_chain; pd[0] on R_core; isotropic (orientation is ignored) */
-  SAS_POLYMER_MICELLE = 14
+  SAS_POLYMER_MICELLE = 14,
+  /* thin-walled hollow rectangular prism (PAPER.md:201 names it among the expensive models; DESIGN.md R-M5): a prism
+   * a x b x c along A, B, C whose contrast sld[0] sits in walls of thickness t on its six faces, to first order in t
+   * (Eq. 1 as a surface integral).  size = a, b, c, t; normalising volume = wall volume 2 t (ab + bc + ca);
+   * pd[0] = common scale of a, b, c */
+  SAS_HOLLOW_PRISM_THIN = 15
 };
 enum {
   SAS_ORIENT_FIXED = 0,

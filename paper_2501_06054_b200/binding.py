@@ -27,7 +27,8 @@ SAMPLE = {"box": 0, "cyl_y": 1}
 LAMBDA_DIST = {"uniform": 0, "triangle": 1}
 MODEL = {"sphere": 0, "core_shell_sphere": 1, "cylinder": 2, "triaxial": 3, "core_shell_triaxial": 4, "flat": 5,
          "parallelepiped": 6, "core_shell_cylinder": 7, "ellipsoid": 8, "barbell": 9, "capped_cylinder": 10,
-         "elliptical_cylinder": 11, "hollow_cylinder": 12, "core_shell_ellipsoid": 13, "polymer_micelle": 14}
+         "elliptical_cylinder": 11, "hollow_cylinder": 12, "core_shell_ellipsoid": 13, "polymer_micelle": 14,
+         "hollow_prism_thin": 15}
 ORIENT = {"fixed": 0, "gauss_quad": 1, "isotropic_mc": 2, "uniform_angles_mc": 3}
 PD = {"none": 0, "schulz": 1, "gauss_mc": 2}
 SQ = {"none": 0, "hard_sphere_py": 1, "hayter_msa": 2}

@@ -197,6 +197,20 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
     const double a = P.msize[0] * x0, b = P.msize[1] * x0, c = P.msize[2] * x0;
     Vol = (a * b) * c;
     F = (s0 * Vol) * ((sinc_r(qA * (0.5 * a)) * sinc_r(qB * (0.5 * b))) * sinc_r(qC * (0.5 * c)));
+  } else if (V == V_HOLLOW_PRISM) {
+    // R-M5: contrast in thin walls on the six faces: F = 2 sld t [bc cos(qA a/2) sinc_b sinc_c + cyclic]
+    const double a = P.msize[0] * x0, b = P.msize[1] * x0, c = P.msize[2] * x0, t = P.msize[3];
+    double sa, ca, sb, cb, sc, cc;
+    const double xa = qA * (0.5 * a), xb = qB * (0.5 * b), xc = qC * (0.5 * c);
+    sincos_d(xa, sa, ca);
+    sincos_d(xb, sb, cb);
+    sincos_d(xc, sc, cc);
+    sa = xa == 0.0 ? 1.0 : sa / xa;
+    sb = xb == 0.0 ? 1.0 : sb / xb;
+    sc = xc == 0.0 ? 1.0 : sc / xc;
+    const double faces = fma((b * c) * ca, sb * sc, fma((a * c) * cb, sa * sc, ((a * b) * cc) * (sa * sb)));
+    Vol = t * (2.0 * fma(a, b, fma(b, c, c * a)));
+    F = (s0 * t) * (2.0 * faces);
   } else if (V == V_CS_CYL) {
     const double R = P.msize[0] * x0, L = P.msize[1] * x1, t = P.msize[2];
     const double Rt = R + t, Lt = L + 2.0 * t;

@@ -139,13 +139,13 @@ sas_status validate_instrument(const sas_instrument_desc* d, std::string& why) {
 sas_status validate_model(const sas_model_desc* m, std::string& why) {
   if (!m) { why = "model descriptor is NULL"; return SAS_EINVAL; }
   if (m->struct_size != sizeof(sas_model_desc)) { why = "sas_model_desc.struct_size mismatch"; return SAS_EINVAL; }
-  if (m->model < SAS_SPHERE || m->model > SAS_POLYMER_MICELLE) { why = "unknown model"; return SAS_EINVAL; }
+  if (m->model < SAS_SPHERE || m->model > SAS_HOLLOW_PRISM_THIN) { why = "unknown model"; return SAS_EINVAL; }
   if (m->precision != SAS_FP32 && m->precision != SAS_FP64) { why = "unknown precision"; return SAS_EINVAL; }
   if (m->orient_kind < SAS_ORIENT_FIXED || m->orient_kind > SAS_ORIENT_UNIFORM_ANGLES_MC) { why = "unknown orient_kind"; return SAS_EINVAL; }
   if (m->sq_kind != SAS_SQ_NONE && m->sq_kind != SAS_SQ_HARD_SPHERE_PY && m->sq_kind != SAS_SQ_HAYTER_MSA) { why = "unknown sq_kind"; return SAS_EINVAL; }
   if (!std::isfinite(m->scale) || !std::isfinite(m->background)) { why = "scale/background not finite"; return SAS_EINVAL; }
-  static const int n_sizes[15] = {1, 2, 2, 3, 4, 0, 3, 3, 2, 3, 3, 3, 3, 3, 4};
-  static const int n_pd[15] = {1, 2, 2, 1, 2, 0, 1, 2, 2, 2, 2, 2, 2, 2, 1};
+  static const int n_sizes[16] = {1, 2, 2, 3, 4, 0, 3, 3, 2, 3, 3, 3, 3, 3, 4, 4};
+  static const int n_pd[16] = {1, 2, 2, 1, 2, 0, 1, 2, 2, 2, 2, 2, 2, 2, 1, 1};
   for (int i = 0; i < n_sizes[m->model]; ++i) {
     // a shell thickness may be 0, every other size must be > 0
     const bool may_be_zero = (m->model == SAS_CORE_SHELL_SPHERE && i == 1) || (m->model == SAS_CORE_SHELL_TRIAXIAL && i == 3) ||
@@ -351,6 +351,10 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
           V = FOUR_PI_3 * (m.size[0] * xa[a] + t) * (m.size[1] * xa[a] + t) * (m.size[2] * xa[a] + t);
         } break;
         case SAS_PARALLELEPIPED: V = (m.size[0] * xa[a]) * (m.size[1] * xa[a]) * (m.size[2] * xa[a]); break;
+        case SAS_HOLLOW_PRISM_THIN: {
+          const double pa = m.size[0] * xa[a], pb = m.size[1] * xa[a], pc = m.size[2] * xa[a];
+          V = m.size[3] * (2.0 * (pa * pb + pb * pc + pc * pa));   // wall volume (R-M5)
+        } break;
         case SAS_CORE_SHELL_CYLINDER: {
           const double Rt = m.size[0] * xa[a] + m.size[2], Lt = m.size[1] * xb[b] + 2.0 * m.size[2];
           V = PI_D * Rt * Rt * Lt;
@@ -399,6 +403,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
       // NEXT-2 models: the node value and its weight; the kernel forms the amplitude itself (models.cuh)
       case SAS_PARALLELEPIPED: case SAS_CORE_SHELL_CYLINDER: case SAS_ELLIPSOID: case SAS_BARBELL: case SAS_CAPPED_CYLINDER:
       case SAS_ELLIPTICAL_CYLINDER: case SAS_HOLLOW_CYLINDER: case SAS_CORE_SHELL_ELLIPSOID: case SAS_POLYMER_MICELLE:
+      case SAS_HOLLOW_PRISM_THIN:
         r[0] = xa[a]; r[2] = wa[a]; break;
       default: break;
     }
@@ -410,6 +415,7 @@ void fill_model(const sas_model_desc& m, ExpParams& P, std::vector<double>& pool
       case SAS_CORE_SHELL_TRIAXIAL: { const double t = m.size[3] * xb[b]; r[0] = t; r[1] = wb[b]; r[2] = t * t; } break;
       case SAS_PARALLELEPIPED: case SAS_CORE_SHELL_CYLINDER: case SAS_ELLIPSOID: case SAS_BARBELL: case SAS_CAPPED_CYLINDER:
       case SAS_ELLIPTICAL_CYLINDER: case SAS_HOLLOW_CYLINDER: case SAS_CORE_SHELL_ELLIPSOID: case SAS_POLYMER_MICELLE:
+      case SAS_HOLLOW_PRISM_THIN:
         r[0] = xb[b]; r[2] = wb[b]; break;
       default: r[1] = wb[b]; break;
     }
@@ -774,6 +780,7 @@ sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v, int g) {
     case V_HOLLOW_CYL: return launch<double, V_HOLLOW_CYL, EV>(c, a);
     case V_CS_ELL: return launch<double, V_CS_ELL, EV>(c, a);
     case V_MICELLE: return launch<double, V_MICELLE, EV>(c, a);
+    case V_HOLLOW_PRISM: return launch<double, V_HOLLOW_PRISM, EV>(c, a);
     default: return fail(c, SAS_EINVAL, "unknown kernel variant");
   }
 }

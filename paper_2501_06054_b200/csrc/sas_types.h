@@ -21,8 +21,8 @@ enum : int { ST_DETECTED = 0, ST_SLIT1 = 1, ST_SLIT2 = 2, ST_MISS_SAMPLE = 3, ST
 enum : int {
   V_SPHERE = 0, V_CS_SPHERE = 1, V_CYL = 2, V_TRIAX = 3, V_CS_TRIAX = 4, V_FLAT = 5, V_CYL_QUAD = 6,
   V_PARA = 7, V_CS_CYL = 8, V_ELL = 9, V_BARBELL = 10, V_CAPPED = 11,  // NEXT-2: generic fp64 node loop
-  V_ELL_CYL = 12, V_HOLLOW_CYL = 13, V_CS_ELL = 14, V_MICELLE = 15,
-  N_VARIANTS = 16
+  V_ELL_CYL = 12, V_HOLLOW_CYL = 13, V_CS_ELL = 14, V_MICELLE = 15, V_HOLLOW_PRISM = 16,
+  N_VARIANTS = 17
 };
 
 // table record widths (in Reals)

@@ -105,6 +105,9 @@ MODEL_COST = {
     "barbell_event_fp64": (U(608, wide=56, imad=3, logic=155, fp64=382, fp32=3, xu=9), U(49.5, logic=6, fp64=43, xu=0.5)),
     # (counted, n3) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
     "micelle_event_fp64": (U(514, wide=19, imad=2, logic=111, fp64=350, fp32=15, xu=17), U(0)),
+    # (counted, n5) thin-walled hollow prism, per event: Philox blocks 2 and 3, one Box-Muller normal, the frame (three
+    # sin/cos of pi x), three fp64 sine/cosine pairs of the half-side phases, the face sum
+    "hollow_prism_event_fp64": (U(518, wide=38, imad=2, logic=154, fp64=313, fp32=5, xu=6), U(0)),
     # (counted, n4) charged spheres, per event: Philox block 3, one Box-Muller normal, sphere Phi, the tail term of
     # S(q); then the 64 nodes of the MSA rule, each one fp64 sine/cosine pair (three-step reduction, two Taylor
     # kernels, quadrant selects) and two accumulations

@@ -58,7 +58,7 @@ def model(**over):
 
 
 def config(i: int, precision: str | None = None):
-    """Return dict(name, instrument, model, n_neutrons, seed) for config i in 0..3 and 5..7,
+    """Return dict(name, instrument, model, n_neutrons, seed) for config i in 0..3 and 5..9,
     or dict(name, instruments[], models[], n_neutrons_each, seed) for config 4."""
     if i == 0:
         return dict(name="c0_sphere_fp64", instrument=instrument(),
@@ -130,6 +130,14 @@ def config(i: int, precision: str | None = None):
                         pd_rel=[0.1, 0.0], scale=0.2, sq_kind="hayter_msa", sq_radius_eff=45.0, sq_volfrac=0.2,
                         sq_contact_kT=5.0, sq_kappa_sigma=2.0),
             n_neutrons=10**9, seed=20250114)
+    if i == 9:
+        # NEXT-2 (not a BASELINE.json config): "Hollow rectangular prism thin walls", the fourth expensive model of
+        # PAPER.md:201 built here (DESIGN.md R-M5), with the paper's per-event size scale and orientation
+        return dict(
+            name="n5_paper_hollow_prism", instrument=instrument(det_nx=256, det_ny=256),
+            model=model(model="hollow_prism_thin", precision="fp64", size=[35.0, 75.0, 120.0, 2.0],
+                        pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0.0], orient_kind="uniform_angles_mc"),
+            n_neutrons=10**9, seed=20250115)
     raise ValueError(i)
 
 

@@ -435,6 +435,13 @@ MORE_MODELS = [
                            sq_radius_eff=60.0, sq_volfrac=0.1, background=0.005)),
     ("micelle_paper", dict(model="polymer_micelle", size=[40.0, 15.0, 4000.0, 30.0], sld=[2e-6, 1e-6, 0],
                            pd_kind=["gauss_mc", "none"], pd_rel=[0.1, 0])),
+    # thin-walled hollow rectangular prism (R-M5): fixed orientation, Schulz scale with random orientation, the
+    # paper's per-event scheme
+    ("hollow_prism_fixed", dict(model="hollow_prism_thin", size=[35.0, 75.0, 120.0, 2.0], theta=0.7, phi=2.0, psi=0.5)),
+    ("hollow_prism_pd_iso", dict(model="hollow_prism_thin", size=[35.0, 75.0, 120.0, 2.0], pd_kind=["schulz", "none"],
+                                 pd_rel=[0.1, 0], pd_nodes=[8, 1], orient_kind="isotropic_mc", background=0.002)),
+    ("hollow_prism_paper", dict(model="hollow_prism_thin", size=[35.0, 75.0, 120.0, 2.0], pd_kind=["gauss_mc", "none"],
+                                pd_rel=[0.1, 0], orient_kind="uniform_angles_mc")),
 ]
 
 
@@ -749,10 +756,10 @@ def test_hayter_msa_in_a_batch_and_its_refusals(sas):
     assert err.value.status == 1
 
 
-@pytest.mark.parametrize("cfg", [5, 6, 7, 8])
+@pytest.mark.parametrize("cfg", [5, 6, 7, 8, 9])
 def test_paper_scheme_workloads_of_the_bench_per_neutron(sas, cfg):
-    """The n1..n4 workloads exactly as bench.py configures them (the paper's per-event averaging on its rod, a
-    barbell, a micelle, charged spheres with the Hayter MSA S(q)): an id prefix per neutron and per bin."""
+    """The n1..n5 workloads exactly as bench.py configures them (the paper's per-event averaging on its rod, a
+    barbell, a micelle, charged spheres with the Hayter MSA S(q), a thin-walled hollow prism): an id prefix per neutron and per bin."""
     c = W.config(cfg)
     check_prefix(sas, c["instrument"], c["model"], c["seed"], 150000, min_detected=6000)
 

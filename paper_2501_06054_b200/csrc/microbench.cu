@@ -13,19 +13,20 @@
 constexpr int CHAINS = 8;
 constexpr int UNROLL = 32;
 
-enum { K_FFMA, K_IMAD, K_IMAD_WIDE, K_LOP3, K_DFMA, K_MUFU_RCP, K_PHILOX, N_KINDS };
+enum { K_FFMA, K_IMAD, K_IMAD_WIDE, K_LOP3, K_DFMA, K_MUFU_RCP, K_PHILOX, K_FFMA2, N_KINDS };
 static const char* NAMES[N_KINDS] = {"FFMA (fp32 fused multiply-add)", "IMAD (32-bit integer multiply-add)",
                                      "IMAD.WIDE.U32 (32x32->64 multiply)", "LOP3 (integer logic)",
                                      "DFMA (fp64 fused multiply-add)", "MUFU.RCP (special function)",
-                                     "Philox4x32-10 block (20 wide multiplies + 20 LOP3)"};
-static const double INSTR_PER_STEP[N_KINDS] = {1, 1, 1, 1, 1, 1, 1};
+                                     "Philox4x32-10 block (20 wide multiplies + 20 LOP3)",
+                                     "FFMA2 (packed fp32 fused multiply-add, two per lane)"};
+static const double INSTR_PER_STEP[N_KINDS] = {1, 1, 1, 1, 1, 1, 1, 1};
 
 template <int KIND>
 __global__ void __launch_bounds__(256, 4) bench(int iters, uint32_t seed, uint32_t* out) {
   uint32_t id = blockIdx.x * blockDim.x + threadIdx.x + seed;
-  float f[CHAINS]; double d[CHAINS]; uint32_t u[CHAINS]; unsigned long long w[CHAINS];
+  float f[CHAINS]; double d[CHAINS]; uint32_t u[CHAINS]; unsigned long long w[CHAINS]; float2 f2[CHAINS];
 #pragma unroll
-  for (int c = 0; c < CHAINS; ++c) { f[c] = 1.0f + id * 1e-9f + c; d[c] = 1.0 + id * 1e-12 + c; u[c] = id * 2654435761u + c; w[c] = u[c]; }
+  for (int c = 0; c < CHAINS; ++c) { f[c] = 1.0f + id * 1e-9f + c; d[c] = 1.0 + id * 1e-12 + c; u[c] = id * 2654435761u + c; w[c] = u[c]; f2[c] = make_float2(f[c], f[c] + 0.5f); }
   const float fa = 1.0000001f, fb = 1e-7f;
   const double da = 1.0000000001, db = 1e-10;
   for (int i = 0; i < iters; ++i) {
@@ -38,13 +39,14 @@ __global__ void __launch_bounds__(256, 4) bench(int iters, uint32_t seed, uint32
         if (KIND == K_IMAD_WIDE) w[c] = (unsigned long long)(uint32_t)(w[c] ^ (w[c] >> 32)) * 0xD2511F53ull;
         if (KIND == K_LOP3) u[c] = u[c] ^ u[(c + 1) % CHAINS] ^ (id + k);
         if (KIND == K_DFMA) d[c] = fma(d[c], da, db);
+        if (KIND == K_FFMA2) f2[c] = __ffma2_rn(f2[c], make_float2(fa, fa), make_float2(fb, fb));
         if (KIND == K_MUFU_RCP) { asm volatile("rcp.approx.ftz.f32 %0, %0;" : "+f"(f[c])); f[c] += fb; }  // + one FADD on the FMA pipe
       }
     }
   }
   uint32_t acc = 0;
 #pragma unroll
-  for (int c = 0; c < CHAINS; ++c) acc ^= __float_as_uint(f[c]) ^ (uint32_t)__double2loint(d[c]) ^ u[c] ^ (uint32_t)w[c] ^ (uint32_t)(w[c] >> 32);
+  for (int c = 0; c < CHAINS; ++c) acc ^= __float_as_uint(f[c]) ^ (uint32_t)__double2loint(d[c]) ^ u[c] ^ (uint32_t)w[c] ^ (uint32_t)(w[c] >> 32) ^ __float_as_uint(f2[c].x) ^ __float_as_uint(f2[c].y);
   if (acc == 0x12345678u) out[id & 1023] = acc;
 }
 
@@ -233,6 +235,7 @@ int main() {
   v[K_FFMA] = run<K_FFMA>(mhz); v[K_IMAD] = run<K_IMAD>(mhz); v[K_IMAD_WIDE] = run<K_IMAD_WIDE>(mhz);
   v[K_LOP3] = run<K_LOP3>(mhz); v[K_DFMA] = run<K_DFMA>(mhz); v[K_MUFU_RCP] = run<K_MUFU_RCP>(mhz);
   v[K_PHILOX] = run_philox(mhz);
+  v[K_FFMA2] = run<K_FFMA2>(mhz);
   printf("SMSP clocks per warp instruction at %.0f MHz (32 resident warps per SM, %d independent chains per thread)\n", mhz, CHAINS);
   for (int k = 0; k < N_KINDS; ++k) printf("  %-52s %7.2f\n", NAMES[k], v[k]);
   const double m0 = run_mix<0>(mhz), m1 = run_mix<1>(mhz), m2 = run_mix<2>(mhz), m3 = run_mix<3>(mhz), sa = run_stage_a(mhz);
@@ -242,7 +245,7 @@ int main() {
   printf("  %-52s %7.2f us\n", "event pair around a kernel that does nothing", fl);
   // one machine-readable line for bench.py
   printf("{\"sm_mhz\": %.0f, \"ffma\": %.4f, \"imad\": %.4f, \"imad_wide\": %.4f, \"lop3\": %.4f, \"dfma\": %.4f, \"mufu\": %.4f, "
-         "\"philox_block\": %.3f, \"wide_lop3\": [%.4f, %.4f, %.4f, %.4f], \"stage_a_core_row\": %.3f, \"event_floor_us\": %.2f}\n",
-         mhz, v[K_FFMA], v[K_IMAD], v[K_IMAD_WIDE], v[K_LOP3], v[K_DFMA], v[K_MUFU_RCP], v[K_PHILOX], m0, m1, m2, m3, sa, fl);
+         "\"philox_block\": %.3f, \"wide_lop3\": [%.4f, %.4f, %.4f, %.4f], \"stage_a_core_row\": %.3f, \"event_floor_us\": %.2f, \"ffma2\": %.4f}\n",
+         mhz, v[K_FFMA], v[K_IMAD], v[K_IMAD_WIDE], v[K_LOP3], v[K_DFMA], v[K_MUFU_RCP], v[K_PHILOX], m0, m1, m2, m3, sa, fl, v[K_FFMA2]);
   return 0;
 }

@@ -9,10 +9,11 @@ bound is the largest of five per-neutron costs, in SMSP clocks per lane (x 32 = 
     int   = c_lop3  x logic-pipe instructions + c_wide_int x 32x32->64 multiplies
     fp64  = c_dfma  x FP64 instructions
     xu    = c_mufu  x MUFU / POPC / conversion instructions
-    fma   = (imul + 2 c_ffma x FP32 operations) / 2              (the two FMA pipes, heavy and lite, 16 lanes each)
+    fma   = (imul + c_ffma2 x FP32 operations) / 2               (the two FMA pipes, heavy and lite, 16 lanes each)
 
 An FP32 operation occupies one of the two FMA pipes for two clocks, a packed one (FFMA2 / FMUL2 / FADD2: two
-operations per lane in one instruction, measured 2.02 clocks per warp instruction) both of them; the integer
+operations per lane in one instruction; c_ffma2, measured by the microbenchmark: 2.02 clocks per warp instruction)
+both of them; the integer
 multiplies run on the heavy pipe only.  The packed node loops of c2 and c3 count one ISSUE slot per packed
 instruction and two FP32 operations: they are bound by `fma`, no longer by `issue`.
 
@@ -41,7 +42,7 @@ SMSP_PER_SM = 4
 SM_MAX_MHZ = 1965.0
 
 # fallback rates: profiles/r2_microbench.md (B200, 1965 MHz); bench.py replaces them with the live run
-RATES = dict(ffma=1.036, imad=2.020, imad_wide=4.05, lop3=2.024, dfma=2.029, mufu=8.04, wide_int=2.05,
+RATES = dict(ffma=1.036, ffma2=2.02, imad=2.020, imad_wide=4.05, lop3=2.024, dfma=2.029, mufu=8.04, wide_int=2.05,
              philox_block=81.0, stage_a_core_row=76.1, source="profiles/r2_microbench.md (not re-measured)")
 
 
@@ -52,7 +53,7 @@ def rates_from_microbench(mb: dict) -> dict:
     w = mb["wide_lop3"]                       # clocks for 1 multiply + (1 + NL) LOP3, NL = 0..3
     slope = (w[3] - w[1]) / 2.0
     wide_int = w[1] - 2.0 * slope             # intercept of the n >= 2 line
-    return dict(ffma=mb["ffma"], imad=mb["imad"], imad_wide=mb["philox_block"] / 20.0, lop3=lop3, dfma=mb["dfma"],
+    return dict(ffma=mb["ffma"], ffma2=mb.get("ffma2", 2.0 * mb["ffma"]), imad=mb["imad"], imad_wide=mb["philox_block"] / 20.0, lop3=lop3, dfma=mb["dfma"],
                 mufu=mb["mufu"], wide_int=wide_int, philox_block=mb["philox_block"],
                 stage_a_core_row=mb["stage_a_core_row"], source="csrc/microbench.cu, run by bench.py on this box")
 
@@ -134,7 +135,8 @@ def clocks(tot, r):
                 int=r["lop3"] * tot["logic"] + r["wide_int"] * tot["wide"],
                 fp64=r["dfma"] * tot["fp64"],
                 xu=r["mufu"] * tot["xu"],
-                fma=0.5 * (r["imad_wide"] * tot["wide"] + r["imad"] * tot["imad"]) + r["ffma"] * tot["fp32"])
+                # an FP32 operation costs half a packed instruction's time on the pair of pipes (measured: ffma2)
+                fma=0.5 * (r["imad_wide"] * tot["wide"] + r["imad"] * tot["imad"]) + 0.5 * r.get("ffma2", 2.0 * r["ffma"]) * tot["fp32"])
 
 
 def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, model_key: str, nodes: int,
@@ -162,7 +164,7 @@ def roofline(neutrons_per_s: float, frac_survive: float, frac_detect: float, mod
         "peak_source": (f"{N_SM} SM x {SMSP_PER_SM} SMSP x 32 lanes x {sm_mhz:.0f} MHz (maximum SM clock); clocks per "
                         f"instruction of each pipe from {r['source']}"),
         "pipe_clocks_per_warp_instruction": {k: round(float(r[k]), 3) for k in
-                                             ("ffma", "imad", "imad_wide", "lop3", "wide_int", "dfma", "mufu")},
+                                             ("ffma", "ffma2", "imad", "imad_wide", "lop3", "wide_int", "dfma", "mufu") if k in r},
         "traffic": traffic,
     }
     if sm_mhz_sampled:

@@ -63,6 +63,7 @@ struct sas_ctx {
   // group = variant + N_VARIANTS * (per-event sizes ? 1 : 0) + 2 N_VARIANTS * (fp64 model arithmetic ? 1 : 0)
   std::vector<uint32_t> group_ids[N_GROUPS];
   size_t group_off[N_GROUPS] = {};
+  bool group_heavy[N_GROUPS] = {};  // consumer-bound group: launched in the 2 producer + 6 consumer split
   uint32_t* d_exp_ids = nullptr;
   double* d_rings = nullptr;  // ring sums of sas_reduce_radial: 3 x SAS_MAX_RINGS doubles + SAS_MAX_RINGS counts
   cudaStream_t stream = nullptr;
@@ -590,6 +591,22 @@ int effective_precision(const sas_model_desc& m, const sas_instrument_desc& ins)
   return SAS_FP32;
 }
 
+// Is a launch of this experiment on the warp-specialised kernel bound by its consumers (stages B and C) rather than
+// by the Philox producers?  Then the block is split into one producer and three consumer warpgroups instead of one
+// and one (trace_kernel_ws.cuh).  Measured at 1e8..1e9 neutrons, heavy split against default: barbell per event
+// +9 %, Hayter MSA +3 %, 32 fp64 sphere nodes +3 %; one fp64 evaluation per neutron (sphere -13 %, per-event
+// cylinder -5 %) and the fp32 node loops (32 sphere nodes -8 %) stay with the default split.
+#ifndef SAS_WS_HEAVY_EVALS
+#define SAS_WS_HEAVY_EVALS 24
+#endif
+bool consumer_bound(const ExpParams& P, int precision) {
+  if (precision != SAS_FP64 || P.model == SAS_FLAT) return false;
+  if (P.model == SAS_BARBELL || P.model == SAS_CAPPED_CYLINDER) return true;  // 64 slices with a Bessel J1 each
+  if (P.sq_kind == SAS_SQ_HAYTER_MSA) return true;                             // 65 fp64 sine/cosine pairs
+  const long evals = (long)std::max(P.n_a, 1) * std::max(P.n_b, 1) * std::max(P.n_th, 1) * std::max(P.n_ph, 1);
+  return evals >= SAS_WS_HEAVY_EVALS;
+}
+
 // (re)build ExpParams + tables of every experiment and upload them
 sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
   c->h_tab.clear();
@@ -638,6 +655,11 @@ sas_status upload_models(sas_ctx* c, const sas_model_desc* models) {
     const bool event = (P.pd_mc[0] | P.pd_mc[1]) != 0 && P.model != SAS_FLAT;
     c->group_ids[v + (event ? (int)N_VARIANTS : 0) + (c->exp_prec[e] == SAS_FP64 ? 2 * (int)N_VARIANTS : 0)].push_back(e);
   }
+  for (int g = 0; g < N_GROUPS; ++g) {
+    size_t n_heavy = 0;
+    for (uint32_t e : c->group_ids[g]) n_heavy += consumer_bound(c->h_exps[e], c->exp_prec[e]) ? 1 : 0;
+    c->group_heavy[g] = !c->group_ids[g].empty() && 2 * n_heavy >= c->group_ids[g].size();
+  }
   std::vector<uint32_t> ids;
   for (int v = 0; v < N_GROUPS; ++v) {
     c->group_off[v] = ids.size();
@@ -675,15 +697,15 @@ constexpr bool use_ws(int v) { return ((SAS_WS_VARIANTS >> v) & 1u) != 0; }
 // occupancy and shared-memory opt-in of one kernel instantiation, asked from the runtime once per (kernel, smem)
 struct KernelPlan { size_t smem = ~(size_t)0; int bps = 0; };
 
-template <typename Real, int V, bool EV>
+template <typename Real, int V, bool EV, int CWG>
 sas_status launch(sas_ctx* c, KernelArgs& a) {
   const bool DUMP = a.d_pixel != nullptr;
   constexpr bool WS = use_ws(V);
-  constexpr int BLOCK_THREADS = WS ? WS_THREADS : block_threads(V);
+  constexpr int BLOCK_THREADS = WS ? WsCfg<CWG>::THREADS : block_threads(V);
   constexpr int ROW_WARPS = WS ? WS_PAIRS : BLOCK_THREADS / 32;  // warps that share the rows of a work item
-  const size_t smem = WS ? ws_smem_bytes<Real>(c->tab_len_max) : trace_smem_bytes<Real>(c->tab_len_max, BLOCK_THREADS / 32);
+  const size_t smem = WS ? ws_smem_bytes<Real, CWG>(c->tab_len_max) : trace_smem_bytes<Real>(c->tab_len_max, BLOCK_THREADS / 32);
   void (*kern)(const KernelArgs);
-  if constexpr (WS) kern = trace_kernel_ws<Real, V, EV>; else kern = trace_kernel<Real, V, EV>;
+  if constexpr (WS) kern = trace_kernel_ws<Real, V, EV, CWG>; else kern = trace_kernel<Real, V, EV>;
   if (smem > 227 * 1024) return fail(c, SAS_EINVAL, "quadrature tables do not fit in shared memory");
   static thread_local KernelPlan plan[8];  // per device ordinal
   KernelPlan& pl = plan[c->device & 7];
@@ -758,29 +780,40 @@ sas_status launch(sas_ctx* c, KernelArgs& a) {
   return SAS_OK;
 }
 
+// The warp-specialised kernel in the split the group asks for: the fp64 instantiations exist in both splits
+// (consumer_bound), everything else in the default one only.
+template <typename Real, int V, bool EV>
+sas_status launch_split(sas_ctx* c, KernelArgs& a, bool heavy) {
+  if constexpr (use_ws(V) && sizeof(Real) == 8 && V != V_FLAT) {
+    if (heavy) return launch<Real, V, EV, SAS_WS_CWG_HEAVY>(c, a);
+  }
+  return launch<Real, V, EV, SAS_WS_CWG>(c, a);
+}
+
 // one launch of the kernel compiled for group g (variant, fixed-node or per-event sizes) over its experiments
 template <typename Real, bool EV>
 sas_status launch_variant(sas_ctx* c, KernelArgs& a, int v, int g) {
   a.exp_ids = c->d_exp_ids + c->group_off[g];
   a.n_exp = (uint32_t)c->group_ids[g].size();
+  const bool heavy = c->group_heavy[g];
   switch (v) {
-    case V_SPHERE: return launch<Real, V_SPHERE, EV>(c, a);
-    case V_CS_SPHERE: return launch<Real, V_CS_SPHERE, EV>(c, a);
-    case V_CYL: return launch<Real, V_CYL, EV>(c, a);
-    case V_TRIAX: return launch<Real, V_TRIAX, EV>(c, a);
-    case V_CS_TRIAX: return launch<Real, V_CS_TRIAX, EV>(c, a);
-    case V_FLAT: return launch<Real, V_FLAT, false>(c, a);
-    case V_CYL_QUAD: return launch<Real, V_CYL_QUAD, false>(c, a);
-    case V_PARA: return launch<double, V_PARA, EV>(c, a);
-    case V_CS_CYL: return launch<double, V_CS_CYL, EV>(c, a);
-    case V_ELL: return launch<double, V_ELL, EV>(c, a);
-    case V_BARBELL: return launch<double, V_BARBELL, EV>(c, a);
-    case V_CAPPED: return launch<double, V_CAPPED, EV>(c, a);
-    case V_ELL_CYL: return launch<double, V_ELL_CYL, EV>(c, a);
-    case V_HOLLOW_CYL: return launch<double, V_HOLLOW_CYL, EV>(c, a);
-    case V_CS_ELL: return launch<double, V_CS_ELL, EV>(c, a);
-    case V_MICELLE: return launch<double, V_MICELLE, EV>(c, a);
-    case V_HOLLOW_PRISM: return launch<double, V_HOLLOW_PRISM, EV>(c, a);
+    case V_SPHERE: return launch_split<Real, V_SPHERE, EV>(c, a, heavy);
+    case V_CS_SPHERE: return launch_split<Real, V_CS_SPHERE, EV>(c, a, heavy);
+    case V_CYL: return launch_split<Real, V_CYL, EV>(c, a, heavy);
+    case V_TRIAX: return launch_split<Real, V_TRIAX, EV>(c, a, heavy);
+    case V_CS_TRIAX: return launch_split<Real, V_CS_TRIAX, EV>(c, a, heavy);
+    case V_FLAT: return launch_split<Real, V_FLAT, false>(c, a, heavy);
+    case V_CYL_QUAD: return launch_split<Real, V_CYL_QUAD, false>(c, a, heavy);
+    case V_PARA: return launch_split<double, V_PARA, EV>(c, a, heavy);
+    case V_CS_CYL: return launch_split<double, V_CS_CYL, EV>(c, a, heavy);
+    case V_ELL: return launch_split<double, V_ELL, EV>(c, a, heavy);
+    case V_BARBELL: return launch_split<double, V_BARBELL, EV>(c, a, heavy);
+    case V_CAPPED: return launch_split<double, V_CAPPED, EV>(c, a, heavy);
+    case V_ELL_CYL: return launch_split<double, V_ELL_CYL, EV>(c, a, heavy);
+    case V_HOLLOW_CYL: return launch_split<double, V_HOLLOW_CYL, EV>(c, a, heavy);
+    case V_CS_ELL: return launch_split<double, V_CS_ELL, EV>(c, a, heavy);
+    case V_MICELLE: return launch_split<double, V_MICELLE, EV>(c, a, heavy);
+    case V_HOLLOW_PRISM: return launch_split<double, V_HOLLOW_PRISM, EV>(c, a, heavy);
     default: return fail(c, SAS_EINVAL, "unknown kernel variant");
   }
 }

@@ -5,7 +5,7 @@
 //       every launched neutron) and stage B0 (Philox block 1 + certain-miss classifier on the 25 % that survive):
 //       pure integer work, bound by the heavy FMA pipe (IMAD.WIDE, 4 clocks each).  Measured (profiles/
 //       r2_ws_probes.md): ONE such warp per sub-partition already saturates that pipe; more only queue behind it.
-//   WS_CWG consumer warpgroups (4 x WS_CWG warps): stage B (fp64 geometry, long dependent chains: latency bound,
+//   CWG consumer warpgroups (4 x CWG warps; 1 or 3, chosen per launch): stage B (fp64 geometry, long dependent chains: latency bound,
 //       wants as many warps as fit) and stage C (model node loops, weight, histogram) on the FP64/FP32/XU pipes.
 //
 // Producer warp p feeds consumer warps p, p + 4, ... (the same sub-partition) through a ring of chunks of 32
@@ -22,7 +22,10 @@
 namespace sas {
 
 #ifndef SAS_WS_CWG
-#define SAS_WS_CWG 1          // consumer warpgroups per block
+#define SAS_WS_CWG 1          // consumer warpgroups per block of the default split (4 producers + 4 consumers per sub-partition)
+#endif
+#ifndef SAS_WS_CWG_HEAVY
+#define SAS_WS_CWG_HEAVY 3    // ... of the split for launches bound by stages B and C (2 producers + 6 consumers)
 #endif
 #ifndef SAS_WS_REGS
 #define SAS_WS_REGS 64        // registers per thread at launch (x threads = the block's pool)
@@ -46,18 +49,26 @@ namespace sas {
 #define SAS_WS_PROD_LAST 0    // the producers are the LAST warpgroup: the sub-partition arbiter serves the highest warp id first
 #endif
 
-constexpr int WS_CWG = SAS_WS_CWG;
-constexpr int WS_THREADS = 128 * (1 + WS_CWG);
-constexpr int WS_MIN_BLOCKS = (65536 / (SAS_WS_REGS * WS_THREADS)) < 1 ? 1 : (65536 / (SAS_WS_REGS * WS_THREADS));
+// The split of a block is a template parameter of the kernel (CWG consumer warpgroups behind one producer
+// warpgroup); the host picks it per launch (sas_api.cu: consumer_bound).  The default split moves 8 registers per
+// thread from the producers to the consumers with setmaxnreg; the heavy split keeps the launch budget for both
+// (2 x 512 threads x 64 registers fill the register file).
+template <int CWG>
+struct WsCfg {
+  static constexpr int THREADS = 128 * (1 + CWG);
+  static constexpr int REGS = SAS_WS_REGS;
+  static constexpr int PROD_REGS = CWG == SAS_WS_CWG ? SAS_WS_PROD_REGS : SAS_WS_REGS;
+  static constexpr int CONS_REGS = CWG == SAS_WS_CWG ? SAS_WS_CONS_REGS : SAS_WS_REGS;
+  static constexpr int MIN_BLOCKS = (65536 / (REGS * THREADS)) < 1 ? 1 : (65536 / (REGS * THREADS));
+  static_assert(PROD_REGS * 128 + CONS_REGS * 128 * CWG <= REGS * THREADS, "setmaxnreg budgets exceed the block's register pool");
+  static_assert(REGS * THREADS * MIN_BLOCKS <= 65536, "register file");
+};
 constexpr int WS_PAIRS = 4;               // producer warps = sub-partitions
 constexpr int WS_G = SAS_WS_G;            // chunks per producer warp
 constexpr int WS_NR = SAS_WS_NR;
 constexpr int WS_NB0 = SAS_WS_NB0;
 constexpr int WS_STACK = 32 * WS_NB0 + 32 * WS_NR;  // stage A -> B0 stack: < one B0 batch + one stage-A step
 static_assert((WS_G & (WS_G - 1)) == 0 && WS_G >= 2, "chunks per producer: a power of two");
-static_assert(SAS_WS_PROD_REGS * 128 + SAS_WS_CONS_REGS * 128 * WS_CWG <= SAS_WS_REGS * WS_THREADS,
-              "setmaxnreg budgets exceed the block's register pool");
-static_assert(SAS_WS_REGS * WS_THREADS * WS_MIN_BLOCKS <= 65536, "register file");
 
 enum : uint32_t { WS_DATA = 0, WS_FLUSH = 1, WS_DONE = 2 };
 
@@ -82,16 +93,17 @@ struct WsConsumer {
   uint32_t oc[6][32];            // outcome counts per lane: row 0 detected, rows 1..5 = ST_*
 };
 
+template <int CWG>
 struct WsShared {
   WsProducer prod[WS_PAIRS];
-  WsConsumer cons[WS_PAIRS * WS_CWG];
+  WsConsumer cons[WS_PAIRS * CWG];
   unsigned int item[2];
   unsigned long long outcomes[8];  // the block's outcome counts (slots of KernelArgs::counters), flushed once per block
 };
 
-template <typename Real>
+template <typename Real, int CWG>
 __host__ __device__ inline size_t ws_smem_bytes(int tab_len_max) {
-  return round16(sizeof(ExpParams)) + round16((size_t)tab_len_max * sizeof(Real)) + round16(sizeof(WsShared));
+  return round16(sizeof(ExpParams)) + round16((size_t)tab_len_max * sizeof(Real)) + round16(sizeof(WsShared<CWG>));
 }
 
 // ---------------------------------------------------------------- mbarrier / register-budget primitives
@@ -188,13 +200,15 @@ __device__ __forceinline__ void philox_words01(const PhiloxKeys& pk, uint32_t c0
   w1 = 0xCD9E8D57u * c2;
 }
 
-template <typename Real, int V, bool EV>
-__global__ void __launch_bounds__(WS_THREADS, WS_MIN_BLOCKS)
+template <typename Real, int V, bool EV, int CWG>
+__global__ void __launch_bounds__(WsCfg<CWG>::THREADS, WsCfg<CWG>::MIN_BLOCKS)
 trace_kernel_ws(const __grid_constant__ KernelArgs a) {
+  using Cfg = WsCfg<CWG>;
+  constexpr int WS_CWG = CWG, WS_THREADS = Cfg::THREADS;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   ExpParams& P = *reinterpret_cast<ExpParams*>(smem_raw);
   Real* tab = reinterpret_cast<Real*>(smem_raw + round16(sizeof(ExpParams)));
-  WsShared& S = *reinterpret_cast<WsShared*>(smem_raw + round16(sizeof(ExpParams)) +
+  WsShared<CWG>& S = *reinterpret_cast<WsShared<CWG>*>(smem_raw + round16(sizeof(ExpParams)) +
                                              round16((size_t)a.tab_len_max * sizeof(Real)));
   const int lane = threadIdx.x & 31;
   const int wid = threadIdx.x >> 5;
@@ -240,7 +254,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
 
   if (is_producer) {
     // ================================================================ producers: stages A and B0
-    if (SAS_WS_PROD_REGS != SAS_WS_REGS) reg_dealloc<SAS_WS_PROD_REGS>();
+    if (Cfg::PROD_REGS != Cfg::REGS) reg_dealloc<Cfg::PROD_REGS>();
     const uint32_t ring = pin(smem_u32(&S.prod[pair]));         // this warp's ring (shared-window address)
     const uint32_t stack0 = pin(smem_u32(S.prod[pair].b_id));   // stack B
     const uint32_t lt = pin(lt_mask);
@@ -377,7 +391,7 @@ trace_kernel_ws(const __grid_constant__ KernelArgs a) {
     }
   } else {
     // ================================================================ consumers: stages B and C
-    if (SAS_WS_CONS_REGS != SAS_WS_REGS) reg_alloc<SAS_WS_CONS_REGS>();
+    if (Cfg::CONS_REGS != Cfg::REGS) reg_alloc<Cfg::CONS_REGS>();
     WsConsumer& cq = S.cons[cwid];
     const uint32_t ring = pin(smem_u32(&S.prod[pair]));
     constexpr uint32_t OFF_ID = (uint32_t)offsetof(WsProducer, id), OFF_FULL = (uint32_t)offsetof(WsProducer, full);

@@ -263,7 +263,8 @@ typedef struct {
   int32_t warp_specialised; /* 1: producer/consumer kernel (trace_kernel_ws.cuh) */
   uint32_t n_exp;        /* experiments of the launch */
   uint32_t n_per_exp;    /* ids per experiment */
-  int32_t grid, block;
+  int32_t grid, block;   /* block: 256 = one producer + one consumer warpgroup, 512 = one + three (launches bound by
+                            the model evaluation; warp-specialised kernel), 128 = unified kernel */
   double ms;
 } sas_launch_record;
 sas_status sas_get_launch_records(sas_ctx* ctx, sas_launch_record* h_records, uint32_t cap, uint32_t* n);

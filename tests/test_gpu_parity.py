@@ -656,6 +656,40 @@ def test_precision_is_decided_per_experiment(sas):
         assert_bins(sp[e], ref, "sum_p", 1e-9 if tol < 1e-11 else 1e-5, e)
 
 
+def test_producer_consumer_split_is_chosen_per_launch_group(sas):
+    """The warp-specialised kernel exists in two block splits: one producer + one consumer
+    warpgroup (256 threads) and one + three (512 threads) for launches bound by stages B and C.  A barbell and a
+    32-node fp64 sphere take the heavy split, a monodisperse sphere and the fp32 node loop the default one; an fp64
+    batch whose sphere group holds two 32-node experiments and one monodisperse one is launched once, in the heavy
+    split (majority), and every experiment is the oracle's per neutron and per bin whichever split served it."""
+    ins = W.instrument(det_nx=128, det_ny=128)
+    mono = W.model(precision="fp64", size=[80.0, 0, 0, 0])
+    poly64 = W.model(precision="fp64", size=[60.0, 0, 0, 0], pd_kind=["schulz", "none"], pd_rel=[0.1, 0.0], pd_nodes=[32, 1])
+    poly32 = dict(poly64, precision="fp32")
+    barbell = W.config(6)["model"]
+    for model, block in ((mono, 256), (poly64, 512), (poly32, 256), (barbell, 512)):
+        tr = sas.Tracer(ins, model)
+        tr.trace(100000, 5)
+        recs = tr.launch_records()
+        tr.close()
+        assert [(r["warp_specialised"], r["block"]) for r in recs] == [(1, block)], (model["model"], recs)
+    seed, n = 78, 200000
+    models = [poly64, mono, poly64]
+    bt = sas.BatchTracer([ins] * 3, models)
+    bt.trace(n, seed)
+    sp, sp2, cn = (a.reshape(3, -1).copy() for a in bt.read_detector())
+    recs = bt.launch_records()
+    bt.close()
+    assert [(r["n_exp"], r["block"]) for r in recs] == [(3, 512)], recs
+    for e, model in enumerate(models):
+        tr = sas.Tracer(ins, model)
+        check_prefix(sas, ins, model, seed, n, exp_index=e, tol=1e-12, min_detected=5000, tracer=tr)
+        tr.close()
+        ref = O.trace_range(ins, model, seed, 0, n, exp_index=e)
+        assert np.array_equal(cn[e], ref["counts"]), e
+        assert_bins(sp[e], ref, "sum_p", 1e-9, e)
+
+
 def test_fp32_request_with_phases_beyond_the_proven_range_runs_in_fp64(sas):
     """The fp32 argument reductions are proven for |x| < 1e3 rad (device_math.cuh).  A Schulz-polydisperse sphere of
     4000 A at q_max = 0.3 reaches 1.6e3: the library serves that experiment in fp64 (include/sas.h) and meets the

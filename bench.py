@@ -136,7 +136,7 @@ def model_key_and_nodes(model):
     if is_event_model(model) and m == "hollow_prism_thin":
         return "hollow_prism_event_fp64", 0
     if is_event_model(model) and m == "sphere" and model["sq_kind"] == "hayter_msa":
-        return "sphere_msa_event_fp64", 64
+        return "sphere_msa_event_fp64", 32   # node pairs of the folded 64-node rule (models.cuh: msa_sq)
     if m == "sphere":
         nodes = pd[0]
         if nodes == 1:

@@ -316,10 +316,15 @@ __device__ __forceinline__ double particle_f2(const ExpParams& P, double q, doub
 }
 
 // R-S2, Hayter-Penfold MSA: S = 1 / |Qhat(K)|^2, K = 2 q R_eff, Qhat = 1 - 12 eta [int_0^1 Q e^{iKx} dx + D' e^{iK}/(k - iK)];
-// the core integral is the 64-node Gauss-Legendre sum whose nodes and weighted Q values the host tabulated in fp64
-// (global memory: 1 KB that every detected neutron of the experiment reads).  Out of line: one call per detected
-// neutron, and the kernels of the other structure factors must not carry its registers.
-constexpr int MSA_N = 64;
+// the core integral is the 64-node Gauss-Legendre sum sum_j c_j e^{iK x_j}, c_j = 12 eta w_j Q(x_j).  The nodes of
+// the rule lie in pairs 1/2 +- y_j, so the sum is regrouped exactly as
+//   e^{iK/2} sum_{j<32} [ (c_j+ + c_j-) cos(K y_j) + i (c_j+ - c_j-) sin(K y_j) ]:
+// 32 sine/cosine pairs per detected neutron instead of 64, arguments half as large; sin K and cos K of the tail term
+// follow from the same sin, cos of K/2.  The host tabulates y_j and the two coefficient rows in fp64 (global memory:
+// 800 B that every detected neutron of the experiment reads).  Out of line: one call per detected neutron, and the
+// kernels of the other structure factors must not carry its registers.
+constexpr int MSA_N = 64;      // nodes of the rule
+constexpr int MSA_H = MSA_N / 2;  // node pairs = table rows
 // Offered for the globular models (sphere family, ellipsoids, micelle) only: an out-of-line call in a kernel costs
 // that kernel's every workload 1-3 % through register allocation (measured on the per-event cylinder and the
 // barbell), and a sphere-sphere structure factor has no meaning for rods and plates anyway (the host refuses it).
@@ -327,17 +332,19 @@ __host__ __device__ constexpr bool msa_offered(int V) {
   return V == V_SPHERE || V == V_CS_SPHERE || V == V_TRIAX || V == V_CS_TRIAX || V == V_ELL || V == V_CS_ELL || V == V_MICELLE;
 }
 __device__ __noinline__ double msa_sq(const double* __restrict__ t, double q) {
-  const double eD = t[2 * MSA_N], k = t[2 * MSA_N + 1], K = q * t[2 * MSA_N + 2];
-  double re = 0.0, im = 0.0;
+  const double eD = t[3 * MSA_H], k = t[3 * MSA_H + 1], K = q * t[3 * MSA_H + 2];
+  double ec = 0.0, os = 0.0;
 #pragma unroll 4
-  for (int j = 0; j < MSA_N; ++j) {
+  for (int j = 0; j < MSA_H; ++j) {
     double s, c;
     sincos_cw(K * t[j], s, c);
-    re = fma(t[MSA_N + j], c, re);
-    im = fma(t[MSA_N + j], s, im);
+    ec = fma(t[MSA_H + j], c, ec);
+    os = fma(t[2 * MSA_H + j], s, os);
   }
-  double sK, cK;
-  sincos_cw(K, sK, cK);
+  double sh, ch;
+  sincos_cw(0.5 * K, sh, ch);
+  double re = fma(ch, ec, -(sh * os)), im = fma(sh, ec, ch * os);   // e^{iK/2} (ec + i os)
+  const double sK = 2.0 * (sh * ch), cK = (ch - sh) * (ch + sh);
   const double den = fma(k, k, K * K);
   re = 1.0 - fma(eD, fma(k, cK, -(K * sK)) / den, re);
   im = -fma(eD, fma(k, sK, K * cK) / den, im);

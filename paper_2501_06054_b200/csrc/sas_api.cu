@@ -484,10 +484,16 @@ sas_status fill_msa(const sas_model_desc& m, const sas_instrument_desc& ins, std
   std::vector<double> x, w;
   legendre_rule_01(64, x, w);
   const double eta12 = 12.0 * m.sq_volfrac, k = m.sq_kappa_sigma;
-  *off = pool.size();
-  pool.insert(pool.end(), x.begin(), x.end());
+  // the nodes lie in pairs 1/2 +- y (ascending: x[j] and x[63 - j]); rows: y_j, c+ + c-, c+ - c- (models.cuh: msa_sq)
+  std::vector<double> cq(64);
   for (int j = 0; j < 64; ++j)
-    pool.push_back(eta12 * w[j] * (((0.5 * u[0]) * (x[j] * x[j] - 1.0) + u[1] * (x[j] - 1.0)) + (u[2] * std::exp(-k * x[j]) - u[3])));
+    cq[j] = eta12 * w[j] * (((0.5 * u[0]) * (x[j] * x[j] - 1.0) + u[1] * (x[j] - 1.0)) + (u[2] * std::exp(-k * x[j]) - u[3]));
+  for (int j = 0; j < 32; ++j)
+    if (!(x[63 - j] > x[j]) || std::fabs((x[63 - j] + x[j]) - 1.0) > 1e-14) { why = "Hayter MSA: the 64-node rule is not symmetric"; return SAS_EUNSUPPORTED; }
+  *off = pool.size();
+  for (int j = 0; j < 32; ++j) pool.push_back(0.5 * (x[63 - j] - x[j]));
+  for (int j = 0; j < 32; ++j) pool.push_back(cq[63 - j] + cq[j]);
+  for (int j = 0; j < 32; ++j) pool.push_back(cq[63 - j] - cq[j]);
   pool.push_back(eta12 * u[4]);
   pool.push_back(k);
   pool.push_back(2.0 * m.sq_radius_eff);
@@ -596,13 +602,16 @@ int effective_precision(const sas_model_desc& m, const sas_instrument_desc& ins)
 // and one (trace_kernel_ws.cuh).  Measured at 1e8..1e9 neutrons, heavy split against default: barbell per event
 // +9 %, Hayter MSA +3 %, 32 fp64 sphere nodes +3 %; one fp64 evaluation per neutron (sphere -13 %, per-event
 // cylinder -5 %) and the fp32 node loops (32 sphere nodes -8 %) stay with the default split.
+#ifndef SAS_WS_MSA_HEAVY
+#define SAS_WS_MSA_HEAVY 1
+#endif
 #ifndef SAS_WS_HEAVY_EVALS
 #define SAS_WS_HEAVY_EVALS 24
 #endif
 bool consumer_bound(const ExpParams& P, int precision) {
   if (precision != SAS_FP64 || P.model == SAS_FLAT) return false;
   if (P.model == SAS_BARBELL || P.model == SAS_CAPPED_CYLINDER) return true;  // 64 slices with a Bessel J1 each
-  if (P.sq_kind == SAS_SQ_HAYTER_MSA) return true;                             // 65 fp64 sine/cosine pairs
+  if (P.sq_kind == SAS_SQ_HAYTER_MSA) return SAS_WS_MSA_HEAVY != 0;            // 33 fp64 sine/cosine pairs
   const long evals = (long)std::max(P.n_a, 1) * std::max(P.n_b, 1) * std::max(P.n_th, 1) * std::max(P.n_ph, 1);
   return evals >= SAS_WS_HEAVY_EVALS;
 }

@@ -56,8 +56,9 @@ struct ExpParams {
   double frame[9];    // particle axes A, B, C in the global frame for fixed / mean orientation (R-A7)
   double msize[4];    // mean sizes (triaxial a, b, c)
   PYCoef py;
-  // Hayter MSA (R-S2): device address of this experiment's table in the fp64 pool -- 64 nodes x_j, 64 products
-  // 12 eta w_j Q(x_j), then 12 eta D', k, 2 R_eff -- read once per detected neutron (models.cuh: msa_sq)
+  // Hayter MSA (R-S2): device address of this experiment's table in the fp64 pool -- the 32 node pairs 1/2 +- y_j of
+  // the 64-node rule: y_j, sums and differences of the products 12 eta w Q(x) of a pair, then 12 eta D', k, 2 R_eff --
+  // read once per detected neutron (models.cuh: msa_sq)
   const double* msa_tab;
   // per-event size sampling (SAS_PD_GAUSS_MC, DESIGN.md R-N1/R-N2): contrasts, 1e8 scale, widths (sizes: msize)
   double ev_sld[2], ev_scale, pd_rel[2];

@@ -123,7 +123,7 @@ def config(i: int, precision: str | None = None):
     if i == 8:
         # NEXT-2 (not a BASELINE.json config): "Hayter MSA", the third expensive model of PAPER.md:201 built here:
         # charged spheres, the paper's per-event Gaussian radius, S(q) from the mean-spherical closure (DESIGN.md
-        # R-S2): 65 fp64 sine/cosine pairs per detected neutron
+        # R-S2): 33 fp64 sine/cosine pairs per detected neutron (the 64-node rule folded about x = 1/2)
         return dict(
             name="n4_paper_hayter_msa", instrument=instrument(det_nx=256, det_ny=256),
             model=model(model="sphere", precision="fp64", size=[40.0, 0, 0, 0], pd_kind=["gauss_mc", "none"],

@@ -109,11 +109,10 @@ MODEL_COST = {
     # (counted, n5) thin-walled hollow prism, per event: Philox blocks 2 and 3, one Box-Muller normal, the frame (three
     # sin/cos of pi x), three fp64 sine/cosine pairs of the half-side phases, the face sum
     "hollow_prism_event_fp64": (U(518, wide=38, imad=2, logic=154, fp64=313, fp32=5, xu=6), U(0)),
-    # (n4) charged spheres, per event: Philox block 3, one Box-Muller normal, sphere Phi, the tail term of S(q)
-    # (counted on the 64-node form; the folded sum adds a complex rotation by K/2 and the double-angle forms of
-    # sin K, cos K: 8 fp64 operations); then the 32 node PAIRS of the MSA rule, each one fp64 sine/cosine pair
-    # (three-step reduction, two Taylor kernels, quadrant selects) and two accumulations (counted)
-    "sphere_msa_event_fp64": (U(320, wide=19, imad=2, logic=84, fp64=203, fp32=4, xu=8), U(39, logic=12, fp64=27)),
+    # (counted, n4) charged spheres, per event: Philox block 3, one Box-Muller normal, sphere Phi, the tail term of
+    # S(q) with the rotation by K/2 of the folded sum; then the 32 node PAIRS of the MSA rule, each one fp64
+    # sine/cosine pair (three-step reduction, two Taylor kernels, quadrant selects) and two accumulations
+    "sphere_msa_event_fp64": (U(323, wide=19, imad=2, logic=85, fp64=205, fp32=4, xu=8), U(39, logic=12, fp64=27)),
 }
 
 RESOURCES = ("issue", "imul", "int", "fp64", "xu", "fma")

@@ -502,6 +502,12 @@ __device__ __forceinline__ double lambda1_r(double x) {
   const double j = (0.5641895835477563 * sqrt(inv)) * fma(P, s - c, Q * (s + c));
   return (2.0 * j) * inv;
 }
+// Lambda of a squared argument: the series range needs no square root (the barbell's slice loop has x^2 =
+// Q_AB^2 rho^2 at hand and paid an fp64 sqrt per slice for x)
+__device__ __forceinline__ double lambda1_sq(double x2) {
+  if (x2 <= SAS_J1_XA * SAS_J1_XA) return clenshaw(c_j1a, fma(x2, SAS_J1_A_SCALE, -1.0));
+  return lambda1_r(sqrt(x2));
+}
 __device__ __forceinline__ double lambda1_x2(double x2) { return lambda1_r(sqrt(x2)); }
 __device__ __forceinline__ double lambda1_x2_small(double x2) { return lambda1_r(sqrt(x2)); }
 template <int LC>

@@ -245,7 +245,7 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
     const double zc = V == V_BARBELL ? 0.5 * L + h : 0.5 * L - h;
     const double z0 = 0.5 * L, z1 = zc + Rb;
     const double half = 0.5 * (z1 - z0), mid = 0.5 * (z1 + z0);
-    const double qab = sqrt(fma(qA, qA, qB * qB));
+    const double qab2 = fma(qA, qA, qB * qB), qab = sqrt(qab2);
     double sum = 0.0;
 #pragma unroll 1
     for (int i = 0; i < GL_N; ++i) {
@@ -254,7 +254,7 @@ __device__ __forceinline__ double particle_amplitude(const ExpParams& P, double 
       const double rho2 = fmax(Rb * Rb - dz * dz, 0.0);
       double sz, cz;
       sincos_d(qC * z, sz, cz);
-      sum = fma(c_gl[GL_N + i], ((PI_D * rho2) * lambda1_r(qab * sqrt(rho2))) * cz, sum);
+      sum = fma(c_gl[GL_N + i], ((PI_D * rho2) * lambda1_sq(qab2 * rho2)) * cz, sum);
     }
     const double pz = z1 - zc, qz = z0 - zc;
     const double Vcyl = (PI_D * (R * R)) * L;

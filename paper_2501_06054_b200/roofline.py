@@ -102,8 +102,9 @@ MODEL_COST = {
     # pi x, sin, Lambda, the weight
     "cylinder_event_fp64": (U(562, wide=56, imad=3, logic=150, fp64=344, fp32=2, xu=7), U(0)),
     # (counted, n2) barbell, per event: everything that executes once per detected warp (size and orientation draws,
-    # frame, cylinder term, weight), then 64 slice evaluations of the two end pieces (fp64 Lambda and cosine each)
-    "barbell_event_fp64": (U(608, wide=56, imad=3, logic=155, fp64=382, fp32=3, xu=9), U(49.5, logic=6, fp64=43, xu=0.5)),
+    # frame, cylinder term, weight), then 64 slice evaluations of the two end pieces (fp64 Lambda of the squared argument
+    # and cosine each; recounted after the square root per slice was removed: 88 per pass of two slices)
+    "barbell_event_fp64": (U(608, wide=56, imad=3, logic=155, fp64=382, fp32=3, xu=9), U(44.0, logic=5.5, fp64=38.5)),
     # (counted, n3) micelle, per event: Philox block 3, one Box-Muller normal, sphere Phi, sinc, expm1, the four terms
     "micelle_event_fp64": (U(514, wide=19, imad=2, logic=111, fp64=350, fp32=15, xu=17), U(0)),
     # (counted, n5) thin-walled hollow prism, per event: Philox blocks 2 and 3, one Box-Muller normal, the frame (three

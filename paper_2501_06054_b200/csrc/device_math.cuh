@@ -28,7 +28,7 @@ __host__ __device__ inline void philox_make_keys(uint64_t seed, PhiloxKeys& pk) 
 
 // 32 x 32 -> 64-bit product as ONE instruction (IMAD.WIDE.U32: 4 clocks of the heavy FMA pipe, one issue slot).
 // Written as mul.wide.u32 because ptxas otherwise may split a __umulhi/mul.lo pair into IMAD.HI + IMAD: the
-// same pipe time but twice the issue slots (profiles/r2_ws_notes.md).
+// same pipe time but twice the issue slots (seen in the SASS of the round-2 kernels; pipe rates: profiles/r2_microbench.md).
 __device__ __forceinline__ void mul_wide(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
   unsigned long long p;
   asm("mul.wide.u32 %0, %1, %2;" : "=l"(p) : "r"(a), "r"(b));

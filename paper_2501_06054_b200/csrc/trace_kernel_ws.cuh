@@ -3,8 +3,8 @@
 //
 //   1 producer warpgroup (4 warps, one per SM sub-partition): stage A (Philox block 0 + integer slit-1 test on
 //       every launched neutron) and stage B0 (Philox block 1 + certain-miss classifier on the 25 % that survive):
-//       pure integer work, bound by the heavy FMA pipe (IMAD.WIDE, 4 clocks each).  Measured (profiles/
-//       r2_ws_probes.md): ONE such warp per sub-partition already saturates that pipe; more only queue behind it.
+//       pure integer work, bound by the multiplier and the logic pipe together (profiles/r2_microbench.md,
+//       r2_stage_split.md).  Four such warps per sub-partition (four blocks per SM) keep those pipes fed, two do not.
 //   CWG consumer warpgroups (4 x CWG warps; 1 or 3, chosen per launch): stage B (fp64 geometry, long dependent chains: latency bound,
 //       wants as many warps as fit) and stage C (model node loops, weight, histogram) on the FP64/FP32/XU pipes.
 //

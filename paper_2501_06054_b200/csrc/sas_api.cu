@@ -600,20 +600,42 @@ int effective_precision(const sas_model_desc& m, const sas_instrument_desc& ins)
 // Is a launch of this experiment on the warp-specialised kernel bound by its consumers (stages B and C) rather than
 // by the Philox producers?  Then the block is split into one producer and three consumer warpgroups instead of one
 // and one (trace_kernel_ws.cuh).  Measured at 1e8..1e9 neutrons, heavy split against default: barbell per event
-// +9 %, Hayter MSA +3 %, 32 fp64 sphere nodes +3 %; one fp64 evaluation per neutron (sphere -13 %, per-event
-// cylinder -5 %) and the fp32 node loops (32 sphere nodes -8 %) stay with the default split.
+// +9 %, Hayter MSA +3 %, 32 fp64 sphere nodes +5 % (break-even at 20-24 nodes), 2 x 2 nodes of a core-shell
+// cylinder +12 %, 3 x 3 of an elliptical cylinder +8 % (2 x 2: even), 5 x 4 nodes of a plain cylinder -7 %; one fp64
+// evaluation per neutron (sphere -13 %, per-event cylinder -5 %) and the fp32 node loops (32 sphere nodes -8 %) stay
+// with the default split.  The rule: node evaluations, each weighted by what one costs next to an fp64 sphere node
+// (slope of the kernel time against the node count: sphere 0.0102, cylinder 0.0045, elliptical cylinder 0.039,
+// core-shell cylinder 0.081 ms per evaluation and 1e8 neutrons; the other models by their instruction mix).
 #ifndef SAS_WS_MSA_HEAVY
 #define SAS_WS_MSA_HEAVY 1
 #endif
 #ifndef SAS_WS_HEAVY_EVALS
 #define SAS_WS_HEAVY_EVALS 24
 #endif
+double eval_weight(int model) {
+  switch (model) {
+    case SAS_SPHERE: return 1.0;                  // measured
+    case SAS_CORE_SHELL_SPHERE: return 2.0;
+    case SAS_CYLINDER: return 0.5;                // measured (0.45)
+    case SAS_TRIAXIAL_ELLIPSOID: return 1.2;
+    case SAS_PARALLELEPIPED: return 3.0;
+    case SAS_CORE_SHELL_CYLINDER: return 8.0;     // measured
+    case SAS_ELLIPSOID: return 1.2;
+    case SAS_ELLIPTICAL_CYLINDER: return 3.8;     // measured
+    case SAS_HOLLOW_CYLINDER: return 6.0;
+    case SAS_CORE_SHELL_ELLIPSOID: return 2.4;
+    case SAS_POLYMER_MICELLE: return 4.0;
+    case SAS_HOLLOW_PRISM_THIN: return 5.0;
+    default: return 1.0;
+  }
+}
 bool consumer_bound(const ExpParams& P, int precision) {
   if (precision != SAS_FP64 || P.model == SAS_FLAT) return false;
   if (P.model == SAS_BARBELL || P.model == SAS_CAPPED_CYLINDER) return true;  // 64 slices with a Bessel J1 each
   if (P.sq_kind == SAS_SQ_HAYTER_MSA) return SAS_WS_MSA_HEAVY != 0;            // 33 fp64 sine/cosine pairs
   const long evals = (long)std::max(P.n_a, 1) * std::max(P.n_b, 1) * std::max(P.n_th, 1) * std::max(P.n_ph, 1);
-  return evals >= SAS_WS_HEAVY_EVALS;
+  if (SAS_WS_HEAVY_EVALS == 0) return true;     // (test builds: every fp64 launch in the heavy split)
+  return evals > 1 && (double)evals * eval_weight(P.model) >= (double)SAS_WS_HEAVY_EVALS;
 }
 
 // (re)build ExpParams + tables of every experiment and upload them
